@@ -1,0 +1,153 @@
+"""ctypes loader for oracle/nf_oracle.c -- the plain double-precision CPU oracle.
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT (see the header of nf_oracle.c).  Every function here
+is a thin marshalling layer over the C functions of the same name (prefix ``nfo_``); the
+arithmetic lives in nf_oracle.c, each routine citing the PAPER.md passage it follows.
+
+Parity status: every function is pinned by tests/test_oracle_pins.py (brute force, closed
+forms, invariants); nothing here is "parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "nf_oracle.c")
+_LIB = os.path.join(_HERE, "libnf_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile nf_oracle.c with gcc (-ffp-contract=off: the float32 binning formulas are a
+    bit-exact contract and must not be fused)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        c_f32p = ctypes.POINTER(ctypes.c_float)
+        c_u32p = ctypes.POINTER(ctypes.c_uint32)
+        c_u64p = ctypes.POINTER(ctypes.c_uint64)
+        c_i64p = ctypes.POINTER(ctypes.c_int64)
+        c_f64p = ctypes.POINTER(ctypes.c_double)
+        lib.nfo_keys.restype = ctypes.c_int64
+        lib.nfo_keys.argtypes = [c_f32p, ctypes.c_int64, ctypes.c_int, ctypes.c_float, c_u32p]
+        lib.nfo_bin.restype = ctypes.c_int64
+        lib.nfo_bin.argtypes = [c_f32p, ctypes.c_int64, ctypes.c_int, ctypes.c_float,
+                                c_f32p, c_u32p, c_u32p, c_u64p]
+        lib.nfo_forces.restype = ctypes.c_int
+        lib.nfo_forces.argtypes = [c_f32p, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                   ctypes.c_float, ctypes.c_double, c_i64p, ctypes.c_int64,
+                                   ctypes.c_int, ctypes.c_int, c_f64p]
+        lib.nfo_interactions.restype = ctypes.c_int64
+        lib.nfo_interactions.argtypes = [c_u32p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+        lib.nfo_spline_over_r.restype = ctypes.c_double
+        lib.nfo_spline_over_r.argtypes = [ctypes.c_double, ctypes.c_double]
+        lib.nfo_plummer_over_r.restype = ctypes.c_double
+        lib.nfo_plummer_over_r.argtypes = [ctypes.c_double, ctypes.c_double]
+        lib.nfo_max_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _f32(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a, a.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
+
+
+def max_threads() -> int:
+    return int(_load().nfo_max_threads())
+
+
+def keys(pos, K: int, box: float):
+    """Cell key per particle; returns (keys uint32[N], n_out_of_range)."""
+    lib = _load()
+    pos, p = _f32(pos)
+    n = pos.shape[0]
+    out = np.empty(n, dtype=np.uint32)
+    nbad = lib.nfo_keys(p, n, int(K), float(box), out.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)))
+    return out, int(nbad)
+
+
+def bin_particles(pos, K: int, box: float):
+    """Stable counting sort by cell.
+    Returns dict(pos_sorted float32[N,4], perm uint32[N], cell_count uint32[K^3],
+    cell_offset uint64[K^3+1], n_out_of_range)."""
+    lib = _load()
+    pos, p = _f32(pos)
+    n = pos.shape[0]
+    ncell = int(K) ** 3
+    ps = np.empty((n, 4), dtype=np.float32)
+    perm = np.empty(n, dtype=np.uint32)
+    cnt = np.empty(ncell, dtype=np.uint32)
+    off = np.empty(ncell + 1, dtype=np.uint64)
+    nbad = lib.nfo_bin(p, n, int(K), float(box),
+                       ps.ctypes.data_as(ctypes.POINTER(ctypes.c_float)),
+                       perm.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)),
+                       cnt.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)),
+                       off.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)))
+    return dict(pos_sorted=ps, perm=perm, cell_count=cnt, cell_offset=off, n_out_of_range=int(nbad))
+
+
+def forces(pos, K: int, R: int, eps: float, box: float, Gm: float, sink_idx=None,
+           softening: str = "spline", nthreads: int = 0):
+    """Near-field accelerations in double (Eq. 2 :243 / Eq. 1 :233).
+    Returns float64[n_sinks, 3] in the order of sink_idx (all particles, input order, if None)."""
+    lib = _load()
+    pos, p = _f32(pos)
+    n = pos.shape[0]
+    if sink_idx is None:
+        sp, ns = None, n
+    else:
+        sink_idx = np.ascontiguousarray(sink_idx, dtype=np.int64)
+        sp, ns = sink_idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), sink_idx.shape[0]
+    acc = np.zeros((ns, 3), dtype=np.float64)
+    soft = {"spline": 0, "plummer": 1}[softening]
+    rc = lib.nfo_forces(p, n, int(K), int(R), float(eps), float(box), float(Gm), sp, ns, soft,
+                        int(nthreads), acc.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    if rc != 0:
+        raise ValueError("nfo_forces: bad arguments (need K >= 2R+1, R >= 0, eps > 0, box > 0)")
+    return acc
+
+
+def interactions(cell_count, K: int, R: int, sink_plane_lo: int = 0, sink_plane_hi=None) -> int:
+    """I = sum_c n_c sum_{c' in N(c)} n_c' (ordered pairs, self pairs included)."""
+    lib = _load()
+    cc = np.ascontiguousarray(cell_count, dtype=np.uint32)
+    hi = int(K) if sink_plane_hi is None else int(sink_plane_hi)
+    return int(lib.nfo_interactions(cc.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)), int(K), int(R),
+                                    int(sink_plane_lo), hi))
+
+
+def spline_over_r(r: float, eps: float) -> float:
+    """|F|/r of Eq. 2."""
+    return float(_load().nfo_spline_over_r(float(r), float(eps)))
+
+
+def plummer_over_r(r: float, eps_p: float) -> float:
+    """|F|/r of Eq. 1."""
+    return float(_load().nfo_plummer_over_r(float(r), float(eps_p)))
+
+
+def parity_error(a_test, a_ref):
+    """Per-particle error metric of BASELINE.json's north_star:
+    e_i = |a_test,i - a_ref,i| / max(|a_ref,i|, rms_k |a_ref,k|)   (2-norms over xyz).
+    Modelled on the paper's own single-vs-double comparison."""
+    a_test = np.asarray(a_test, dtype=np.float64)
+    a_ref = np.asarray(a_ref, dtype=np.float64)
+    mag = np.sqrt((a_ref ** 2).sum(axis=1))
+    rms = np.sqrt((mag ** 2).mean()) if mag.size else 0.0
+    den = np.maximum(mag, rms)
+    den = np.where(den > 0, den, 1.0)
+    return np.sqrt(((a_test - a_ref) ** 2).sum(axis=1)) / den
