@@ -1,0 +1,197 @@
+/*
+ * nf.h -- C ABI of libnf: the near-field force of the Abacus N-body method on one B200.
+ *
+ * Source of every definition: arXiv:1810.02916, Sec. 2.1 "Method" and Sec. 4.3
+ * "Softening".  Readings of points the paper leaves open are listed in DESIGN.md ("Readings").
+ *
+ *   - "the domain is decomposed into K^3 cubic cells, and every particle belongs to one
+ *     cell"                                              -> nf_bin
+ *   - "Particles in cells separated by fewer than near-field radius R cells (typically 2)
+ *     interact via the near-field force, which we compute as a direct pairwise summation of
+ *     1/r^2 forces (or some appropriately softened form)"; 2R+1 slabs are
+ *     needed, i.e. the (2R+1)^3 neighbour cells          -> nf_forces
+ *   - compact spline softening, Eq. 2; Plummer, Eq. 1
+ *   - "positions are stored as offsets relative to cell centers"
+ *   - the slab pipeline: "load a rolling window of slabs ... compute forces ... on the
+ *     central slab, write out the trailing slab, and then load a slab at the leading edge"
+ *     (PAPER.md:41), fed from pinned host memory        -> nf_stream_slabs
+ *
+ * Conventions
+ *   - Plain C types only.  "dev" pointers are CUDA device pointers on the context's device,
+ *     "host" pointers are host memory (pinned where stated).  `stream` is a cudaStream_t
+ *     passed as void* (NULL = the legacy default stream).
+ *   - The caller owns every input and output buffer.  The library never frees or retains a
+ *     caller buffer past the stream-ordered work of the call that received it.  The context
+ *     owns only scratch memory.
+ *   - Every call returns an int status (NF_OK = 0).  Argument checks happen on the host
+ *     before any launch.  No exceptions, no exit(), no output to stdout/stderr.
+ *     nf_last_error() gives a human-readable detail for the last non-zero status.
+ *   - nf_bin and nf_forces are asynchronous: they enqueue work on `stream` and return.
+ *     They may synchronise only when scratch memory has to grow (avoid with nf_reserve).
+ *   - There is no CPU fallback anywhere in this library.
+ *   - A context must not be used from two threads at once.
+ */
+#ifndef NF_H
+#define NF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nf_ctx nf_ctx;
+
+enum {
+    NF_OK = 0,
+    NF_ERR_ARG = 1,    /* null pointer, N < 0, K < 2R+1, K > NF_MAX_K, R < 0, eps <= 0, box <= 0, ... */
+    NF_ERR_NOMEM = 2,  /* device or host allocation failed */
+    NF_ERR_CUDA = 3,   /* CUDA runtime error; nf_last_error() names it */
+    NF_ERR_RANGE = 4   /* positions outside [0, box) were seen and clamped into the edge cell */
+};
+
+enum {
+    NF_SOFT_SPLINE = 0, /* Eq. 2: F = [10 - 15u + 6u^2] r/eps^3 (u = r/eps < 1), r/r^3 beyond */
+    NF_SOFT_PLUMMER = 1 /* Eq. 1: F = r/(r^2 + eps^2)^(3/2) */
+};
+
+#define NF_MAX_K 1024 /* K^3 must fit a uint32 key; radix digits are per-axis cell indices */
+#define NF_MAX_R 3
+
+/* Library version: major*10000 + minor*100 + patch. */
+int nf_version(void);
+
+/* Create / destroy a context on CUDA device `device`.  The context owns scratch memory
+ * (sort keys, histograms, work lists, slab ring buffers) and internal streams/events. */
+int nf_create(nf_ctx **out, int device);
+int nf_destroy(nf_ctx *ctx);
+
+/* Text for the last non-zero status returned on this context ("" if none).  The pointer is
+ * valid until the next call on the context.  ctx may be NULL (returns a static string). */
+const char *nf_last_error(const nf_ctx *ctx);
+
+/* Pre-size scratch for up to maxN particles and K cells per side so that later nf_bin /
+ * nf_forces calls with N <= maxN never allocate (and therefore never synchronise). */
+int nf_reserve(nf_ctx *ctx, int64_t maxN, int K);
+
+/*
+ * nf_bin -- cell assignment + STABLE counting sort into cell-contiguous arrays.
+ * (PAPER.md:37 cells; :41/:47 slab = all Y,Z at one X => x is the slowest index; :51 offsets.)
+ *
+ *   pos_xyz      dev in   N x 3 float32, global positions, each coordinate in [0, box)
+ *   N            number of particles, 0 <= N < 2^32
+ *   K            cells per side, 1 <= K <= NF_MAX_K
+ *   box          periodic box length L > 0
+ *   pos_sorted   dev out  N x 4 float32 (16-byte aligned): xyz = offset of the particle from
+ *                         the centre of its own cell, w = 0 (reserved: mass)
+ *   perm         dev out  N uint32: original index of the particle in each sorted slot
+ *   cell_count   dev out  K^3 uint32, linear cell index (cx*K + cy)*K + cz (z fastest)
+ *   cell_offset  dev out  K^3+1 uint64, exclusive prefix sum of cell_count
+ *
+ * Bit-exact contract, all in float32, no fused
+ * multiply-add:  invw = (float)K / box;  c = (int)floorf(x * invw) clamped to [0, K-1];
+ * hw = 0.5f * (box / (float)K);  centre = (float)(2c+1) * hw;  offset = x - centre.
+ * Ties (same cell) keep their input order (perm increases within a cell), so the output is
+ * unique.  Particles outside [0, box) (or NaN) are clamped into the edge cell and counted;
+ * read the count with nf_out_of_range().
+ */
+int nf_bin(nf_ctx *ctx, const float *pos_xyz, int64_t N, int K, float box,
+           float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,
+           void *stream);
+
+/* Synchronises `stream`, stores the number of out-of-range particles seen by the last nf_bin
+ * (or nf_stream_slabs) on this context in *n, and returns NF_ERR_RANGE if it is non-zero. */
+int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream);
+
+/*
+ * nf_forces -- near-field accelerations for every particle (fully periodic box).
+ *
+ *   a_i = Gm * sum over the (2R+1)^3 periodic neighbour cells c' of cell(i), over j in c':
+ *         f(|d|) d,   d = (o_j - o_i) + (c' - c) * w   (cell-centred offsets, w = box/K),
+ *   f(r) = min(10 - 15u + 6u^2, u^-3) / eps^3, u = r/eps  (== Eq. 2, see fn. 4 PAPER.md:239),
+ *   or the Plummer law.  Pairs with r = 0 (self, coincident particles) contribute zero.
+ *   The periodic image of a source is fixed by the cell offset (reading c8).
+ *
+ *   pos_sorted, cell_offset, cell_count   dev in   as written by nf_bin
+ *   perm         dev in, nullable: if given, accelerations are written in the caller's
+ *                original order (acc[perm[s]] = a of sorted slot s), else in sorted order
+ *   N, K, box    as for nf_bin;  requires K >= 2R+1 (else a cell would be listed twice)
+ *   R            near-field radius in cells, 0 <= R <= NF_MAX_R  (the paper uses 2)
+ *   eps          softening length > 0: eps_s of Eq. 2, or eps_p of Eq. 1 (no 2.16 factor is
+ *                applied inside the library; see nf_spline_equivalent_eps)
+ *   Gm           G times the (equal) particle mass
+ *   softening    NF_SOFT_SPLINE or NF_SOFT_PLUMMER
+ *   acc_xyz      dev out  N x 3 float32
+ *
+ * float32 in, float32 accumulate (per source tile, with a compensated outer sum), float32
+ * out.  Deterministic: no floating-point atomics; the same inputs give the same bits.
+ */
+int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
+              const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
+              float eps, float box, float Gm, int softening, float *acc_xyz, void *stream);
+
+/* Number of ordered (sink, source) pairs nf_forces evaluates for these cell counts:
+ * I = sum_c n_c * sum_{c' in N(c)} n_c'  (self pairs included, padding excluded; the
+ * "pairwise interactions" of PAPER.md:107).  Computed on the device, synchronises `stream`,
+ * result in *interactions (host). */
+int nf_interactions(nf_ctx *ctx, const uint32_t *cell_count, int K, int R,
+                    int64_t *interactions, void *stream);
+
+/* eps_s = 2.16 eps_p: the spline softening with the same minimum pairwise
+ * dynamical time as a Plummer softening eps_p.  Pure host helper. */
+float nf_spline_equivalent_eps(float eps_plummer);
+
+/* Statistics of one nf_stream_slabs call (all times in seconds, measured with CUDA events). */
+typedef struct nf_stream_stats {
+    int64_t particles_in;    /* particles copied host -> device (sink + ghost planes) */
+    int64_t particles_out;   /* accelerations copied device -> host (sink planes) */
+    int64_t interactions;    /* ordered pairs evaluated */
+    int64_t out_of_range;    /* particles clamped (see nf_bin) or found in the wrong plane */
+    double h2d_bytes, d2h_bytes;
+    double h2d_seconds, d2h_seconds;      /* sum of the individual copies' durations */
+    double kernel_seconds;                /* sum of bin + force kernel durations */
+    double wall_seconds;                  /* first H2D start to last D2H end */
+    double h2d_gbps, d2h_gbps;            /* bytes / copy seconds */
+    double overlap_fraction;              /* 1 - (wall - kernel)/ (h2d + d2h seconds), clamped to [0,1] */
+} nf_stream_stats;
+
+/*
+ * nf_stream_slabs -- the slab-ordered pass over P consecutive x-planes of
+ * cells, from pinned host memory, with H2D / D2H copies on side streams overlapping the
+ * kernels.
+ *
+ *   plane_pos_host  host in   P + 2R pointers (pinned memory); plane q holds plane_n[q] x 3
+ *                             float32 global positions of the particles whose x-cell index
+ *                             is (plane0 + q) mod K; the first and last R planes are ghosts
+ *                             (sources only)
+ *   plane_n         host in   P + 2R particle counts
+ *   P               number of sink planes, >= 1
+ *   K               cells per side of the full box (y and z have K cells and are periodic
+ *                   with period box; cell width w = box / K)
+ *   R, eps, Gm, softening     as for nf_forces
+ *   plane0          x-cell index of the first ghost plane, may be negative or wrap past K
+ *                   (the plane index is taken modulo K; the caller supplies the wrapped
+ *                   planes' particles with their stored coordinates in [0, box))
+ *   plane_acc_host  host out  P pointers (pinned): plane_n[R+p] x 3 float32 accelerations of
+ *                             sink plane p, in that plane's input order
+ *   stats           host out, nullable
+ *
+ * x is open inside the chunk: only the P + 2R supplied planes act as sources.  Requires
+ * K >= 2R+1 and P + 2R <= K.  Returns after the last D2H copy has completed (the call
+ * synchronises); `stream` orders the call after prior work on that stream.
+ */
+int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,
+                    int P, int K, int R, float eps, float box, int plane0, float Gm,
+                    int softening, float *const *plane_acc_host, nf_stream_stats *stats,
+                    void *stream);
+
+/* Timing of the kernels of the last nf_forces call on this context (CUDA events recorded on
+ * the call's stream around the interaction kernel).  Synchronises on the end event.
+ * *kernel_ms = duration of the interaction kernel alone; *total_ms = whole nf_forces call
+ * (work-list build + kernel + scale/un-permute).  Either pointer may be NULL. */
+int nf_last_forces_timing(nf_ctx *ctx, float *kernel_ms, float *total_ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NF_H */

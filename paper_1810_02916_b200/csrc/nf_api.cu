@@ -1,0 +1,201 @@
+// nf_api.cu -- extern "C" entry points declared in include/nf.h (argument checks, scratch
+// sizing, dispatch).  Every step of the path runs in the kernels of nf_bin.cu / nf_forces.cu.
+#include <new>
+
+#include "nf_common.cuh"
+
+static const char *const k_no_ctx = "nf: null context";
+
+int nf_scratch_reserve(nf_ctx *ctx, size_t bytes)
+{
+    if (bytes <= ctx->scratch_bytes) return NF_OK;
+    NF_CUDA(ctx, cudaDeviceSynchronize());
+    if (ctx->scratch) NF_CUDA(ctx, cudaFree(ctx->scratch));
+    ctx->scratch = nullptr;
+    ctx->scratch_bytes = 0;
+    size_t want = nf_align_up(bytes + bytes / 16, 1 << 20);
+    cudaError_t e = cudaMalloc((void **)&ctx->scratch, want);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        NF_SET_ERR(ctx, "cudaMalloc of %zu scratch bytes failed: %s", want, cudaGetErrorString(e));
+        return NF_ERR_NOMEM;
+    }
+    ctx->scratch_bytes = want;
+    return NF_OK;
+}
+
+extern "C" {
+
+int nf_version(void) { return NF_VERSION_NUM; }
+
+int nf_create(nf_ctx **out, int device)
+{
+    if (!out) return NF_ERR_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return NF_ERR_CUDA;
+    }
+    nf_ctx *ctx = new (std::nothrow) nf_ctx();
+    if (!ctx) return NF_ERR_NOMEM;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->device = device;
+    int rc = NF_OK;
+    do {
+        if (cudaSetDevice(device) != cudaSuccess) { rc = NF_ERR_CUDA; break; }
+        if (cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { rc = NF_ERR_CUDA; break; }
+        if (cudaMalloc((void **)&ctx->counters, 16 * sizeof(unsigned long long)) != cudaSuccess) { rc = NF_ERR_NOMEM; break; }
+        if (cudaMemset(ctx->counters, 0, 16 * sizeof(unsigned long long)) != cudaSuccess) { rc = NF_ERR_CUDA; break; }
+        if (cudaMallocHost((void **)&ctx->h_counters, 16 * sizeof(unsigned long long)) != cudaSuccess) { rc = NF_ERR_NOMEM; break; }
+        memset(ctx->h_counters, 0, 16 * sizeof(unsigned long long));
+        if (cudaEventCreate(&ctx->ev_total0) != cudaSuccess || cudaEventCreate(&ctx->ev_kern0) != cudaSuccess ||
+            cudaEventCreate(&ctx->ev_kern1) != cudaSuccess || cudaEventCreate(&ctx->ev_total1) != cudaSuccess) { rc = NF_ERR_CUDA; break; }
+        if (cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking) != cudaSuccess) { rc = NF_ERR_CUDA; break; }
+    } while (0);
+    if (rc != NF_OK) {
+        cudaGetLastError();
+        nf_destroy(ctx);
+        return rc;
+    }
+    *out = ctx;
+    return NF_OK;
+}
+
+int nf_destroy(nf_ctx *ctx)
+{
+    if (!ctx) return NF_OK;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    if (ctx->scratch) cudaFree(ctx->scratch);
+    if (ctx->counters) cudaFree(ctx->counters);
+    if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
+    if (ctx->ev_total0) cudaEventDestroy(ctx->ev_total0);
+    if (ctx->ev_kern0) cudaEventDestroy(ctx->ev_kern0);
+    if (ctx->ev_kern1) cudaEventDestroy(ctx->ev_kern1);
+    if (ctx->ev_total1) cudaEventDestroy(ctx->ev_total1);
+    if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
+    if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
+    nf_slab_state_free(ctx);
+    cudaGetLastError();
+    delete ctx;
+    return NF_OK;
+}
+
+const char *nf_last_error(const nf_ctx *ctx) { return ctx ? ctx->err : k_no_ctx; }
+
+static int check_common(nf_ctx *ctx, int64_t N, int K, float box)
+{
+    NF_ARG(ctx, N >= 0 && N < ((int64_t)1 << 32), "N = %lld out of range [0, 2^32)", (long long)N);
+    NF_ARG(ctx, K >= 1 && K <= NF_MAX_K, "K = %d out of range [1, %d]", K, NF_MAX_K);
+    NF_ARG(ctx, box > 0.0f && box < 3.0e38f, "box must be positive and finite");
+    return NF_OK;
+}
+
+static size_t forces_scratch_full(int K)
+{
+    nf_force_params p{};
+    p.K = K;
+    p.n_planes = K;
+    return nf_forces_scratch_bytes(p);
+}
+
+int nf_reserve(nf_ctx *ctx, int64_t maxN, int K)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_TRY(check_common(ctx, maxN, K, 1.0f));
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    size_t need = nf_bin_scratch_bytes(maxN, K, false);
+    size_t f = forces_scratch_full(K);
+    return nf_scratch_reserve(ctx, need > f ? need : f);
+}
+
+int nf_bin(nf_ctx *ctx, const float *pos_xyz, int64_t N, int K, float box, float *pos_sorted,
+           uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_TRY(check_common(ctx, N, K, box));
+    NF_ARG(ctx, cell_count && cell_offset, "nf_bin: cell_count / cell_offset must not be null");
+    NF_ARG(ctx, N == 0 || (pos_xyz && pos_sorted && perm), "nf_bin: null particle array with N > 0");
+    NF_ARG(ctx, ((uintptr_t)pos_sorted & 15) == 0, "nf_bin: pos_sorted must be 16-byte aligned");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    NF_TRY(nf_scratch_reserve(ctx, nf_bin_scratch_bytes(N, K, false)));
+    nf_scratch_reset(ctx);
+    NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, sizeof(unsigned long long), (cudaStream_t)stream));
+    return nf_bin_impl(ctx, pos_xyz, N, K, box, -1, pos_sorted, perm, cell_count, cell_offset, (cudaStream_t)stream);
+}
+
+int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, n != nullptr, "nf_out_of_range: null output");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    NF_CUDA(ctx, cudaStreamSynchronize(st));
+    *n = (int64_t)ctx->h_counters[0];
+    if (*n) {
+        NF_SET_ERR(ctx, "%lld particle(s) outside [0, box) were clamped into edge cells", (long long)*n);
+        return NF_ERR_RANGE;
+    }
+    return NF_OK;
+}
+
+static int check_force_args(nf_ctx *ctx, int K, int R, float eps, float Gm, int softening)
+{
+    NF_ARG(ctx, R >= 0 && R <= NF_MAX_R, "R = %d out of range [0, %d]", R, NF_MAX_R);
+    NF_ARG(ctx, K >= 2 * R + 1, "K = %d < 2R+1 = %d would list a neighbour cell twice", K, 2 * R + 1);
+    NF_ARG(ctx, eps > 0.0f && eps < 3.0e38f, "eps must be positive and finite");
+    NF_ARG(ctx, Gm == Gm && fabsf(Gm) < 3.0e38f, "Gm must be finite");
+    NF_ARG(ctx, softening == NF_SOFT_SPLINE || softening == NF_SOFT_PLUMMER, "unknown softening %d", softening);
+    return NF_OK;
+}
+
+int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
+              const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
+              float eps, float box, float Gm, int softening, float *acc_xyz, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_TRY(check_common(ctx, N, K, box));
+    NF_TRY(check_force_args(ctx, K, R, eps, Gm, softening));
+    NF_ARG(ctx, cell_offset && cell_count, "nf_forces: cell_offset / cell_count must not be null");
+    NF_ARG(ctx, N == 0 || (pos_sorted && acc_xyz), "nf_forces: null particle array with N > 0");
+    NF_ARG(ctx, ((uintptr_t)pos_sorted & 15) == 0, "nf_forces: pos_sorted must be 16-byte aligned");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (N == 0) return NF_OK;
+    nf_force_params p{};
+    p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
+    p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening;
+    NF_TRY(nf_scratch_reserve(ctx, nf_forces_scratch_bytes(p)));
+    nf_scratch_reset(ctx);
+    nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
+    if (!d_planes) { NF_SET_ERR(ctx, "nf_forces: internal scratch arena too small"); return NF_ERR_NOMEM; }
+    cudaStream_t st = (cudaStream_t)stream;
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(pos_sorted), cell_offset, perm, acc_xyz, st));
+    return nf_forces_impl(ctx, p, d_planes, st, true);
+}
+
+int nf_interactions(nf_ctx *ctx, const uint32_t *cell_count, int K, int R, int64_t *interactions, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, cell_count && interactions, "nf_interactions: null argument");
+    NF_ARG(ctx, K >= 1 && K <= NF_MAX_K && R >= 0 && R <= NF_MAX_R && K >= 2 * R + 1, "nf_interactions: bad K / R");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    return nf_interactions_impl(ctx, cell_count, K, R, interactions, (cudaStream_t)stream);
+}
+
+float nf_spline_equivalent_eps(float eps_plummer) { return 2.16f * eps_plummer; }
+
+int nf_last_forces_timing(nf_ctx *ctx, float *kernel_ms, float *total_ms)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, ctx->forces_timed, "nf_last_forces_timing: no nf_forces call has been timed yet");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    NF_CUDA(ctx, cudaEventSynchronize(ctx->ev_total1));
+    if (kernel_ms) NF_CUDA(ctx, cudaEventElapsedTime(kernel_ms, ctx->ev_kern0, ctx->ev_kern1));
+    if (total_ms) NF_CUDA(ctx, cudaEventElapsedTime(total_ms, ctx->ev_total0, ctx->ev_total1));
+    return NF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,242 @@
+// nf_bin.cu -- cell assignment and STABLE counting sort by cell.
+//
+// PAPER.md:37 "the domain is decomposed into K^3 cubic cells, and every particle belongs to
+// one cell"; :47 a slab spans all Y,Z at one X (x slowest, z fastest); :51 positions are
+// stored as float32 offsets from the cell centre.
+//
+// Pipeline (all on the caller's stream):
+//   keys      one thread per particle: float32 cell index per axis (bit-exact contract in
+//             include/nf.h), key = (cx*K+cy)*K+cz, cell histogram by integer atomics
+//   scan      cell_offset = exclusive scan of cell_count (uint64)
+//   radix     LSD radix sort of (key, original index) with one digit per axis (cz, cy, cx),
+//             each pass a stable counting sort over <= K bins: per-tile digit histogram,
+//             device-wide scan, stable scatter with warp-level match/ballot ranking.
+//             LSD + stable passes => ties keep input order => perm increases within a cell.
+//   gather    sorted slot s: i = perm[s]; offset = x_i - centre(cell) -> float4
+//
+// The sort is deterministic (no atomics decide an output position).
+#include "nf_common.cuh"
+
+namespace {
+
+constexpr int RS_THREADS = 256;
+constexpr int RS_WARPS = RS_THREADS / 32;
+constexpr int RS_ROUNDS = 16;                       // rounds of 32 elements per warp
+constexpr int RS_WARP_ELEMS = RS_ROUNDS * 32;       // 512
+constexpr int RS_TILE = RS_WARPS * RS_WARP_ELEMS;   // 4096
+
+// float32 cell index, include/nf.h contract: c = (int)floorf(x * invw) clamped to [0, K-1].
+// __fmul_rn is never contracted into an FMA.
+__device__ __forceinline__ int cell_index(float x, float invw, int K, int *bad)
+{
+    float fl = floorf(__fmul_rn(x, invw));
+    int b = !(fl >= 0.0f && fl <= (float)(K - 1));
+    int c;
+    if (!(fl >= 0.0f)) c = 0;
+    else if (fl > (float)(K - 1)) c = K - 1;
+    else c = (int)fl;
+    *bad |= b;
+    return c;
+}
+
+__global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pos, int64_t N, int K, float invw, int plane_cx,
+                                              uint32_t *__restrict__ keys, uint32_t *__restrict__ cell_count,
+                                              unsigned long long *__restrict__ n_bad)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int bad = 0;
+    if (i < N) {
+        float x = pos[3 * i + 0], y = pos[3 * i + 1], z = pos[3 * i + 2];
+        int cx = cell_index(x, invw, K, &bad);
+        int cy = cell_index(y, invw, K, &bad);
+        int cz = cell_index(z, invw, K, &bad);
+        uint32_t key;
+        if (plane_cx >= 0) {
+            bad |= (cx != plane_cx);
+            key = (uint32_t)cy * (uint32_t)K + (uint32_t)cz;
+        } else {
+            key = ((uint32_t)cx * (uint32_t)K + (uint32_t)cy) * (uint32_t)K + (uint32_t)cz;
+        }
+        keys[i] = key;
+        atomicAdd(&cell_count[key], 1u);
+    }
+    unsigned m = __ballot_sync(0xffffffffu, bad);
+    if (m && (threadIdx.x & 31) == 0) atomicAdd(n_bad, (unsigned long long)__popc(m));
+}
+
+__device__ __forceinline__ uint32_t digit_of(uint32_t key, uint32_t div, uint32_t K) { return (key / div) % K; }
+
+// per-tile digit histogram -> hist[digit * ntiles + tile]
+__global__ void __launch_bounds__(RS_THREADS) k_radix_hist(const uint32_t *__restrict__ keys, int64_t N, uint32_t div, uint32_t K,
+                                                           uint32_t *__restrict__ hist, uint32_t ntiles)
+{
+    extern __shared__ uint32_t sh[];
+    for (uint32_t d = threadIdx.x; d < K; d += RS_THREADS) sh[d] = 0;
+    __syncthreads();
+    int64_t base = (int64_t)blockIdx.x * RS_TILE;
+#pragma unroll 4
+    for (int k = 0; k < RS_TILE / RS_THREADS; k++) {
+        int64_t i = base + (int64_t)k * RS_THREADS + threadIdx.x;
+        if (i < N) atomicAdd(&sh[digit_of(keys[i], div, K)], 1u);
+    }
+    __syncthreads();
+    for (uint32_t d = threadIdx.x; d < K; d += RS_THREADS) hist[(size_t)d * ntiles + blockIdx.x] = sh[d];
+}
+
+// stable scatter.  Warp w of the tile owns elements [tile*4096 + w*512, +512) in index order.
+// idx_in == nullptr means "identity" (first pass).
+__global__ void __launch_bounds__(RS_THREADS) k_radix_scatter(const uint32_t *__restrict__ keys_in, const uint32_t *__restrict__ idx_in,
+                                                              int64_t N, uint32_t div, uint32_t K,
+                                                              const uint32_t *__restrict__ hist_scanned, uint32_t ntiles,
+                                                              uint32_t *__restrict__ keys_out, uint32_t *__restrict__ idx_out)
+{
+    extern __shared__ uint32_t sh[];  // [RS_WARPS][K]
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned lt = (1u << lane) - 1u;
+    for (uint32_t d = threadIdx.x; d < K * RS_WARPS; d += RS_THREADS) sh[d] = 0;
+    __syncthreads();
+    uint32_t *cnt = sh + (size_t)w * K;
+    const int64_t wbase = (int64_t)blockIdx.x * RS_TILE + (int64_t)w * RS_WARP_ELEMS;
+    uint32_t key[RS_ROUNDS];
+    // count pass
+#pragma unroll
+    for (int r = 0; r < RS_ROUNDS; r++) {
+        int64_t i = wbase + r * 32 + lane;
+        bool valid = i < N;
+        key[r] = valid ? keys_in[i] : 0u;
+        unsigned act = __ballot_sync(0xffffffffu, valid);
+        if (valid) {
+            uint32_t d = digit_of(key[r], div, K);
+            unsigned peers = __match_any_sync(act, d);
+            if ((peers & lt) == 0) cnt[d] += __popc(peers);  // leader = lowest lane of the group
+        }
+        __syncwarp();
+    }
+    __syncthreads();
+    // exclusive scan across warps for every digit, seeded with the tile's global base
+    for (uint32_t d = threadIdx.x; d < K; d += RS_THREADS) {
+        uint32_t run = hist_scanned[(size_t)d * ntiles + blockIdx.x];
+#pragma unroll
+        for (int ww = 0; ww < RS_WARPS; ww++) {
+            uint32_t t = sh[(size_t)ww * K + d];
+            sh[(size_t)ww * K + d] = run;
+            run += t;
+        }
+    }
+    __syncthreads();
+    // rank + scatter pass
+#pragma unroll
+    for (int r = 0; r < RS_ROUNDS; r++) {
+        int64_t i = wbase + r * 32 + lane;
+        bool valid = i < N;
+        unsigned act = __ballot_sync(0xffffffffu, valid);
+        if (valid) {
+            uint32_t d = digit_of(key[r], div, K);
+            unsigned peers = __match_any_sync(act, d);
+            int leader = __ffs(peers) - 1;
+            uint32_t base = 0;
+            if (lane == leader) {
+                base = cnt[d];
+                cnt[d] = base + __popc(peers);
+            }
+            base = __shfl_sync(peers, base, leader);
+            uint32_t dst = base + __popc(peers & lt);
+            keys_out[dst] = key[r];
+            idx_out[dst] = idx_in ? idx_in[i] : (uint32_t)i;
+        }
+        __syncwarp();
+    }
+}
+
+// gather positions into cell order and re-centre.  Offset contract:
+// hw = 0.5f*(box/(float)K); centre = (float)(2c+1)*hw; o = x - centre (no FMA contraction).
+__global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pos, const uint32_t *__restrict__ keys_sorted,
+                                                const uint32_t *__restrict__ perm, int64_t N, int K, float hw, int plane_cx,
+                                                float4 *__restrict__ pos_sorted)
+{
+    int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    uint32_t key = keys_sorted[s];
+    uint32_t i = perm[s];
+    int cz = (int)(key % (uint32_t)K);
+    int cy = (int)((key / (uint32_t)K) % (uint32_t)K);
+    int cx = plane_cx >= 0 ? plane_cx : (int)(key / ((uint32_t)K * (uint32_t)K));
+    float x = pos[3 * (size_t)i + 0], y = pos[3 * (size_t)i + 1], z = pos[3 * (size_t)i + 2];
+    float4 o;
+    o.x = __fsub_rn(x, __fmul_rn((float)(2 * cx + 1), hw));
+    o.y = __fsub_rn(y, __fmul_rn((float)(2 * cy + 1), hw));
+    o.z = __fsub_rn(z, __fmul_rn((float)(2 * cz + 1), hw));
+    o.w = 0.0f;
+    pos_sorted[s] = o;
+}
+
+}  // namespace
+
+size_t nf_bin_scratch_bytes(int64_t N, int K, bool plane)
+{
+    size_t n = (size_t)(N > 0 ? N : 1);
+    size_t ntiles = (n + RS_TILE - 1) / RS_TILE;
+    size_t ncell = plane ? (size_t)K * K : (size_t)K * K * K;
+    size_t b = 0;
+    b += 3 * nf_align_up(n * sizeof(uint32_t), 256);                 // keysA, keysB, idxB
+    b += nf_align_up((size_t)K * ntiles * sizeof(uint32_t), 256);    // digit histograms
+    b += nf_align_up(nf_scan_temp_elems((size_t)K * ntiles) * sizeof(uint32_t), 256);
+    b += nf_align_up(nf_scan_temp_elems(ncell) * sizeof(uint64_t), 256);
+    return b + 4096;
+}
+
+int nf_bin_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, int plane_cx,
+                float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,
+                cudaStream_t st)
+{
+    const bool plane = plane_cx >= 0;
+    const size_t ncell = plane ? (size_t)K * K : (size_t)K * K * K;
+    const int npass = plane ? 2 : 3;
+    const size_t n = (size_t)N;
+    const size_t ntiles = n ? (n + RS_TILE - 1) / RS_TILE : 1;
+
+    uint32_t *keysA = nf_scratch_take<uint32_t>(ctx, n ? n : 1);
+    uint32_t *keysB = nf_scratch_take<uint32_t>(ctx, n ? n : 1);
+    uint32_t *idxB = nf_scratch_take<uint32_t>(ctx, n ? n : 1);
+    uint32_t *hist = nf_scratch_take<uint32_t>(ctx, (size_t)K * ntiles);
+    uint32_t *tmp32 = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems((size_t)K * ntiles));
+    uint64_t *tmp64 = nf_scratch_take<uint64_t>(ctx, nf_scan_temp_elems(ncell));
+    if (!keysA || !keysB || !idxB || !hist || !tmp32 || !tmp64) {
+        NF_SET_ERR(ctx, "nf_bin: internal scratch arena too small");
+        return NF_ERR_NOMEM;
+    }
+
+    NF_CUDA(ctx, cudaMemsetAsync(cell_count, 0, ncell * sizeof(uint32_t), st));
+    if (N > 0) {
+        float invw = (float)K / box;
+        k_keys<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, N, K, invw, plane_cx, keysA, cell_count, ctx->counters);
+        NF_CUDA(ctx, cudaGetLastError());
+    }
+    NF_TRY(nf_exclusive_scan_u32_u64(ctx, cell_count, cell_offset, ncell, tmp64, st));
+    if (N == 0) return NF_OK;
+
+    // LSD passes: digit cz (div 1), cy (div K), cx (div K^2).  Destinations alternate so that
+    // the last pass writes the index array into `perm`.
+    const uint32_t *kin = keysA;
+    const uint32_t *iin = nullptr;
+    uint32_t div = 1;
+    for (int p = 0; p < npass; p++) {
+        bool to_perm = ((npass - 1 - p) % 2) == 0;
+        uint32_t *kout = (kin == keysA) ? keysB : keysA;
+        uint32_t *iout = to_perm ? perm : idxB;
+        size_t sh_hist = (size_t)K * sizeof(uint32_t);
+        size_t sh_scat = (size_t)K * RS_WARPS * sizeof(uint32_t);
+        k_radix_hist<<<(unsigned)ntiles, RS_THREADS, sh_hist, st>>>(kin, N, div, (uint32_t)K, hist, (uint32_t)ntiles);
+        NF_CUDA(ctx, cudaGetLastError());
+        NF_TRY(nf_exclusive_scan_u32(ctx, hist, hist, (size_t)K * ntiles, tmp32, st));
+        k_radix_scatter<<<(unsigned)ntiles, RS_THREADS, sh_scat, st>>>(kin, iin, N, div, (uint32_t)K, hist, (uint32_t)ntiles, kout, iout);
+        NF_CUDA(ctx, cudaGetLastError());
+        kin = kout;
+        iin = iout;
+        div *= (uint32_t)K;
+    }
+    float hw = 0.5f * (box / (float)K);
+    k_gather<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, kin, perm, N, K, hw, plane_cx, reinterpret_cast<float4 *>(pos_sorted));
+    NF_CUDA(ctx, cudaGetLastError());
+    return NF_OK;
+}

@@ -1,0 +1,116 @@
+// nf_common.cuh -- context, error handling and scratch arena shared by the libnf sources.
+// Part of the CUDA product path; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/nf.h"
+
+#define NF_VERSION_NUM 100
+
+struct nf_ctx {
+    int device;
+    int sm_count;
+    char err[512];
+    // bump-allocated device scratch (grown on demand; growth synchronises the device)
+    char *scratch;
+    size_t scratch_bytes;
+    size_t scratch_used;
+    // small persistent device counters: [0] out-of-range particles, [1] interactions, [2] work cursor
+    unsigned long long *counters;
+    unsigned long long *h_counters;  // pinned host mirror
+    // timing of the last nf_forces
+    cudaEvent_t ev_total0, ev_kern0, ev_kern1, ev_total1;
+    bool forces_timed;
+    // slab streaming resources (created lazily)
+    cudaStream_t s_h2d, s_d2h;
+    void *slab_state;
+};
+
+#define NF_SET_ERR(ctx, ...)                                        \
+    do {                                                            \
+        if (ctx) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__); \
+    } while (0)
+
+#define NF_CUDA(ctx, call)                                                                   \
+    do {                                                                                     \
+        cudaError_t e__ = (call);                                                            \
+        if (e__ != cudaSuccess) {                                                            \
+            NF_SET_ERR(ctx, "CUDA error %d (%s) at %s:%d: %s", (int)e__, cudaGetErrorName(e__), \
+                       __FILE__, __LINE__, cudaGetErrorString(e__));                         \
+            return e__ == cudaErrorMemoryAllocation ? NF_ERR_NOMEM : NF_ERR_CUDA;            \
+        }                                                                                    \
+    } while (0)
+
+#define NF_ARG(ctx, cond, ...)           \
+    do {                                 \
+        if (!(cond)) {                   \
+            NF_SET_ERR(ctx, __VA_ARGS__); \
+            return NF_ERR_ARG;           \
+        }                                \
+    } while (0)
+
+#define NF_TRY(call)              \
+    do {                          \
+        int rc__ = (call);        \
+        if (rc__ != NF_OK) return rc__; \
+    } while (0)
+
+static inline size_t nf_align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Scratch arena: reset at the start of each API call, then carve.
+int nf_scratch_reserve(nf_ctx *ctx, size_t bytes);  // ensure capacity (may sync + realloc)
+static inline void nf_scratch_reset(nf_ctx *ctx) { ctx->scratch_used = 0; }
+template <class T>
+static inline T *nf_scratch_take(nf_ctx *ctx, size_t count)
+{
+    size_t off = nf_align_up(ctx->scratch_used, 256);
+    size_t end = off + nf_align_up(count * sizeof(T), 256);
+    if (end > ctx->scratch_bytes) return nullptr;
+    ctx->scratch_used = end;
+    return reinterpret_cast<T *>(ctx->scratch + off);
+}
+
+// ---- internal entry points shared between translation units ---------------------------
+// exclusive scans (nf_scan.cu); temp must hold nf_scan_temp_elems(n) elements of the out type
+size_t nf_scan_temp_elems(size_t n);
+int nf_exclusive_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t *out, size_t n, uint32_t *temp, cudaStream_t st);
+int nf_exclusive_scan_u32_u64(nf_ctx *ctx, const uint32_t *in, uint64_t *out, size_t n, uint64_t *temp, cudaStream_t st);
+
+// binning (nf_bin.cu).  plane_cx < 0: full box, keys (cx*K+cy)*K+cz over K^3 cells;
+// plane_cx >= 0: one x-plane, keys cy*K+cz over K^2 cells, particles must have cx == plane_cx.
+size_t nf_bin_scratch_bytes(int64_t N, int K, bool plane);
+int nf_bin_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, int plane_cx,
+                float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,
+                cudaStream_t st);
+
+// forces (nf_forces.cu).  A "plane table" describes the x-planes available as sources and
+// sinks: plane p (0 <= p < n_planes) has its own cell-contiguous arrays.
+struct nf_plane_view {
+    const float4 *pos;        // sorted cell-centred offsets of this plane's particles
+    const uint64_t *off;      // K*K+1 exclusive offsets within this plane's arrays
+    const uint32_t *perm;     // nullable
+    float *acc;               // output for this plane (n x 3), nullable for ghost planes
+};
+struct nf_force_params {
+    int K;            // cells per side in y and z
+    int n_planes;     // number of x-planes in the table
+    int periodic_x;   // 1: plane index wraps modulo n_planes (full box); 0: open
+    int sink_lo, sink_hi;  // sink planes [lo, hi)
+    int R;
+    float eps, box, Gm;
+    int softening;
+};
+size_t nf_forces_scratch_bytes(const nf_force_params &p);
+// d_planes: DEVICE array of p.n_planes views (fill with nf_fill_planes_full or copy from pinned memory)
+int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d_planes,
+                   cudaStream_t st, bool record_timing);
+// the full box seen as K planes sharing one set of arrays: plane cx starts at cell cx*K*K
+int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const uint64_t *off,
+                        const uint32_t *perm, float *acc, cudaStream_t st);
+// ordered pairs evaluated for the sink planes of a plane table (device result added to ctx->counters[1])
+int nf_interactions_planes(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d_planes, cudaStream_t st);
+void nf_slab_state_free(nf_ctx *ctx);
+int nf_interactions_impl(nf_ctx *ctx, const uint32_t *cell_count, int K, int R, int64_t *out, cudaStream_t st);

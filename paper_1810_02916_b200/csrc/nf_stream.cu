@@ -1,0 +1,253 @@
+// nf_stream.cu -- nf_stream_slabs: the slab pipeline of PAPER.md:41 ("load a rolling window of
+// slabs into memory, compute forces ... on the central slab, write out the trailing slab, and
+// then load a slab at the leading edge") with the slabs held in pinned host memory
+// instead of on disk.
+//
+// Three streams: H2D copies (ctx->s_h2d), kernels (the caller's stream), D2H copies
+// (ctx->s_d2h), ordered by events.  A ring of W = 2R+1+LOOKAHEAD device slots holds the
+// resident planes; each slot owns raw positions, cell-sorted offsets, perm, per-plane cell
+// counts / offsets and the accelerations of the plane.
+#include <new>
+#include <vector>
+
+#include "nf_common.cuh"
+
+namespace {
+
+constexpr int LOOKAHEAD = 2;  // "we allow Abacus to read ahead by a few slabs"
+
+struct Slot {
+    float *raw;        // n x 3
+    float *sorted;     // n x 4
+    uint32_t *perm;    // n
+    uint32_t *count;   // K*K
+    uint64_t *off;     // K*K + 1
+    float *acc;        // n x 3
+};
+
+struct SlabState {
+    char *mem = nullptr;
+    size_t mem_bytes = 0;
+    nf_plane_view *h_views = nullptr;  // pinned, [P+2R]
+    nf_plane_view *d_views = nullptr;
+    int views_cap = 0;
+};
+
+void free_state(SlabState *s)
+{
+    if (!s) return;
+    if (s->mem) cudaFree(s->mem);
+    if (s->h_views) cudaFreeHost(s->h_views);
+    if (s->d_views) cudaFree(s->d_views);
+    delete s;
+}
+
+struct EventPool {
+    std::vector<cudaEvent_t> ev;
+    ~EventPool() { for (auto e : ev) cudaEventDestroy(e); }
+    cudaEvent_t get(bool timing)
+    {
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreateWithFlags(&e, timing ? cudaEventDefault : cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        ev.push_back(e);
+        return e;
+    }
+};
+
+}  // namespace
+
+void nf_slab_state_free(nf_ctx *ctx)
+{
+    free_state(static_cast<SlabState *>(ctx->slab_state));
+    ctx->slab_state = nullptr;
+}
+
+extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,
+                               int P, int K, int R, float eps, float box, int plane0, float Gm,
+                               int softening, float *const *plane_acc_host, nf_stream_stats *stats,
+                               void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, plane_pos_host && plane_n && plane_acc_host, "nf_stream_slabs: null pointer table");
+    NF_ARG(ctx, P >= 1, "nf_stream_slabs: P must be >= 1");
+    NF_ARG(ctx, K >= 1 && K <= NF_MAX_K, "K = %d out of range [1, %d]", K, NF_MAX_K);
+    NF_ARG(ctx, R >= 0 && R <= NF_MAX_R, "R = %d out of range [0, %d]", R, NF_MAX_R);
+    NF_ARG(ctx, K >= 2 * R + 1, "K = %d < 2R+1", K);
+    NF_ARG(ctx, P + 2 * R <= K, "P + 2R = %d planes exceed K = %d", P + 2 * R, K);
+    NF_ARG(ctx, eps > 0.0f && eps < 3.0e38f, "eps must be positive and finite");
+    NF_ARG(ctx, box > 0.0f && box < 3.0e38f, "box must be positive and finite");
+    NF_ARG(ctx, softening == NF_SOFT_SPLINE || softening == NF_SOFT_PLUMMER, "unknown softening %d", softening);
+    const int NP = P + 2 * R;
+    int64_t max_n = 1;
+    for (int q = 0; q < NP; q++) {
+        NF_ARG(ctx, plane_n[q] >= 0 && plane_n[q] < ((int64_t)1 << 32), "plane_n[%d] out of range", q);
+        NF_ARG(ctx, plane_n[q] == 0 || plane_pos_host[q], "plane_pos_host[%d] is null", q);
+        if (plane_n[q] > max_n) max_n = plane_n[q];
+    }
+    for (int p = 0; p < P; p++) NF_ARG(ctx, plane_n[R + p] == 0 || plane_acc_host[p], "plane_acc_host[%d] is null", p);
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    // host pointers must be pinned (page-locked): "Pinning memory"
+    for (int q = 0; q < NP; q++) {
+        if (plane_n[q] == 0) continue;
+        cudaPointerAttributes at;
+        cudaError_t e = cudaPointerGetAttributes(&at, plane_pos_host[q]);
+        if (e != cudaSuccess || (at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged)) {
+            cudaGetLastError();
+            NF_SET_ERR(ctx, "plane_pos_host[%d] is not pinned host memory", q);
+            return NF_ERR_ARG;
+        }
+    }
+    for (int p = 0; p < P; p++) {
+        if (plane_n[R + p] == 0) continue;
+        cudaPointerAttributes at;
+        cudaError_t e = cudaPointerGetAttributes(&at, plane_acc_host[p]);
+        if (e != cudaSuccess || (at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged)) {
+            cudaGetLastError();
+            NF_SET_ERR(ctx, "plane_acc_host[%d] is not pinned host memory", p);
+            return NF_ERR_ARG;
+        }
+    }
+
+    cudaStream_t st = (cudaStream_t)stream;
+    const int W = 2 * R + 1 + LOOKAHEAD;
+    const size_t ncell = (size_t)K * K;
+
+    // ---- device memory: ring slots + shared scratch for binning ----
+    SlabState *S = static_cast<SlabState *>(ctx->slab_state);
+    if (!S) {
+        S = new (std::nothrow) SlabState();
+        if (!S) { NF_SET_ERR(ctx, "host allocation failed"); return NF_ERR_NOMEM; }
+        ctx->slab_state = S;
+    }
+    const size_t n = (size_t)max_n;
+    const size_t slot_bytes = nf_align_up(n * 12, 256) + nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
+                              nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256) + nf_align_up(n * 12, 256);
+    const size_t need = slot_bytes * W;
+    if (need > S->mem_bytes) {
+        NF_CUDA(ctx, cudaDeviceSynchronize());
+        if (S->mem) NF_CUDA(ctx, cudaFree(S->mem));
+        S->mem = nullptr; S->mem_bytes = 0;
+        cudaError_t e = cudaMalloc((void **)&S->mem, need);
+        if (e != cudaSuccess) { cudaGetLastError(); NF_SET_ERR(ctx, "cudaMalloc of %zu bytes for the slab ring failed", need); return NF_ERR_NOMEM; }
+        S->mem_bytes = need;
+    }
+    if (NP > S->views_cap) {
+        NF_CUDA(ctx, cudaDeviceSynchronize());
+        if (S->h_views) NF_CUDA(ctx, cudaFreeHost(S->h_views));
+        if (S->d_views) NF_CUDA(ctx, cudaFree(S->d_views));
+        S->h_views = nullptr; S->d_views = nullptr; S->views_cap = 0;
+        NF_CUDA(ctx, cudaMallocHost((void **)&S->h_views, sizeof(nf_plane_view) * NP));
+        NF_CUDA(ctx, cudaMalloc((void **)&S->d_views, sizeof(nf_plane_view) * NP));
+        S->views_cap = NP;
+    }
+    nf_force_params fp{};
+    fp.K = K; fp.n_planes = NP; fp.periodic_x = 0; fp.R = R; fp.eps = eps; fp.box = box; fp.Gm = Gm; fp.softening = softening;
+    size_t scratch_need = nf_bin_scratch_bytes(max_n, K, true);
+    size_t fs = nf_forces_scratch_bytes(fp);
+    NF_TRY(nf_scratch_reserve(ctx, scratch_need > fs ? scratch_need : fs));
+
+    std::vector<Slot> slots(W);
+    for (int s = 0; s < W; s++) {
+        char *b = S->mem + slot_bytes * s;
+        slots[s].raw = (float *)b;                b += nf_align_up(n * 12, 256);
+        slots[s].sorted = (float *)b;             b += nf_align_up(n * 16, 256);
+        slots[s].perm = (uint32_t *)b;            b += nf_align_up(n * 4, 256);
+        slots[s].count = (uint32_t *)b;           b += nf_align_up(ncell * 4, 256);
+        slots[s].off = (uint64_t *)b;             b += nf_align_up((ncell + 1) * 8, 256);
+        slots[s].acc = (float *)b;
+    }
+    // plane views (device pointers are fixed by the slot assignment q % W)
+    for (int q = 0; q < NP; q++) {
+        const Slot &sl = slots[q % W];
+        S->h_views[q].pos = (const float4 *)sl.sorted;
+        S->h_views[q].off = sl.off;
+        S->h_views[q].perm = sl.perm;
+        S->h_views[q].acc = sl.acc;
+    }
+    NF_CUDA(ctx, cudaMemcpyAsync(S->d_views, S->h_views, sizeof(nf_plane_view) * NP, cudaMemcpyHostToDevice, st));
+    NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st));
+
+    EventPool pool;
+    std::vector<cudaEvent_t> h2d0(NP), h2d1(NP), bin0(NP), bin1(NP), frc0(P), frc1(P), d2h0(P), d2h1(P);
+    for (int q = 0; q < NP; q++) { h2d0[q] = pool.get(true); h2d1[q] = pool.get(true); bin0[q] = pool.get(true); bin1[q] = pool.get(true); }
+    for (int p = 0; p < P; p++) { frc0[p] = pool.get(true); frc1[p] = pool.get(true); d2h0[p] = pool.get(true); d2h1[p] = pool.get(true); }
+    cudaEvent_t ev_begin = pool.get(true), ev_end = pool.get(true), ev_ready = pool.get(false);
+    for (auto e : pool.ev) if (!e) { NF_SET_ERR(ctx, "cudaEventCreate failed"); return NF_ERR_CUDA; }
+
+    NF_CUDA(ctx, cudaEventRecord(ev_ready, st));        // order the whole call after prior work on `stream`
+    NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, ev_ready, 0));
+    NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_d2h, ev_ready, 0));
+    NF_CUDA(ctx, cudaEventRecord(ev_begin, ctx->s_h2d));
+
+    for (int q = 0; q < NP; q++) {
+        const Slot &sl = slots[q % W];
+        // slot reuse: plane q-W lived here.  It was last read as a source by sink plane
+        // (q-W)+R, and (if it was a sink) its accelerations were copied out by d2h1.
+        const int prev = q - W;
+        if (prev >= 0) {
+            int last_sink = prev;  // chunk plane prev+R is the last sink that reads plane prev; its sink number is prev
+            if (last_sink >= 0 && last_sink < P) NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, frc1[last_sink], 0));
+            int own_sink = prev - R;
+            if (own_sink >= 0 && own_sink < P) NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, d2h1[own_sink], 0));
+        }
+        NF_CUDA(ctx, cudaEventRecord(h2d0[q], ctx->s_h2d));
+        if (plane_n[q] > 0)
+            NF_CUDA(ctx, cudaMemcpyAsync(sl.raw, plane_pos_host[q], (size_t)plane_n[q] * 12, cudaMemcpyHostToDevice, ctx->s_h2d));
+        NF_CUDA(ctx, cudaEventRecord(h2d1[q], ctx->s_h2d));
+
+        NF_CUDA(ctx, cudaStreamWaitEvent(st, h2d1[q], 0));
+        NF_CUDA(ctx, cudaEventRecord(bin0[q], st));
+        nf_scratch_reset(ctx);
+        const int cx = ((plane0 + q) % K + K) % K;
+        // counters[0] accumulates out-of-range / wrong-plane particles over all planes
+        NF_TRY(nf_bin_impl(ctx, sl.raw, plane_n[q], K, box, cx, sl.sorted, sl.perm, sl.count, sl.off, st));
+        NF_CUDA(ctx, cudaEventRecord(bin1[q], st));
+
+        const int sp = q - R;        // chunk plane whose neighbourhood is now complete
+        const int p = sp - R;        // its sink number
+        if (p >= 0 && p < P) {
+            fp.sink_lo = sp; fp.sink_hi = sp + 1;
+            NF_CUDA(ctx, cudaEventRecord(frc0[p], st));
+            NF_TRY(nf_forces_impl(ctx, fp, S->d_views, st, false));
+            NF_TRY(nf_interactions_planes(ctx, fp, S->d_views, st));
+            NF_CUDA(ctx, cudaEventRecord(frc1[p], st));
+            NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_d2h, frc1[p], 0));
+            NF_CUDA(ctx, cudaEventRecord(d2h0[p], ctx->s_d2h));
+            if (plane_n[sp] > 0)
+                NF_CUDA(ctx, cudaMemcpyAsync(plane_acc_host[p], slots[sp % W].acc, (size_t)plane_n[sp] * 12, cudaMemcpyDeviceToHost, ctx->s_d2h));
+            NF_CUDA(ctx, cudaEventRecord(d2h1[p], ctx->s_d2h));
+        }
+    }
+    NF_CUDA(ctx, cudaStreamWaitEvent(st, d2h1[P - 1], 0));
+    NF_CUDA(ctx, cudaEventRecord(ev_end, st));
+    NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->counters, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    NF_CUDA(ctx, cudaStreamSynchronize(st));
+    NF_CUDA(ctx, cudaStreamSynchronize(ctx->s_d2h));
+    NF_CUDA(ctx, cudaStreamSynchronize(ctx->s_h2d));
+
+    if (stats) {
+        memset(stats, 0, sizeof(*stats));
+        float ms = 0.f;
+        for (int q = 0; q < NP; q++) {
+            stats->particles_in += plane_n[q];
+            NF_CUDA(ctx, cudaEventElapsedTime(&ms, h2d0[q], h2d1[q])); stats->h2d_seconds += ms * 1e-3;
+            NF_CUDA(ctx, cudaEventElapsedTime(&ms, bin0[q], bin1[q])); stats->kernel_seconds += ms * 1e-3;
+        }
+        for (int p = 0; p < P; p++) {
+            stats->particles_out += plane_n[R + p];
+            NF_CUDA(ctx, cudaEventElapsedTime(&ms, frc0[p], frc1[p])); stats->kernel_seconds += ms * 1e-3;
+            NF_CUDA(ctx, cudaEventElapsedTime(&ms, d2h0[p], d2h1[p])); stats->d2h_seconds += ms * 1e-3;
+        }
+        NF_CUDA(ctx, cudaEventElapsedTime(&ms, ev_begin, ev_end)); stats->wall_seconds = ms * 1e-3;
+        stats->h2d_bytes = 12.0 * (double)stats->particles_in;
+        stats->d2h_bytes = 12.0 * (double)stats->particles_out;
+        stats->h2d_gbps = stats->h2d_seconds > 0 ? stats->h2d_bytes / stats->h2d_seconds * 1e-9 : 0.0;
+        stats->d2h_gbps = stats->d2h_seconds > 0 ? stats->d2h_bytes / stats->d2h_seconds * 1e-9 : 0.0;
+        stats->interactions = (int64_t)ctx->h_counters[1];
+        stats->out_of_range = (int64_t)ctx->h_counters[0];
+        const double copy_s = stats->h2d_seconds + stats->d2h_seconds;
+        double hidden = copy_s > 0 ? 1.0 - (stats->wall_seconds - stats->kernel_seconds) / copy_s : 0.0;
+        stats->overlap_fraction = hidden < 0 ? 0.0 : (hidden > 1 ? 1.0 : hidden);
+    }
+    return NF_OK;
+}

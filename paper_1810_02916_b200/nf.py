@@ -1,0 +1,207 @@
+"""Thin Python binding over the C-ABI library libnf.so (include/nf.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of csrc/.
+PyTorch is used for device memory and streams.  There is NO CPU fallback: if libnf.so is
+missing or no CUDA device is present, the constructor raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import List, Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnf.so")
+
+NF_OK, NF_ERR_ARG, NF_ERR_NOMEM, NF_ERR_CUDA, NF_ERR_RANGE = 0, 1, 2, 3, 4
+SOFT_SPLINE, SOFT_PLUMMER = 0, 1
+_SOFT = {"spline": SOFT_SPLINE, "plummer": SOFT_PLUMMER}
+
+# every symbol include/nf.h declares
+EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve", "nf_bin",
+           "nf_out_of_range", "nf_forces", "nf_interactions", "nf_spline_equivalent_eps",
+           "nf_stream_slabs", "nf_last_forces_timing"]
+
+
+class NFError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"libnf status {status}: {msg}")
+        self.status = status
+
+
+class StreamStats(ctypes.Structure):
+    _fields_ = [("particles_in", ctypes.c_int64), ("particles_out", ctypes.c_int64),
+                ("interactions", ctypes.c_int64), ("out_of_range", ctypes.c_int64),
+                ("h2d_bytes", ctypes.c_double), ("d2h_bytes", ctypes.c_double),
+                ("h2d_seconds", ctypes.c_double), ("d2h_seconds", ctypes.c_double),
+                ("kernel_seconds", ctypes.c_double), ("wall_seconds", ctypes.c_double),
+                ("h2d_gbps", ctypes.c_double), ("d2h_gbps", ctypes.c_double),
+                ("overlap_fraction", ctypes.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
+    """dlopen libnf.so and declare the prototypes of include/nf.h.  Raises if it is missing:
+    build it with ``python -m paper_1810_02916_b200.build``."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} not found: run `python -m paper_1810_02916_b200.build` (no CPU fallback exists)")
+    lib = ctypes.CDLL(path)
+    vp, i32, i64, f32 = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_float
+    lib.nf_version.restype = i32
+    lib.nf_create.restype = i32
+    lib.nf_create.argtypes = [ctypes.POINTER(vp), i32]
+    lib.nf_destroy.restype = i32
+    lib.nf_destroy.argtypes = [vp]
+    lib.nf_last_error.restype = ctypes.c_char_p
+    lib.nf_last_error.argtypes = [vp]
+    lib.nf_reserve.restype = i32
+    lib.nf_reserve.argtypes = [vp, i64, i32]
+    lib.nf_bin.restype = i32
+    lib.nf_bin.argtypes = [vp, vp, i64, i32, f32, vp, vp, vp, vp, vp]
+    lib.nf_out_of_range.restype = i32
+    lib.nf_out_of_range.argtypes = [vp, ctypes.POINTER(i64), vp]
+    lib.nf_forces.restype = i32
+    lib.nf_forces.argtypes = [vp, vp, vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp]
+    lib.nf_interactions.restype = i32
+    lib.nf_interactions.argtypes = [vp, vp, i32, i32, ctypes.POINTER(i64), vp]
+    lib.nf_spline_equivalent_eps.restype = f32
+    lib.nf_spline_equivalent_eps.argtypes = [f32]
+    lib.nf_stream_slabs.restype = i32
+    lib.nf_stream_slabs.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(i64), i32, i32, i32, f32, f32, i32, f32,
+                                    i32, ctypes.POINTER(vp), ctypes.POINTER(StreamStats), vp]
+    lib.nf_last_forces_timing.restype = i32
+    lib.nf_last_forces_timing.argtypes = [vp, ctypes.POINTER(f32), ctypes.POINTER(f32)]
+    _lib = lib
+    return lib
+
+
+@dataclass
+class Binned:
+    """Output of nf_bin (all device tensors)."""
+    pos_sorted: torch.Tensor   # float32 [N, 4]: cell-centred offsets, w = 0
+    perm: torch.Tensor         # int32 view of uint32 [N]
+    cell_count: torch.Tensor   # int32 view of uint32 [K^3]
+    cell_offset: torch.Tensor  # int64 view of uint64 [K^3 + 1]
+    N: int
+    K: int
+    box: float
+
+
+def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+class Context:
+    """nf_create / nf_destroy."""
+
+    def __init__(self, device: int = 0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1810_02916_b200.nf needs a CUDA device (there is no CPU fallback)")
+        self.lib = load_library()
+        self.device = torch.device("cuda", device)
+        self._h = ctypes.c_void_p()
+        torch.cuda.init()
+        with torch.cuda.device(self.device):
+            torch.zeros(1, device=self.device)      # make sure the primary context exists
+            rc = self.lib.nf_create(ctypes.byref(self._h), device)
+        if rc != NF_OK:
+            raise NFError(rc, "nf_create failed")
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self.lib.nf_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int, allow=()):
+        if rc != NF_OK and rc not in allow:
+            raise NFError(rc, self.lib.nf_last_error(self._h).decode())
+        return rc
+
+    def _stream(self, stream: Optional[torch.cuda.Stream]):
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        return ctypes.c_void_p(s.cuda_stream)
+
+    def reserve(self, maxN: int, K: int):
+        self._check(self.lib.nf_reserve(self._h, int(maxN), int(K)))
+
+    def bin(self, pos: torch.Tensor, K: int, box: float, stream=None) -> Binned:
+        """nf_bin: pos float32 [N, 3] on the device -> cell-contiguous arrays."""
+        assert pos.is_cuda and pos.dtype == torch.float32 and pos.dim() == 2 and pos.shape[1] == 3 and pos.is_contiguous()
+        N = pos.shape[0]
+        dev = pos.device
+        ncell = int(K) ** 3
+        out = Binned(torch.empty(N, 4, dtype=torch.float32, device=dev),
+                     torch.empty(N, dtype=torch.int32, device=dev),
+                     torch.empty(ncell, dtype=torch.int32, device=dev),
+                     torch.empty(ncell + 1, dtype=torch.int64, device=dev), N, int(K), float(box))
+        self._check(self.lib.nf_bin(self._h, _ptr(pos), N, int(K), float(box), _ptr(out.pos_sorted), _ptr(out.perm),
+                                    _ptr(out.cell_count), _ptr(out.cell_offset), self._stream(stream)))
+        return out
+
+    def out_of_range(self, stream=None) -> int:
+        n = ctypes.c_int64(0)
+        self._check(self.lib.nf_out_of_range(self._h, ctypes.byref(n), self._stream(stream)), allow=(NF_ERR_RANGE,))
+        return int(n.value)
+
+    def forces(self, b: Binned, R: int, eps: float, Gm: float, softening: str = "spline",
+               original_order: bool = True, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """nf_forces: accelerations float32 [N, 3] (caller's order if original_order)."""
+        acc = out if out is not None else torch.empty(b.N, 3, dtype=torch.float32, device=b.pos_sorted.device)
+        assert acc.is_cuda and acc.dtype == torch.float32 and acc.shape == (b.N, 3) and acc.is_contiguous()
+        self._check(self.lib.nf_forces(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset), _ptr(b.cell_count),
+                                       _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
+                                       float(b.box), float(Gm), _SOFT[softening], _ptr(acc), self._stream(stream)))
+        return acc
+
+    def interactions(self, b: Binned, R: int, stream=None) -> int:
+        n = ctypes.c_int64(0)
+        self._check(self.lib.nf_interactions(self._h, _ptr(b.cell_count), b.K, int(R), ctypes.byref(n), self._stream(stream)))
+        return int(n.value)
+
+    def last_forces_timing(self):
+        """(kernel_ms, total_ms) of the last forces() call, from CUDA events on its stream."""
+        k, t = ctypes.c_float(0), ctypes.c_float(0)
+        self._check(self.lib.nf_last_forces_timing(self._h, ctypes.byref(k), ctypes.byref(t)))
+        return float(k.value), float(t.value)
+
+    def stream_slabs(self, planes: Sequence[torch.Tensor], P: int, K: int, R: int, eps: float, box: float,
+                     plane0: int, Gm: float, softening: str = "spline",
+                     out: Optional[List[torch.Tensor]] = None, stream=None):
+        """nf_stream_slabs: planes = P + 2R pinned host float32 [n_q, 3] tensors; returns
+        (list of P pinned host float32 [n, 3] acceleration tensors, stats dict)."""
+        NP = P + 2 * R
+        assert len(planes) == NP
+        for t in planes:
+            assert (not t.is_cuda) and t.dtype == torch.float32 and t.dim() == 2 and t.shape[1] == 3 and t.is_contiguous()
+            assert t.shape[0] == 0 or t.is_pinned(), "plane tensors must be pinned host memory"
+        if out is None:
+            out = [torch.empty(planes[R + p].shape[0], 3, dtype=torch.float32).pin_memory() for p in range(P)]
+        pos_ptrs = (ctypes.c_void_p * NP)(*[t.data_ptr() if t.shape[0] else None for t in planes])
+        ns = (ctypes.c_int64 * NP)(*[t.shape[0] for t in planes])
+        acc_ptrs = (ctypes.c_void_p * P)(*[t.data_ptr() if t.shape[0] else None for t in out])
+        stats = StreamStats()
+        self._check(self.lib.nf_stream_slabs(self._h, pos_ptrs, ns, int(P), int(K), int(R), float(eps), float(box),
+                                             int(plane0), float(Gm), _SOFT[softening], acc_ptrs, ctypes.byref(stats),
+                                             self._stream(stream)))
+        return out, stats.as_dict()
+
+
+def spline_equivalent_eps(eps_plummer: float) -> float:
+    return float(load_library().nf_spline_equivalent_eps(float(eps_plummer)))

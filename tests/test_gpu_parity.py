@@ -1,0 +1,224 @@
+"""Parity of the CUDA path (through the C-ABI, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Bars (BASELINE.json north_star): cell
+assignment and sort bit-exact; accelerations within a per-particle relative error
+|a_gpu - a_ref| / max(|a_ref|, rms|a_ref|) of 1e-5 at the median and 1e-3 at the maximum.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1810_02916_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+MEDIAN_TOL = 1e-5
+MAX_TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_1810_02916_b200 import nf
+    c = nf.Context(0)
+    yield c
+    c.close()
+
+
+def u32(t):
+    return t.cpu().numpy().view(np.uint32)
+
+
+def u64(t):
+    return t.cpu().numpy().view(np.uint64)
+
+
+def check_bin(ctx, pos_np, K, box):
+    ref = oracle.bin_particles(pos_np, K, box)
+    b = ctx.bin(torch.from_numpy(pos_np).cuda(), K, box)
+    nbad = ctx.out_of_range()
+    assert nbad == ref["n_out_of_range"]
+    assert np.array_equal(u32(b.cell_count), ref["cell_count"])
+    assert np.array_equal(u64(b.cell_offset), ref["cell_offset"])
+    assert np.array_equal(u32(b.perm), ref["perm"])
+    # bit-for-bit: compare the float32 bit patterns (a NaN input stays NaN; its payload is not compared)
+    got = b.pos_sorted.cpu().numpy()
+    nan = np.isnan(ref["pos_sorted"])
+    assert np.array_equal(np.isnan(got), nan)
+    assert np.array_equal(got.view(np.uint32)[~nan], ref["pos_sorted"].view(np.uint32)[~nan])
+    return b, ref
+
+
+def check_forces(ctx, pos_np, K, R, eps, box, Gm, softening="spline", sink_idx=None, med=MEDIAN_TOL, mx=MAX_TOL):
+    b = ctx.bin(torch.from_numpy(pos_np).cuda(), K, box)
+    acc = ctx.forces(b, R, eps, Gm, softening=softening).cpu().numpy()
+    assert np.isfinite(acc).all()
+    ref = oracle.forces(pos_np, K, R, eps, box, Gm, sink_idx=sink_idx, softening=softening)
+    got = acc if sink_idx is None else acc[sink_idx]
+    err = oracle.parity_error(got, ref)
+    assert np.median(err) <= med, f"median error {np.median(err):.3e}"
+    assert err.max() <= mx, f"max error {err.max():.3e}"
+    assert ctx.interactions(b, R) == oracle.interactions(u32(b.cell_count), K, R)
+    return acc, ref, err
+
+
+# ------------------------------------------------------------------------------- binning
+@pytest.mark.parametrize("which,N,K", [(1, 32 ** 3, 8), (3, 200_003, 16), (2, 48 ** 3, 12), (1, 5000, 7), (1, 4097, 13), (1, 31, 3)])
+def test_bin_bit_exact(ctx, which, N, K):
+    cfg = inputs.scaled(inputs.config(which), N if which != 2 else N, K)
+    if cfg.kind == "lattice":
+        cfg = inputs.scaled(inputs.config(2), N, K)
+    pos = inputs.make_positions(cfg).numpy()
+    check_bin(ctx, pos, K, cfg.box)
+
+
+def test_bin_edge_cases(ctx):
+    K, box = 10, 1.0
+    top = np.nextafter(np.float32(1.0), np.float32(0))
+    pos = np.array([[top, 0.0, 0.5], [1.0, 0.2, 0.2], [-0.1, 0.3, 0.3], [0.0, 0.0, 0.0], [0.5, np.nan, 0.5]], np.float32)
+    check_bin(ctx, pos, K, box)
+    check_bin(ctx, np.zeros((0, 3), np.float32), K, box)                       # empty input
+    check_bin(ctx, np.full((3000, 3), 0.3, np.float32), K, box)                # everything in one cell
+    rng = np.random.default_rng(1)
+    check_bin(ctx, (rng.random((70_000, 3)) * 500).astype(np.float32).clip(0, 499.99), 64, 500.0)
+    check_bin(ctx, rng.random((1000, 3)).astype(np.float32), 1, 1.0)           # a single cell
+
+
+def test_bin_is_deterministic(ctx):
+    cfg = inputs.scaled(inputs.config(3), 100_000, 8)
+    pos = inputs.make_positions(cfg).cuda()
+    a = ctx.bin(pos, 8, cfg.box)
+    b = ctx.bin(pos, 8, cfg.box)
+    assert torch.equal(a.perm, b.perm) and torch.equal(a.pos_sorted, b.pos_sorted)
+
+
+# ------------------------------------------------------------------------------- forces
+def test_forces_c1_uniform(ctx):
+    cfg = inputs.config(1)
+    pos = inputs.make_positions(cfg).numpy()
+    acc, ref, err = check_forces(ctx, pos, cfg.K, cfg.R, cfg.eps, cfg.box, cfg.Gm)
+    # zero net force on a fully periodic box
+    mag = np.sqrt((acc.astype(np.float64) ** 2).sum(axis=1))
+    assert np.abs(acc.astype(np.float64).sum(axis=0)).max() < 1e-5 * mag.sum()
+
+
+def test_forces_lattice_small(ctx):
+    """Perturbed lattice (C2 recipe at 64^3): near-cancelling forces, the accumulation-order
+    stress test (SURVEY.md Sec. 7 hard part 3)."""
+    cfg = inputs.scaled(inputs.config(2), 64 ** 3, 16)
+    pos = inputs.make_positions(cfg).numpy()
+    check_forces(ctx, pos, cfg.K, cfg.R, cfg.eps, cfg.box, cfg.Gm)
+
+
+def test_forces_clustered_small(ctx):
+    """C3 recipe at 2 x 64^3 particles, K = 16: cells with >1000 particles beside cells with ~30;
+    many pairs inside eps."""
+    cfg = inputs.scaled(inputs.config(3), 2 * 64 ** 3, 16)
+    cfg = inputs.dataclasses.replace(cfg, n_halos=48)
+    pos = inputs.make_positions(cfg).numpy()
+    rng = np.random.default_rng(0)
+    sink_idx = np.sort(rng.choice(cfg.N, 60_000, replace=False))
+    check_forces(ctx, pos, cfg.K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=sink_idx)
+
+
+@pytest.mark.parametrize("K,R", [(5, 2), (6, 2), (7, 2), (8, 2), (9, 2), (11, 2), (3, 1), (4, 1), (7, 3), (12, 3), (2, 0)])
+def test_forces_small_K_and_R(ctx, K, R):
+    """Degenerate neighbourhoods: K = 2R+1 (every cell neighbours every other exactly once),
+    K just above it, other R."""
+    rng = np.random.default_rng(10 * K + R)
+    n = 3000
+    box = 2.0
+    pos = (rng.random((n, 3)) * box).astype(np.float32)
+    pos[:300] = (pos[0] + 0.01 * rng.standard_normal((300, 3))).astype(np.float32) % np.float32(box)
+    pos[5] = pos[6]                                   # coincident particles: r = 0 contributes nothing
+    pos = np.clip(pos, 0, np.nextafter(np.float32(box), np.float32(0)))
+    check_forces(ctx, pos, K, R, 0.004, box, 1.0 / n)
+
+
+def test_forces_plummer(ctx):
+    cfg = inputs.scaled(inputs.config(3), 40_000, 8)
+    pos = inputs.make_positions(cfg).numpy()
+    check_forces(ctx, pos, cfg.K, cfg.R, cfg.eps, cfg.box, cfg.Gm, softening="plummer")
+
+
+def test_two_particle_closed_form_gpu(ctx):
+    """The golden closed-form values (Eq. 2 by hand) straight through the CUDA path."""
+    import os
+    rows = []
+    with open(os.path.join(os.path.dirname(__file__), "golden", "spline_closed_form.txt")) as fh:
+        for line in fh:
+            line = line.split("#")[0].strip()
+            if line:
+                rows.append([float(t) for t in line.split()])
+    K, R, box, Gm = 8, 2, 1.0, 0.75
+    w = box / K
+    eps = w / 16
+    for u, expect in rows:
+        r = u * eps
+        for p0, dirn in [(np.array([3.5 * w, 2.5 * w, 4.5 * w]), np.array([1.0, 0, 0])),
+                         (np.array([3.0 * w - r / 2, 2.5 * w, 4.5 * w]), np.array([1.0, 0, 0])),
+                         (np.array([1.5 * w, 0.5 * w, box - r / 2]), np.array([0, 0, 1.0])),
+                         (np.array([1.5 * w, box - r / 2, 0.5 * w]), np.array([0, 1.0, 0]))]:
+            pos = np.mod(np.stack([p0, p0 + r * dirn]), box).astype(np.float32)
+            d = pos[1].astype(np.float64) - pos[0].astype(np.float64)
+            d -= np.round(d / box) * box
+            ur = np.linalg.norm(d) / eps
+            exp_r = ur * (10 - 15 * ur + 6 * ur * ur) if ur < 1 else ur ** -2
+            b = ctx.bin(torch.from_numpy(pos).cuda(), K, box)
+            a = ctx.forces(b, R, eps, Gm).cpu().numpy().astype(np.float64)
+            assert np.linalg.norm(a[0]) * eps ** 2 / Gm == pytest.approx(exp_r, rel=2e-6)
+            assert exp_r == pytest.approx(expect, rel=1e-4)
+            assert np.dot(a[0], d) > 0 and np.allclose(a[0], -a[1], rtol=1e-6)
+    # Chebyshev cell distance R+1: exactly zero
+    pos = np.array([[0.99 * w, 0.5 * w, 0.5 * w], [3.01 * w, 0.5 * w, 0.5 * w]], np.float32)
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box)
+    assert (ctx.forces(b, R, eps, Gm).cpu().numpy() == 0).all()
+
+
+def test_forces_sorted_order_and_determinism(ctx):
+    cfg = inputs.scaled(inputs.config(3), 50_000, 8)
+    pos = inputs.make_positions(cfg).cuda()
+    b = ctx.bin(pos, cfg.K, cfg.box)
+    a1 = ctx.forces(b, cfg.R, cfg.eps, cfg.Gm)
+    a2 = ctx.forces(b, cfg.R, cfg.eps, cfg.Gm)
+    assert torch.equal(a1, a2)                                   # deterministic: same bits run to run
+    a_sorted = ctx.forces(b, cfg.R, cfg.eps, cfg.Gm, original_order=False)
+    assert torch.equal(a_sorted, a1[b.perm.long() & 0xFFFFFFFF])
+
+
+def test_argument_errors(ctx):
+    from paper_1810_02916_b200 import nf
+    pos = torch.rand(100, 3, device="cuda")
+    b = ctx.bin(pos, 4, 1.0)
+    with pytest.raises(nf.NFError) as e:
+        ctx.forces(b, 2, 0.01, 1.0)           # K < 2R+1
+    assert e.value.status == nf.NF_ERR_ARG
+    with pytest.raises(nf.NFError):
+        ctx.forces(ctx.bin(pos, 8, 1.0), 2, -1.0, 1.0)
+    with pytest.raises(nf.NFError):
+        ctx.bin(pos, 0, 1.0)
+
+
+# ------------------------------------------------------------------------------- slabs
+def test_stream_slabs_small(ctx):
+    """nf_stream_slabs on a thin C5-recipe chunk: x open inside the chunk, y/z periodic.  The
+    oracle is the fully periodic oracle on the chunk's particles only (K is large enough that
+    no periodic image in x aliases), evaluated for the sink planes."""
+    cfg = inputs.dataclasses.replace(inputs.config(5), K=32, planes=6, plane0=29 - 32, n_halos=4096,
+                                     r_trunc=2 * 500.0 / 32 / 2, a_lo=0.3, a_hi=2.0, eps=0.15)
+    cfg = inputs.dataclasses.replace(cfg, plane0=3)
+    planes = inputs.make_slab_planes(cfg, density_scale=(32 * 4) ** 3 / 2048 ** 3)
+    R, P = cfg.R, cfg.planes
+    pinned = [p.pin_memory() for p in planes]
+    Gm = 1.0 / sum(p.shape[0] for p in planes)
+    out, stats = ctx.stream_slabs(pinned, P, cfg.K, R, cfg.eps, cfg.box, cfg.plane0, Gm)
+    allpos = torch.cat(planes).numpy()
+    starts = np.cumsum([0] + [p.shape[0] for p in planes])
+    sink_idx = np.arange(starts[R], starts[R + P])
+    ref = oracle.forces(allpos, cfg.K, R, cfg.eps, cfg.box, Gm, sink_idx=sink_idx)
+    got = torch.cat(out).numpy()
+    err = oracle.parity_error(got, ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
+    assert stats["out_of_range"] == 0
+    assert stats["particles_in"] == allpos.shape[0] and stats["particles_out"] == sink_idx.size
+    cnt = oracle.bin_particles(allpos, cfg.K, cfg.box)["cell_count"]
+    assert stats["interactions"] == oracle.interactions(cnt, cfg.K, R, cfg.plane0 + R, cfg.plane0 + R + P)
