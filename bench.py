@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- the near-field force hot path (nf_bin + nf_forces) on seeded synthetic input.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (cell assignment,
+histogram, scan, stable scatter + re-centre, work list, interaction kernel, scale/un-permute)
+over one batch of synthetic particles.  The default workload is BASELINE.json's configs[3]
+("C4", the clustered 1024^3 box the 60 % roofline target is quoted on); it fits one B200.
+
+One JSON line is printed by rank 0 (DESIGN.md "Measurement" explains every key):
+  value      pairwise interactions/s over the whole step, inputs resident in HBM
+  e2e        the same through nf_forces_host: pinned HOST buffers, H2D + D2H inside the timing
+  roofline   interaction kernel alone against the FP32 ALU peak, 20 flop per interaction
+  cpu_baseline   the CPU oracle, as it stands, on a bounded sample of the same workload
+
+`--impl reference` times the CPU oracle (this tier's reference arm) on bounded samples.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1810_02916_b200 import inputs  # noqa: E402
+
+FLOP_PER_INTERACTION = 20          # BASELINE.json convention (the paper counts 23)
+FP32_LANES_PER_SM = 128
+
+
+def read_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            d = json.load(fh)
+        return float(d.get("sm_max_mhz", 1965.0)), float(d.get("hbm_gbs", 6650.0)), "measured"
+    return 1965.0, 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+            out, _ = self.p.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [t.strip() for t in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        # "under load": samples in the upper half of the power range
+        thr = 0.5 * (min(pw) + max(pw))
+        load = [s for s, p in zip(sm, pw) if p >= thr] or sm
+        return {"sm_mhz": statistics.median(load), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(pos_dev: torch.Tensor, cfg, m: int, c0=(3, 5, 7)):
+    """A block of m^3 sink cells with every source they need, for the CPU oracle: the particles
+    whose coordinates lie within the block padded by R+1 cells (selected by coordinate range --
+    the oracle does its own cell assignment with the full K and box)."""
+    if cfg.K <= m + 2 * (cfg.R + 1):      # small box: hand the oracle everything
+        return pos_dev.cpu().numpy(), None
+    w = cfg.box / cfg.K
+    lo = [(c - cfg.R - 1) * w for c in c0]
+    hi = [(c + m + cfg.R + 1) * w for c in c0]
+    idx = inputs.select_box(pos_dev, lo, hi, cfg.box)
+    sub = pos_dev[idx].cpu().numpy()
+    return sub, idx
+
+
+def time_oracle(sub, cfg, m, c0, budget_s=20.0):
+    """Oracle forces for the sinks in the inner m^3 block; returns (interactions, seconds, cores, n_sinks)."""
+    import numpy as np
+    import oracle
+    keys, _ = oracle.keys(sub, cfg.K, cfg.box)
+    K = cfg.K
+    cz, cy, cx = keys % K, (keys // K) % K, keys // (K * K)
+    inner = np.ones(len(keys), bool)
+    for c, lo in ((cx, c0[0]), (cy, c0[1]), (cz, c0[2])):
+        if K > m + 2 * (cfg.R + 1):
+            inner &= ((c.astype(np.int64) - lo) % K) < m
+    sink_idx = np.nonzero(inner)[0]
+    # interactions of those sinks: count neighbours through the oracle's own cell counts
+    cnt = np.bincount(keys, minlength=K ** 3).astype(np.uint32)
+    # pilot to size the timed sample
+    rng = np.random.default_rng(1)
+    pilot = np.sort(rng.choice(sink_idx, min(len(sink_idx), 2000), replace=False))
+    t0 = time.perf_counter()
+    oracle.forces(sub, K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=pilot)
+    tp = max(time.perf_counter() - t0, 1e-4)
+    n_timed = int(min(len(sink_idx), max(len(pilot), len(pilot) * budget_s / tp)))
+    timed = np.sort(rng.choice(sink_idx, n_timed, replace=False))
+    t0 = time.perf_counter()
+    acc = oracle.forces(sub, K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=timed)
+    dt = time.perf_counter() - t0
+    # ordered pairs evaluated for the timed sinks
+    kk = keys[timed].astype(np.int64)
+    tz, ty, tx = kk % K, (kk // K) % K, kk // (K * K)
+    cnt3 = cnt.reshape(K, K, K).astype(np.int64)
+    inter = 0
+    R = cfg.R
+    for dx in range(-R, R + 1):
+        for dy in range(-R, R + 1):
+            for dz in range(-R, R + 1):
+                inter += int(cnt3[(tx + dx) % K, (ty + dy) % K, (tz + dz) % K].sum())
+    return inter, dt, oracle.max_threads(), n_timed, timed, acc
+
+
+def run_reference(args, cfg):
+    """This tier's reference arm: the CPU oracle, as it stands, on the host cores."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    m = 6
+    pos = inputs.make_positions(cfg, device=dev)
+    sub, _ = oracle_sample(pos, cfg, m)
+    del pos
+    per_step = []
+    inter_step = 0
+    budget = 8.0
+    for it in range(args.warmup + args.steps):
+        inter, dt, cores, n_sinks, _, _ = time_oracle(sub, cfg, m, (3, 5, 7), budget_s=budget)
+        if it >= args.warmup:
+            per_step.append(dt)
+            inter_step = inter
+    ms = 1e3 * sum(per_step) / len(per_step)
+    value = inter_step / (ms * 1e-3)
+    line = {"impl": "reference", "metric": "near_field_pairwise_interactions_per_s", "value": value,
+            "unit": "interactions/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "N": cfg.N, "K": cfg.K, "R": cfg.R, "sample": f"{n_sinks} sinks of a {m}^3-cell block, all their sources"},
+            "cpu_baseline": {"value": value, "unit": "interactions/s", "cores": cores, "kind": "oracle",
+                             "sample": f"{n_sinks} sinks of a {m}^3-cell block with all their sources, {inter_step} pairs per step"},
+            "e2e": {"value": value, "unit": "interactions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number 1..4 (default 4 = C4)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = max(args.warmup, 0)
+    cfg = inputs.config(args.config)
+
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    from paper_1810_02916_b200 import nf
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # every rank owns an independently seeded box of the same recipe (weak scaling)
+    rcfg = cfg if rank == 0 else inputs.dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    pos = inputs.make_positions(rcfg, device=dev)
+    N, K, R = rcfg.N, rcfg.K, rcfg.R
+    ctx = nf.Context(local)
+    ctx.reserve(N, K)
+    b = ctx.bin(pos, K, rcfg.box)
+    acc = torch.empty(N, 3, dtype=torch.float32, device=dev)
+    I = ctx.interactions(b, R)
+    flush = None
+    small = N * 28 < (256 << 20)
+    if small:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        ctx.bin(pos, K, rcfg.box, out=b)
+        ctx.forces(b, R, rcfg.eps, rcfg.Gm, out=acc)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    launches0 = ctx.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kern_ms = []
+    barrier()
+    for s in range(args.steps):
+        if flush is not None:
+            flush.fill_(s)
+        ev[s][0].record()
+        step()
+        ev[s][1].record()
+        kern_ms.append(ctx.last_forces_timing()[0])   # synchronises on the step's end event
+    barrier()
+    launches = ctx.launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    step_ms = [a.elapsed_time(bb) for a, bb in ev]
+    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
+    I_all = torch.tensor([float(I)], dtype=torch.float64, device=dev)
+    N_all = torch.tensor([float(N)], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(I_all)
+        dist.all_reduce(N_all)
+    ms_per_step = float(total_ms.item()) / args.steps
+    value = float(I_all.item()) / (ms_per_step * 1e-3)
+    k_ms = sum(kern_ms) / len(kern_ms)
+
+    # sample for the CPU oracle (taken now, while the positions are still on the device)
+    cpu_sub = None
+    if not args.no_cpu and world == 1 and rank == 0:
+        cpu_sub, _ = oracle_sample(pos, rcfg, 6)
+
+    # ---- end to end through nf_forces_host (pinned host buffers, copies inside the timing) ----
+    e2e = None
+    if not args.no_e2e:
+        try:
+            del b, acc
+            torch.cuda.empty_cache()
+            hpos = torch.empty(N, 3, dtype=torch.float32).pin_memory()
+            hpos.copy_(pos)
+            del pos
+            torch.cuda.empty_cache()
+            hacc = torch.empty(N, 3, dtype=torch.float32).pin_memory()
+            ctx.reserve_host(N, K)
+            n_e2e = max(1, min(args.steps, 3))
+            for _ in range(2):
+                ctx.forces_host(hpos, K, R, rcfg.eps, rcfg.box, rcfg.Gm, out=hacc)
+            barrier()
+            t0 = time.perf_counter()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(n_e2e):
+                ctx.forces_host(hpos, K, R, rcfg.eps, rcfg.box, rcfg.Gm, out=hacc)
+            e1.record()
+            barrier()
+            wall = (time.perf_counter() - t0) / n_e2e
+            dev_s = e0.elapsed_time(e1) * 1e-3 / n_e2e
+            t = torch.tensor([max(wall, dev_s)], dtype=torch.float64, device=dev)
+            if dist is not None:
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e = {"value": float(I_all.item()) / float(t.item()), "unit": "interactions/s",
+                   "h2d_bytes_per_step": 12 * N, "d2h_bytes_per_step": 12 * N,
+                   "ms_per_step": 1e3 * float(t.item()), "api": "nf_forces_host", "steps": n_e2e,
+                   "result_checksum": float(hacc[:: max(1, N // 4096)].double().abs().sum())}
+        except Exception as exc:  # keep the device-timed line even if the host leg cannot run
+            e2e = {"value": None, "unit": "interactions/s", "error": repr(exc)[:200]}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    sm_max_mhz, hbm_gbs, peak_src = read_peaks()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak_tflops = sms * sm_max_mhz * 1e6 * 2 * FP32_LANES_PER_SM / 1e12
+    achieved = FLOP_PER_INTERACTION * I / (k_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "interaction kernel (nf_forces)", "achieved": achieved,
+                "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
+                "peak_source": f"{sms} SMs x {sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz) x 2 x {FP32_LANES_PER_SM} FP32 lanes",
+                "flop_per_interaction": FLOP_PER_INTERACTION, "kernel_ms": k_ms,
+                "kernel_interactions_per_s": I / (k_ms * 1e-3), "kernel_share_of_step": k_ms / ms_per_step,
+                "frac_at_sampled_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max_mhz)
+                                          if clocks and clocks.get("sm_mhz") else None)}
+
+    cpu = None
+    if cpu_sub is not None:
+        m = 6
+        inter, dt, cores, n_sinks, _, _ = time_oracle(cpu_sub, rcfg, m, (3, 5, 7), budget_s=15.0)
+        cpu = {"value": inter / dt, "unit": "interactions/s", "cores": cores, "kind": "oracle",
+               "sample": f"{n_sinks} sinks drawn from a {m}^3-cell block of {rcfg.name} with all their sources: "
+                         f"{inter} pairs in {dt:.2f} s, float64"}
+
+    line = {"metric": "near_field_pairwise_interactions_per_s", "value": value, "unit": "interactions/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": rcfg.name, "N": N, "K": K, "R": R, "eps": rcfg.eps, "box": rcfg.box,
+                       "interactions_per_step_per_gpu": I, "interactions_per_particle": I / N,
+                       "l2": "flushed between timed steps (256 MiB write)" if small else "inputs larger than L2",
+                       "parallelism": f"{world} independent boxes, one per GPU" if world > 1 else "1 GPU"},
+            "particles_per_s": float(N_all.item()) / (ms_per_step * 1e-3),
+            "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -130,6 +130,25 @@ int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
               const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
               float eps, float box, float Gm, int softening, float *acc_xyz, void *stream);
 
+/*
+ * nf_forces_host -- the whole path from HOST buffers: H2D copy of the positions, nf_bin,
+ * nf_forces, D2H copy of the accelerations (the paper's GPU rate "includes
+ * PCIe bus transfer overheads").  All device buffers come from the context's scratch arena
+ * (about 60 bytes per particle; pre-size with nf_reserve_host to avoid the first-call
+ * allocation).
+ *
+ *   pos_host   host in   N x 3 float32 global positions (pinned memory recommended; pageable
+ *                        memory works but the copies are then staged by the driver)
+ *   acc_host   host out  N x 3 float32 accelerations in the caller's order
+ *   other arguments as for nf_bin / nf_forces.
+ *
+ * The call returns after the D2H copy has completed (it synchronises `stream`).  Returns
+ * NF_ERR_RANGE (after completing the computation) if positions outside [0, box) were clamped.
+ */
+int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, float eps,
+                   float box, float Gm, int softening, float *acc_host, void *stream);
+int nf_reserve_host(nf_ctx *ctx, int64_t maxN, int K);
+
 /* Number of ordered (sink, source) pairs nf_forces evaluates for these cell counts:
  * I = sum_c n_c * sum_{c' in N(c)} n_c'  (self pairs included, padding excluded; the
  * "pairwise interactions" of PAPER.md:107).  Computed on the device, synchronises `stream`,
@@ -190,6 +209,10 @@ int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const int64
  * *kernel_ms = duration of the interaction kernel alone; *total_ms = whole nf_forces call
  * (work-list build + kernel + scale/un-permute).  Either pointer may be NULL. */
 int nf_last_forces_timing(nf_ctx *ctx, float *kernel_ms, float *total_ms);
+
+/* Number of CUDA kernels this context has launched since nf_create (memcpy / memset nodes are
+ * not counted).  Host-side counter; does not synchronise.  Used by bench.py's gpu_launches. */
+int nf_launch_count(const nf_ctx *ctx, int64_t *launches);
 
 #ifdef __cplusplus
 }

@@ -176,6 +176,64 @@ int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
     return nf_forces_impl(ctx, p, d_planes, st, true);
 }
 
+static size_t host_path_bytes(int64_t N, int K)
+{
+    const size_t n = (size_t)(N > 0 ? N : 1), ncell = (size_t)K * K * K;
+    size_t b = nf_align_up(n * 12, 256) * 2 + nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
+               nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256);
+    return b + nf_bin_scratch_bytes(N, K, false) + forces_scratch_full(K) + 4096;
+}
+
+int nf_reserve_host(nf_ctx *ctx, int64_t maxN, int K)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_TRY(check_common(ctx, maxN, K, 1.0f));
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    return nf_scratch_reserve(ctx, host_path_bytes(maxN, K));
+}
+
+int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, float eps,
+                   float box, float Gm, int softening, float *acc_host, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_TRY(check_common(ctx, N, K, box));
+    NF_TRY(check_force_args(ctx, K, R, eps, Gm, softening));
+    NF_ARG(ctx, N == 0 || (pos_host && acc_host), "nf_forces_host: null particle array with N > 0");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (N == 0) return NF_OK;
+    NF_TRY(nf_scratch_reserve(ctx, host_path_bytes(N, K)));
+    nf_scratch_reset(ctx);
+    const size_t n = (size_t)N, ncell = (size_t)K * K * K;
+    float *raw = nf_scratch_take<float>(ctx, n * 3);
+    float *acc = nf_scratch_take<float>(ctx, n * 3);
+    float *sorted = nf_scratch_take<float>(ctx, n * 4);
+    uint32_t *perm = nf_scratch_take<uint32_t>(ctx, n);
+    uint32_t *count = nf_scratch_take<uint32_t>(ctx, ncell);
+    uint64_t *off = nf_scratch_take<uint64_t>(ctx, ncell + 1);
+    nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
+    if (!raw || !acc || !sorted || !perm || !count || !off || !d_planes) {
+        NF_SET_ERR(ctx, "nf_forces_host: internal scratch arena too small");
+        return NF_ERR_NOMEM;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, sizeof(unsigned long long), st));
+    NF_CUDA(ctx, cudaMemcpyAsync(raw, pos_host, n * 12, cudaMemcpyHostToDevice, st));
+    NF_TRY(nf_bin_impl(ctx, raw, N, K, box, -1, sorted, perm, count, off, st));
+    nf_force_params p{};
+    p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
+    p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening;
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), off, perm, acc, st));
+    NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
+    NF_CUDA(ctx, cudaMemcpyAsync(acc_host, acc, n * 12, cudaMemcpyDeviceToHost, st));
+    NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    NF_CUDA(ctx, cudaStreamSynchronize(st));
+    if (ctx->h_counters[0]) {
+        NF_SET_ERR(ctx, "%lld particle(s) outside [0, box) were clamped into edge cells", (long long)ctx->h_counters[0]);
+        return NF_ERR_RANGE;
+    }
+    return NF_OK;
+}
+
 int nf_interactions(nf_ctx *ctx, const uint32_t *cell_count, int K, int R, int64_t *interactions, void *stream)
 {
     if (!ctx) return NF_ERR_ARG;
@@ -195,6 +253,13 @@ int nf_last_forces_timing(nf_ctx *ctx, float *kernel_ms, float *total_ms)
     NF_CUDA(ctx, cudaEventSynchronize(ctx->ev_total1));
     if (kernel_ms) NF_CUDA(ctx, cudaEventElapsedTime(kernel_ms, ctx->ev_kern0, ctx->ev_kern1));
     if (total_ms) NF_CUDA(ctx, cudaEventElapsedTime(total_ms, ctx->ev_total0, ctx->ev_total1));
+    return NF_OK;
+}
+
+int nf_launch_count(const nf_ctx *ctx, int64_t *launches)
+{
+    if (!ctx || !launches) return NF_ERR_ARG;
+    *launches = (int64_t)ctx->launches;
     return NF_OK;
 }
 

@@ -210,7 +210,7 @@ int nf_bin_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, int 
     if (N > 0) {
         float invw = (float)K / box;
         k_keys<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, N, K, invw, plane_cx, keysA, cell_count, ctx->counters);
-        NF_CUDA(ctx, cudaGetLastError());
+        NF_LAUNCHED(ctx);
     }
     NF_TRY(nf_exclusive_scan_u32_u64(ctx, cell_count, cell_offset, ncell, tmp64, st));
     if (N == 0) return NF_OK;
@@ -227,16 +227,16 @@ int nf_bin_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, int 
         size_t sh_hist = (size_t)K * sizeof(uint32_t);
         size_t sh_scat = (size_t)K * RS_WARPS * sizeof(uint32_t);
         k_radix_hist<<<(unsigned)ntiles, RS_THREADS, sh_hist, st>>>(kin, N, div, (uint32_t)K, hist, (uint32_t)ntiles);
-        NF_CUDA(ctx, cudaGetLastError());
+        NF_LAUNCHED(ctx);
         NF_TRY(nf_exclusive_scan_u32(ctx, hist, hist, (size_t)K * ntiles, tmp32, st));
         k_radix_scatter<<<(unsigned)ntiles, RS_THREADS, sh_scat, st>>>(kin, iin, N, div, (uint32_t)K, hist, (uint32_t)ntiles, kout, iout);
-        NF_CUDA(ctx, cudaGetLastError());
+        NF_LAUNCHED(ctx);
         kin = kout;
         iin = iout;
         div *= (uint32_t)K;
     }
     float hw = 0.5f * (box / (float)K);
     k_gather<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, kin, perm, N, K, hw, plane_cx, reinterpret_cast<float4 *>(pos_sorted));
-    NF_CUDA(ctx, cudaGetLastError());
+    NF_LAUNCHED(ctx);
     return NF_OK;
 }

@@ -24,6 +24,7 @@ struct nf_ctx {
     // timing of the last nf_forces
     cudaEvent_t ev_total0, ev_kern0, ev_kern1, ev_total1;
     bool forces_timed;
+    long long launches;  // kernels launched by this context since nf_create
     // slab streaming resources (created lazily)
     cudaStream_t s_h2d, s_d2h;
     void *slab_state;
@@ -42,6 +43,13 @@ struct nf_ctx {
                        __FILE__, __LINE__, cudaGetErrorString(e__));                         \
             return e__ == cudaErrorMemoryAllocation ? NF_ERR_NOMEM : NF_ERR_CUDA;            \
         }                                                                                    \
+    } while (0)
+
+// after every kernel launch: count it (nf_launch_count) and pick up launch errors
+#define NF_LAUNCHED(ctx)                      \
+    do {                                      \
+        (ctx)->launches++;                    \
+        NF_CUDA(ctx, cudaGetLastError());     \
     } while (0)
 
 #define NF_ARG(ctx, cond, ...)           \

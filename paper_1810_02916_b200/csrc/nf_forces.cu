@@ -228,7 +228,7 @@ int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float
                         const uint32_t *perm, float *acc, cudaStream_t st)
 {
     k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, off, perm, acc);
-    NF_CUDA(ctx, cudaGetLastError());
+    NF_LAUNCHED(ctx);
     return NF_OK;
 }
 
@@ -238,7 +238,7 @@ int nf_interactions_planes(nf_ctx *ctx, const nf_force_params &p, const nf_plane
     if (n_sink_planes <= 0) return NF_OK;
     dim3 grid((unsigned)((p.K * p.K + 255) / 256), (unsigned)n_sink_planes);
     k_interactions_planes<<<grid, 256, 0, st>>>(d_planes, p, ctx->counters + 1);
-    NF_CUDA(ctx, cudaGetLastError());
+    NF_LAUNCHED(ctx);
     return NF_OK;
 }
 
@@ -252,7 +252,7 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
     if (n_sink_planes > 0) {
         dim3 grid((unsigned)(p.K * p.K), (unsigned)n_sink_planes);
         k_forces_cell<<<grid, CELL_THREADS, 0, st>>>(d_planes, p, fc);
-        NF_CUDA(ctx, cudaGetLastError());
+        NF_LAUNCHED(ctx);
     }
     if (record_timing) {
         NF_CUDA(ctx, cudaEventRecord(ctx->ev_kern1, st));
@@ -268,7 +268,7 @@ int nf_interactions_impl(nf_ctx *ctx, const uint32_t *cell_count, int K, int R, 
     const size_t ncell = (size_t)K * K * K;
     unsigned blocks = (unsigned)min((size_t)ctx->sm_count * 8, (ncell + 255) / 256);
     k_interactions<<<blocks, 256, 0, st>>>(cell_count, K, R, ctx->counters + 1);
-    NF_CUDA(ctx, cudaGetLastError());
+    NF_LAUNCHED(ctx);
     NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters + 1, ctx->counters + 1, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     NF_CUDA(ctx, cudaStreamSynchronize(st));
     *out = (int64_t)ctx->h_counters[1];

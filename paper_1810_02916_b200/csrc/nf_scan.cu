@@ -90,15 +90,15 @@ int scan_impl(nf_ctx *ctx, const TIn *in, TOut *out, size_t n, TOut *temp, cudaS
     size_t nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
     if (nblk == 1) {
         scan_apply<TIn, TOut><<<1, SCAN_THREADS, 0, st>>>(in, n, nullptr, out, write_total);
-        NF_CUDA(ctx, cudaGetLastError());
+        NF_LAUNCHED(ctx);
         return NF_OK;
     }
     TOut *sums = temp;
     scan_reduce<TIn, TOut><<<(unsigned)nblk, SCAN_THREADS, 0, st>>>(in, n, sums);
-    NF_CUDA(ctx, cudaGetLastError());
+    NF_LAUNCHED(ctx);
     NF_TRY((scan_impl<TOut, TOut>(ctx, sums, sums, nblk, temp + nf_align_up(nblk, 64), st, 0)));
     scan_apply<TIn, TOut><<<(unsigned)nblk, SCAN_THREADS, 0, st>>>(in, n, sums, out, write_total);
-    NF_CUDA(ctx, cudaGetLastError());
+    NF_LAUNCHED(ctx);
     return NF_OK;
 }
 

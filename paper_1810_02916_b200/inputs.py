@@ -226,3 +226,21 @@ def make_slab_planes(cfg: Config, device="cpu", n_planes_total: Optional[int] = 
         planes.append(x[s:s + n].contiguous())
         s += n
     return planes
+
+
+def select_box(pos: torch.Tensor, lo, hi, box: float) -> torch.Tensor:
+    """Indices of the particles whose coordinates lie in the periodic axis-aligned box
+    [lo, hi) (per axis, lo may be negative and hi may exceed `box`; hi - lo < box).  A plain
+    geometric filter used to cut samples out of the big configs for the CPU oracle; it does no
+    cell assignment."""
+    mask = torch.ones(pos.shape[0], dtype=torch.bool, device=pos.device)
+    for ax in range(3):
+        x = pos[:, ax]
+        l, h = float(lo[ax]), float(hi[ax])
+        assert h - l < box
+        l_w, h_w = l % box, h % box
+        if l_w < h_w:
+            mask &= (x >= l_w) & (x < h_w)
+        else:
+            mask &= (x >= l_w) | (x < h_w)
+    return torch.nonzero(mask).flatten()

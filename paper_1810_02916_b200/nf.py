@@ -23,7 +23,7 @@ _SOFT = {"spline": SOFT_SPLINE, "plummer": SOFT_PLUMMER}
 # every symbol include/nf.h declares
 EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve", "nf_bin",
            "nf_out_of_range", "nf_forces", "nf_interactions", "nf_spline_equivalent_eps",
-           "nf_stream_slabs", "nf_last_forces_timing"]
+           "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host"]
 
 
 class NFError(RuntimeError):
@@ -82,6 +82,12 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
                                     i32, ctypes.POINTER(vp), ctypes.POINTER(StreamStats), vp]
     lib.nf_last_forces_timing.restype = i32
     lib.nf_last_forces_timing.argtypes = [vp, ctypes.POINTER(f32), ctypes.POINTER(f32)]
+    lib.nf_forces_host.restype = i32
+    lib.nf_forces_host.argtypes = [vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp]
+    lib.nf_reserve_host.restype = i32
+    lib.nf_reserve_host.argtypes = [vp, i64, i32]
+    lib.nf_launch_count.restype = i32
+    lib.nf_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     _lib = lib
     return lib
 
@@ -141,16 +147,19 @@ class Context:
     def reserve(self, maxN: int, K: int):
         self._check(self.lib.nf_reserve(self._h, int(maxN), int(K)))
 
-    def bin(self, pos: torch.Tensor, K: int, box: float, stream=None) -> Binned:
-        """nf_bin: pos float32 [N, 3] on the device -> cell-contiguous arrays."""
+    def bin(self, pos: torch.Tensor, K: int, box: float, out: Optional[Binned] = None, stream=None) -> Binned:
+        """nf_bin: pos float32 [N, 3] on the device -> cell-contiguous arrays (written into
+        ``out`` if given, so repeated calls reuse the same device buffers)."""
         assert pos.is_cuda and pos.dtype == torch.float32 and pos.dim() == 2 and pos.shape[1] == 3 and pos.is_contiguous()
         N = pos.shape[0]
         dev = pos.device
         ncell = int(K) ** 3
-        out = Binned(torch.empty(N, 4, dtype=torch.float32, device=dev),
-                     torch.empty(N, dtype=torch.int32, device=dev),
-                     torch.empty(ncell, dtype=torch.int32, device=dev),
-                     torch.empty(ncell + 1, dtype=torch.int64, device=dev), N, int(K), float(box))
+        if out is None:
+            out = Binned(torch.empty(N, 4, dtype=torch.float32, device=dev),
+                         torch.empty(N, dtype=torch.int32, device=dev),
+                         torch.empty(ncell, dtype=torch.int32, device=dev),
+                         torch.empty(ncell + 1, dtype=torch.int64, device=dev), N, int(K), float(box))
+        assert out.N == N and out.K == int(K) and out.box == float(box)
         self._check(self.lib.nf_bin(self._h, _ptr(pos), N, int(K), float(box), _ptr(out.pos_sorted), _ptr(out.perm),
                                     _ptr(out.cell_count), _ptr(out.cell_offset), self._stream(stream)))
         return out
@@ -170,6 +179,24 @@ class Context:
                                        float(b.box), float(Gm), _SOFT[softening], _ptr(acc), self._stream(stream)))
         return acc
 
+    def reserve_host(self, maxN: int, K: int):
+        self._check(self.lib.nf_reserve_host(self._h, int(maxN), int(K)))
+
+    def forces_host(self, pos_host: torch.Tensor, K: int, R: int, eps: float, box: float, Gm: float,
+                    softening: str = "spline", out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """nf_forces_host: the whole path from a HOST float32 [N, 3] tensor (pinned recommended) to
+        a host float32 [N, 3] acceleration tensor; H2D, binning, forces and D2H all inside the call."""
+        assert (not pos_host.is_cuda) and pos_host.dtype == torch.float32 and pos_host.dim() == 2 \
+            and pos_host.shape[1] == 3 and pos_host.is_contiguous()
+        N = pos_host.shape[0]
+        if out is None:
+            out = torch.empty(N, 3, dtype=torch.float32).pin_memory()
+        assert (not out.is_cuda) and out.dtype == torch.float32 and out.shape == (N, 3) and out.is_contiguous()
+        self._check(self.lib.nf_forces_host(self._h, _ptr(pos_host), N, int(K), int(R), float(eps), float(box),
+                                            float(Gm), _SOFT[softening], _ptr(out), self._stream(stream)),
+                    allow=(NF_ERR_RANGE,))
+        return out
+
     def interactions(self, b: Binned, R: int, stream=None) -> int:
         n = ctypes.c_int64(0)
         self._check(self.lib.nf_interactions(self._h, _ptr(b.cell_count), b.K, int(R), ctypes.byref(n), self._stream(stream)))
@@ -180,6 +207,12 @@ class Context:
         k, t = ctypes.c_float(0), ctypes.c_float(0)
         self._check(self.lib.nf_last_forces_timing(self._h, ctypes.byref(k), ctypes.byref(t)))
         return float(k.value), float(t.value)
+
+    def launch_count(self) -> int:
+        """Kernels launched by this context so far (host counter)."""
+        n = ctypes.c_int64(0)
+        self._check(self.lib.nf_launch_count(self._h, ctypes.byref(n)))
+        return int(n.value)
 
     def stream_slabs(self, planes: Sequence[torch.Tensor], P: int, K: int, R: int, eps: float, box: float,
                      plane0: int, Gm: float, softening: str = "spline",
