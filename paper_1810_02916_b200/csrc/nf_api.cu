@@ -93,11 +93,14 @@ static int check_common(nf_ctx *ctx, int64_t N, int K, float box)
     return NF_OK;
 }
 
-static size_t forces_scratch_full(int K)
+static size_t forces_scratch_full(int64_t N, int K)
 {
     nf_force_params p{};
     p.K = K;
     p.n_planes = K;
+    p.sink_lo = 0;
+    p.sink_hi = K;
+    p.max_sinks = N;
     return nf_forces_scratch_bytes(p);
 }
 
@@ -107,7 +110,7 @@ int nf_reserve(nf_ctx *ctx, int64_t maxN, int K)
     NF_TRY(check_common(ctx, maxN, K, 1.0f));
     NF_CUDA(ctx, cudaSetDevice(ctx->device));
     size_t need = nf_bin_scratch_bytes(maxN, K, false);
-    size_t f = forces_scratch_full(K);
+    size_t f = forces_scratch_full(maxN, K);
     return nf_scratch_reserve(ctx, need > f ? need : f);
 }
 
@@ -166,7 +169,7 @@ int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
     if (N == 0) return NF_OK;
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
-    p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening;
+    p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
     NF_TRY(nf_scratch_reserve(ctx, nf_forces_scratch_bytes(p)));
     nf_scratch_reset(ctx);
     nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
@@ -181,7 +184,7 @@ static size_t host_path_bytes(int64_t N, int K)
     const size_t n = (size_t)(N > 0 ? N : 1), ncell = (size_t)K * K * K;
     size_t b = nf_align_up(n * 12, 256) * 2 + nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
                nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256);
-    return b + nf_bin_scratch_bytes(N, K, false) + forces_scratch_full(K) + 4096;
+    return b + nf_bin_scratch_bytes(N, K, false) + forces_scratch_full(N, K) + 4096;
 }
 
 int nf_reserve_host(nf_ctx *ctx, int64_t maxN, int K)
@@ -221,7 +224,7 @@ int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, 
     NF_TRY(nf_bin_impl(ctx, raw, N, K, box, -1, sorted, perm, count, off, st));
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
-    p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening;
+    p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
     NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), off, perm, acc, st));
     NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
     NF_CUDA(ctx, cudaMemcpyAsync(acc_host, acc, n * 12, cudaMemcpyDeviceToHost, st));

@@ -110,6 +110,7 @@ struct nf_force_params {
     int R;
     float eps, box, Gm;
     int softening;
+    long long max_sinks;  // upper bound on the particles in the sink planes (sizes the work list)
 };
 size_t nf_forces_scratch_bytes(const nf_force_params &p);
 // d_planes: DEVICE array of p.n_planes views (fill with nf_fill_planes_full or copy from pinned memory)

@@ -5,11 +5,8 @@
 // PAPER.md:243 Eq. 2 compact spline, evaluated as min(10 - 15u + 6u^2, u^-3)/eps^3 (fn. 4, :239);
 // PAPER.md:233 Eq. 1 Plummer;  PAPER.md:51 cell-centred float32 offsets.
 //
-// Two kernels:
-//   k_forces_cell   -- general path (any K >= 2R+1): one block per sink cell, source cells
-//                      staged through shared memory one at a time, sink shifted into each
-//                      source cell's frame (d = o_j - (o_i - dc*w), the cell-centred form).
-//   k_forces_pencil -- fast path (K >= 4R): see the block comment above it.
+// k_task_count / k_task_fill build the work list (chunks of <= 256 sinks of one cell);
+// k_forces_tile is the interaction kernel (see the block comment above it).
 #include "nf_common.cuh"
 
 namespace {
@@ -48,81 +45,259 @@ struct PlaneTable {
 };
 
 // ------------------------------------------------------------------------------------------
-// General kernel.  grid = (K*K, sink planes); block = 128 threads; block handles sink cell
-// (plane, cy, cz).  Sinks are processed 128 at a time, one per thread.
+// Packed FP32 (sm_100 FFMA2 / FADD2 / FMUL2): one 64-bit register holds the same quantity for
+// TWO SINKS; the source coordinate is a scalar operand broadcast to both halves (ptxas emits
+// the .F32 broadcast operand form, so no duplicating moves).  13 (spline) or 11 (r^-3 only)
+// FMA-pipe instructions per source serve two interactions per lane.
 // ------------------------------------------------------------------------------------------
-constexpr int CELL_THREADS = 128;
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk(float a, float b) { u64 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void upk(u64 r, float &a, float &b) { asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(r)); }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 d; asm("sub.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 d; asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 
-__global__ void __launch_bounds__(CELL_THREADS) k_forces_cell(const nf_plane_view *__restrict__ planes, nf_force_params p, ForceConsts fc)
+// One source against the lane's two sinks.  MODE 0: spline, min(poly, r^-3); 1: r^-3 only
+// (valid when the cell separation guarantees r >= eps, or for Plummer where r2_floor = eps^2).
+template <int MODE>
+__device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64 ys, const u64 zs, const ForceConsts &fc,
+                                         u64 &ax, u64 &ay, u64 &az)
 {
-    __shared__ float4 tile[CELL_THREADS];
-    const int K = p.K, R = p.R;
-    const int sink_plane = p.sink_lo + blockIdx.y;
-    const int cyz = blockIdx.x;
-    const int cy = cyz / K, cz = cyz % K;
-    const nf_plane_view sp = planes[sink_plane];
-    const uint64_t s0 = sp.off[cyz], s1 = sp.off[cyz + 1];
-    if (s0 == s1) return;
-    const float w = (p.box / (float)K) * fc.scale;
+    const u64 dx = sub2(pk(q.x, q.x), xs), dy = sub2(pk(q.y, q.y), ys), dz = sub2(pk(q.z, q.z), zs);
+    u64 r2 = fma2(dz, dz, pk(fc.r2_floor, fc.r2_floor));
+    r2 = fma2(dy, dy, r2);
+    r2 = fma2(dx, dx, r2);
+    float r2a, r2b;
+    upk(r2, r2a, r2b);
+    const u64 ri = pk(rsqrt_approx(r2a), rsqrt_approx(r2b));
+    u64 f = mul2(mul2(ri, ri), ri);
+    if (MODE == 0) {
+        const u64 poly = fma2(r2, fma2(pk(fc.B, fc.B), ri, pk(fc.C, fc.C)), pk(fc.A, fc.A));
+        float pa, pb, fa, fb;
+        upk(poly, pa, pb);
+        upk(f, fa, fb);
+        f = pk(fminf(pa, fa), fminf(pb, fb));
+    }
+    ax = fma2(f, dx, ax);
+    ay = fma2(f, dy, ay);
+    az = fma2(f, dz, az);
+}
 
-    for (uint64_t sb = s0; sb < s1; sb += CELL_THREADS) {
-        const uint64_t si = sb + threadIdx.x;
-        const bool active = si < s1;
-        float4 me = active ? sp.pos[si] : make_float4(0.f, 0.f, 0.f, 0.f);
-        const float xi = me.x * fc.scale, yi = me.y * fc.scale, zi = me.z * fc.scale;
-        float ahx = 0.f, ahy = 0.f, ahz = 0.f, alx = 0.f, aly = 0.f, alz = 0.f;
-        for (int dx = -R; dx <= R; dx++) {
+template <int MODE>
+__device__ __forceinline__ void run_sources(const float4 *__restrict__ src, int q, const u64 xs, const u64 ys, const u64 zs,
+                                            const ForceConsts &fc, u64 &ax, u64 &ay, u64 &az)
+{
+    int k = 0;
+#pragma unroll 1
+    for (; k + 4 <= q; k += 4) {
+        const float4 q0 = src[k], q1 = src[k + 1], q2 = src[k + 2], q3 = src[k + 3];
+        interact<MODE>(q0, xs, ys, zs, fc, ax, ay, az);
+        interact<MODE>(q1, xs, ys, zs, fc, ax, ay, az);
+        interact<MODE>(q2, xs, ys, zs, fc, ax, ay, az);
+        interact<MODE>(q3, xs, ys, zs, fc, ax, ay, az);
+    }
+#pragma unroll 1
+    for (; k < q; k++) interact<MODE>(src[k], xs, ys, zs, fc, ax, ay, az);
+}
+
+// ------------------------------------------------------------------------------------------
+// Work list.  A task is a chunk of <= TILE_SINKS consecutive sinks of ONE cell of a sink plane.
+// ------------------------------------------------------------------------------------------
+constexpr int TILE_T = 128;                 // threads per block
+constexpr int TILE_SINKS = 2 * TILE_T;      // sinks per task at most (two per lane, one phase)
+constexpr int TILE_CAP = 512;               // sources staged per pass (float4 each)
+
+struct Task {
+    uint32_t cyz;     // cell index within the plane, cy*K + cz
+    uint16_t plane;   // sink plane (index into the plane table)
+    uint16_t chunk;   // chunk of TILE_SINKS sinks within the cell
+};
+
+__global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restrict__ planes, nf_force_params p, uint32_t *__restrict__ tc)
+{
+    const int cyz = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cyz >= p.K * p.K) return;
+    const uint64_t *off = planes[p.sink_lo + blockIdx.y].off;
+    const uint64_t n = off[cyz + 1] - off[cyz];
+    tc[(size_t)blockIdx.y * p.K * p.K + cyz] = (uint32_t)((n + TILE_SINKS - 1) / TILE_SINKS);
+}
+
+// ctl[0] = work cursor (zeroed here), ctl[1] = number of tasks
+__global__ void __launch_bounds__(256) k_task_fill(const uint32_t *__restrict__ tc, const uint32_t *__restrict__ to, nf_force_params p,
+                                                   Task *__restrict__ tasks, uint32_t *__restrict__ ctl)
+{
+    const int cyz = blockIdx.x * blockDim.x + threadIdx.x;
+    const int KK = p.K * p.K;
+    if (cyz >= KK) return;
+    const size_t c = (size_t)blockIdx.y * KK + cyz;
+    const uint32_t n = tc[c], o = to[c];
+    for (uint32_t k = 0; k < n; k++) {
+        Task t;
+        t.cyz = (uint32_t)cyz;
+        t.plane = (uint16_t)(p.sink_lo + blockIdx.y);
+        t.chunk = (uint16_t)k;
+        tasks[o + k] = t;
+    }
+    if (cyz == KK - 1 && blockIdx.y == gridDim.y - 1) {
+        ctl[0] = 0;
+        ctl[1] = o + n;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Interaction kernel.  Persistent blocks of TILE_T threads pull tasks from the work list.
+//
+// Task = n <= 256 sinks of cell (plane, cy, cz).  Lane mapping: L = ceil(n/2) "sink lanes"
+// each hold two sinks in packed registers; the P = floor(T/L) "phases" split every source run
+// between them, so small cells still fill the block (lane use L*P/T).  For each of the
+// (2R+1)^2 source columns (dx, dy) the 2R+1 cells cz-R..cz+R are one z-run (contiguous in
+// memory because z is the fastest cell index; the periodic wrap splits it): the run is staged
+// through shared memory once, already multiplied by `scale` and with the z shift of its cell
+// added, so that same-cell differences stay exact, and every phase processes a
+// contiguous q = ceil(m/P) slice of it (missing entries are far-away sentinels: zero force).
+// float32 partial sums per run, double outer sum over runs and phases; no atomics on floats.
+// ------------------------------------------------------------------------------------------
+struct RunTab {
+    unsigned long long start[2 * NF_MAX_R + 1];   // first particle of each cell segment
+    int cum[2 * NF_MAX_R + 2];                    // cumulative particle count before segment s
+    int pad_;
+};
+
+template <int R>
+__global__ void __launch_bounds__(TILE_T) k_forces_tile(const nf_plane_view *__restrict__ planes, const nf_force_params p, const ForceConsts fc,
+                                                        const Task *__restrict__ tasks, uint32_t *__restrict__ ctl)
+{
+    constexpr int W = 2 * R + 1;
+    __shared__ __align__(16) float4 buf[TILE_CAP];
+    __shared__ RunTab tab[2];
+    __shared__ uint32_t s_task;
+    const int tid = threadIdx.x;
+    const int K = p.K;
+    const float w = (p.box / (float)K) * fc.scale;
+    const float SENT = 1.0e15f;   // sentinel source: r2 ~ 1e30, r^-3 flushes to zero
+    const bool far_ok = !fc.plummer && w > 1.001f * sqrtf(fc.eps2);
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_task = atomicAdd(&ctl[0], 1u);
+        __syncthreads();
+        const uint32_t ti = s_task;
+        if (ti >= ctl[1]) return;
+        const Task task = tasks[ti];
+        const int sink_plane = task.plane;
+        const int cy = (int)(task.cyz / (uint32_t)K), cz = (int)(task.cyz % (uint32_t)K);
+        const nf_plane_view sp = planes[sink_plane];
+        const uint64_t c0 = sp.off[task.cyz], c1 = sp.off[task.cyz + 1];
+        const uint64_t s0 = c0 + (uint64_t)task.chunk * TILE_SINKS;
+        const int n = (int)min((uint64_t)TILE_SINKS, c1 - s0);
+        const int L = (n + 1) >> 1;
+        const int P = TILE_T / L;
+        const int sl = tid % L, ph = tid / L;
+        const bool active = ph < P;
+        // the lane's two sinks (the second is a duplicate of the first when n is odd)
+        const uint64_t i0 = s0 + 2 * (uint64_t)sl;
+        const uint64_t i1 = (2 * sl + 1 < n) ? i0 + 1 : i0;
+        const float4 m0 = sp.pos[i0], m1 = sp.pos[i1];
+        const u64 xi = pk(m0.x * fc.scale, m1.x * fc.scale), yi = pk(m0.y * fc.scale, m1.y * fc.scale),
+                  zi = pk(m0.z * fc.scale, m1.z * fc.scale);
+        double ax0 = 0.0, ay0 = 0.0, az0 = 0.0, ax1 = 0.0, ay1 = 0.0, az1 = 0.0;
+
+        // segment table of a run: lanes 0..W-1 of warp 0 each look up one cell of the z-window
+        auto build_tab = [&](int r, RunTab &t) {
+            const int dx = r / W - R, dy = r % W - R;
+            int px = sink_plane + dx;
+            bool have = true;
+            if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
+            else if (px < 0 || px >= p.n_planes) { have = false; px = sink_plane; }
+            const int qy = ((cy + dy) % K + K) % K;
+            const int s = tid;     // segment index (only tid < W matter)
+            unsigned long long st = 0;
+            int cnt = 0;
+            if (s < W && have) {
+                const int qz = ((cz + s - R) % K + K) % K;
+                const uint64_t *qo = planes[px].off + (size_t)qy * K + qz;
+                st = qo[0];
+                cnt = (int)(qo[1] - st);
+            }
+            int inc = cnt;
+#pragma unroll
+            for (int d = 1; d < 8; d <<= 1) {
+                int v = __shfl_up_sync(0xffffffffu, inc, d);
+                if ((tid & 31) >= d) inc += v;
+            }
+            if (s < W) { t.start[s] = st; t.cum[s] = inc - cnt; }
+            if (s == W - 1) t.cum[W] = inc;
+        };
+        if (tid < 32) build_tab(0, tab[0]);
+
+        for (int r = 0; r < W * W; r++) {
+            const int dx = r / W - R, dy = r % W - R;
             int px = sink_plane + dx;
             if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
-            else if (px < 0 || px >= p.n_planes) continue;
-            const nf_plane_view qp = planes[px];
-            const float xs = xi - (float)dx * w;  // sink in the source cell's frame
-            for (int dy = -R; dy <= R; dy++) {
-                const int qy = ((cy + dy) % K + K) % K;
-                const float ys = yi - (float)dy * w;
-                for (int dz = -R; dz <= R; dz++) {
-                    const int qz = ((cz + dz) % K + K) % K;
-                    const float zs = zi - (float)dz * w;
-                    const uint64_t j0 = qp.off[qy * K + qz], j1 = qp.off[qy * K + qz + 1];
-                    float ax = 0.f, ay = 0.f, az = 0.f;
-                    for (uint64_t jb = j0; jb < j1; jb += CELL_THREADS) {
-                        __syncthreads();
-                        const uint64_t j = jb + threadIdx.x;
-                        if (j < j1) {
-                            float4 q = qp.pos[j];
-                            tile[threadIdx.x] = make_float4(q.x * fc.scale, q.y * fc.scale, q.z * fc.scale, 0.f);
-                        }
-                        __syncthreads();
-                        const int n = (int)min((uint64_t)CELL_THREADS, j1 - jb);
-#pragma unroll 4
-                        for (int t = 0; t < n; t++) {
-                            const float4 q = tile[t];
-                            const float ddx = q.x - xs, ddy = q.y - ys, ddz = q.z - zs;
-                            float r2 = fmaf(ddz, ddz, fc.r2_floor);
-                            r2 = fmaf(ddy, ddy, r2);
-                            r2 = fmaf(ddx, ddx, r2);
-                            const float ri = rsqrt_approx(r2);
-                            float f = ri * ri * ri;
-                            if (!fc.plummer) {
-                                const float poly = fmaf(r2, fmaf(fc.B, ri, fc.C), fc.A);
-                                f = fminf(poly, f);
-                            }
-                            ax = fmaf(f, ddx, ax);
-                            ay = fmaf(f, ddy, ay);
-                            az = fmaf(f, ddz, az);
-                        }
+            else if (px < 0 || px >= p.n_planes) px = sink_plane;   // run is empty (tab has m = 0)
+            const float4 *__restrict__ qpos = planes[px].pos;
+            const u64 xs = sub2(xi, pk((float)dx * w, (float)dx * w));   // sink in the source column's frame
+            const u64 ys = sub2(yi, pk((float)dy * w, (float)dy * w));
+            const bool near = !fc.plummer && (!far_ok || (dx >= -1 && dx <= 1 && dy >= -1 && dy <= 1));
+            u64 ax = 0, ay = 0, az = 0;
+            const RunTab &t = tab[r & 1];
+            bool first = true;
+            int m = 0;
+            for (int b0 = 0; first || b0 < m; first = false) {
+                __syncthreads();                       // previous pass is done with buf; tab[r&1] is visible
+                m = t.cum[W];
+                const int mc = min(m - b0, TILE_CAP - P);     // sources in this pass
+                const int q = (mc + P - 1) / P;               // per-phase slice (P*q <= TILE_CAP)
+                for (int i = tid; i < P * q; i += TILE_T) {
+                    float4 v = make_float4(SENT, SENT, SENT, 0.f);
+                    if (i < mc) {
+                        const int g = b0 + i;
+                        int s = 0;
+#pragma unroll
+                        for (int k = 1; k < W; k++) s += (g >= t.cum[k]);
+                        const float4 o = qpos[t.start[s] + (unsigned long long)(g - t.cum[s])];
+                        v.x = o.x * fc.scale;
+                        v.y = o.y * fc.scale;
+                        v.z = fmaf(o.z, fc.scale, (float)(s - R) * w);
                     }
-                    comp_add(ahx, alx, ax);
-                    comp_add(ahy, aly, ay);
-                    comp_add(ahz, alz, az);
+                    buf[i] = v;
                 }
+                if (b0 == 0 && tid < 32 && r + 1 < W * W) build_tab(r + 1, tab[(r + 1) & 1]);
+                __syncthreads();
+                if (active && q > 0) {
+                    if (near) run_sources<0>(buf + ph * q, q, xs, ys, zi, fc, ax, ay, az);
+                    else run_sources<1>(buf + ph * q, q, xs, ys, zi, fc, ax, ay, az);
+                }
+                b0 += mc > 0 ? mc : 1;
             }
+            float a, b;
+            upk(ax, a, b); ax0 += (double)a; ax1 += (double)b;
+            upk(ay, a, b); ay0 += (double)a; ay1 += (double)b;
+            upk(az, a, b); az0 += (double)a; az1 += (double)b;
         }
-        if (active && sp.acc) {
-            const uint64_t o = sp.perm ? (uint64_t)sp.perm[si] : si;
-            sp.acc[3 * o + 0] = (ahx + alx) * fc.out_scale;
-            sp.acc[3 * o + 1] = (ahy + aly) * fc.out_scale;
-            sp.acc[3 * o + 2] = (ahz + alz) * fc.out_scale;
+
+        // reduce the phases (fixed order), scale and write
+        __syncthreads();
+        double *red = reinterpret_cast<double *>(buf);       // [P][L][6] doubles <= 128*48 B = 6 KiB
+        if (active) {
+            double *d = red + ((size_t)ph * L + sl) * 6;
+            d[0] = ax0; d[1] = ay0; d[2] = az0; d[3] = ax1; d[4] = ay1; d[5] = az1;
+        }
+        __syncthreads();
+        for (int i = tid; i < n; i += TILE_T) {
+            const int l = i >> 1, h = (i & 1) * 3;
+            double sx = 0.0, sy = 0.0, sz = 0.0;
+            for (int pp = 0; pp < P; pp++) {
+                const double *d = red + ((size_t)pp * L + l) * 6 + h;
+                sx += d[0]; sy += d[1]; sz += d[2];
+            }
+            if (sp.acc) {
+                const uint64_t si = s0 + (uint64_t)i;
+                const uint64_t o = sp.perm ? (uint64_t)sp.perm[si] : si;
+                sp.acc[3 * o + 0] = (float)(sx * (double)fc.out_scale);
+                sp.acc[3 * o + 1] = (float)(sy * (double)fc.out_scale);
+                sp.acc[3 * o + 2] = (float)(sz * (double)fc.out_scale);
+            }
         }
     }
 }
@@ -219,9 +394,25 @@ ForceConsts make_consts(const nf_force_params &p)
 
 }  // namespace
 
+static size_t n_sink_cells(const nf_force_params &p)
+{
+    const int n_sink_planes = p.sink_hi - p.sink_lo;
+    return (size_t)(n_sink_planes > 0 ? n_sink_planes : 0) * p.K * p.K;
+}
+static size_t max_tasks(const nf_force_params &p)
+{
+    return n_sink_cells(p) + (size_t)(p.max_sinks > 0 ? p.max_sinks : 0) / TILE_SINKS + 1;
+}
+
+// scratch taken by nf_forces_impl (work list) plus room for a plane table of n_planes views
 size_t nf_forces_scratch_bytes(const nf_force_params &p)
 {
-    return nf_align_up((size_t)p.n_planes * sizeof(nf_plane_view), 256) + 4096;
+    const size_t nc = n_sink_cells(p);
+    size_t b = nf_align_up((size_t)p.n_planes * sizeof(nf_plane_view), 256);
+    b += 2 * nf_align_up(nc * sizeof(uint32_t), 256);                               // tc, to
+    b += nf_align_up(nf_scan_temp_elems(nc) * sizeof(uint32_t), 256);               // scan temp
+    b += nf_align_up(max_tasks(p) * sizeof(Task), 256);                             // tasks
+    return b + 256 + 4096;
 }
 
 int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const uint64_t *off,
@@ -242,17 +433,54 @@ int nf_interactions_planes(nf_ctx *ctx, const nf_force_params &p, const nf_plane
     return NF_OK;
 }
 
+template <int R>
+static int launch_tile(nf_ctx *ctx, const nf_force_params &p, const ForceConsts &fc, const nf_plane_view *d_planes,
+                       const Task *tasks, uint32_t *ctl, cudaStream_t st)
+{
+    int occ = 0;
+    NF_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_forces_tile<R>, TILE_T, 0));
+    if (occ < 1) occ = 1;
+    const size_t want = max_tasks(p);
+    size_t blocks = (size_t)ctx->sm_count * occ;
+    if (blocks > want) blocks = want;
+    k_forces_tile<R><<<(unsigned)blocks, TILE_T, 0, st>>>(d_planes, p, fc, tasks, ctl);
+    NF_LAUNCHED(ctx);
+    return NF_OK;
+}
+
 int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d_planes,
                    cudaStream_t st, bool record_timing)
 {
     if (record_timing) NF_CUDA(ctx, cudaEventRecord(ctx->ev_total0, st));
     const ForceConsts fc = make_consts(p);
-    if (record_timing) NF_CUDA(ctx, cudaEventRecord(ctx->ev_kern0, st));
     const int n_sink_planes = p.sink_hi - p.sink_lo;
+    const size_t nc = n_sink_cells(p);
+    uint32_t *tc = nf_scratch_take<uint32_t>(ctx, nc ? nc : 1);
+    uint32_t *to = nf_scratch_take<uint32_t>(ctx, nc ? nc : 1);
+    uint32_t *tmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(nc));
+    Task *tasks = nf_scratch_take<Task>(ctx, max_tasks(p));
+    uint32_t *ctl = nf_scratch_take<uint32_t>(ctx, 2);
+    if (!tc || !to || !tmp || !tasks || !ctl) {
+        NF_SET_ERR(ctx, "nf_forces: internal scratch arena too small");
+        return NF_ERR_NOMEM;
+    }
     if (n_sink_planes > 0) {
-        dim3 grid((unsigned)(p.K * p.K), (unsigned)n_sink_planes);
-        k_forces_cell<<<grid, CELL_THREADS, 0, st>>>(d_planes, p, fc);
+        // work list
+        dim3 grid((unsigned)((p.K * p.K + 255) / 256), (unsigned)n_sink_planes);
+        k_task_count<<<grid, 256, 0, st>>>(d_planes, p, tc);
         NF_LAUNCHED(ctx);
+        NF_TRY(nf_exclusive_scan_u32(ctx, tc, to, nc, tmp, st));
+        k_task_fill<<<grid, 256, 0, st>>>(tc, to, p, tasks, ctl);
+        NF_LAUNCHED(ctx);
+    }
+    if (record_timing) NF_CUDA(ctx, cudaEventRecord(ctx->ev_kern0, st));
+    if (n_sink_planes > 0) {
+        switch (p.R) {
+        case 0: NF_TRY(launch_tile<0>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
+        case 1: NF_TRY(launch_tile<1>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
+        case 2: NF_TRY(launch_tile<2>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
+        default: NF_TRY(launch_tile<3>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
+        }
     }
     if (record_timing) {
         NF_CUDA(ctx, cudaEventRecord(ctx->ev_kern1, st));

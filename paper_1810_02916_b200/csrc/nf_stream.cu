@@ -142,9 +142,9 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
     }
     nf_force_params fp{};
     fp.K = K; fp.n_planes = NP; fp.periodic_x = 0; fp.R = R; fp.eps = eps; fp.box = box; fp.Gm = Gm; fp.softening = softening;
-    size_t scratch_need = nf_bin_scratch_bytes(max_n, K, true);
-    size_t fs = nf_forces_scratch_bytes(fp);
-    NF_TRY(nf_scratch_reserve(ctx, scratch_need > fs ? scratch_need : fs));
+    fp.sink_lo = 0; fp.sink_hi = 1; fp.max_sinks = max_n;     // one sink plane per nf_forces_impl call
+    // binning and the force work list of a plane take their scratch one after the other
+    NF_TRY(nf_scratch_reserve(ctx, nf_bin_scratch_bytes(max_n, K, true) + nf_forces_scratch_bytes(fp)));
 
     std::vector<Slot> slots(W);
     for (int s = 0; s < W; s++) {
