@@ -30,20 +30,6 @@ struct ForceConsts {
     int plummer;
 };
 
-// two-term compensated accumulation: (hi, lo) += x
-__device__ __forceinline__ void comp_add(float &hi, float &lo, float x)
-{
-    float s = hi + x;
-    float bb = s - hi;
-    float err = (hi - (s - bb)) + (x - bb);
-    hi = s;
-    lo += err;
-}
-
-struct PlaneTable {
-    const float4 *pos[1];  // flexible: n_planes entries follow in device memory
-};
-
 // ------------------------------------------------------------------------------------------
 // Packed FP32 (sm_100 FFMA2 / FADD2 / FMUL2): one 64-bit register holds the same quantity for
 // TWO SINKS; the source coordinate is a scalar operand broadcast to both halves (ptxas emits
@@ -83,21 +69,29 @@ __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64
     az = fma2(f, dz, az);
 }
 
+// q (a multiple of 4, >= 4) consecutive sources against the lane's two sinks; the loads of the
+// next group of four are issued before the arithmetic of the current one.
 template <int MODE>
 __device__ __forceinline__ void run_sources(const float4 *__restrict__ src, int q, const u64 xs, const u64 ys, const u64 zs,
                                             const ForceConsts &fc, u64 &ax, u64 &ay, u64 &az)
 {
-    int k = 0;
+    const float4 *end = src + q;
+    float4 a0 = src[0], a1 = src[1], a2 = src[2], a3 = src[3];
+    src += 4;
 #pragma unroll 1
-    for (; k + 4 <= q; k += 4) {
-        const float4 q0 = src[k], q1 = src[k + 1], q2 = src[k + 2], q3 = src[k + 3];
-        interact<MODE>(q0, xs, ys, zs, fc, ax, ay, az);
-        interact<MODE>(q1, xs, ys, zs, fc, ax, ay, az);
-        interact<MODE>(q2, xs, ys, zs, fc, ax, ay, az);
-        interact<MODE>(q3, xs, ys, zs, fc, ax, ay, az);
+    while (src < end) {
+        const float4 b0 = src[0], b1 = src[1], b2 = src[2], b3 = src[3];
+        src += 4;
+        interact<MODE>(a0, xs, ys, zs, fc, ax, ay, az);
+        interact<MODE>(a1, xs, ys, zs, fc, ax, ay, az);
+        interact<MODE>(a2, xs, ys, zs, fc, ax, ay, az);
+        interact<MODE>(a3, xs, ys, zs, fc, ax, ay, az);
+        a0 = b0; a1 = b1; a2 = b2; a3 = b3;
     }
-#pragma unroll 1
-    for (; k < q; k++) interact<MODE>(src[k], xs, ys, zs, fc, ax, ay, az);
+    interact<MODE>(a0, xs, ys, zs, fc, ax, ay, az);
+    interact<MODE>(a1, xs, ys, zs, fc, ax, ay, az);
+    interact<MODE>(a2, xs, ys, zs, fc, ax, ay, az);
+    interact<MODE>(a3, xs, ys, zs, fc, ax, ay, az);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -105,7 +99,7 @@ __device__ __forceinline__ void run_sources(const float4 *__restrict__ src, int 
 // ------------------------------------------------------------------------------------------
 constexpr int TILE_T = 128;                 // threads per block
 constexpr int TILE_SINKS = 2 * TILE_T;      // sinks per task at most (two per lane, one phase)
-constexpr int TILE_CAP = 512;               // sources staged per pass (float4 each)
+constexpr int TILE_CAP = 2048;              // float4 slots of the source buffer (32 KiB)
 
 struct Task {
     uint32_t cyz;     // cell index within the plane, cy*K + cz
@@ -150,31 +144,35 @@ __global__ void __launch_bounds__(256) k_task_fill(const uint32_t *__restrict__ 
 // Task = n <= 256 sinks of cell (plane, cy, cz).  Lane mapping: L = ceil(n/2) "sink lanes"
 // each hold two sinks in packed registers; the P = floor(T/L) "phases" split every source run
 // between them, so small cells still fill the block (lane use L*P/T).  For each of the
-// (2R+1)^2 source columns (dx, dy) the 2R+1 cells cz-R..cz+R are one z-run (contiguous in
-// memory because z is the fastest cell index; the periodic wrap splits it): the run is staged
-// through shared memory once, already multiplied by `scale` and with the z shift of its cell
-// added, so that same-cell differences stay exact, and every phase processes a
-// contiguous q = ceil(m/P) slice of it (missing entries are far-away sentinels: zero force).
+// (2R+1)^2 source columns (dx, dy) the 2R+1 cells cz-R..cz+R form one z-run (contiguous in
+// memory because z is the fastest cell index; the periodic wrap splits it).  A run of m sources
+// is staged into shared memory as P slices of q = roundup4(ceil(m/P)) slots, already multiplied
+// by `scale` and with the z shift of its cell added, so that same-cell differences stay exact
+// (PAPER.md:51); unused slots hold a far-away sentinel (zero force).  Several runs are staged
+// per pass (as many as fit the buffer), then every phase sweeps its slice of each run.
 // float32 partial sums per run, double outer sum over runs and phases; no atomics on floats.
 // ------------------------------------------------------------------------------------------
-struct RunTab {
-    unsigned long long start[2 * NF_MAX_R + 1];   // first particle of each cell segment
-    int cum[2 * NF_MAX_R + 2];                    // cumulative particle count before segment s
-    int pad_;
+template <int R>
+struct TaskTab {
+    static constexpr int W = 2 * R + 1;
+    uint32_t start[W * W][W];    // first particle of each cell segment, relative to its plane's arrays
+    int cum[W * W][W + 1];       // particles of the run before segment s; cum[r][W] = m_r
+    int px[W * W];               // plane of the run (-1: outside the open chunk)
+    int q[W * W];                // padded slice length of the run for this task's P
 };
 
 template <int R>
-__global__ void __launch_bounds__(TILE_T) k_forces_tile(const nf_plane_view *__restrict__ planes, const nf_force_params p, const ForceConsts fc,
-                                                        const Task *__restrict__ tasks, uint32_t *__restrict__ ctl)
+__global__ void __launch_bounds__(TILE_T, 6) k_forces_tile(const nf_plane_view *__restrict__ planes, const nf_force_params p, const ForceConsts fc,
+                                                           const Task *__restrict__ tasks, uint32_t *__restrict__ ctl)
 {
-    constexpr int W = 2 * R + 1;
+    constexpr int W = 2 * R + 1, NR = W * W;
     __shared__ __align__(16) float4 buf[TILE_CAP];
-    __shared__ RunTab tab[2];
+    __shared__ TaskTab<R> tab;
     __shared__ uint32_t s_task;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int K = p.K;
     const float w = (p.box / (float)K) * fc.scale;
-    const float SENT = 1.0e15f;   // sentinel source: r2 ~ 1e30, r^-3 flushes to zero
+    const float4 SENT = make_float4(1.0e15f, 1.0e15f, 1.0e15f, 0.f);   // r2 ~ 1e30: r^-3 flushes to zero
     const bool far_ok = !fc.plummer && w > 1.001f * sqrtf(fc.eps2);
 
     for (;;) {
@@ -194,6 +192,26 @@ __global__ void __launch_bounds__(TILE_T) k_forces_tile(const nf_plane_view *__r
         const int P = TILE_T / L;
         const int sl = tid % L, ph = tid / L;
         const bool active = ph < P;
+
+        // ---- segment table of the task: (run, cell of the z-window) -> start, count ----
+        for (int e = tid; e < NR * W; e += TILE_T) {
+            const int r = e / W, s = e - r * W;
+            const int dx = r / W - R, dy = r - (r / W) * W - R;
+            int px = sink_plane + dx;
+            if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
+            else if (px < 0 || px >= p.n_planes) px = -1;
+            uint32_t st = 0;
+            int cnt = 0;
+            if (px >= 0) {
+                const int qy = ((cy + dy) % K + K) % K, qz = ((cz + s - R) % K + K) % K;
+                const uint64_t *qo = planes[px].off + (size_t)qy * K + qz;
+                st = (uint32_t)qo[0];
+                cnt = (int)(qo[1] - qo[0]);
+            }
+            tab.start[r][s] = st;
+            tab.cum[r][s + 1] = cnt;      // counts first, prefix-summed below
+            if (s == 0) tab.px[r] = px;
+        }
         // the lane's two sinks (the second is a duplicate of the first when n is odd)
         const uint64_t i0 = s0 + 2 * (uint64_t)sl;
         const uint64_t i1 = (2 * sl + 1 < n) ? i0 + 1 : i0;
@@ -201,82 +219,97 @@ __global__ void __launch_bounds__(TILE_T) k_forces_tile(const nf_plane_view *__r
         const u64 xi = pk(m0.x * fc.scale, m1.x * fc.scale), yi = pk(m0.y * fc.scale, m1.y * fc.scale),
                   zi = pk(m0.z * fc.scale, m1.z * fc.scale);
         double ax0 = 0.0, ay0 = 0.0, az0 = 0.0, ax1 = 0.0, ay1 = 0.0, az1 = 0.0;
-
-        // segment table of a run: lanes 0..W-1 of warp 0 each look up one cell of the z-window
-        auto build_tab = [&](int r, RunTab &t) {
-            const int dx = r / W - R, dy = r % W - R;
-            int px = sink_plane + dx;
-            bool have = true;
-            if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
-            else if (px < 0 || px >= p.n_planes) { have = false; px = sink_plane; }
-            const int qy = ((cy + dy) % K + K) % K;
-            const int s = tid;     // segment index (only tid < W matter)
-            unsigned long long st = 0;
-            int cnt = 0;
-            if (s < W && have) {
-                const int qz = ((cz + s - R) % K + K) % K;
-                const uint64_t *qo = planes[px].off + (size_t)qy * K + qz;
-                st = qo[0];
-                cnt = (int)(qo[1] - st);
-            }
-            int inc = cnt;
+        __syncthreads();
+        if (tid < NR) {
+            int c = 0;
+            tab.cum[tid][0] = 0;
 #pragma unroll
-            for (int d = 1; d < 8; d <<= 1) {
-                int v = __shfl_up_sync(0xffffffffu, inc, d);
-                if ((tid & 31) >= d) inc += v;
-            }
-            if (s < W) { t.start[s] = st; t.cum[s] = inc - cnt; }
-            if (s == W - 1) t.cum[W] = inc;
-        };
-        if (tid < 32) build_tab(0, tab[0]);
+            for (int s = 1; s <= W; s++) { c += tab.cum[tid][s]; tab.cum[tid][s] = c; }
+            tab.q[tid] = ((c + P - 1) / P + 3) & ~3;
+        }
+        __syncthreads();
 
-        for (int r = 0; r < W * W; r++) {
-            const int dx = r / W - R, dy = r % W - R;
-            int px = sink_plane + dx;
-            if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
-            else if (px < 0 || px >= p.n_planes) px = sink_plane;   // run is empty (tab has m = 0)
-            const float4 *__restrict__ qpos = planes[px].pos;
-            const u64 xs = sub2(xi, pk((float)dx * w, (float)dx * w));   // sink in the source column's frame
-            const u64 ys = sub2(yi, pk((float)dy * w, (float)dy * w));
-            const bool near = !fc.plummer && (!far_ok || (dx >= -1 && dx <= 1 && dy >= -1 && dy <= 1));
-            u64 ax = 0, ay = 0, az = 0;
-            const RunTab &t = tab[r & 1];
-            bool first = true;
-            int m = 0;
-            for (int b0 = 0; first || b0 < m; first = false) {
-                __syncthreads();                       // previous pass is done with buf; tab[r&1] is visible
-                m = t.cum[W];
-                const int mc = min(m - b0, TILE_CAP - P);     // sources in this pass
-                const int q = (mc + P - 1) / P;               // per-phase slice (P*q <= TILE_CAP)
-                for (int i = tid; i < P * q; i += TILE_T) {
-                    float4 v = make_float4(SENT, SENT, SENT, 0.f);
-                    if (i < mc) {
-                        const int g = b0 + i;
-                        int s = 0;
-#pragma unroll
-                        for (int k = 1; k < W; k++) s += (g >= t.cum[k]);
-                        const float4 o = qpos[t.start[s] + (unsigned long long)(g - t.cum[s])];
-                        v.x = o.x * fc.scale;
-                        v.y = o.y * fc.scale;
-                        v.z = fmaf(o.z, fc.scale, (float)(s - R) * w);
+        // padded slice length of a run of m sources
+        auto slice = [&](int m) { return ((m + P - 1) / P + 3) & ~3; };
+        const int q_cap = (TILE_CAP / P) & ~3;            // longest slice the buffer can hold
+
+        int r = 0, m_done = 0;                            // next run, sources of it already processed
+        while (r < NR) {
+            // ---- choose the pass: whole runs r..r_end-1, or one piece of an oversized run ----
+            int r_end = r, slots = 0;
+            bool piece = false;
+            if (m_done == 0) {
+                while (r_end < NR) {
+                    const int need = P * tab.q[r_end];
+                    if (slots + need > TILE_CAP) break;
+                    slots += need;
+                    r_end++;
+                }
+            }
+            int mc = 0, qc = 0;
+            if (r_end == r) {                             // run r does not fit: take P*q_cap sources of it
+                piece = true;
+                mc = min(tab.cum[r][W] - m_done, P * q_cap);
+                qc = slice(mc);
+                r_end = r + 1;
+            }
+            __syncthreads();                              // the previous pass is done with buf
+            // ---- stage: one warp per cell segment, lanes over its particles ----
+            {
+                int base = 0;
+                for (int rr = r; rr < r_end; rr++) {
+                    const int m = piece ? mc : tab.cum[rr][W];
+                    const int q = piece ? qc : tab.q[rr];
+                    const int px = tab.px[rr];
+                    if (m > 0) {
+                        const float4 *__restrict__ qpos = planes[px].pos;
+                        for (int sg = warp; sg < W; sg += TILE_T / 32) {
+                            const int lo = tab.cum[rr][sg], hi = tab.cum[rr][sg + 1];
+                            const int a = max(lo, m_done), b = min(hi, m_done + m);     // part of the segment in this pass
+                            const uint32_t st = tab.start[rr][sg];
+                            const float zsh = (float)(sg - R) * w;
+                            for (int g = a + lane; g < b; g += 32) {
+                                const float4 o = qpos[st + (uint32_t)(g - lo)];
+                                buf[base + g - m_done] = make_float4(o.x * fc.scale, o.y * fc.scale, fmaf(o.z, fc.scale, zsh), 0.f);
+                            }
+                        }
+                        for (int i = m + tid; i < P * q; i += TILE_T) buf[base + i] = SENT;
                     }
-                    buf[i] = v;
+                    base += P * q;
                 }
-                if (b0 == 0 && tid < 32 && r + 1 < W * W) build_tab(r + 1, tab[(r + 1) & 1]);
-                __syncthreads();
-                if (active && q > 0) {
-                    if (near) run_sources<0>(buf + ph * q, q, xs, ys, zi, fc, ax, ay, az);
-                    else run_sources<1>(buf + ph * q, q, xs, ys, zi, fc, ax, ay, az);
-                }
-                b0 += mc > 0 ? mc : 1;
             }
-            float a, b;
-            upk(ax, a, b); ax0 += (double)a; ax1 += (double)b;
-            upk(ay, a, b); ay0 += (double)a; ay1 += (double)b;
-            upk(az, a, b); az0 += (double)a; az1 += (double)b;
+            __syncthreads();
+            // ---- compute: every phase sweeps its slice of each staged run ----
+            if (active) {
+                int base = 0;
+                for (int rr = r; rr < r_end; rr++) {
+                    const int m = piece ? mc : tab.cum[rr][W];
+                    if (m == 0) continue;
+                    const int q = piece ? qc : tab.q[rr];
+                    const int dx = rr / W - R, dy = rr - (rr / W) * W - R;
+                    const u64 xs = sub2(xi, pk((float)dx * w, (float)dx * w));   // sinks in the source column's frame
+                    const u64 ys = sub2(yi, pk((float)dy * w, (float)dy * w));
+                    const bool near = !fc.plummer && (!far_ok || (dx >= -1 && dx <= 1 && dy >= -1 && dy <= 1));
+                    u64 ax = 0, ay = 0, az = 0;
+                    const float4 *src = buf + base + ph * q;
+                    if (near) run_sources<0>(src, q, xs, ys, zi, fc, ax, ay, az);
+                    else run_sources<1>(src, q, xs, ys, zi, fc, ax, ay, az);
+                    float a, b;
+                    upk(ax, a, b); ax0 += (double)a; ax1 += (double)b;
+                    upk(ay, a, b); ay0 += (double)a; ay1 += (double)b;
+                    upk(az, a, b); az0 += (double)a; az1 += (double)b;
+                    base += P * q;
+                }
+            }
+            if (piece) {
+                m_done += mc;
+                if (m_done >= tab.cum[r][W]) { m_done = 0; r++; }
+            } else {
+                r = r_end;
+            }
         }
 
-        // reduce the phases (fixed order), scale and write
+        // ---- reduce the phases (fixed order), scale and write ----
         __syncthreads();
         double *red = reinterpret_cast<double *>(buf);       // [P][L][6] doubles <= 128*48 B = 6 KiB
         if (active) {
