@@ -5,8 +5,9 @@
 // PAPER.md:243 Eq. 2 compact spline, evaluated as min(10 - 15u + 6u^2, u^-3)/eps^3 (fn. 4, :239);
 // PAPER.md:233 Eq. 1 Plummer;  PAPER.md:51 cell-centred float32 offsets.
 //
-// k_task_count / k_task_fill build the work list (chunks of <= 256 sinks of one cell);
-// k_forces_tile is the interaction kernel (see the block comment above it).
+// k_encode                      scaled, z-block-encoded copy of the sorted offsets (TMA source)
+// k_task_count / k_task_fill    work list: tasks of 4L sinks of one cell, dense cells first
+// k_forces_warp                 the interaction kernel (see the block comment above it)
 #include "nf_common.cuh"
 
 namespace {
@@ -17,6 +18,12 @@ __device__ __forceinline__ float rsqrt_approx(float x)
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float min3(float a, float b, float c)
+{
+    float y;
+    asm("min.ftz.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c));   // FMNMX3 (sm_100)
+    return y;
+}
 
 // Force-law constants in internal units.  Positions are multiplied by `scale` = 2^k (exact)
 // with 2^k ~ 1/eps, so eps' = eps*scale lies in [2^-1/2, 2^1/2) and A, B, C are O(1..100)
@@ -24,17 +31,17 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 struct ForceConsts {
     float A, B, C;      // 10/eps'^3, -15/eps'^4, 6/eps'^5   (spline)
     float r2_floor;     // addend of r'^2: tiny (spline; keeps r = 0 finite) or eps'^2 (Plummer)
-    float eps2;         // eps'^2 (spline: below this the polynomial branch can win the min)
+    float eps2_test;    // spline: eps'^2 (+ margin); a tile whose smallest r'^2 is below it is redone with the min form.  Plummer: 0
     float scale;        // 2^k
+    float ws;           // cell width in internal units, (box / K) * scale
     float out_scale;    // Gm * scale^2: a = out_scale * sum f' d'
-    int plummer;
 };
 
 // ------------------------------------------------------------------------------------------
 // Packed FP32 (sm_100 FFMA2 / FADD2 / FMUL2): one 64-bit register holds the same quantity for
 // TWO SINKS; the source coordinate is a scalar operand broadcast to both halves (ptxas emits
-// the .F32 broadcast operand form, so no duplicating moves).  13 (spline) or 11 (r^-3 only)
-// FMA-pipe instructions per source serve two interactions per lane.
+// the .F32 broadcast operand form, so no duplicating moves).  11 FMA-pipe instructions per
+// source serve two interactions per lane (13 with the spline polynomial).
 // ------------------------------------------------------------------------------------------
 typedef unsigned long long u64;
 __device__ __forceinline__ u64 pk(float a, float b) { u64 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
@@ -43,11 +50,14 @@ __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.ft
 __device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 d; asm("sub.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 d; asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 
-// One source against the lane's two sinks.  MODE 0: spline, min(poly, r^-3); 1: r^-3 only
-// (valid when the cell separation guarantees r >= eps, or for Plummer where r2_floor = eps^2).
+// One source against two of the lane's sinks.
+// MODE 0: Eq. 2 as min(poly, r^-3).
+// MODE 1: r^-3 only, and the smallest r^2 seen is tracked in rmin: exact whenever no pair of
+//         the tile lies inside eps (the caller checks rmin and redoes the tile with MODE 0
+//         otherwise).  Also the Plummer law (r2_floor = eps^2, eps2_test = 0).
 template <int MODE>
 __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64 ys, const u64 zs, const ForceConsts &fc,
-                                         u64 &ax, u64 &ay, u64 &az)
+                                         u64 &ax, u64 &ay, u64 &az, float &rmin)
 {
     const u64 dx = sub2(pk(q.x, q.x), xs), dy = sub2(pk(q.y, q.y), ys), dz = sub2(pk(q.z, q.z), zs);
     u64 r2 = fma2(dz, dz, pk(fc.r2_floor, fc.r2_floor));
@@ -63,265 +73,412 @@ __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64
         upk(poly, pa, pb);
         upk(f, fa, fb);
         f = pk(fminf(pa, fa), fminf(pb, fb));
+    } else {
+        rmin = min3(rmin, r2a, r2b);
     }
     ax = fma2(f, dx, ax);
     ay = fma2(f, dy, ay);
     az = fma2(f, dz, az);
 }
 
-// q (a multiple of 4, >= 4) consecutive sources against the lane's two sinks; the loads of the
-// next group of four are issued before the arithmetic of the current one.
+// q (a multiple of 2, >= 2) consecutive sources against the lane's FOUR sinks (two packed
+// pairs); the loads of the next two sources are issued before the arithmetic of the current.
 template <int MODE>
-__device__ __forceinline__ void run_sources(const float4 *__restrict__ src, int q, const u64 xs, const u64 ys, const u64 zs,
-                                            const ForceConsts &fc, u64 &ax, u64 &ay, u64 &az)
+__device__ __forceinline__ void sweep(const float4 *__restrict__ src, int q, const u64 (&xs)[2], const u64 (&ys)[2], const u64 (&zs)[2],
+                                      const ForceConsts &fc, u64 (&ax)[2], u64 (&ay)[2], u64 (&az)[2], float &rmin)
 {
     const float4 *end = src + q;
-    float4 a0 = src[0], a1 = src[1], a2 = src[2], a3 = src[3];
-    src += 4;
+    float4 a0 = src[0], a1 = src[1];
+    src += 2;
 #pragma unroll 1
     while (src < end) {
-        const float4 b0 = src[0], b1 = src[1], b2 = src[2], b3 = src[3];
-        src += 4;
-        interact<MODE>(a0, xs, ys, zs, fc, ax, ay, az);
-        interact<MODE>(a1, xs, ys, zs, fc, ax, ay, az);
-        interact<MODE>(a2, xs, ys, zs, fc, ax, ay, az);
-        interact<MODE>(a3, xs, ys, zs, fc, ax, ay, az);
-        a0 = b0; a1 = b1; a2 = b2; a3 = b3;
+        const float4 b0 = src[0], b1 = src[1];
+        src += 2;
+        interact<MODE>(a0, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
+        interact<MODE>(a0, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
+        interact<MODE>(a1, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
+        interact<MODE>(a1, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
+        a0 = b0; a1 = b1;
     }
-    interact<MODE>(a0, xs, ys, zs, fc, ax, ay, az);
-    interact<MODE>(a1, xs, ys, zs, fc, ax, ay, az);
-    interact<MODE>(a2, xs, ys, zs, fc, ax, ay, az);
-    interact<MODE>(a3, xs, ys, zs, fc, ax, ay, az);
+    interact<MODE>(a0, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
+    interact<MODE>(a0, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
+    interact<MODE>(a1, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
+    interact<MODE>(a1, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
+}
+
+// ---- mbarrier / bulk-copy (TMA 1D) primitives --------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok)
+                     : "r"(bar), "r"(parity)
+                     : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// ------------------------------------------------------------------------------------------
+// Encoded positions.  The interaction kernel fetches source cells with bulk copies straight
+// into shared memory, so whatever a lane needs per source must already be in the array:
+//   enc.xy = offset.xy * scale                 (exact: scale is a power of two)
+//   enc.z  = offset.z * scale + e(cz) * ws,    e(cz) = (cz mod ZB) - (ZB-1)/2
+// i.e. z is measured from the centre of the cell's block of ZB = 8 cells, so that a whole run
+// of consecutive cells inside one z-block shares ONE shift of the sink coordinates.  |enc.z| <
+// 4 ws: the rounding of the encoding (<= 2^-23 ws) is the same size as that of the x/y column
+// shifts, and differences inside one cell stay exact.
+// ------------------------------------------------------------------------------------------
+constexpr int ZB = 8;
+
+__global__ void __launch_bounds__(256) k_encode(const float4 *__restrict__ pos, const uint64_t *__restrict__ off, size_t ncell, int K,
+                                                float scale, float ws, float4 *__restrict__ enc)
+{
+    const size_t c = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (c >= ncell) return;
+    const int lane = threadIdx.x & 31;
+    const uint64_t s0 = off[c], s1 = off[c + 1];
+    const int cz = (int)(c % (size_t)K);
+    const float ez = ((float)(cz % ZB) - 0.5f * (float)(ZB - 1)) * ws;
+    for (uint64_t s = s0 + lane; s < s1; s += 32) {
+        const float4 o = pos[s];
+        enc[s] = make_float4(o.x * scale, o.y * scale, fmaf(o.z, scale, ez), 0.f);
+    }
 }
 
 // ------------------------------------------------------------------------------------------
-// Work list.  A task is a chunk of <= TILE_SINKS consecutive sinks of ONE cell of a sink plane.
+// Work list.  A task is 4L consecutive sinks (L <= 32 lanes, four sinks each) of ONE cell; the
+// P = floor(32/L) "phases" of the warp split every source tile between them.  A cell of n
+// sinks becomes floor(n/128) full tasks (L = 32) plus the split of the remainder that
+// minimises  sum over tasks (1/P + C0)  -- warp time per source swept plus a fixed per-task
+// cost -- found by dynamic programming on the host (c_split).  Lane use is ~96 % for
+// Poisson(64) cells against ~91 % for an even split.
 // ------------------------------------------------------------------------------------------
-constexpr int TILE_T = 128;                 // threads per block
-constexpr int TILE_SINKS = 2 * TILE_T;      // sinks per task at most (two per lane, one phase)
-constexpr int TILE_CAP = 2048;              // float4 slots of the source buffer (32 KiB)
+constexpr int SPLIT_MAX = 4;       // tasks per remainder (< 128 sinks) at most
+constexpr int HEAVY_N = 256;       // cells with at least this many sinks are scheduled first
 
 struct Task {
     uint32_t cyz;     // cell index within the plane, cy*K + cz
+    uint32_t first;   // first sink of the task within the cell
     uint16_t plane;   // sink plane (index into the plane table)
-    uint16_t chunk;   // chunk of TILE_SINKS sinks within the cell
+    uint16_t L;       // lanes holding sinks (1..32); the task covers min(4L, n - first) sinks
 };
+
+struct SplitTable {
+    uint8_t nt[128];
+    uint8_t L[128][SPLIT_MAX];
+};
+__constant__ SplitTable c_split;
 
 __global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restrict__ planes, nf_force_params p, uint32_t *__restrict__ tc)
 {
     const int cyz = blockIdx.x * blockDim.x + threadIdx.x;
-    if (cyz >= p.K * p.K) return;
+    const int KK = p.K * p.K;
+    if (cyz >= KK) return;
+    const size_t nc = (size_t)gridDim.y * KK, c = (size_t)blockIdx.y * KK + cyz;
     const uint64_t *off = planes[p.sink_lo + blockIdx.y].off;
     const uint64_t n = off[cyz + 1] - off[cyz];
-    tc[(size_t)blockIdx.y * p.K * p.K + cyz] = (uint32_t)((n + TILE_SINKS - 1) / TILE_SINKS);
+    const uint32_t nt = (uint32_t)(n >> 7) + c_split.nt[n & 127];
+    const bool heavy = n >= HEAVY_N;
+    tc[c] = heavy ? nt : 0u;            // first half of the list: dense cells
+    tc[nc + c] = heavy ? 0u : nt;
 }
 
 // ctl[0] = work cursor (zeroed here), ctl[1] = number of tasks
-__global__ void __launch_bounds__(256) k_task_fill(const uint32_t *__restrict__ tc, const uint32_t *__restrict__ to, nf_force_params p,
-                                                   Task *__restrict__ tasks, uint32_t *__restrict__ ctl)
+__global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restrict__ planes, const uint32_t *__restrict__ tc,
+                                                   const uint32_t *__restrict__ to, nf_force_params p, Task *__restrict__ tasks,
+                                                   uint32_t *__restrict__ ctl)
 {
     const int cyz = blockIdx.x * blockDim.x + threadIdx.x;
     const int KK = p.K * p.K;
     if (cyz >= KK) return;
-    const size_t c = (size_t)blockIdx.y * KK + cyz;
-    const uint32_t n = tc[c], o = to[c];
-    for (uint32_t k = 0; k < n; k++) {
-        Task t;
-        t.cyz = (uint32_t)cyz;
-        t.plane = (uint16_t)(p.sink_lo + blockIdx.y);
-        t.chunk = (uint16_t)k;
-        tasks[o + k] = t;
+    const size_t nc = (size_t)gridDim.y * KK, c = (size_t)blockIdx.y * KK + cyz;
+    const uint64_t *off = planes[p.sink_lo + blockIdx.y].off;
+    const uint64_t n = off[cyz + 1] - off[cyz];
+    const size_t e = n >= HEAVY_N ? c : nc + c;
+    uint32_t o = to[e];
+    Task t;
+    t.cyz = (uint32_t)cyz;
+    t.plane = (uint16_t)(p.sink_lo + blockIdx.y);
+    uint32_t first = 0;
+    for (uint64_t k = 0; k < (n >> 7); k++) {
+        t.first = first;
+        t.L = 32;
+        tasks[o++] = t;
+        first += 128;
+    }
+    const int rem = (int)(n & 127);
+    for (int k = 0; k < c_split.nt[rem]; k++) {
+        t.first = first;
+        t.L = c_split.L[rem][k];
+        tasks[o++] = t;
+        first += 4u * t.L;
     }
     if (cyz == KK - 1 && blockIdx.y == gridDim.y - 1) {
         ctl[0] = 0;
-        ctl[1] = o + n;
+        ctl[1] = to[2 * nc - 1] + tc[2 * nc - 1];
     }
 }
 
 // ------------------------------------------------------------------------------------------
-// Interaction kernel.  Persistent blocks of TILE_T threads pull tasks from the work list.
+// Interaction kernel.  Every WARP is an independent worker: it pulls tasks from the work list,
+// streams the task's source cells through its own double-buffered shared-memory tiles with
+// bulk copies (cp.async.bulk + mbarrier; one lane issues, nobody stages by hand), and never
+// meets a block barrier.
 //
-// Task = n <= 256 sinks of cell (plane, cy, cz).  Lane mapping: L = ceil(n/2) "sink lanes"
-// each hold two sinks in packed registers; the P = floor(T/L) "phases" split every source run
-// between them, so small cells still fill the block (lane use L*P/T).  For each of the
-// (2R+1)^2 source columns (dx, dy) the 2R+1 cells cz-R..cz+R form one z-run (contiguous in
-// memory because z is the fastest cell index; the periodic wrap splits it).  A run of m sources
-// is staged into shared memory as P slices of q = roundup4(ceil(m/P)) slots, already multiplied
-// by `scale` and with the z shift of its cell added, so that same-cell differences stay exact
-// (PAPER.md:51); unused slots hold a far-away sentinel (zero force).  Several runs are staged
-// per pass (as many as fit the buffer), then every phase sweeps its slice of each run.
-// float32 partial sums per run, double outer sum over runs and phases; no atomics on floats.
+// Task = 4L sinks of cell (plane, cy, cz): lane = (sl, ph), sl < L holds sinks 4sl..4sl+3 as two
+// packed pairs, the P = floor(32/L) phases split every tile of sources between them.
+// Sources: for each of the (2R+1)^2 columns (dx, dy) the cells cz-R..cz+R are contiguous in
+// memory (z is the fastest cell index).  They are cut into "pieces" = maximal runs of cells that
+// are contiguous AND share one z shift (same z-block of the encoding, same periodic image), and
+// pieces into tiles of <= TILE_CAP - P*UNR sources.  Per tile the sink coordinates are shifted
+// into the tile's frame (x, y by the column offset, z by the piece's shift), the tail of the
+// buffer is padded with far-away sentinels (zero force) up to P equal slices, and each phase
+// sweeps its slice with broadcast LDS.128.
+// Spline: the sweep evaluates r^-3 only and tracks the smallest r^2; if any lane of the warp saw
+// a pair inside eps the tile is redone with the min form of Eq. 2 (and the rest of that column
+// uses the min form directly).  Exact, because the two laws agree for r >= eps.
+// float32 partial sums per tile, double outer sum over tiles and phases in a fixed order:
+// deterministic, no floating-point atomics.
 // ------------------------------------------------------------------------------------------
+constexpr int WARPS = 4;                    // warps per block (independent workers)
+constexpr int TILE_CAP = 512;               // float4 slots per tile buffer (8 KiB)
+constexpr int UNR = 2;                      // sources per sweep iteration
+
 template <int R>
-struct TaskTab {
-    static constexpr int W = 2 * R + 1;
-    uint32_t start[W * W][W];    // first particle of each cell segment, relative to its plane's arrays
-    int cum[W * W][W + 1];       // particles of the run before segment s; cum[r][W] = m_r
-    int px[W * W];               // plane of the run (-1: outside the open chunk)
-    int q[W * W];                // padded slice length of the run for this task's P
+struct WarpShared {
+    static constexpr int W = 2 * R + 1, NR = W * W;
+    float4 buf[2][TILE_CAP];
+    uint4 piece[NR * W];                    // x: first particle, y: count, z: column | (k + 128) << 8 | dxi << 16 | self << 24
+    const float4 *enc[W];                   // encoded positions of the W source planes (by dx + R; null = outside the chunk)
+    unsigned long long bar[2];
+};
+
+struct TileDesc {
+    uint32_t start, n, meta;                // n == 0: no more tiles
 };
 
 template <int R>
-__global__ void __launch_bounds__(TILE_T, 6) k_forces_tile(const nf_plane_view *__restrict__ planes, const nf_force_params p, const ForceConsts fc,
-                                                           const Task *__restrict__ tasks, uint32_t *__restrict__ ctl)
+__global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_view *__restrict__ planes, const nf_force_params p,
+                                                               const ForceConsts fc, const Task *__restrict__ tasks,
+                                                               uint32_t *__restrict__ ctl)
 {
     constexpr int W = 2 * R + 1, NR = W * W;
-    __shared__ __align__(16) float4 buf[TILE_CAP];
-    __shared__ TaskTab<R> tab;
-    __shared__ uint32_t s_task;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    WarpShared<R> &S = reinterpret_cast<WarpShared<R> *>(smem_raw)[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
     const int K = p.K;
-    const float w = (p.box / (float)K) * fc.scale;
     const float4 SENT = make_float4(1.0e15f, 1.0e15f, 1.0e15f, 0.f);   // r2 ~ 1e30: r^-3 flushes to zero
-    const bool far_ok = !fc.plummer && w > 1.001f * sqrtf(fc.eps2);
+    const uint32_t bar0 = smem_u32(&S.bar[0]), bar1 = smem_u32(&S.bar[1]);
+    const uint32_t n_tasks = ctl[1];
+
+    if (lane == 0) {
+        mbar_init(bar0, 1);
+        mbar_init(bar1, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    fence_proxy_async();
+    __syncwarp();
+    uint32_t parity = 0;                    // bit b: parity to wait for on buffer b
 
     for (;;) {
-        __syncthreads();
-        if (tid == 0) s_task = atomicAdd(&ctl[0], 1u);
-        __syncthreads();
-        const uint32_t ti = s_task;
-        if (ti >= ctl[1]) return;
+        uint32_t ti = 0;
+        if (lane == 0) ti = atomicAdd(&ctl[0], 1u);
+        ti = __shfl_sync(0xffffffffu, ti, 0);
+        if (ti >= n_tasks) return;
         const Task task = tasks[ti];
         const int sink_plane = task.plane;
         const int cy = (int)(task.cyz / (uint32_t)K), cz = (int)(task.cyz % (uint32_t)K);
         const nf_plane_view sp = planes[sink_plane];
         const uint64_t c0 = sp.off[task.cyz], c1 = sp.off[task.cyz + 1];
-        const uint64_t s0 = c0 + (uint64_t)task.chunk * TILE_SINKS;
-        const int n = (int)min((uint64_t)TILE_SINKS, c1 - s0);
-        const int L = (n + 1) >> 1;
-        const int P = TILE_T / L;
-        const int sl = tid % L, ph = tid / L;
+        const uint64_t s0 = c0 + task.first;
+        const int L = task.L;
+        const int n = (int)min((uint64_t)(4 * L), c1 - s0);
+        const int P = 32 / L;
+        const int sl = lane % L, ph = lane / L;
         const bool active = ph < P;
+        const int tile_max = TILE_CAP - P * UNR;
 
-        // ---- segment table of the task: (run, cell of the z-window) -> start, count ----
-        for (int e = tid; e < NR * W; e += TILE_T) {
-            const int r = e / W, s = e - r * W;
-            const int dx = r / W - R, dy = r - (r / W) * W - R;
-            int px = sink_plane + dx;
+        // ---- piece table: lane r builds the pieces of column r ----
+        if (lane < W) {
+            int px = sink_plane + lane - R;
             if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
             else if (px < 0 || px >= p.n_planes) px = -1;
-            uint32_t st = 0;
-            int cnt = 0;
-            if (px >= 0) {
-                const int qy = ((cy + dy) % K + K) % K, qz = ((cz + s - R) % K + K) % K;
-                const uint64_t *qo = planes[px].off + (size_t)qy * K + qz;
-                st = (uint32_t)qo[0];
-                cnt = (int)(qo[1] - qo[0]);
-            }
-            tab.start[r][s] = st;
-            tab.cum[r][s + 1] = cnt;      // counts first, prefix-summed below
-            if (s == 0) tab.px[r] = px;
+            S.enc[lane] = px >= 0 ? planes[px].enc : nullptr;
         }
-        // the lane's two sinks (the second is a duplicate of the first when n is odd)
-        const uint64_t i0 = s0 + 2 * (uint64_t)sl;
-        const uint64_t i1 = (2 * sl + 1 < n) ? i0 + 1 : i0;
-        const float4 m0 = sp.pos[i0], m1 = sp.pos[i1];
-        const u64 xi = pk(m0.x * fc.scale, m1.x * fc.scale), yi = pk(m0.y * fc.scale, m1.y * fc.scale),
-                  zi = pk(m0.z * fc.scale, m1.z * fc.scale);
-        double ax0 = 0.0, ay0 = 0.0, az0 = 0.0, ax1 = 0.0, ay1 = 0.0, az1 = 0.0;
-        __syncthreads();
-        if (tid < NR) {
-            int c = 0;
-            tab.cum[tid][0] = 0;
+        int n_pieces = 0;
+        for (int rb = 0; rb < NR; rb += 32) {
+            const int r = rb + lane;
+            uint32_t st[W], cn[W];
+            int kz[W];
+            bool newp[W];
+            int np = 0;
+            const int dxi = r / W, dyi = r - dxi * W;
+            if (r < NR) {
+                int px = sink_plane + dxi - R;
+                if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
+                else if (px < 0 || px >= p.n_planes) px = -1;
+                const int qy = ((cy + dyi - R) % K + K) % K;
+                const uint64_t *qo = px >= 0 ? planes[px].off + (size_t)qy * K : nullptr;
+                uint32_t prev_end = 0;
+                int prev_k = 0;
+                bool have = false;
 #pragma unroll
-            for (int s = 1; s <= W; s++) { c += tab.cum[tid][s]; tab.cum[tid][s] = c; }
-            tab.q[tid] = ((c + P - 1) / P + 3) & ~3;
-        }
-        __syncthreads();
-
-        // padded slice length of a run of m sources
-        auto slice = [&](int m) { return ((m + P - 1) / P + 3) & ~3; };
-        const int q_cap = (TILE_CAP / P) & ~3;            // longest slice the buffer can hold
-
-        int r = 0, m_done = 0;                            // next run, sources of it already processed
-        while (r < NR) {
-            // ---- choose the pass: whole runs r..r_end-1, or one piece of an oversized run ----
-            int r_end = r, slots = 0;
-            bool piece = false;
-            if (m_done == 0) {
-                while (r_end < NR) {
-                    const int need = P * tab.q[r_end];
-                    if (slots + need > TILE_CAP) break;
-                    slots += need;
-                    r_end++;
+                for (int s = 0; s < W; s++) {
+                    const int qz = ((cz + s - R) % K + K) % K;
+                    st[s] = 0; cn[s] = 0;
+                    if (qo) { st[s] = (uint32_t)qo[qz]; cn[s] = (uint32_t)(qo[qz + 1] - qo[qz]); }
+                    kz[s] = (s - R) - (qz % ZB) + (cz % ZB);
+                    const bool self = r == NR / 2 && s == R;      // the sinks' own cell: a piece of its own (flagged)
+                    newp[s] = cn[s] > 0 && (self || !(have && prev_end == st[s] && prev_k == kz[s]));
+                    if (cn[s] > 0) { have = !self; prev_end = st[s] + cn[s]; prev_k = kz[s]; }
+                    np += newp[s] ? 1 : 0;
                 }
             }
-            int mc = 0, qc = 0;
-            if (r_end == r) {                             // run r does not fit: take P*q_cap sources of it
-                piece = true;
-                mc = min(tab.cum[r][W] - m_done, P * q_cap);
-                qc = slice(mc);
-                r_end = r + 1;
+            int incl = np;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += v;
             }
-            __syncthreads();                              // the previous pass is done with buf
-            // ---- stage: one warp per cell segment, lanes over its particles ----
-            {
-                int base = 0;
-                for (int rr = r; rr < r_end; rr++) {
-                    const int m = piece ? mc : tab.cum[rr][W];
-                    const int q = piece ? qc : tab.q[rr];
-                    const int px = tab.px[rr];
-                    if (m > 0) {
-                        const float4 *__restrict__ qpos = planes[px].pos;
-                        for (int sg = warp; sg < W; sg += TILE_T / 32) {
-                            const int lo = tab.cum[rr][sg], hi = tab.cum[rr][sg + 1];
-                            const int a = max(lo, m_done), b = min(hi, m_done + m);     // part of the segment in this pass
-                            const uint32_t st = tab.start[rr][sg];
-                            const float zsh = (float)(sg - R) * w;
-                            for (int g = a + lane; g < b; g += 32) {
-                                const float4 o = qpos[st + (uint32_t)(g - lo)];
-                                buf[base + g - m_done] = make_float4(o.x * fc.scale, o.y * fc.scale, fmaf(o.z, fc.scale, zsh), 0.f);
-                            }
-                        }
-                        for (int i = m + tid; i < P * q; i += TILE_T) buf[base + i] = SENT;
+            int slot = n_pieces + incl - np - 1;
+            if (r < NR) {
+#pragma unroll
+                for (int s = 0; s < W; s++) {
+                    if (cn[s] == 0) continue;
+                    if (newp[s]) {
+                        slot++;
+                        const uint32_t self = (r == NR / 2 && s == R) ? 1u << 24 : 0u;
+                        S.piece[slot] = make_uint4(st[s], cn[s], (uint32_t)r | ((uint32_t)(kz[s] + 128) << 8) | ((uint32_t)dxi << 16) | self, 0u);
+                    } else {
+                        S.piece[slot].y += cn[s];
                     }
-                    base += P * q;
                 }
             }
-            __syncthreads();
-            // ---- compute: every phase sweeps its slice of each staged run ----
+            n_pieces += __shfl_sync(0xffffffffu, incl, 31);
+        }
+
+        // ---- the lane's four sinks (slots past n repeat the last sink; they are never written) ----
+        u64 xi[2], yi[2], zi[2];
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+            const int j0 = min(4 * sl + 2 * h, n - 1), j1 = min(4 * sl + 2 * h + 1, n - 1);
+            const float4 m0 = sp.enc[s0 + j0], m1 = sp.enc[s0 + j1];
+            xi[h] = pk(m0.x, m1.x); yi[h] = pk(m0.y, m1.y); zi[h] = pk(m0.z, m1.z);
+        }
+        double tot[12];
+#pragma unroll
+        for (int i = 0; i < 12; i++) tot[i] = 0.0;
+        __syncwarp();
+
+        // ---- tile cursor (warp-uniform) ----
+        int cur_piece = 0;
+        uint32_t cur_off = 0;
+        auto next_tile = [&]() {
+            TileDesc d;
+            d.start = 0; d.n = 0; d.meta = 0;
+            if (cur_piece < n_pieces) {
+                const uint4 pc = S.piece[cur_piece];
+                const uint32_t nt = (pc.y + tile_max - 1) / tile_max;          // balanced tiles
+                const uint32_t tl = (pc.y + nt - 1) / nt;
+                d.start = pc.x + cur_off;
+                d.n = min(tl, pc.y - cur_off);
+                d.meta = pc.z;
+                cur_off += d.n;
+                if (cur_off >= pc.y) { cur_piece++; cur_off = 0; }
+            }
+            return d;
+        };
+        auto issue = [&](const TileDesc &d, int b) {
+            if (d.n && lane == 0) {
+                fence_proxy_async();          // earlier generic accesses to the buffer (sentinels, reduction scratch) come first
+                const uint32_t bar = b ? bar1 : bar0;
+                mbar_expect_tx(bar, d.n * 16u);
+                bulk_g2s(smem_u32(&S.buf[b][0]), S.enc[(d.meta >> 16) & 0xff] + d.start, d.n * 16u, bar);
+            }
+        };
+
+        TileDesc d0 = next_tile();
+        issue(d0, 0);
+        TileDesc d1 = next_tile();
+        issue(d1, 1);
+        int b = 0, sticky_col = -1;
+        while (d0.n) {
+            mbar_wait(b ? bar1 : bar0, (parity >> b) & 1u);
+            parity ^= 1u << b;
+            float4 *buf = S.buf[b];
+            const int tn = (int)d0.n;
+            const int q = ((tn + P - 1) / P + UNR - 1) & ~(UNR - 1);
+            for (int i = tn + lane; i < P * q; i += 32) buf[i] = SENT;
+            __syncwarp();
+            const int col = (int)(d0.meta & 0xff), kzs = (int)((d0.meta >> 8) & 0xff) - 128;
+            const int dxi = col / W, dyi = col - dxi * W;
+            const float sx = (float)(dxi - R) * fc.ws, sy = (float)(dyi - R) * fc.ws, sz = (float)kzs * fc.ws;
+            u64 xs[2], ys[2], zs[2];
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                xs[h] = sub2(xi[h], pk(sx, sx));       // sinks in the tile's frame
+                ys[h] = sub2(yi[h], pk(sy, sy));
+                zs[h] = sub2(zi[h], pk(sz, sz));
+            }
+            u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
+            float rmin = 3.0e38f;
+            const float4 *src = buf + ph * q;
+            // the sinks' own cell holds every sink as a source (r = 0), which would always trip the
+            // close-pair test: it takes the min form directly, as does the rest of a column after a hit
+            const bool direct = sticky_col == col || (d0.meta >> 24) != 0;
             if (active) {
-                int base = 0;
-                for (int rr = r; rr < r_end; rr++) {
-                    const int m = piece ? mc : tab.cum[rr][W];
-                    if (m == 0) continue;
-                    const int q = piece ? qc : tab.q[rr];
-                    const int dx = rr / W - R, dy = rr - (rr / W) * W - R;
-                    const u64 xs = sub2(xi, pk((float)dx * w, (float)dx * w));   // sinks in the source column's frame
-                    const u64 ys = sub2(yi, pk((float)dy * w, (float)dy * w));
-                    const bool near = !fc.plummer && (!far_ok || (dx >= -1 && dx <= 1 && dy >= -1 && dy <= 1));
-                    u64 ax = 0, ay = 0, az = 0;
-                    const float4 *src = buf + base + ph * q;
-                    if (near) run_sources<0>(src, q, xs, ys, zi, fc, ax, ay, az);
-                    else run_sources<1>(src, q, xs, ys, zi, fc, ax, ay, az);
-                    float a, b;
-                    upk(ax, a, b); ax0 += (double)a; ax1 += (double)b;
-                    upk(ay, a, b); ay0 += (double)a; ay1 += (double)b;
-                    upk(az, a, b); az0 += (double)a; az1 += (double)b;
-                    base += P * q;
-                }
+                if (direct) sweep<0>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                else sweep<1>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
             }
-            if (piece) {
-                m_done += mc;
-                if (m_done >= tab.cum[r][W]) { m_done = 0; r++; }
-            } else {
-                r = r_end;
+            if (!direct && __any_sync(0xffffffffu, rmin < fc.eps2_test)) {
+                sticky_col = col;
+                ax[0] = ax[1] = ay[0] = ay[1] = az[0] = az[1] = 0;
+                if (active) sweep<0>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
             }
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                float a, c;
+                upk(ax[h], a, c); tot[6 * h + 0] += (double)a; tot[6 * h + 3] += (double)c;
+                upk(ay[h], a, c); tot[6 * h + 1] += (double)a; tot[6 * h + 4] += (double)c;
+                upk(az[h], a, c); tot[6 * h + 2] += (double)a; tot[6 * h + 5] += (double)c;
+            }
+            __syncwarp();                                  // every lane is done with buf
+            const TileDesc d2 = next_tile();
+            issue(d2, b);
+            d0 = d1;
+            d1 = d2;
+            b ^= 1;
         }
 
         // ---- reduce the phases (fixed order), scale and write ----
-        __syncthreads();
-        double *red = reinterpret_cast<double *>(buf);       // [P][L][6] doubles <= 128*48 B = 6 KiB
+        double *red = reinterpret_cast<double *>(&S.buf[0][0]);     // [P][L][12] doubles <= 3 KiB
         if (active) {
-            double *d = red + ((size_t)ph * L + sl) * 6;
-            d[0] = ax0; d[1] = ay0; d[2] = az0; d[3] = ax1; d[4] = ay1; d[5] = az1;
+            double *d = red + (size_t)(ph * L + sl) * 12;
+#pragma unroll
+            for (int i = 0; i < 12; i++) d[i] = tot[i];
         }
-        __syncthreads();
-        for (int i = tid; i < n; i += TILE_T) {
-            const int l = i >> 1, h = (i & 1) * 3;
+        __syncwarp();
+        for (int i = lane; i < n; i += 32) {
+            const int l = i >> 2, h = (i & 3) * 3;
             double sx = 0.0, sy = 0.0, sz = 0.0;
             for (int pp = 0; pp < P; pp++) {
-                const double *d = red + ((size_t)pp * L + l) * 6 + h;
+                const double *d = red + (size_t)(pp * L + l) * 12 + h;
                 sx += d[0]; sy += d[1]; sz += d[2];
             }
             if (sp.acc) {
@@ -332,6 +489,7 @@ __global__ void __launch_bounds__(TILE_T, 6) k_forces_tile(const nf_plane_view *
                 sp.acc[3 * o + 2] = (float)(sz * (double)fc.out_scale);
             }
         }
+        __syncwarp();
     }
 }
 
@@ -361,12 +519,14 @@ __global__ void __launch_bounds__(256) k_interactions(const uint32_t *__restrict
     if ((threadIdx.x & 31) == 0 && local) atomicAdd(out, local);  // integer atomics: order-independent
 }
 
-__global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, const uint64_t *off, const uint32_t *perm, float *acc)
+__global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, const float4 *enc, const uint64_t *off,
+                              const uint32_t *perm, float *acc)
 {
     int cx = blockIdx.x * blockDim.x + threadIdx.x;
     if (cx >= K) return;
     nf_plane_view v;
     v.pos = pos;
+    v.enc = enc;
     v.off = off + (size_t)cx * K * K;
     v.perm = perm;
     v.acc = acc;
@@ -414,15 +574,54 @@ ForceConsts make_consts(const nf_force_params &p)
     float scale = ldexpf(1.0f, -e);    // eps*scale in [0.5, 1)
     if (p.eps * scale < 0.70710678f) scale *= 2.0f;  // -> [0.7071, 1.4142)
     const double es = (double)p.eps * (double)scale;
+    const bool plummer = p.softening == NF_SOFT_PLUMMER;
     fc.scale = scale;
-    fc.plummer = p.softening == NF_SOFT_PLUMMER;
+    fc.ws = (p.box / (float)p.K) * scale;
     fc.A = (float)(10.0 / (es * es * es));
     fc.B = (float)(-15.0 / (es * es * es * es));
     fc.C = (float)(6.0 / (es * es * es * es * es));
-    fc.eps2 = (float)(es * es);
-    fc.r2_floor = fc.plummer ? fc.eps2 : 8.673617379884035e-19f;  // 2^-60
+    fc.r2_floor = plummer ? (float)(es * es) : 8.673617379884035e-19f;  // 2^-60
+    fc.eps2_test = plummer ? 0.0f : (float)(es * es * 1.0001);
     fc.out_scale = (float)((double)p.Gm * (double)scale * (double)scale);
     return fc;
+}
+
+// split of a remainder of n < 128 sinks into tasks of 4L sinks: minimise sum(1/P + C0), P = floor(32/L)
+void make_split_table(SplitTable &t)
+{
+    const double C0 = 0.02, INF = 1e30;
+    static double dp[SPLIT_MAX + 1][128];
+    static int ch[SPLIT_MAX + 1][128];
+    for (int k = 0; k <= SPLIT_MAX; k++)
+        for (int m = 0; m < 128; m++) { dp[k][m] = m == 0 ? 0.0 : INF; ch[k][m] = 0; }
+    for (int k = 1; k <= SPLIT_MAX; k++)
+        for (int m = 1; m < 128; m++) {
+            dp[k][m] = dp[k - 1][m];
+            ch[k][m] = 0;                                  // 0: use the (k-1)-task solution
+            for (int L = 1; L <= 32; L++) {
+                const int prev = m - 4 * L > 0 ? m - 4 * L : 0;
+                const double c = dp[k - 1][prev] + 1.0 / (32 / L) + C0;
+                if (c < dp[k][m] - 1e-12) { dp[k][m] = c; ch[k][m] = L; }
+            }
+        }
+    memset(&t, 0, sizeof(t));
+    for (int n = 1; n < 128; n++) {
+        int m = n, k = SPLIT_MAX, cnt = 0;
+        uint8_t Ls[SPLIT_MAX];
+        while (m > 0 && k > 0) {
+            const int L = ch[k][m];
+            if (L == 0) { k--; continue; }
+            Ls[cnt++] = (uint8_t)L;
+            m = m - 4 * L > 0 ? m - 4 * L : 0;
+            k--;
+        }
+        // largest tasks first, so that the last (smallest) one takes the cell's tail
+        for (int i = 0; i < cnt; i++)
+            for (int j = i + 1; j < cnt; j++)
+                if (Ls[j] > Ls[i]) { uint8_t x = Ls[i]; Ls[i] = Ls[j]; Ls[j] = x; }
+        t.nt[n] = (uint8_t)cnt;
+        for (int i = 0; i < cnt; i++) t.L[n][i] = Ls[i];
+    }
 }
 
 }  // namespace
@@ -434,7 +633,7 @@ static size_t n_sink_cells(const nf_force_params &p)
 }
 static size_t max_tasks(const nf_force_params &p)
 {
-    return n_sink_cells(p) + (size_t)(p.max_sinks > 0 ? p.max_sinks : 0) / TILE_SINKS + 1;
+    return n_sink_cells(p) * SPLIT_MAX + (size_t)(p.max_sinks > 0 ? p.max_sinks : 0) / 128 + 1;
 }
 
 // scratch taken by nf_forces_impl (work list) plus room for a plane table of n_planes views
@@ -442,16 +641,34 @@ size_t nf_forces_scratch_bytes(const nf_force_params &p)
 {
     const size_t nc = n_sink_cells(p);
     size_t b = nf_align_up((size_t)p.n_planes * sizeof(nf_plane_view), 256);
-    b += 2 * nf_align_up(nc * sizeof(uint32_t), 256);                               // tc, to
-    b += nf_align_up(nf_scan_temp_elems(nc) * sizeof(uint32_t), 256);               // scan temp
+    b += 2 * nf_align_up(2 * nc * sizeof(uint32_t), 256);                           // tc, to
+    b += nf_align_up(nf_scan_temp_elems(2 * nc) * sizeof(uint32_t), 256);           // scan temp
     b += nf_align_up(max_tasks(p) * sizeof(Task), 256);                             // tasks
     return b + 256 + 4096;
 }
 
-int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const uint64_t *off,
+int nf_forces_init(nf_ctx *ctx)
+{
+    SplitTable t;
+    make_split_table(t);
+    NF_CUDA(ctx, cudaMemcpyToSymbol(c_split, &t, sizeof(t)));
+    return NF_OK;
+}
+
+int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const uint64_t *off,
                         const uint32_t *perm, float *acc, cudaStream_t st)
 {
-    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, off, perm, acc);
+    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, enc, off, perm, acc);
+    NF_LAUNCHED(ctx);
+    return NF_OK;
+}
+
+int nf_encode_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, float4 *enc,
+                   cudaStream_t st)
+{
+    if (ncell == 0) return NF_OK;
+    const ForceConsts fc = make_consts(p);
+    k_encode<<<(unsigned)((ncell + 7) / 8), 256, 0, st>>>(pos, off, ncell, p.K, fc.scale, fc.ws, enc);
     NF_LAUNCHED(ctx);
     return NF_OK;
 }
@@ -467,16 +684,18 @@ int nf_interactions_planes(nf_ctx *ctx, const nf_force_params &p, const nf_plane
 }
 
 template <int R>
-static int launch_tile(nf_ctx *ctx, const nf_force_params &p, const ForceConsts &fc, const nf_plane_view *d_planes,
+static int launch_warp(nf_ctx *ctx, const nf_force_params &p, const ForceConsts &fc, const nf_plane_view *d_planes,
                        const Task *tasks, uint32_t *ctl, cudaStream_t st)
 {
+    const size_t smem = sizeof(WarpShared<R>) * WARPS;
+    NF_CUDA(ctx, cudaFuncSetAttribute(k_forces_warp<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    NF_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_forces_tile<R>, TILE_T, 0));
+    NF_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_forces_warp<R>, WARPS * 32, smem));
     if (occ < 1) occ = 1;
-    const size_t want = max_tasks(p);
+    const size_t want = (max_tasks(p) + WARPS - 1) / WARPS;
     size_t blocks = (size_t)ctx->sm_count * occ;
     if (blocks > want) blocks = want;
-    k_forces_tile<R><<<(unsigned)blocks, TILE_T, 0, st>>>(d_planes, p, fc, tasks, ctl);
+    k_forces_warp<R><<<(unsigned)blocks, WARPS * 32, smem, st>>>(d_planes, p, fc, tasks, ctl);
     NF_LAUNCHED(ctx);
     return NF_OK;
 }
@@ -488,9 +707,9 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
     const ForceConsts fc = make_consts(p);
     const int n_sink_planes = p.sink_hi - p.sink_lo;
     const size_t nc = n_sink_cells(p);
-    uint32_t *tc = nf_scratch_take<uint32_t>(ctx, nc ? nc : 1);
-    uint32_t *to = nf_scratch_take<uint32_t>(ctx, nc ? nc : 1);
-    uint32_t *tmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(nc));
+    uint32_t *tc = nf_scratch_take<uint32_t>(ctx, nc ? 2 * nc : 1);
+    uint32_t *to = nf_scratch_take<uint32_t>(ctx, nc ? 2 * nc : 1);
+    uint32_t *tmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(2 * nc));
     Task *tasks = nf_scratch_take<Task>(ctx, max_tasks(p));
     uint32_t *ctl = nf_scratch_take<uint32_t>(ctx, 2);
     if (!tc || !to || !tmp || !tasks || !ctl) {
@@ -502,17 +721,17 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
         dim3 grid((unsigned)((p.K * p.K + 255) / 256), (unsigned)n_sink_planes);
         k_task_count<<<grid, 256, 0, st>>>(d_planes, p, tc);
         NF_LAUNCHED(ctx);
-        NF_TRY(nf_exclusive_scan_u32(ctx, tc, to, nc, tmp, st));
-        k_task_fill<<<grid, 256, 0, st>>>(tc, to, p, tasks, ctl);
+        NF_TRY(nf_exclusive_scan_u32(ctx, tc, to, 2 * nc, tmp, st));
+        k_task_fill<<<grid, 256, 0, st>>>(d_planes, tc, to, p, tasks, ctl);
         NF_LAUNCHED(ctx);
     }
     if (record_timing) NF_CUDA(ctx, cudaEventRecord(ctx->ev_kern0, st));
     if (n_sink_planes > 0) {
         switch (p.R) {
-        case 0: NF_TRY(launch_tile<0>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
-        case 1: NF_TRY(launch_tile<1>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
-        case 2: NF_TRY(launch_tile<2>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
-        default: NF_TRY(launch_tile<3>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
+        case 0: NF_TRY(launch_warp<0>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
+        case 1: NF_TRY(launch_warp<1>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
+        case 2: NF_TRY(launch_warp<2>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
+        default: NF_TRY(launch_warp<3>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
         }
     }
     if (record_timing) {
