@@ -48,6 +48,7 @@ __device__ __forceinline__ u64 pk(float a, float b) { u64 r; asm("mov.b64 %0, {%
 __device__ __forceinline__ void upk(u64 r, float &a, float &b) { asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(r)); }
 __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
 __device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 d; asm("sub.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 d; asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 d; asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 
 // One source against two of the lane's sinks.
@@ -82,28 +83,38 @@ __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64
 }
 
 // q (a multiple of 2, >= 2) consecutive sources against the lane's FOUR sinks (two packed
-// pairs); the loads of the next two sources are issued before the arithmetic of the current.
+// pairs).  Two register sets alternate (the loads of the next two sources are issued before
+// the arithmetic of the current two), so no register is moved.
+template <int MODE>
+__device__ __forceinline__ void pair4(const float4 a0, const float4 a1, const u64 (&xs)[2], const u64 (&ys)[2], const u64 (&zs)[2],
+                                      const ForceConsts &fc, u64 (&ax)[2], u64 (&ay)[2], u64 (&az)[2], float &rmin)
+{
+    interact<MODE>(a0, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
+    interact<MODE>(a0, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
+    interact<MODE>(a1, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
+    interact<MODE>(a1, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
+}
 template <int MODE>
 __device__ __forceinline__ void sweep(const float4 *__restrict__ src, int q, const u64 (&xs)[2], const u64 (&ys)[2], const u64 (&zs)[2],
                                       const ForceConsts &fc, u64 (&ax)[2], u64 (&ay)[2], u64 (&az)[2], float &rmin)
 {
     const float4 *end = src + q;
-    float4 a0 = src[0], a1 = src[1];
-    src += 2;
-#pragma unroll 1
-    while (src < end) {
-        const float4 b0 = src[0], b1 = src[1];
+    if (q & 2) {
+        const float4 c0 = src[0], c1 = src[1];
+        pair4<MODE>(c0, c1, xs, ys, zs, fc, ax, ay, az, rmin);
         src += 2;
-        interact<MODE>(a0, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
-        interact<MODE>(a0, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
-        interact<MODE>(a1, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
-        interact<MODE>(a1, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
-        a0 = b0; a1 = b1;
     }
-    interact<MODE>(a0, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
-    interact<MODE>(a0, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
-    interact<MODE>(a1, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
-    interact<MODE>(a1, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
+    if (src < end) {
+        float4 a0 = src[0], a1 = src[1];
+#pragma unroll 1
+        do {
+            const float4 b0 = src[2], b1 = src[3];
+            pair4<MODE>(a0, a1, xs, ys, zs, fc, ax, ay, az, rmin);
+            a0 = src[4]; a1 = src[5];          // past the slice in the last round: loaded, never used
+            src += 4;
+            pair4<MODE>(b0, b1, xs, ys, zs, fc, ax, ay, az, rmin);
+        } while (src < end);
+    }
 }
 
 // ---- mbarrier / bulk-copy (TMA 1D) primitives --------------------------------------------
@@ -310,9 +321,10 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
         const int L = task.L;
         const int n = (int)min((uint64_t)(4 * L), c1 - s0);
         const int P = 32 / L;
+        const uint32_t inv_P = (65536u + P - 1) / P;     // floor(x / P) == (x * inv_P) >> 16 for x < 1024
         const int sl = lane % L, ph = lane / L;
         const bool active = ph < P;
-        const int tile_max = TILE_CAP - P * UNR;
+        const int tile_max = TILE_CAP - P * UNR - 2;   // 2 slots of slack: the sweep loads one pair ahead
 
         // ---- piece table: lane r builds the pieces of column r ----
         if (lane < W) {
@@ -386,6 +398,14 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
         for (int i = 0; i < 12; i++) tot[i] = 0.0;
         __syncwarp();
 
+        // balanced tile length of every piece (no division on the per-tile path)
+        for (int i = lane; i < n_pieces; i += 32) {
+            const uint32_t cnt = S.piece[i].y;
+            const uint32_t nt = (cnt + tile_max - 1) / tile_max;
+            S.piece[i].w = (cnt + nt - 1) / nt;
+        }
+        __syncwarp();
+
         // ---- tile cursor (warp-uniform) ----
         int cur_piece = 0;
         uint32_t cur_off = 0;
@@ -394,10 +414,8 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             d.start = 0; d.n = 0; d.meta = 0;
             if (cur_piece < n_pieces) {
                 const uint4 pc = S.piece[cur_piece];
-                const uint32_t nt = (pc.y + tile_max - 1) / tile_max;          // balanced tiles
-                const uint32_t tl = (pc.y + nt - 1) / nt;
                 d.start = pc.x + cur_off;
-                d.n = min(tl, pc.y - cur_off);
+                d.n = min(pc.w, pc.y - cur_off);
                 d.meta = pc.z;
                 cur_off += d.n;
                 if (cur_off >= pc.y) { cur_piece++; cur_off = 0; }
@@ -412,22 +430,30 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                 bulk_g2s(smem_u32(&S.buf[b][0]), S.enc[(d.meta >> 16) & 0xff] + d.start, d.n * 16u, bar);
             }
         };
+        // float32 sums of the tiles of one dx plane, flushed into the double totals when dx changes
+        u64 gx[2] = {0, 0}, gy[2] = {0, 0}, gz[2] = {0, 0};
+        auto flush_group = [&]() {
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                float a, c;
+                upk(gx[h], a, c); tot[6 * h + 0] += (double)a; tot[6 * h + 3] += (double)c;
+                upk(gy[h], a, c); tot[6 * h + 1] += (double)a; tot[6 * h + 4] += (double)c;
+                upk(gz[h], a, c); tot[6 * h + 2] += (double)a; tot[6 * h + 5] += (double)c;
+                gx[h] = gy[h] = gz[h] = 0;
+            }
+        };
 
         TileDesc d0 = next_tile();
         issue(d0, 0);
         TileDesc d1 = next_tile();
         issue(d1, 1);
-        int b = 0, sticky_col = -1;
+        int b = 0, sticky_col = -1, g_dxi = 0;
         while (d0.n) {
-            mbar_wait(b ? bar1 : bar0, (parity >> b) & 1u);
-            parity ^= 1u << b;
-            float4 *buf = S.buf[b];
             const int tn = (int)d0.n;
-            const int q = ((tn + P - 1) / P + UNR - 1) & ~(UNR - 1);
-            for (int i = tn + lane; i < P * q; i += 32) buf[i] = SENT;
-            __syncwarp();
-            const int col = (int)(d0.meta & 0xff), kzs = (int)((d0.meta >> 8) & 0xff) - 128;
-            const int dxi = col / W, dyi = col - dxi * W;
+            const int q = ((int)(((uint32_t)(tn + P - 1) * inv_P) >> 16) + UNR - 1) & ~(UNR - 1);   // ceil(tn / P), even
+            const int col = (int)(d0.meta & 0xff), kzs = (int)((d0.meta >> 8) & 0xff) - 128, dxi = (int)((d0.meta >> 16) & 0xff);
+            const int dyi = col - dxi * W;
+            if (dxi != g_dxi) { flush_group(); g_dxi = dxi; }
             const float sx = (float)(dxi - R) * fc.ws, sy = (float)(dyi - R) * fc.ws, sz = (float)kzs * fc.ws;
             u64 xs[2], ys[2], zs[2];
 #pragma unroll
@@ -436,6 +462,11 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                 ys[h] = sub2(yi[h], pk(sy, sy));
                 zs[h] = sub2(zi[h], pk(sz, sz));
             }
+            float4 *buf = S.buf[b];
+            for (int i = tn + lane; i < P * q; i += 32) buf[i] = SENT;     // slots the bulk copy does not write
+            mbar_wait(b ? bar1 : bar0, (parity >> b) & 1u);
+            parity ^= 1u << b;
+            __syncwarp();
             u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
             float rmin = 3.0e38f;
             const float4 *src = buf + ph * q;
@@ -453,10 +484,9 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             }
 #pragma unroll
             for (int h = 0; h < 2; h++) {
-                float a, c;
-                upk(ax[h], a, c); tot[6 * h + 0] += (double)a; tot[6 * h + 3] += (double)c;
-                upk(ay[h], a, c); tot[6 * h + 1] += (double)a; tot[6 * h + 4] += (double)c;
-                upk(az[h], a, c); tot[6 * h + 2] += (double)a; tot[6 * h + 5] += (double)c;
+                gx[h] = add2(gx[h], ax[h]);
+                gy[h] = add2(gy[h], ay[h]);
+                gz[h] = add2(gz[h], az[h]);
             }
             __syncwarp();                                  // every lane is done with buf
             const TileDesc d2 = next_tile();
@@ -465,6 +495,7 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             d1 = d2;
             b ^= 1;
         }
+        flush_group();
 
         // ---- reduce the phases (fixed order), scale and write ----
         double *red = reinterpret_cast<double *>(&S.buf[0][0]);     // [P][L][12] doubles <= 3 KiB
