@@ -188,10 +188,14 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--n-side", type=int, default=0,
+                    help="profiling aid: the same recipe at n_side^3 particles and K = n_side/4 (not the bench workload)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = max(args.warmup, 0)
     cfg = inputs.config(args.config)
+    if args.n_side:
+        cfg = inputs.scaled(cfg, args.n_side ** 3, args.n_side // 4)
 
     if args.impl == "reference":
         run_reference(args, cfg)

@@ -92,8 +92,9 @@ int nf_reserve(nf_ctx *ctx, int64_t maxN, int K);
  * multiply-add:  invw = (float)K / box;  c = (int)floorf(x * invw) clamped to [0, K-1];
  * hw = 0.5f * (box / (float)K);  centre = (float)(2c+1) * hw;  offset = x - centre.
  * Ties (same cell) keep their input order (perm increases within a cell), so the output is
- * unique.  Particles outside [0, box) (or NaN) are clamped into the edge cell and counted;
- * read the count with nf_out_of_range().
+ * unique.  Particles whose coordinate is outside [0, box) (or NaN) are clamped into the edge
+ * cell and counted; read the count with nf_out_of_range().  A coordinate just below box whose
+ * product x * invw rounds up to K is valid: it lands in cell K-1 and is not counted.
  */
 int nf_bin(nf_ctx *ctx, const float *pos_xyz, int64_t N, int K, float box,
            float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,

@@ -41,12 +41,14 @@
 /* ---- cell assignment: "every particle belongs to one cell" ------------------
  * Float32 contract: invw = (float)K / box (one float32 division);
  * t = x * invw (one float32 multiply); c = (int)floorf(t), clamped to [0, K-1].
- * Returns 1 if the unclamped index was outside [0, K-1] (or x was NaN). */
-static int cell_of(float x, float invw, int K, int *c_out)
+ * Returns 1 if x itself is outside [0, box) or NaN (reading c9).  An x just below
+ * box whose product x*invw rounds up to K is a valid position: it is clamped into cell K-1 and
+ * NOT reported. */
+static int cell_of(float x, float invw, float box, int K, int *c_out)
 {
     float t = x * invw;
     float fl = floorf(t);
-    int bad = !(fl >= 0.0f && fl <= (float)(K - 1));
+    int bad = !(x >= 0.0f && x < box);
     int c;
     if (!(fl >= 0.0f)) c = 0;               /* negative or NaN */
     else if (fl > (float)(K - 1)) c = K - 1;
@@ -62,9 +64,9 @@ int64_t nfo_keys(const float *pos, int64_t N, int K, float box, uint32_t *key)
     int64_t nbad = 0;
     for (int64_t i = 0; i < N; i++) {
         int cx, cy, cz;
-        int b = cell_of(pos[3 * i + 0], invw, K, &cx);
-        b |= cell_of(pos[3 * i + 1], invw, K, &cy);
-        b |= cell_of(pos[3 * i + 2], invw, K, &cz);
+        int b = cell_of(pos[3 * i + 0], invw, box, K, &cx);
+        b |= cell_of(pos[3 * i + 1], invw, box, K, &cy);
+        b |= cell_of(pos[3 * i + 2], invw, box, K, &cz);
         key[i] = (uint32_t)(((int64_t)cx * K + cy) * K + cz);
         nbad += b;
     }

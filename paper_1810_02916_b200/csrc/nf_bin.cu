@@ -27,10 +27,12 @@ constexpr int RS_TILE = RS_WARPS * RS_WARP_ELEMS;   // 4096
 
 // float32 cell index, include/nf.h contract: c = (int)floorf(x * invw) clamped to [0, K-1].
 // __fmul_rn is never contracted into an FMA.
-__device__ __forceinline__ int cell_index(float x, float invw, int K, int *bad)
+// "Out of range" is x outside [0, box) or NaN; an x just below box whose product rounds up to K
+// is valid and silently clamped into cell K-1 (reading c9).
+__device__ __forceinline__ int cell_index(float x, float invw, float box, int K, int *bad)
 {
     float fl = floorf(__fmul_rn(x, invw));
-    int b = !(fl >= 0.0f && fl <= (float)(K - 1));
+    int b = !(x >= 0.0f && x < box);
     int c;
     if (!(fl >= 0.0f)) c = 0;
     else if (fl > (float)(K - 1)) c = K - 1;
@@ -39,7 +41,7 @@ __device__ __forceinline__ int cell_index(float x, float invw, int K, int *bad)
     return c;
 }
 
-__global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pos, int64_t N, int K, float invw, int plane_cx,
+__global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pos, int64_t N, int K, float invw, float box, int plane_cx,
                                               uint32_t *__restrict__ keys, uint32_t *__restrict__ cell_count,
                                               unsigned long long *__restrict__ n_bad)
 {
@@ -47,9 +49,9 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pos, int
     int bad = 0;
     if (i < N) {
         float x = pos[3 * i + 0], y = pos[3 * i + 1], z = pos[3 * i + 2];
-        int cx = cell_index(x, invw, K, &bad);
-        int cy = cell_index(y, invw, K, &bad);
-        int cz = cell_index(z, invw, K, &bad);
+        int cx = cell_index(x, invw, box, K, &bad);
+        int cy = cell_index(y, invw, box, K, &bad);
+        int cz = cell_index(z, invw, box, K, &bad);
         uint32_t key;
         if (plane_cx >= 0) {
             bad |= (cx != plane_cx);
@@ -209,7 +211,7 @@ int nf_bin_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, int 
     NF_CUDA(ctx, cudaMemsetAsync(cell_count, 0, ncell * sizeof(uint32_t), st));
     if (N > 0) {
         float invw = (float)K / box;
-        k_keys<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, N, K, invw, plane_cx, keysA, cell_count, ctx->counters);
+        k_keys<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, N, K, invw, box, plane_cx, keysA, cell_count, ctx->counters);
         NF_LAUNCHED(ctx);
     }
     NF_TRY(nf_exclusive_scan_u32_u64(ctx, cell_count, cell_offset, ncell, tmp64, st));

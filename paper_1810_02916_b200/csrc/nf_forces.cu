@@ -47,6 +47,7 @@ typedef unsigned long long u64;
 __device__ __forceinline__ u64 pk(float a, float b) { u64 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
 __device__ __forceinline__ void upk(u64 r, float &a, float &b) { asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(r)); }
 __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ void fma2_acc(u64 &acc, u64 a, u64 b) { asm("fma.rn.ftz.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b)); }
 __device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 d; asm("sub.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 d; asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 d; asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
@@ -77,9 +78,9 @@ __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64
     } else {
         rmin = min3(rmin, r2a, r2b);
     }
-    ax = fma2(f, dx, ax);
-    ay = fma2(f, dy, ay);
-    az = fma2(f, dz, az);
+    fma2_acc(ax, f, dx);
+    fma2_acc(ay, f, dy);
+    fma2_acc(az, f, dz);
 }
 
 // q (a multiple of 2, >= 2) consecutive sources against the lane's FOUR sinks (two packed
@@ -106,7 +107,7 @@ __device__ __forceinline__ void sweep(const float4 *__restrict__ src, int q, con
     }
     if (src < end) {
         float4 a0 = src[0], a1 = src[1];
-#pragma unroll 1
+#pragma unroll 2
         do {
             const float4 b0 = src[2], b1 = src[3];
             pair4<MODE>(a0, a1, xs, ys, zs, fc, ax, ay, az, rmin);
@@ -340,7 +341,10 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             int kz[W];
             bool newp[W];
             int np = 0;
-            const int dxi = r / W, dyi = r - dxi * W;
+            // columns are visited in mirror pairs (0, NR-1, 1, NR-2, ...) so that the running float32
+            // sums stay near the net force instead of growing to a half-space sum and cancelling later
+            const int col = (r & 1) ? NR - 1 - (r >> 1) : (r >> 1);
+            const int dxi = col / W, dyi = col - dxi * W;
             if (r < NR) {
                 int px = sink_plane + dxi - R;
                 if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
@@ -356,7 +360,7 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                     st[s] = 0; cn[s] = 0;
                     if (qo) { st[s] = (uint32_t)qo[qz]; cn[s] = (uint32_t)(qo[qz + 1] - qo[qz]); }
                     kz[s] = (s - R) - (qz % ZB) + (cz % ZB);
-                    const bool self = r == NR / 2 && s == R;      // the sinks' own cell: a piece of its own (flagged)
+                    const bool self = col == NR / 2 && s == R;    // the sinks' own cell: a piece of its own (flagged)
                     newp[s] = cn[s] > 0 && (self || !(have && prev_end == st[s] && prev_k == kz[s]));
                     if (cn[s] > 0) { have = !self; prev_end = st[s] + cn[s]; prev_k = kz[s]; }
                     np += newp[s] ? 1 : 0;
@@ -375,8 +379,8 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                     if (cn[s] == 0) continue;
                     if (newp[s]) {
                         slot++;
-                        const uint32_t self = (r == NR / 2 && s == R) ? 1u << 24 : 0u;
-                        S.piece[slot] = make_uint4(st[s], cn[s], (uint32_t)r | ((uint32_t)(kz[s] + 128) << 8) | ((uint32_t)dxi << 16) | self, 0u);
+                        const uint32_t self = (col == NR / 2 && s == R) ? 1u << 24 : 0u;
+                        S.piece[slot] = make_uint4(st[s], cn[s], (uint32_t)col | ((uint32_t)(kz[s] + 128) << 8) | ((uint32_t)dxi << 16) | self, 0u);
                     } else {
                         S.piece[slot].y += cn[s];
                     }
@@ -393,9 +397,6 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             const float4 m0 = sp.enc[s0 + j0], m1 = sp.enc[s0 + j1];
             xi[h] = pk(m0.x, m1.x); yi[h] = pk(m0.y, m1.y); zi[h] = pk(m0.z, m1.z);
         }
-        double tot[12];
-#pragma unroll
-        for (int i = 0; i < 12; i++) tot[i] = 0.0;
         __syncwarp();
 
         // balanced tile length of every piece (no division on the per-tile path)
@@ -430,30 +431,19 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                 bulk_g2s(smem_u32(&S.buf[b][0]), S.enc[(d.meta >> 16) & 0xff] + d.start, d.n * 16u, bar);
             }
         };
-        // float32 sums of the tiles of one dx plane, flushed into the double totals when dx changes
+        // running float32 sums over the task's tiles (per-tile sums are formed from zero and added here)
         u64 gx[2] = {0, 0}, gy[2] = {0, 0}, gz[2] = {0, 0};
-        auto flush_group = [&]() {
-#pragma unroll
-            for (int h = 0; h < 2; h++) {
-                float a, c;
-                upk(gx[h], a, c); tot[6 * h + 0] += (double)a; tot[6 * h + 3] += (double)c;
-                upk(gy[h], a, c); tot[6 * h + 1] += (double)a; tot[6 * h + 4] += (double)c;
-                upk(gz[h], a, c); tot[6 * h + 2] += (double)a; tot[6 * h + 5] += (double)c;
-                gx[h] = gy[h] = gz[h] = 0;
-            }
-        };
 
         TileDesc d0 = next_tile();
         issue(d0, 0);
         TileDesc d1 = next_tile();
         issue(d1, 1);
-        int b = 0, sticky_col = -1, g_dxi = 0;
+        int b = 0, sticky_col = -1;
         while (d0.n) {
             const int tn = (int)d0.n;
             const int q = ((int)(((uint32_t)(tn + P - 1) * inv_P) >> 16) + UNR - 1) & ~(UNR - 1);   // ceil(tn / P), even
             const int col = (int)(d0.meta & 0xff), kzs = (int)((d0.meta >> 8) & 0xff) - 128, dxi = (int)((d0.meta >> 16) & 0xff);
             const int dyi = col - dxi * W;
-            if (dxi != g_dxi) { flush_group(); g_dxi = dxi; }
             const float sx = (float)(dxi - R) * fc.ws, sy = (float)(dyi - R) * fc.ws, sz = (float)kzs * fc.ws;
             u64 xs[2], ys[2], zs[2];
 #pragma unroll
@@ -495,14 +485,17 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             d1 = d2;
             b ^= 1;
         }
-        flush_group();
-
         // ---- reduce the phases (fixed order), scale and write ----
         double *red = reinterpret_cast<double *>(&S.buf[0][0]);     // [P][L][12] doubles <= 3 KiB
         if (active) {
             double *d = red + (size_t)(ph * L + sl) * 12;
 #pragma unroll
-            for (int i = 0; i < 12; i++) d[i] = tot[i];
+            for (int h = 0; h < 2; h++) {
+                float a, c;
+                upk(gx[h], a, c); d[6 * h + 0] = (double)a; d[6 * h + 3] = (double)c;
+                upk(gy[h], a, c); d[6 * h + 1] = (double)a; d[6 * h + 4] = (double)c;
+                upk(gz[h], a, c); d[6 * h + 2] = (double)a; d[6 * h + 5] = (double)c;
+            }
         }
         __syncwarp();
         for (int i = lane; i < n; i += 32) {

@@ -1,0 +1,133 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times
+(nf_bin + nf_forces through the C ABI on the whole box), checked on sampled outputs the oracle
+can compute one by one, plus properties that hold at any size:
+
+  - C2 (128^3 perturbed lattice) and C3 (256^3 clustered): binning bit-exact in full; forces of
+    a seeded sample of sinks (random particles + every particle of the fullest cells) against the
+    oracle run on the full input.
+  - C4 (1024^3 clustered, the config the roofline target is quoted on): the oracle cannot hold
+    2^30 particles, so it gets the particles of two padded blocks of cells (one interior, one
+    wrapping around the box corner) cut out by a plain coordinate filter; every sink of the inner
+    blocks then has all of its sources.  Binning is compared bit for bit on those cells.
+  - everywhere: no NaN/Inf, zero net force, interaction count from the cell counts.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1810_02916_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+MEDIAN_TOL = 1e-5
+MAX_TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_1810_02916_b200 import nf
+    c = nf.Context(0)
+    yield c
+    c.close()
+
+
+def u32(t):
+    return t.cpu().numpy().view(np.uint32)
+
+
+def net_force_ok(acc: torch.Tensor):
+    """no NaN/Inf and zero net force on a fully periodic box (pair antisymmetry), in chunks"""
+    net = torch.zeros(3, dtype=torch.float64, device=acc.device)
+    mag = 0.0
+    for lo in range(0, acc.shape[0], 1 << 26):
+        a = acc[lo:lo + (1 << 26)]
+        assert torch.isfinite(a).all()
+        a = a.double()
+        net += a.sum(dim=0)
+        mag += a.norm(dim=1).sum().item()
+    assert net.abs().max().item() < 1e-5 * mag, (net, mag)
+
+
+@pytest.mark.parametrize("which", [2, 3])
+def test_full_box_sampled_sinks(ctx, which):
+    cfg = inputs.config(which)
+    pos = inputs.make_positions(cfg, device="cuda")
+    b = ctx.bin(pos, cfg.K, cfg.box)
+    acc = ctx.forces(b, cfg.R, cfg.eps, cfg.Gm)
+    net_force_ok(acc)
+    pos_np = pos.cpu().numpy()
+    # binning, in full, bit for bit
+    ref = oracle.bin_particles(pos_np, cfg.K, cfg.box)
+    assert ctx.out_of_range() == ref["n_out_of_range"] == 0
+    assert np.array_equal(u32(b.cell_count), ref["cell_count"])
+    assert np.array_equal(b.cell_offset.cpu().numpy().view(np.uint64), ref["cell_offset"])
+    assert np.array_equal(u32(b.perm), ref["perm"])
+    assert np.array_equal(b.pos_sorted.cpu().numpy().view(np.uint32), ref["pos_sorted"].view(np.uint32))
+    assert ctx.interactions(b, cfg.R) == oracle.interactions(ref["cell_count"], cfg.K, cfg.R)
+    # forces: 30 000 random sinks + all particles of the 8 fullest cells
+    rng = np.random.default_rng(which)
+    sinks = [rng.choice(cfg.N, 30_000, replace=False)]
+    for c in np.argsort(ref["cell_count"])[-8:]:
+        o0, o1 = int(ref["cell_offset"][c]), int(ref["cell_offset"][c + 1])
+        sinks.append(ref["perm"][o0:o1].astype(np.int64))
+    sink_idx = np.unique(np.concatenate(sinks))
+    a_ref = oracle.forces(pos_np, cfg.K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=sink_idx)
+    # the metric's rms is taken over the sampled sinks
+    err = oracle.parity_error(acc[torch.from_numpy(sink_idx).cuda()].cpu().numpy(), a_ref)
+    assert np.median(err) <= MEDIAN_TOL, f"median error {np.median(err):.3e}"
+    assert err.max() <= MAX_TOL, f"max error {err.max():.3e}"
+
+
+def test_c4_full_size_blocks(ctx):
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90 * (1 << 30):
+        pytest.skip("needs ~90 GB of free device memory")
+    cfg = inputs.config(4)
+    K, R, m = cfg.K, cfg.R, 5
+    pos = inputs.make_positions(cfg, device="cuda")
+    ctx.reserve(cfg.N, K)
+    b = ctx.bin(pos, K, cfg.box)
+    assert ctx.out_of_range() == 0
+    acc = ctx.forces(b, R, cfg.eps, cfg.Gm)
+    # properties at full size
+    net_force_ok(acc)
+    cnt = b.cell_count.long()
+    assert int(cnt.sum()) == cfg.N
+    assert torch.equal(torch.cumsum(cnt, 0), b.cell_offset[1:])
+    nb = torch.zeros_like(cnt.view(K, K, K))
+    c3 = cnt.view(K, K, K)
+    for dx in range(-R, R + 1):
+        for dy in range(-R, R + 1):
+            for dz in range(-R, R + 1):
+                nb += torch.roll(c3, shifts=(dx, dy, dz), dims=(0, 1, 2))
+    assert ctx.interactions(b, R) == int((c3 * nb).sum())
+    w = cfg.box / K
+    off = b.cell_offset.cpu().numpy()
+    for c0 in [(3, 5, 7), (K - 2, K - 3, K - 1)]:          # interior block; block wrapping around the box corner
+        lo = [(c - R - 1) * w for c in c0]
+        hi = [(c + m + R + 1) * w for c in c0]
+        idx = inputs.select_box(pos, lo, hi, cfg.box)       # increasing original indices
+        sub = pos[idx].cpu().numpy()
+        idx_np = idx.cpu().numpy()
+        ref = oracle.bin_particles(sub, K, cfg.box)
+        keys, nbad = oracle.keys(sub, K, cfg.box)
+        assert nbad == 0
+        cx, cy, cz = keys // (K * K), (keys // K) % K, keys % K
+        inner = np.ones(len(keys), bool)
+        for c, l0 in ((cx, c0[0]), (cy, c0[1]), (cz, c0[2])):
+            inner &= ((c.astype(np.int64) - l0) % K) < m
+        # binning of the inner cells, bit for bit (the sub-sample keeps the input order, so the
+        # stable order inside a cell is the same)
+        for key in np.unique(keys[inner])[:: 7]:
+            g0, g1 = int(off[key]), int(off[key + 1])
+            r0, r1 = int(ref["cell_offset"][key]), int(ref["cell_offset"][key + 1])
+            assert g1 - g0 == r1 - r0
+            assert np.array_equal(u32(b.perm[g0:g1]), idx_np[ref["perm"][r0:r1]].astype(np.uint32))
+            assert np.array_equal(b.pos_sorted[g0:g1].cpu().numpy().view(np.uint32), ref["pos_sorted"][r0:r1].view(np.uint32))
+        sink_local = np.nonzero(inner)[0]
+        a_ref = oracle.forces(sub, K, R, cfg.eps, cfg.box, cfg.Gm, sink_idx=sink_local)
+        got = acc[idx[torch.from_numpy(sink_local).cuda()]].cpu().numpy()
+        err = oracle.parity_error(got, a_ref)
+        assert np.median(err) <= MEDIAN_TOL, f"median error {np.median(err):.3e} at block {c0}"
+        assert err.max() <= MAX_TOL, f"max error {err.max():.3e} at block {c0}"

@@ -81,6 +81,8 @@ def test_bin_edge_cases(ctx):
     rng = np.random.default_rng(1)
     check_bin(ctx, (rng.random((70_000, 3)) * 500).astype(np.float32).clip(0, 499.99), 64, 500.0)
     check_bin(ctx, rng.random((1000, 3)).astype(np.float32), 1, 1.0)           # a single cell
+    top = np.nextafter(np.float32(500.0), np.float32(0))                         # 499.99997 * 0.512f rounds to 256.0f: valid, cell K-1
+    check_bin(ctx, np.array([[top, top, 1.0], [500.0, 1.0, 1.0], [3.0, top, 499.0]], np.float32), 256, 500.0)
 
 
 def test_bin_is_deterministic(ctx):

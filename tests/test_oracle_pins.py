@@ -355,6 +355,13 @@ def test_binning_edge_cases():
     assert key[1] == (9 * K + 2) * K + 2 and key[2] == (0 * K + 3) * K + 3 and key[3] == 0
     b = oracle.bin_particles(np.zeros((0, 3), np.float32), K, box)
     assert b["cell_count"].sum() == 0 and b["cell_offset"][-1] == 0
+    # DESIGN.md reading c9: a valid x just below box whose float32 product x * (K / box) rounds up
+    # to K (499.99997 * 0.512f == 256.0f) is clamped into cell K-1 and is NOT out of range
+    K, box = 256, 500.0
+    top = np.nextafter(np.float32(box), np.float32(0))
+    assert np.float32(top) * (np.float32(K) / np.float32(box)) == np.float32(K)
+    key, nbad = oracle.keys(np.array([[top, top, 1.0], [np.float32(box), 1.0, 1.0]], np.float32), K, box)
+    assert nbad == 1 and key[0] == ((K - 1) * K + (K - 1)) * K + 0 and key[1] // (K * K) == K - 1
 
 
 def test_interaction_count():
