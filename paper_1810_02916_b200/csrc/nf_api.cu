@@ -102,7 +102,7 @@ static size_t forces_scratch_full(int64_t N, int K)
     p.sink_lo = 0;
     p.sink_hi = K;
     p.max_sinks = N;
-    return nf_forces_scratch_bytes(p) + nf_align_up((size_t)(N > 0 ? N : 1) * 16, 256);   // + encoded positions
+    return nf_forces_scratch_bytes(p) + 2 * nf_align_up((size_t)(N > 0 ? N : 1) * 16, 256);   // + the two encoded copies
 }
 
 int nf_reserve(nf_ctx *ctx, int64_t maxN, int K)
@@ -175,11 +175,12 @@ int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
     NF_TRY(nf_scratch_reserve(ctx, forces_scratch_full(N, K)));
     nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
     float4 *enc = nf_scratch_take<float4>(ctx, (size_t)N);
-    if (!d_planes || !enc) { NF_SET_ERR(ctx, "nf_forces: internal scratch arena too small"); return NF_ERR_NOMEM; }
+    float4 *enc_h = nf_scratch_take<float4>(ctx, (size_t)N);
+    if (!d_planes || !enc || !enc_h) { NF_SET_ERR(ctx, "nf_forces: internal scratch arena too small"); return NF_ERR_NOMEM; }
     cudaStream_t st = (cudaStream_t)stream;
     const float4 *ps = reinterpret_cast<const float4 *>(pos_sorted);
-    NF_TRY(nf_encode_impl(ctx, p, ps, cell_offset, (size_t)K * K * K, enc, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, ps, enc, cell_offset, perm, acc_xyz, st));
+    NF_TRY(nf_encode_impl(ctx, p, ps, cell_offset, (size_t)K * K * K, enc, enc_h, st));
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, ps, enc, enc_h, cell_offset, perm, acc_xyz, st));
     return nf_forces_impl(ctx, p, d_planes, st, true);
 }
 
@@ -219,7 +220,8 @@ int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, 
     uint64_t *off = nf_scratch_take<uint64_t>(ctx, ncell + 1);
     nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
     float4 *enc = nf_scratch_take<float4>(ctx, n);
-    if (!raw || !acc || !sorted || !perm || !count || !off || !d_planes || !enc) {
+    float4 *enc_h = nf_scratch_take<float4>(ctx, n);
+    if (!raw || !acc || !sorted || !perm || !count || !off || !d_planes || !enc || !enc_h) {
         NF_SET_ERR(ctx, "nf_forces_host: internal scratch arena too small");
         return NF_ERR_NOMEM;
     }
@@ -230,8 +232,8 @@ int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, 
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
-    NF_TRY(nf_encode_impl(ctx, p, reinterpret_cast<const float4 *>(sorted), off, ncell, enc, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, off, perm, acc, st));
+    NF_TRY(nf_encode_impl(ctx, p, reinterpret_cast<const float4 *>(sorted), off, ncell, enc, enc_h, st));
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, acc, st));
     NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
     NF_CUDA(ctx, cudaMemcpyAsync(acc_host, acc, n * 12, cudaMemcpyDeviceToHost, st));
     NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));

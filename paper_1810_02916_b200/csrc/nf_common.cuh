@@ -98,7 +98,8 @@ int nf_bin_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, int 
 // sinks: plane p (0 <= p < n_planes) has its own cell-contiguous arrays.
 struct nf_plane_view {
     const float4 *pos;        // sorted cell-centred offsets of this plane's particles
-    const float4 *enc;        // the same particles, scaled and z-block-encoded (nf_encode_impl)
+    const float4 *enc;        // the same particles, scaled and z-block-encoded (nf_encode_impl), blocks from cz = 0
+    const float4 *enc_h;      // ... and with the z-blocks shifted by half a block
     const uint64_t *off;      // K*K+1 exclusive offsets within this plane's arrays
     const uint32_t *perm;     // nullable
     float *acc;               // output for this plane (n x 3), nullable for ghost planes
@@ -118,11 +119,12 @@ size_t nf_forces_scratch_bytes(const nf_force_params &p);
 int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d_planes,
                    cudaStream_t st, bool record_timing);
 // the full box seen as K planes sharing one set of arrays: plane cx starts at cell cx*K*K
-int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const uint64_t *off,
-                        const uint32_t *perm, float *acc, cudaStream_t st);
-// enc[s] = encoded copy of pos[s] for the ncell cells described by off (cell index % K = cz); depends on p.eps, p.box, p.K
+int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
+                        const uint64_t *off, const uint32_t *perm, float *acc, cudaStream_t st);
+// enc[s], enc_h[s] = the two encoded copies of pos[s] for the ncell cells described by off (cell index % K = cz);
+// they depend on p.eps, p.box, p.K
 int nf_encode_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, float4 *enc,
-                   cudaStream_t st);
+                   float4 *enc_h, cudaStream_t st);
 // once per context: uploads the task-split table
 int nf_forces_init(nf_ctx *ctx);
 // ordered pairs evaluated for the sink planes of a plane table (device result added to ctx->counters[1])

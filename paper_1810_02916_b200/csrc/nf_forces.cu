@@ -35,7 +35,9 @@ struct ForceConsts {
     float scale;        // 2^k
     float ws;           // cell width in internal units, (box / K) * scale
     float out_scale;    // Gm * scale^2: a = out_scale * sum f' d'
+    int flags;          // FC_FAR_OK: a cell width exceeds eps, so cells two or more apart hold no pair inside eps;  FC_PLUMMER
 };
+constexpr int FC_FAR_OK = 1, FC_PLUMMER = 2;
 
 // ------------------------------------------------------------------------------------------
 // Packed FP32 (sm_100 FFMA2 / FADD2 / FMUL2): one 64-bit register holds the same quantity for
@@ -56,7 +58,10 @@ __device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 d; asm("mul.rn.ftz.f32x2
 // MODE 0: Eq. 2 as min(poly, r^-3).
 // MODE 1: r^-3 only, and the smallest r^2 seen is tracked in rmin: exact whenever no pair of
 //         the tile lies inside eps (the caller checks rmin and redoes the tile with MODE 0
-//         otherwise).  Also the Plummer law (r2_floor = eps^2, eps2_test = 0).
+//         otherwise).
+// MODE 2: r^-3 only, nothing tracked: tiles that cannot hold a pair inside eps (source cells two
+//         or more cells away from the sinks' cell when a cell is wider than eps), and the
+//         Plummer law (r2_floor = eps^2).
 template <int MODE>
 __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64 ys, const u64 zs, const ForceConsts &fc,
                                          u64 &ax, u64 &ay, u64 &az, float &rmin)
@@ -75,7 +80,7 @@ __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64
         upk(poly, pa, pb);
         upk(f, fa, fb);
         f = pk(fminf(pa, fa), fminf(pb, fb));
-    } else {
+    } else if (MODE == 1) {
         rmin = min3(rmin, r2a, r2b);
     }
     fma2_acc(ax, f, dx);
@@ -150,16 +155,19 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // Encoded positions.  The interaction kernel fetches source cells with bulk copies straight
 // into shared memory, so whatever a lane needs per source must already be in the array:
 //   enc.xy = offset.xy * scale                 (exact: scale is a power of two)
-//   enc.z  = offset.z * scale + e(cz) * ws,    e(cz) = (cz mod ZB) - (ZB-1)/2
+//   enc.z  = offset.z * scale + e(cz) * ws,    e(cz) = ((cz + phi) mod ZB) - (ZB-1)/2
 // i.e. z is measured from the centre of the cell's block of ZB = 8 cells, so that a whole run
-// of consecutive cells inside one z-block shares ONE shift of the sink coordinates.  |enc.z| <
-// 4 ws: the rounding of the encoding (<= 2^-23 ws) is the same size as that of the x/y column
-// shifts, and differences inside one cell stay exact.
+// of consecutive cells inside one z-block shares ONE shift of the sink coordinates.  Two copies
+// are kept, with the blocks starting at phi = 0 and at phi = ZB/2: for R <= 2 the 2R+1 cells
+// cz-R..cz+R always lie inside one block of one of the two, so a column of source cells is one
+// contiguous piece in one frame (a task picks the copy by its cz).  |enc.z| < 4 ws: the rounding
+// of the encoding (<= 2^-23 ws) is the same size as that of the x/y column shifts, and
+// differences inside one cell stay exact.
 // ------------------------------------------------------------------------------------------
 constexpr int ZB = 8;
 
 __global__ void __launch_bounds__(256) k_encode(const float4 *__restrict__ pos, const uint64_t *__restrict__ off, size_t ncell, int K,
-                                                float scale, float ws, float4 *__restrict__ enc)
+                                                float scale, float ws, float4 *__restrict__ enc, float4 *__restrict__ enc_h)
 {
     const size_t c = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (c >= ncell) return;
@@ -167,9 +175,12 @@ __global__ void __launch_bounds__(256) k_encode(const float4 *__restrict__ pos, 
     const uint64_t s0 = off[c], s1 = off[c + 1];
     const int cz = (int)(c % (size_t)K);
     const float ez = ((float)(cz % ZB) - 0.5f * (float)(ZB - 1)) * ws;
+    const float eh = ((float)((cz + ZB / 2) % ZB) - 0.5f * (float)(ZB - 1)) * ws;
     for (uint64_t s = s0 + lane; s < s1; s += 32) {
         const float4 o = pos[s];
-        enc[s] = make_float4(o.x * scale, o.y * scale, fmaf(o.z, scale, ez), 0.f);
+        const float x = o.x * scale, y = o.y * scale;
+        enc[s] = make_float4(x, y, fmaf(o.z, scale, ez), 0.f);
+        enc_h[s] = make_float4(x, y, fmaf(o.z, scale, eh), 0.f);
     }
 }
 
@@ -178,7 +189,8 @@ __global__ void __launch_bounds__(256) k_encode(const float4 *__restrict__ pos, 
 // P = floor(32/L) "phases" of the warp split every source tile between them.  A cell of n
 // sinks becomes floor(n/128) full tasks (L = 32) plus the split of the remainder that
 // minimises  sum over tasks (1/P + C0)  -- warp time per source swept plus a fixed per-task
-// cost -- found by dynamic programming on the host (c_split).  Lane use is ~96 % for
+// cost (C0 = per-tile overhead, ~13 source steps, over a typical tile of ~300 sources) -- found
+// by dynamic programming on the host (c_split).  Lane use is ~96 % for
 // Poisson(64) cells against ~91 % for an even split.
 // ------------------------------------------------------------------------------------------
 constexpr int SPLIT_MAX = 4;       // tasks per remainder (< 128 sinks) at most
@@ -264,7 +276,8 @@ __global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restri
 // sweeps its slice with broadcast LDS.128.
 // Spline: the sweep evaluates r^-3 only and tracks the smallest r^2; if any lane of the warp saw
 // a pair inside eps the tile is redone with the min form of Eq. 2 (and the rest of that column
-// uses the min form directly).  Exact, because the two laws agree for r >= eps.
+// uses the min form directly).  Exact, because the two laws agree for r >= eps.  Columns two or
+// more cells away in x or y are at least a cell width from the sinks: no pair inside eps, nothing tracked.
 // float32 partial sums per tile, double outer sum over tiles and phases in a fixed order:
 // deterministic, no floating-point atomics.
 // ------------------------------------------------------------------------------------------
@@ -327,12 +340,14 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
         const bool active = ph < P;
         const int tile_max = TILE_CAP - P * UNR - 2;   // 2 slots of slack: the sweep loads one pair ahead
 
+        // which of the two encoded copies: the one whose z-blocks do not cut cz-R..cz+R (if any)
+        const int zphi = ((cz - R + ZB * 4) / ZB != (cz + R + ZB * 4) / ZB) ? ZB / 2 : 0;
         // ---- piece table: lane r builds the pieces of column r ----
         if (lane < W) {
             int px = sink_plane + lane - R;
             if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
             else if (px < 0 || px >= p.n_planes) px = -1;
-            S.enc[lane] = px >= 0 ? planes[px].enc : nullptr;
+            S.enc[lane] = px >= 0 ? (zphi ? planes[px].enc_h : planes[px].enc) : nullptr;
         }
         int n_pieces = 0;
         for (int rb = 0; rb < NR; rb += 32) {
@@ -359,7 +374,7 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                     const int qz = ((cz + s - R) % K + K) % K;
                     st[s] = 0; cn[s] = 0;
                     if (qo) { st[s] = (uint32_t)qo[qz]; cn[s] = (uint32_t)(qo[qz + 1] - qo[qz]); }
-                    kz[s] = (s - R) - (qz % ZB) + (cz % ZB);
+                    kz[s] = (s - R) - ((qz + zphi) % ZB) + ((cz + zphi) % ZB);
                     const bool self = col == NR / 2 && s == R;    // the sinks' own cell: a piece of its own (flagged)
                     newp[s] = cn[s] > 0 && (self || !(have && prev_end == st[s] && prev_k == kz[s]));
                     if (cn[s] > 0) { have = !self; prev_end = st[s] + cn[s]; prev_k = kz[s]; }
@@ -394,7 +409,8 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
 #pragma unroll
         for (int h = 0; h < 2; h++) {
             const int j0 = min(4 * sl + 2 * h, n - 1), j1 = min(4 * sl + 2 * h + 1, n - 1);
-            const float4 m0 = sp.enc[s0 + j0], m1 = sp.enc[s0 + j1];
+            const float4 *se = zphi ? sp.enc_h : sp.enc;
+            const float4 m0 = se[s0 + j0], m1 = se[s0 + j1];
             xi[h] = pk(m0.x, m1.x); yi[h] = pk(m0.y, m1.y); zi[h] = pk(m0.z, m1.z);
         }
         __syncwarp();
@@ -460,14 +476,20 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
             float rmin = 3.0e38f;
             const float4 *src = buf + ph * q;
-            // the sinks' own cell holds every sink as a source (r = 0), which would always trip the
-            // close-pair test: it takes the min form directly, as does the rest of a column after a hit
-            const bool direct = sticky_col == col || (d0.meta >> 24) != 0;
+            // Which law the tile needs (warp-uniform).  The sinks' own cell holds every sink as a source
+            // (r = 0), which would always trip the close-pair test: it takes the min form directly, as
+            // does the rest of a column after a hit.  Columns two or more cells away in x or y cannot
+            // hold a pair inside eps (FC_FAR_OK), and Plummer has no second branch: nothing to track.
+            int mode = 1;
+            if (fc.flags & FC_PLUMMER) mode = 2;
+            else if (sticky_col == col || (d0.meta >> 24) != 0) mode = 0;
+            else if ((fc.flags & FC_FAR_OK) && max(abs(dxi - R), abs(dyi - R)) >= 2) mode = 2;
             if (active) {
-                if (direct) sweep<0>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-                else sweep<1>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                if (mode == 1) sweep<1>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                else if (mode == 2) sweep<2>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                else sweep<0>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
             }
-            if (!direct && __any_sync(0xffffffffu, rmin < fc.eps2_test)) {
+            if (mode == 1 && __any_sync(0xffffffffu, rmin < fc.eps2_test)) {
                 sticky_col = col;
                 ax[0] = ax[1] = ay[0] = ay[1] = az[0] = az[1] = 0;
                 if (active) sweep<0>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
@@ -543,14 +565,15 @@ __global__ void __launch_bounds__(256) k_interactions(const uint32_t *__restrict
     if ((threadIdx.x & 31) == 0 && local) atomicAdd(out, local);  // integer atomics: order-independent
 }
 
-__global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, const float4 *enc, const uint64_t *off,
-                              const uint32_t *perm, float *acc)
+__global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
+                              const uint64_t *off, const uint32_t *perm, float *acc)
 {
     int cx = blockIdx.x * blockDim.x + threadIdx.x;
     if (cx >= K) return;
     nf_plane_view v;
     v.pos = pos;
     v.enc = enc;
+    v.enc_h = enc_h;
     v.off = off + (size_t)cx * K * K;
     v.perm = perm;
     v.acc = acc;
@@ -607,13 +630,15 @@ ForceConsts make_consts(const nf_force_params &p)
     fc.r2_floor = plummer ? (float)(es * es) : 8.673617379884035e-19f;  // 2^-60
     fc.eps2_test = plummer ? 0.0f : (float)(es * es * 1.0001);
     fc.out_scale = (float)((double)p.Gm * (double)scale * (double)scale);
+    // sources two or more cells away are at least one cell width (minus rounding) from every sink of the cell
+    fc.flags = (plummer ? FC_PLUMMER : 0) | ((double)fc.ws * 0.999 > es * 1.0001 ? FC_FAR_OK : 0);
     return fc;
 }
 
 // split of a remainder of n < 128 sinks into tasks of 4L sinks: minimise sum(1/P + C0), P = floor(32/L)
 void make_split_table(SplitTable &t)
 {
-    const double C0 = 0.02, INF = 1e30;
+    const double C0 = 0.045, INF = 1e30;
     static double dp[SPLIT_MAX + 1][128];
     static int ch[SPLIT_MAX + 1][128];
     for (int k = 0; k <= SPLIT_MAX; k++)
@@ -679,20 +704,20 @@ int nf_forces_init(nf_ctx *ctx)
     return NF_OK;
 }
 
-int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const uint64_t *off,
-                        const uint32_t *perm, float *acc, cudaStream_t st)
+int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
+                        const uint64_t *off, const uint32_t *perm, float *acc, cudaStream_t st)
 {
-    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, enc, off, perm, acc);
+    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, enc, enc_h, off, perm, acc);
     NF_LAUNCHED(ctx);
     return NF_OK;
 }
 
 int nf_encode_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, float4 *enc,
-                   cudaStream_t st)
+                   float4 *enc_h, cudaStream_t st)
 {
     if (ncell == 0) return NF_OK;
     const ForceConsts fc = make_consts(p);
-    k_encode<<<(unsigned)((ncell + 7) / 8), 256, 0, st>>>(pos, off, ncell, p.K, fc.scale, fc.ws, enc);
+    k_encode<<<(unsigned)((ncell + 7) / 8), 256, 0, st>>>(pos, off, ncell, p.K, fc.scale, fc.ws, enc, enc_h);
     NF_LAUNCHED(ctx);
     return NF_OK;
 }

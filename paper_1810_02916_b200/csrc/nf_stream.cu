@@ -20,6 +20,7 @@ struct Slot {
     float *raw;        // n x 3
     float *sorted;     // n x 4
     float *enc;        // n x 4: scaled, z-block-encoded copy read by the interaction kernel
+    float *enc_h;      // n x 4: the same with the z-blocks shifted by half a block
     uint32_t *perm;    // n
     uint32_t *count;   // K*K
     uint64_t *off;     // K*K + 1
@@ -121,7 +122,7 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         ctx->slab_state = S;
     }
     const size_t n = (size_t)max_n;
-    const size_t slot_bytes = nf_align_up(n * 12, 256) + 2 * nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
+    const size_t slot_bytes = nf_align_up(n * 12, 256) + 3 * nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
                               nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256) + nf_align_up(n * 12, 256);
     const size_t need = slot_bytes * W;
     if (need > S->mem_bytes) {
@@ -153,6 +154,7 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         slots[s].raw = (float *)b;                b += nf_align_up(n * 12, 256);
         slots[s].sorted = (float *)b;             b += nf_align_up(n * 16, 256);
         slots[s].enc = (float *)b;                b += nf_align_up(n * 16, 256);
+        slots[s].enc_h = (float *)b;              b += nf_align_up(n * 16, 256);
         slots[s].perm = (uint32_t *)b;            b += nf_align_up(n * 4, 256);
         slots[s].count = (uint32_t *)b;           b += nf_align_up(ncell * 4, 256);
         slots[s].off = (uint64_t *)b;             b += nf_align_up((ncell + 1) * 8, 256);
@@ -163,6 +165,7 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         const Slot &sl = slots[q % W];
         S->h_views[q].pos = (const float4 *)sl.sorted;
         S->h_views[q].enc = (const float4 *)sl.enc;
+        S->h_views[q].enc_h = (const float4 *)sl.enc_h;
         S->h_views[q].off = sl.off;
         S->h_views[q].perm = sl.perm;
         S->h_views[q].acc = sl.acc;
@@ -204,7 +207,7 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         const int cx = ((plane0 + q) % K + K) % K;
         // counters[0] accumulates out-of-range / wrong-plane particles over all planes
         NF_TRY(nf_bin_impl(ctx, sl.raw, plane_n[q], K, box, cx, sl.sorted, sl.perm, sl.count, sl.off, st));
-        NF_TRY(nf_encode_impl(ctx, fp, (const float4 *)sl.sorted, sl.off, ncell, (float4 *)sl.enc, st));
+        NF_TRY(nf_encode_impl(ctx, fp, (const float4 *)sl.sorted, sl.off, ncell, (float4 *)sl.enc, (float4 *)sl.enc_h, st));
         NF_CUDA(ctx, cudaEventRecord(bin1[q], st));
 
         const int sp = q - R;        // chunk plane whose neighbourhood is now complete
