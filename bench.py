@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- the near-field force hot path (nf_bin + nf_forces) on seeded synthetic input.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..4] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (cell assignment,
 histogram, scan, stable scatter + re-centre, work list, interaction kernel, scale/un-permute)
@@ -13,6 +13,9 @@ One JSON line is printed by rank 0 (DESIGN.md "Measurement" explains every key):
   e2e        the same through nf_forces_host: pinned HOST buffers, H2D + D2H inside the timing
   roofline   interaction kernel alone against the FP32 ALU peak, 20 flop per interaction
   cpu_baseline   the CPU oracle, as it stands, on a bounded sample of the same workload
+
+`--config 5` is the slab-streaming workload (C5): a step is one nf_stream_slabs call over the
+16 + 4 planes, from and to pinned host memory, so `value` already contains the copies.
 
 `--impl reference` times the CPU oracle (this tier's reference arm) on bounded samples.
 """
@@ -36,6 +39,10 @@ from paper_1810_02916_b200 import inputs  # noqa: E402
 
 FLOP_PER_INTERACTION = 20          # BASELINE.json convention (the paper counts 23)
 FP32_LANES_PER_SM = 128
+ORACLE_BLOCK = 24                  # the oracle's sample: sinks of a 24^3-cell block (~0.9 M sinks at 64 per cell)
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_forces_warp launch, from the `ncu --set full`
+# captures summarised under profiles/ (the file named there gives the command); None = not captured
+NCU_TRAFFIC_BYTES = {}
 
 
 def read_peaks():
@@ -153,7 +160,9 @@ def run_reference(args, cfg):
     import oracle
     oracle.build()
     dev = "cuda" if torch.cuda.is_available() else "cpu"
-    m = 6
+    m = ORACLE_BLOCK
+    if cfg.kind == "slab":          # C5: the oracle is timed on the C4 box of the same recipe (same eps, halo catalogue, 64 per cell)
+        cfg = inputs.config(4)
     pos = inputs.make_positions(cfg, device=dev)
     sub, _ = oracle_sample(pos, cfg, m)
     del pos
@@ -179,12 +188,112 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def run_stream(args, cfg):
+    """C5: nf_stream_slabs over P + 2R planes held in pinned host memory.
+    One rank per GPU, every rank its own seeded chunk (weak scaling, no data-path collective)."""
+    from paper_1810_02916_b200 import nf
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    rcfg = cfg if rank == 0 else inputs.dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    planes_dev = inputs.make_slab_planes(rcfg, device=dev)
+    planes = []
+    for t in planes_dev:
+        h = torch.empty(t.shape, dtype=torch.float32).pin_memory()
+        h.copy_(t)
+        planes.append(h)
+    del planes_dev, t
+    torch.cuda.empty_cache()
+    P, R, K = rcfg.planes, rcfg.R, rcfg.K
+    n_in = sum(t.shape[0] for t in planes)
+    n_out = sum(planes[R + p].shape[0] for p in range(P))
+    Gm = 1.0 / float(rcfg.density_n) ** 3
+    ctx = nf.Context(local)
+    out = [torch.empty(planes[R + p].shape[0], 3, dtype=torch.float32).pin_memory() for p in range(P)]
+    stats = None
+    for _ in range(max(args.warmup, 1)):
+        _, stats = ctx.stream_slabs(planes, P, K, R, rcfg.eps, rcfg.box, rcfg.plane0, Gm, out=out)
+    I = stats["interactions"]
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    launches0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    all_stats = []
+    barrier()
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(args.steps):
+        _, st = ctx.stream_slabs(planes, P, K, R, rcfg.eps, rcfg.box, rcfg.plane0, Gm, out=out)
+        all_stats.append(st)
+    e1.record()
+    barrier()
+    wall = time.perf_counter() - t0
+    launches = ctx.launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    t = torch.tensor([max(wall, e0.elapsed_time(e1) * 1e-3)], dtype=torch.float64, device=dev)
+    tot = torch.tensor([float(I), float(n_out)], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    ms_per_step = 1e3 * float(t.item()) / args.steps
+    value = float(tot[0].item()) / (ms_per_step * 1e-3)
+    mean = lambda k: sum(s[k] for s in all_stats) / len(all_stats)
+    sm_max_mhz, hbm_gbs, peak_src = read_peaks()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak_tflops = sms * sm_max_mhz * 1e6 * 2 * FP32_LANES_PER_SM / 1e12
+    f_ms = 1e3 * mean("force_seconds")
+    achieved = FLOP_PER_INTERACTION * I / (f_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "interaction kernel (16 launches, one per sink plane, with their work-list kernels)",
+                "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                "traffic": NCU_TRAFFIC_BYTES.get(rcfg.name),
+                "peak_source": f"{sms} SMs x {sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz) x 2 x {FP32_LANES_PER_SM} FP32 lanes",
+                "flop_per_interaction": FLOP_PER_INTERACTION, "kernel_ms": f_ms,
+                "kernel_interactions_per_s": I / (f_ms * 1e-3), "kernel_share_of_step": f_ms / ms_per_step}
+    e2e = {"value": value, "unit": "interactions/s", "h2d_bytes_per_step": int(mean("h2d_bytes")),
+           "d2h_bytes_per_step": int(mean("d2h_bytes")), "ms_per_step": ms_per_step, "api": "nf_stream_slabs",
+           "note": "this workload lives in pinned host memory by definition: value and e2e are the same measurement",
+           "result_checksum": float(sum(float(o[:: max(1, o.shape[0] // 256)].double().abs().sum()) for o in out))}
+    copies = {"h2d_gbps": mean("h2d_gbps"), "d2h_gbps": mean("d2h_gbps"), "overlap_fraction": mean("overlap_fraction"),
+              "h2d_seconds": mean("h2d_seconds"), "d2h_seconds": mean("d2h_seconds"),
+              "kernel_seconds": mean("kernel_seconds"), "wall_seconds": mean("wall_seconds")}
+    line = {"metric": "near_field_pairwise_interactions_per_s", "value": value, "unit": "interactions/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": rcfg.name, "planes": P, "ghost_planes": 2 * R, "K": K, "R": R, "eps": rcfg.eps,
+                       "box": rcfg.box, "particles_in": n_in, "particles_out": n_out,
+                       "interactions_per_step_per_gpu": I, "interactions_per_particle": I / max(n_out, 1),
+                       "l2": "inputs larger than L2 (streamed from pinned host memory)",
+                       "parallelism": f"{world} independent chunks, one per GPU" if world > 1 else "1 GPU"},
+            "particles_per_s": float(tot[1].item()) / (ms_per_step * 1e-3),
+            "e2e": e2e, "copies": copies, "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
+            "cpu_baseline": None}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number 1..4 (default 4 = C4)")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number 1..5 (default 4 = C4; 5 = slab streaming)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -203,6 +312,9 @@ def main():
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    if cfg.kind == "slab":
+        run_stream(args, cfg)
+        return
     from paper_1810_02916_b200 import nf
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -271,7 +383,7 @@ def main():
     # sample for the CPU oracle (taken now, while the positions are still on the device)
     cpu_sub = None
     if not args.no_cpu and world == 1 and rank == 0:
-        cpu_sub, _ = oracle_sample(pos, rcfg, 6)
+        cpu_sub, _ = oracle_sample(pos, rcfg, ORACLE_BLOCK)
 
     # ---- end to end through nf_forces_host (pinned host buffers, copies inside the timing) ----
     e2e = None
@@ -318,7 +430,7 @@ def main():
     peak_tflops = sms * sm_max_mhz * 1e6 * 2 * FP32_LANES_PER_SM / 1e12
     achieved = FLOP_PER_INTERACTION * I / (k_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "interaction kernel (nf_forces)", "achieved": achieved,
-                "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
+                "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": NCU_TRAFFIC_BYTES.get(rcfg.name),
                 "peak_source": f"{sms} SMs x {sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz) x 2 x {FP32_LANES_PER_SM} FP32 lanes",
                 "flop_per_interaction": FLOP_PER_INTERACTION, "kernel_ms": k_ms,
                 "kernel_interactions_per_s": I / (k_ms * 1e-3), "kernel_share_of_step": k_ms / ms_per_step,
@@ -327,7 +439,7 @@ def main():
 
     cpu = None
     if cpu_sub is not None:
-        m = 6
+        m = ORACLE_BLOCK
         inter, dt, cores, n_sinks, _, _ = time_oracle(cpu_sub, rcfg, m, (3, 5, 7), budget_s=15.0)
         cpu = {"value": inter / dt, "unit": "interactions/s", "cores": cores, "kind": "oracle",
                "sample": f"{n_sinks} sinks drawn from a {m}^3-cell block of {rcfg.name} with all their sources: "

@@ -173,6 +173,7 @@ typedef struct nf_stream_stats {
     double wall_seconds;                  /* first H2D start to last D2H end */
     double h2d_gbps, d2h_gbps;            /* bytes / copy seconds */
     double overlap_fraction;              /* 1 - (wall - kernel)/ (h2d + d2h seconds), clamped to [0,1] */
+    double force_seconds;                 /* the part of kernel_seconds spent in work-list build + interaction kernel */
 } nf_stream_stats;
 
 /*

@@ -41,7 +41,7 @@ __device__ __forceinline__ TOut block_exclusive(TOut v, TOut *total)
 }
 
 template <class TIn, class TOut>
-__global__ void __launch_bounds__(SCAN_THREADS) scan_reduce(const TIn *__restrict__ in, size_t n, TOut *__restrict__ sums)
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(const TIn *__restrict__ in, size_t n, TOut *__restrict__ sums)
 {
     __shared__ TOut total;
     size_t base = (size_t)blockIdx.x * SCAN_TILE;
@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_reduce(const TIn *__restric
 
 // in-place safe (in may alias out when TIn == TOut): all loads of a tile happen before its stores
 template <class TIn, class TOut>
-__global__ void __launch_bounds__(SCAN_THREADS) scan_apply(const TIn *in, size_t n, const TOut *__restrict__ block_offsets, TOut *out, int write_total)
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const TIn *in, size_t n, const TOut *__restrict__ block_offsets, TOut *out, int write_total)
 {
     __shared__ TOut total;
     size_t base = (size_t)blockIdx.x * SCAN_TILE + (size_t)threadIdx.x * SCAN_ITEMS;
@@ -89,15 +89,15 @@ int scan_impl(nf_ctx *ctx, const TIn *in, TOut *out, size_t n, TOut *temp, cudaS
     }
     size_t nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
     if (nblk == 1) {
-        scan_apply<TIn, TOut><<<1, SCAN_THREADS, 0, st>>>(in, n, nullptr, out, write_total);
+        k_scan_apply<TIn, TOut><<<1, SCAN_THREADS, 0, st>>>(in, n, nullptr, out, write_total);
         NF_LAUNCHED(ctx);
         return NF_OK;
     }
     TOut *sums = temp;
-    scan_reduce<TIn, TOut><<<(unsigned)nblk, SCAN_THREADS, 0, st>>>(in, n, sums);
+    k_scan_reduce<TIn, TOut><<<(unsigned)nblk, SCAN_THREADS, 0, st>>>(in, n, sums);
     NF_LAUNCHED(ctx);
     NF_TRY((scan_impl<TOut, TOut>(ctx, sums, sums, nblk, temp + nf_align_up(nblk, 64), st, 0)));
-    scan_apply<TIn, TOut><<<(unsigned)nblk, SCAN_THREADS, 0, st>>>(in, n, sums, out, write_total);
+    k_scan_apply<TIn, TOut><<<(unsigned)nblk, SCAN_THREADS, 0, st>>>(in, n, sums, out, write_total);
     NF_LAUNCHED(ctx);
     return NF_OK;
 }

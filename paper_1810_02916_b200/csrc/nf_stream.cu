@@ -242,7 +242,7 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         }
         for (int p = 0; p < P; p++) {
             stats->particles_out += plane_n[R + p];
-            NF_CUDA(ctx, cudaEventElapsedTime(&ms, frc0[p], frc1[p])); stats->kernel_seconds += ms * 1e-3;
+            NF_CUDA(ctx, cudaEventElapsedTime(&ms, frc0[p], frc1[p])); stats->kernel_seconds += ms * 1e-3; stats->force_seconds += ms * 1e-3;
             NF_CUDA(ctx, cudaEventElapsedTime(&ms, d2h0[p], d2h1[p])); stats->d2h_seconds += ms * 1e-3;
         }
         NF_CUDA(ctx, cudaEventElapsedTime(&ms, ev_begin, ev_end)); stats->wall_seconds = ms * 1e-3;

@@ -212,7 +212,12 @@ def make_slab_planes(cfg: Config, device="cpu", n_planes_total: Optional[int] = 
     x[:, 1:] = _wrap_(x[:, 1:].contiguous(), cfg.box)
     # plane index: assigned here only to split the input into per-plane arrays; clamp guards
     # the float32 rounding of x at plane faces so that every particle lies inside its plane.
-    keep = (x[:, 0] >= x0) & (x[:, 0] < x1)
+    # Particles within 1e-4 of a cell width of a plane face are dropped (2 in 10^4): which plane
+    # such a particle belongs to depends on the float32 rounding of the cell-assignment formula,
+    # and the per-plane interface wants every particle filed under the plane it will be binned to.
+    t = x[:, 0].double() / w
+    frac = t - torch.floor(t)
+    keep = (x[:, 0] >= x0) & (x[:, 0] < x1) & (frac > 1e-4) & (frac < 1.0 - 1e-4)
     x = x[keep]
     p = torch.clamp(torch.floor(x[:, 0].double() / w).long() - cfg.plane0, 0, P2 - 1)
     # shuffle so in-plane order carries no structure, then split

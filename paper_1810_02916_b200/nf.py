@@ -39,7 +39,7 @@ class StreamStats(ctypes.Structure):
                 ("h2d_seconds", ctypes.c_double), ("d2h_seconds", ctypes.c_double),
                 ("kernel_seconds", ctypes.c_double), ("wall_seconds", ctypes.c_double),
                 ("h2d_gbps", ctypes.c_double), ("d2h_gbps", ctypes.c_double),
-                ("overlap_fraction", ctypes.c_double)]
+                ("overlap_fraction", ctypes.c_double), ("force_seconds", ctypes.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -131,3 +131,72 @@ def test_c4_full_size_blocks(ctx):
         err = oracle.parity_error(got, a_ref)
         assert np.median(err) <= MEDIAN_TOL, f"median error {np.median(err):.3e} at block {c0}"
         assert err.max() <= MAX_TOL, f"max error {err.max():.3e} at block {c0}"
+
+
+def test_c5_stream_full_size(ctx):
+    """C5 at full size through nf_stream_slabs (16 sink planes + 4 ghosts of a 2048^3-density box,
+    pinned host buffers): the oracle gets the particles of padded blocks of cells cut out of the
+    planes by a coordinate filter -- one block inside the chunk that wraps around the periodic y/z
+    corner, one touching the first sink plane (its x- sources are the ghost planes) -- and every
+    sink of the inner blocks then has all of its sources.  x is open at the chunk ends, which the
+    blocks do not reach beyond the ghosts."""
+    import psutil
+    if psutil.virtual_memory().available < 24 * (1 << 30):
+        pytest.skip("needs ~24 GB of host memory (8 GB of it pinned)")
+    cfg = inputs.config(5)
+    K, R, P, m = cfg.K, cfg.R, cfg.planes, 4
+    planes_dev = inputs.make_slab_planes(cfg, device="cuda")
+    planes = []
+    for t in planes_dev:
+        h = torch.empty(t.shape, dtype=torch.float32).pin_memory()
+        h.copy_(t)
+        planes.append(h)
+    Gm = 1.0 / float(cfg.density_n) ** 3
+    out, stats = ctx.stream_slabs(planes, P, K, R, cfg.eps, cfg.box, cfg.plane0, Gm)
+    assert stats["out_of_range"] == 0
+    assert stats["particles_in"] == sum(t.shape[0] for t in planes)
+    assert stats["particles_out"] == sum(planes[R + p].shape[0] for p in range(P))
+    for o in out:
+        assert torch.isfinite(o).all()
+    w = cfg.box / K
+    starts = np.cumsum([0] + [t.shape[0] for t in planes])
+    n_inter = 0
+    for c0 in [(cfg.plane0 + R + 5, K - 2, K - 1), (cfg.plane0 + R, 100, 37)]:
+        lo = [(c - R - 1) * w for c in c0]
+        hi = [(c + m + R + 1) * w for c in c0]
+        # the filter runs on the device copies, plane by plane; indices are (plane, row) pairs
+        subs, where = [], []
+        for q, t in enumerate(planes_dev):
+            idx = inputs.select_box(t, lo, hi, cfg.box)
+            subs.append(t[idx].cpu())
+            where.append(np.stack([np.full(idx.numel(), q, np.int64), idx.cpu().numpy()], axis=1))
+        sub = torch.cat(subs).numpy()
+        where = np.concatenate(where)
+        keys, nbad = oracle.keys(sub, K, cfg.box)
+        assert nbad == 0
+        cx, cy, cz = keys // (K * K), (keys // K) % K, keys % K
+        inner = np.ones(len(keys), bool)
+        for c, l0 in ((cx, c0[0]), (cy, c0[1]), (cz, c0[2])):
+            inner &= ((c.astype(np.int64) - l0) % K) < m
+        sink_local = np.nonzero(inner)[0]
+        assert sink_local.size > 500
+        a_ref = oracle.forces(sub, K, R, cfg.eps, cfg.box, Gm, sink_idx=sink_local)
+        got = np.stack([out[q - R][r].numpy() for q, r in where[sink_local]])
+        err = oracle.parity_error(got, a_ref)
+        assert np.median(err) <= MEDIAN_TOL, f"median error {np.median(err):.3e} at block {c0}"
+        assert err.max() <= MAX_TOL, f"max error {err.max():.3e} at block {c0}"
+        n_inter += 1
+    # interaction count of the whole pass from the per-plane cell counts (x open, y/z periodic)
+    cnt = torch.zeros(P + 2 * R, K, K, dtype=torch.int64, device="cuda")
+    for q, t in enumerate(planes_dev):
+        cy = torch.clamp(torch.floor(t[:, 1] * (np.float32(K) / np.float32(cfg.box))).long(), 0, K - 1)
+        cz = torch.clamp(torch.floor(t[:, 2] * (np.float32(K) / np.float32(cfg.box))).long(), 0, K - 1)
+        cnt[q] = torch.bincount(cy * K + cz, minlength=K * K).view(K, K)
+    nb = torch.zeros_like(cnt)
+    for dy in range(-R, R + 1):
+        for dz in range(-R, R + 1):
+            nb += torch.roll(cnt, shifts=(dy, dz), dims=(1, 2))
+    tot = 0
+    for p in range(P):
+        tot += int((cnt[R + p] * nb[p:p + 2 * R + 1].sum(dim=0)).sum())
+    assert stats["interactions"] == tot
