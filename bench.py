@@ -39,10 +39,10 @@ from paper_1810_02916_b200 import inputs  # noqa: E402
 
 FLOP_PER_INTERACTION = 20          # BASELINE.json convention (the paper counts 23)
 FP32_LANES_PER_SM = 128
-ORACLE_BLOCK = 24                  # the oracle's sample: sinks of a 24^3-cell block (~0.9 M sinks at 64 per cell)
+ORACLE_BLOCK = 44                  # the oracle's sample is drawn from the sinks of a 44^3-cell block (~5 M sinks at 64 per cell)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_forces_warp launch, from the `ncu --set full`
 # captures summarised under profiles/ (the file named there gives the command); None = not captured
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"C4-clustered-1024^3": 169.98e9}   # profiles/r01_interaction_kernel_c4_dram.md
 
 
 def read_peaks():
@@ -128,13 +128,17 @@ def time_oracle(sub, cfg, m, c0, budget_s=20.0):
     sink_idx = np.nonzero(inner)[0]
     # interactions of those sinks: count neighbours through the oracle's own cell counts
     cnt = np.bincount(keys, minlength=K ** 3).astype(np.uint32)
-    # pilot to size the timed sample
+    # two pilots (2 000 and 20 000 sinks) separate the call's fixed cost (its own binning of `sub`)
+    # from the per-sink cost; the timed sample is then sized to ~budget_s of CPU work
     rng = np.random.default_rng(1)
-    pilot = np.sort(rng.choice(sink_idx, min(len(sink_idx), 2000), replace=False))
-    t0 = time.perf_counter()
-    oracle.forces(sub, K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=pilot)
-    tp = max(time.perf_counter() - t0, 1e-4)
-    n_timed = int(min(len(sink_idx), max(len(pilot), len(pilot) * budget_s / tp)))
+    tp = []
+    for n_p in (2000, 20000):
+        pilot = np.sort(rng.choice(sink_idx, min(len(sink_idx), n_p), replace=False))
+        t0 = time.perf_counter()
+        oracle.forces(sub, K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=pilot)
+        tp.append((len(pilot), max(time.perf_counter() - t0, 1e-4)))
+    per_sink = max((tp[1][1] - tp[0][1]) / max(tp[1][0] - tp[0][0], 1), 1e-9)
+    n_timed = int(min(len(sink_idx), max(tp[1][0], budget_s / per_sink)))
     timed = np.sort(rng.choice(sink_idx, n_timed, replace=False))
     t0 = time.perf_counter()
     acc = oracle.forces(sub, K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=timed)

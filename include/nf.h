@@ -55,6 +55,12 @@ enum {
     NF_SOFT_PLUMMER = 1 /* Eq. 1: F = r/(r^2 + eps^2)^(3/2) */
 };
 
+/* Flag OR-ed into the `softening` argument of nf_forces / nf_forces_ex: sources carry their own
+ * masses in the .w lane of pos_sorted (written by nf_bin_m) and `Gm` is then G alone:
+ * a_i = G * sum_j m_j f(|d|) d.  The paper's runs use equal masses; SURVEY.md Sec. 8(f) rank 1. */
+#define NF_MASS_W 0x100
+#define NF_SOFT_LAW_MASK 0xff
+
 #define NF_MAX_K 1024 /* K^3 must fit a uint32 key; radix digits are per-axis cell indices */
 #define NF_MAX_R 3
 
@@ -100,6 +106,13 @@ int nf_bin(nf_ctx *ctx, const float *pos_xyz, int64_t N, int K, float box,
            float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,
            void *stream);
 
+/* nf_bin_m -- nf_bin with per-particle masses: mass (dev in, N float32, caller's order, nullable)
+ * is carried into the .w lane of pos_sorted (pos_sorted[s].w = mass[perm[s]]; 0 when mass is
+ * NULL, which makes nf_bin_m identical to nf_bin).  Everything else as for nf_bin. */
+int nf_bin_m(nf_ctx *ctx, const float *pos_xyz, const float *mass, int64_t N, int K, float box,
+             float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,
+             void *stream);
+
 /* Synchronises `stream`, stores the number of out-of-range particles seen by the last nf_bin
  * (or nf_stream_slabs) on this context in *n, and returns NF_ERR_RANGE if it is non-zero. */
 int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream);
@@ -121,7 +134,7 @@ int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream);
  *   eps          softening length > 0: eps_s of Eq. 2, or eps_p of Eq. 1 (no 2.16 factor is
  *                applied inside the library; see nf_spline_equivalent_eps)
  *   Gm           G times the (equal) particle mass
- *   softening    NF_SOFT_SPLINE or NF_SOFT_PLUMMER
+ *   softening    NF_SOFT_SPLINE or NF_SOFT_PLUMMER, optionally | NF_MASS_W
  *   acc_xyz      dev out  N x 3 float32
  *
  * float32 in, float32 accumulate (per source tile, with a compensated outer sum), float32
@@ -130,6 +143,23 @@ int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream);
 int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
               const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
               float eps, float box, float Gm, int softening, float *acc_xyz, void *stream);
+
+/*
+ * nf_forces_ex -- nf_forces with the outputs the time-step criterion needs (PAPER.md:194, :207:
+ * "TimeStepAccel times the maximum of v_rms/a_max computed within each cell"; SURVEY.md Sec. 8(f)
+ * rank 2), reduced inside the interaction kernel's epilogue:
+ *
+ *   cell_amax   dev out, nullable  K^3 float32: max over the particles of each cell of |a_i|
+ *               (2-norm of the float32 acceleration written to acc_xyz); 0 for empty cells.
+ *               Exact and order-independent: an integer atomicMax on the float bit patterns.
+ *   softening   may carry NF_MASS_W (per-particle source masses, see above)
+ *
+ * nf_forces(...) is nf_forces_ex(..., cell_amax = NULL, ...).
+ */
+int nf_forces_ex(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
+                 const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
+                 float eps, float box, float Gm, int softening, float *acc_xyz,
+                 float *cell_amax, void *stream);
 
 /*
  * nf_forces_host -- the whole path from HOST buffers: H2D copy of the positions, nf_bin,

@@ -9,6 +9,7 @@ from .nf_oracle import (  # noqa: F401
     keys,
     bin_particles,
     forces,
+    cell_amax,
     interactions,
     spline_over_r,
     plummer_over_r,

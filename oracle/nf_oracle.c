@@ -142,10 +142,14 @@ double nfo_plummer_over_r(double r, double eps_p)
  * sink_idx: original indices of the sinks to evaluate (NULL = all N, in input order).
  * acc: n_sinks x 3 doubles, in the order of sink_idx.
  * softening: 0 = spline (Eq. 2, eps = eps_s), 1 = Plummer (Eq. 1, eps = eps_p).
+ * mass: NULL = equal masses (the paper's case; Gm = G*m), else N float32 source
+ *       masses in input order and a_i = Gm * sum_j m_j F d/|d| with Gm = G (SURVEY.md Sec. 8(f) rank 1:
+ *       the pair force of PAPER.md:37 between unequal masses is G m_i m_j F, so the acceleration of i
+ *       carries m_j).
  * Returns 0, or -1 on bad arguments (K < 2R+1 would list a cell twice). */
-int nfo_forces(const float *pos, int64_t N, int K, int R, double eps, float box, double Gm,
-               const int64_t *sink_idx, int64_t n_sinks, int softening, int nthreads,
-               double *acc)
+int nfo_forces_m(const float *pos, const float *mass, int64_t N, int K, int R, double eps, float box, double Gm,
+                 const int64_t *sink_idx, int64_t n_sinks, int softening, int nthreads,
+                 double *acc)
 {
     if (K < 2 * R + 1 || R < 0 || !(eps > 0.0) || !(box > 0.0f) || N < 0) return -1;
     int64_t ncell = (int64_t)K * K * K;
@@ -158,11 +162,13 @@ int nfo_forces(const float *pos, int64_t N, int K, int R, double eps, float box,
     memcpy(cursor, off, sizeof(uint64_t) * (size_t)ncell);
     /* cell-contiguous copies of the GLOBAL positions, promoted to double */
     double *X = (double *)malloc(sizeof(double) * 3 * (size_t)(N > 0 ? N : 1));
+    double *M = mass ? (double *)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1)) : NULL;
     for (int64_t i = 0; i < N; i++) {
         uint64_t s = cursor[key[i]]++;
         X[3 * s + 0] = (double)pos[3 * i + 0];
         X[3 * s + 1] = (double)pos[3 * i + 1];
         X[3 * s + 2] = (double)pos[3 * i + 2];
+        if (M) M[s] = (double)mass[i];
     }
     free(cursor);
     if (sink_idx == NULL) n_sinks = N;
@@ -201,6 +207,7 @@ int nfo_forces(const float *pos, int64_t N, int K, int R, double eps, float box,
                         double r = sqrt(r2);
                         double f = softening ? nfo_plummer_over_r(r, eps)
                                              : nfo_spline_over_r(r, eps);
+                        if (M) f *= M[j];
                         ax += f * ddx;
                         ay += f * ddy;
                         az += f * ddz;
@@ -213,9 +220,29 @@ int nfo_forces(const float *pos, int64_t N, int K, int R, double eps, float box,
         acc[3 * s + 2] = Gm * az;
     }
     free(X);
+    free(M);
     free(off);
     free(key);
     return 0;
+}
+
+int nfo_forces(const float *pos, int64_t N, int K, int R, double eps, float box, double Gm,
+               const int64_t *sink_idx, int64_t n_sinks, int softening, int nthreads,
+               double *acc)
+{
+    return nfo_forces_m(pos, NULL, N, K, R, eps, box, Gm, sink_idx, n_sinks, softening, nthreads, acc);
+}
+
+/* Per-cell maximum of |a| (2-norm), the quantity the time-step criterion takes "within each cell"
+ * (PAPER.md:194, :207).  acc: N x 3 doubles in input order; key: the particles' cell keys;
+ * amax: ncell doubles, 0 for empty cells.  The definition written out. */
+void nfo_cell_amax(const double *acc, const uint32_t *key, int64_t N, int64_t ncell, double *amax)
+{
+    for (int64_t c = 0; c < ncell; c++) amax[c] = 0.0;
+    for (int64_t i = 0; i < N; i++) {
+        double a = sqrt(acc[3 * i] * acc[3 * i] + acc[3 * i + 1] * acc[3 * i + 1] + acc[3 * i + 2] * acc[3 * i + 2]);
+        if (a > amax[key[i]]) amax[key[i]] = a;
+    }
 }
 
 /* Number of ordered (sink, source) pairs the near field requires, self pairs included

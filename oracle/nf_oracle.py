@@ -50,6 +50,12 @@ def _load():
         lib.nfo_forces.argtypes = [c_f32p, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                    ctypes.c_float, ctypes.c_double, c_i64p, ctypes.c_int64,
                                    ctypes.c_int, ctypes.c_int, c_f64p]
+        lib.nfo_forces_m.restype = ctypes.c_int
+        lib.nfo_forces_m.argtypes = [c_f32p, c_f32p, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                     ctypes.c_float, ctypes.c_double, c_i64p, ctypes.c_int64,
+                                     ctypes.c_int, ctypes.c_int, c_f64p]
+        lib.nfo_cell_amax.restype = None
+        lib.nfo_cell_amax.argtypes = [c_f64p, c_u32p, ctypes.c_int64, ctypes.c_int64, c_f64p]
         lib.nfo_interactions.restype = ctypes.c_int64
         lib.nfo_interactions.argtypes = [c_u32p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
         lib.nfo_spline_over_r.restype = ctypes.c_double
@@ -101,9 +107,10 @@ def bin_particles(pos, K: int, box: float):
 
 
 def forces(pos, K: int, R: int, eps: float, box: float, Gm: float, sink_idx=None,
-           softening: str = "spline", nthreads: int = 0):
+           softening: str = "spline", nthreads: int = 0, mass=None):
     """Near-field accelerations in double (Eq. 2 :243 / Eq. 1 :233).
-    Returns float64[n_sinks, 3] in the order of sink_idx (all particles, input order, if None)."""
+    Returns float64[n_sinks, 3] in the order of sink_idx (all particles, input order, if None).
+    mass: None = equal masses (Gm = G*m); else float32[N] source masses and Gm = G."""
     lib = _load()
     pos, p = _f32(pos)
     n = pos.shape[0]
@@ -114,11 +121,27 @@ def forces(pos, K: int, R: int, eps: float, box: float, Gm: float, sink_idx=None
         sp, ns = sink_idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), sink_idx.shape[0]
     acc = np.zeros((ns, 3), dtype=np.float64)
     soft = {"spline": 0, "plummer": 1}[softening]
-    rc = lib.nfo_forces(p, n, int(K), int(R), float(eps), float(box), float(Gm), sp, ns, soft,
-                        int(nthreads), acc.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    mp = None
+    if mass is not None:
+        mass = np.ascontiguousarray(mass, dtype=np.float32)
+        assert mass.shape == (n,)
+        mp = mass.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
+    rc = lib.nfo_forces_m(p, mp, n, int(K), int(R), float(eps), float(box), float(Gm), sp, ns, soft,
+                          int(nthreads), acc.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
     if rc != 0:
         raise ValueError("nfo_forces: bad arguments (need K >= 2R+1, R >= 0, eps > 0, box > 0)")
     return acc
+
+
+def cell_amax(acc, key, ncell: int):
+    """Per-cell maximum of |a|; acc float64[N,3] in input order, key uint32[N]."""
+    lib = _load()
+    acc = np.ascontiguousarray(acc, dtype=np.float64)
+    key = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.zeros(int(ncell), dtype=np.float64)
+    lib.nfo_cell_amax(acc.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), key.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)),
+                      acc.shape[0], int(ncell), out.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    return out
 
 
 def interactions(cell_count, K: int, R: int, sink_plane_lo: int = 0, sink_plane_hi=None) -> int:

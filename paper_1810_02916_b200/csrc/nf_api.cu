@@ -118,6 +118,12 @@ int nf_reserve(nf_ctx *ctx, int64_t maxN, int K)
 int nf_bin(nf_ctx *ctx, const float *pos_xyz, int64_t N, int K, float box, float *pos_sorted,
            uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset, void *stream)
 {
+    return nf_bin_m(ctx, pos_xyz, nullptr, N, K, box, pos_sorted, perm, cell_count, cell_offset, stream);
+}
+
+int nf_bin_m(nf_ctx *ctx, const float *pos_xyz, const float *mass, int64_t N, int K, float box, float *pos_sorted,
+             uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset, void *stream)
+{
     if (!ctx) return NF_ERR_ARG;
     NF_TRY(check_common(ctx, N, K, box));
     NF_ARG(ctx, cell_count && cell_offset, "nf_bin: cell_count / cell_offset must not be null");
@@ -127,7 +133,7 @@ int nf_bin(nf_ctx *ctx, const float *pos_xyz, int64_t N, int K, float box, float
     NF_TRY(nf_scratch_reserve(ctx, nf_bin_scratch_bytes(N, K, false)));
     nf_scratch_reset(ctx);
     NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, sizeof(unsigned long long), (cudaStream_t)stream));
-    return nf_bin_impl(ctx, pos_xyz, N, K, box, -1, pos_sorted, perm, cell_count, cell_offset, (cudaStream_t)stream);
+    return nf_bin_impl(ctx, pos_xyz, mass, N, K, box, -1, pos_sorted, perm, cell_count, cell_offset, (cudaStream_t)stream);
 }
 
 int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream)
@@ -152,13 +158,22 @@ static int check_force_args(nf_ctx *ctx, int K, int R, float eps, float Gm, int 
     NF_ARG(ctx, K >= 2 * R + 1, "K = %d < 2R+1 = %d would list a neighbour cell twice", K, 2 * R + 1);
     NF_ARG(ctx, eps > 0.0f && eps < 3.0e38f, "eps must be positive and finite");
     NF_ARG(ctx, Gm == Gm && fabsf(Gm) < 3.0e38f, "Gm must be finite");
-    NF_ARG(ctx, softening == NF_SOFT_SPLINE || softening == NF_SOFT_PLUMMER, "unknown softening %d", softening);
+    const int law = softening & NF_SOFT_LAW_MASK;
+    NF_ARG(ctx, (law == NF_SOFT_SPLINE || law == NF_SOFT_PLUMMER) && (softening & ~(NF_SOFT_LAW_MASK | NF_MASS_W)) == 0,
+           "unknown softening %d", softening);
     return NF_OK;
 }
 
 int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
               const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
               float eps, float box, float Gm, int softening, float *acc_xyz, void *stream)
+{
+    return nf_forces_ex(ctx, pos_sorted, cell_offset, cell_count, perm, N, K, R, eps, box, Gm, softening, acc_xyz, nullptr, stream);
+}
+
+int nf_forces_ex(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
+                 const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
+                 float eps, float box, float Gm, int softening, float *acc_xyz, float *cell_amax, void *stream)
 {
     if (!ctx) return NF_ERR_ARG;
     NF_TRY(check_common(ctx, N, K, box));
@@ -167,7 +182,10 @@ int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
     NF_ARG(ctx, N == 0 || (pos_sorted && acc_xyz), "nf_forces: null particle array with N > 0");
     NF_ARG(ctx, ((uintptr_t)pos_sorted & 15) == 0, "nf_forces: pos_sorted must be 16-byte aligned");
     NF_CUDA(ctx, cudaSetDevice(ctx->device));
-    if (N == 0) return NF_OK;
+    if (N == 0) {
+        if (cell_amax) NF_CUDA(ctx, cudaMemsetAsync(cell_amax, 0, sizeof(float) * (size_t)K * K * K, (cudaStream_t)stream));
+        return NF_OK;
+    }
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
@@ -180,7 +198,8 @@ int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
     cudaStream_t st = (cudaStream_t)stream;
     const float4 *ps = reinterpret_cast<const float4 *>(pos_sorted);
     NF_TRY(nf_encode_impl(ctx, p, ps, cell_offset, (size_t)K * K * K, enc, enc_h, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, ps, enc, enc_h, cell_offset, perm, acc_xyz, st));
+    if (cell_amax) NF_CUDA(ctx, cudaMemsetAsync(cell_amax, 0, sizeof(float) * (size_t)K * K * K, st));
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, ps, enc, enc_h, cell_offset, perm, acc_xyz, cell_amax, st));
     return nf_forces_impl(ctx, p, d_planes, st, true);
 }
 
@@ -207,6 +226,7 @@ int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, 
     NF_TRY(check_common(ctx, N, K, box));
     NF_TRY(check_force_args(ctx, K, R, eps, Gm, softening));
     NF_ARG(ctx, N == 0 || (pos_host && acc_host), "nf_forces_host: null particle array with N > 0");
+    NF_ARG(ctx, (softening & NF_MASS_W) == 0, "nf_forces_host takes no masses: NF_MASS_W is not accepted");
     NF_CUDA(ctx, cudaSetDevice(ctx->device));
     if (N == 0) return NF_OK;
     NF_TRY(nf_scratch_reserve(ctx, host_path_bytes(N, K)));
@@ -228,12 +248,12 @@ int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, 
     cudaStream_t st = (cudaStream_t)stream;
     NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, sizeof(unsigned long long), st));
     NF_CUDA(ctx, cudaMemcpyAsync(raw, pos_host, n * 12, cudaMemcpyHostToDevice, st));
-    NF_TRY(nf_bin_impl(ctx, raw, N, K, box, -1, sorted, perm, count, off, st));
+    NF_TRY(nf_bin_impl(ctx, raw, nullptr, N, K, box, -1, sorted, perm, count, off, st));
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
     NF_TRY(nf_encode_impl(ctx, p, reinterpret_cast<const float4 *>(sorted), off, ncell, enc, enc_h, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, acc, st));
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, acc, nullptr, st));
     NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
     NF_CUDA(ctx, cudaMemcpyAsync(acc_host, acc, n * 12, cudaMemcpyDeviceToHost, st));
     NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));

@@ -152,7 +152,8 @@ __global__ void __launch_bounds__(RS_THREADS) k_radix_scatter(const uint32_t *__
 
 // gather positions into cell order and re-centre.  Offset contract:
 // hw = 0.5f*(box/(float)K); centre = (float)(2c+1)*hw; o = x - centre (no FMA contraction).
-__global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pos, const uint32_t *__restrict__ keys_sorted,
+__global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pos, const float *__restrict__ mass,
+                                                const uint32_t *__restrict__ keys_sorted,
                                                 const uint32_t *__restrict__ perm, int64_t N, int K, float hw, int plane_cx,
                                                 float4 *__restrict__ pos_sorted)
 {
@@ -168,7 +169,7 @@ __global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pos, c
     o.x = __fsub_rn(x, __fmul_rn((float)(2 * cx + 1), hw));
     o.y = __fsub_rn(y, __fmul_rn((float)(2 * cy + 1), hw));
     o.z = __fsub_rn(z, __fmul_rn((float)(2 * cz + 1), hw));
-    o.w = 0.0f;
+    o.w = mass ? mass[i] : 0.0f;           // the spare lane carries the particle's mass when one is given
     pos_sorted[s] = o;
 }
 
@@ -187,7 +188,7 @@ size_t nf_bin_scratch_bytes(int64_t N, int K, bool plane)
     return b + 4096;
 }
 
-int nf_bin_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, int plane_cx,
+int nf_bin_impl(nf_ctx *ctx, const float *pos, const float *mass, int64_t N, int K, float box, int plane_cx,
                 float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,
                 cudaStream_t st)
 {
@@ -238,7 +239,7 @@ int nf_bin_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, int 
         div *= (uint32_t)K;
     }
     float hw = 0.5f * (box / (float)K);
-    k_gather<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, kin, perm, N, K, hw, plane_cx, reinterpret_cast<float4 *>(pos_sorted));
+    k_gather<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, mass, kin, perm, N, K, hw, plane_cx, reinterpret_cast<float4 *>(pos_sorted));
     NF_LAUNCHED(ctx);
     return NF_OK;
 }

@@ -90,7 +90,7 @@ int nf_exclusive_scan_u32_u64(nf_ctx *ctx, const uint32_t *in, uint64_t *out, si
 // binning (nf_bin.cu).  plane_cx < 0: full box, keys (cx*K+cy)*K+cz over K^3 cells;
 // plane_cx >= 0: one x-plane, keys cy*K+cz over K^2 cells, particles must have cx == plane_cx.
 size_t nf_bin_scratch_bytes(int64_t N, int K, bool plane);
-int nf_bin_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, int plane_cx,
+int nf_bin_impl(nf_ctx *ctx, const float *pos, const float *mass /* nullable */, int64_t N, int K, float box, int plane_cx,
                 float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,
                 cudaStream_t st);
 
@@ -103,6 +103,7 @@ struct nf_plane_view {
     const uint64_t *off;      // K*K+1 exclusive offsets within this plane's arrays
     const uint32_t *perm;     // nullable
     float *acc;               // output for this plane (n x 3), nullable for ghost planes
+    float *amax;              // nullable: K*K per-cell maxima of |a| (zeroed by the caller; integer atomicMax on the float bits)
 };
 struct nf_force_params {
     int K;            // cells per side in y and z
@@ -120,7 +121,7 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
                    cudaStream_t st, bool record_timing);
 // the full box seen as K planes sharing one set of arrays: plane cx starts at cell cx*K*K
 int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
-                        const uint64_t *off, const uint32_t *perm, float *acc, cudaStream_t st);
+                        const uint64_t *off, const uint32_t *perm, float *acc, float *cell_amax, cudaStream_t st);
 // enc[s], enc_h[s] = the two encoded copies of pos[s] for the ncell cells described by off (cell index % K = cz);
 // they depend on p.eps, p.box, p.K
 int nf_encode_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, float4 *enc,

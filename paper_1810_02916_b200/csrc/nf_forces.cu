@@ -62,7 +62,7 @@ __device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 d; asm("mul.rn.ftz.f32x2
 // MODE 2: r^-3 only, nothing tracked: tiles that cannot hold a pair inside eps (source cells two
 //         or more cells away from the sinks' cell when a cell is wider than eps), and the
 //         Plummer law (r2_floor = eps^2).
-template <int MODE>
+template <int MODE, bool MASS>
 __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64 ys, const u64 zs, const ForceConsts &fc,
                                          u64 &ax, u64 &ay, u64 &az, float &rmin)
 {
@@ -83,6 +83,7 @@ __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64
     } else if (MODE == 1) {
         rmin = min3(rmin, r2a, r2b);
     }
+    if (MASS) f = mul2(f, pk(q.w, q.w));            // per-particle source mass (the .w lane)
     fma2_acc(ax, f, dx);
     fma2_acc(ay, f, dy);
     fma2_acc(az, f, dz);
@@ -91,23 +92,23 @@ __device__ __forceinline__ void interact(const float4 q, const u64 xs, const u64
 // q (a multiple of 2, >= 2) consecutive sources against the lane's FOUR sinks (two packed
 // pairs).  Two register sets alternate (the loads of the next two sources are issued before
 // the arithmetic of the current two), so no register is moved.
-template <int MODE>
+template <int MODE, bool MASS>
 __device__ __forceinline__ void pair4(const float4 a0, const float4 a1, const u64 (&xs)[2], const u64 (&ys)[2], const u64 (&zs)[2],
                                       const ForceConsts &fc, u64 (&ax)[2], u64 (&ay)[2], u64 (&az)[2], float &rmin)
 {
-    interact<MODE>(a0, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
-    interact<MODE>(a0, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
-    interact<MODE>(a1, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
-    interact<MODE>(a1, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
+    interact<MODE, MASS>(a0, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
+    interact<MODE, MASS>(a0, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
+    interact<MODE, MASS>(a1, xs[0], ys[0], zs[0], fc, ax[0], ay[0], az[0], rmin);
+    interact<MODE, MASS>(a1, xs[1], ys[1], zs[1], fc, ax[1], ay[1], az[1], rmin);
 }
-template <int MODE>
+template <int MODE, bool MASS>
 __device__ __forceinline__ void sweep(const float4 *__restrict__ src, int q, const u64 (&xs)[2], const u64 (&ys)[2], const u64 (&zs)[2],
                                       const ForceConsts &fc, u64 (&ax)[2], u64 (&ay)[2], u64 (&az)[2], float &rmin)
 {
     const float4 *end = src + q;
     if (q & 2) {
         const float4 c0 = src[0], c1 = src[1];
-        pair4<MODE>(c0, c1, xs, ys, zs, fc, ax, ay, az, rmin);
+        pair4<MODE, MASS>(c0, c1, xs, ys, zs, fc, ax, ay, az, rmin);
         src += 2;
     }
     if (src < end) {
@@ -115,10 +116,10 @@ __device__ __forceinline__ void sweep(const float4 *__restrict__ src, int q, con
 #pragma unroll 2
         do {
             const float4 b0 = src[2], b1 = src[3];
-            pair4<MODE>(a0, a1, xs, ys, zs, fc, ax, ay, az, rmin);
+            pair4<MODE, MASS>(a0, a1, xs, ys, zs, fc, ax, ay, az, rmin);
             a0 = src[4]; a1 = src[5];          // past the slice in the last round: loaded, never used
             src += 4;
-            pair4<MODE>(b0, b1, xs, ys, zs, fc, ax, ay, az, rmin);
+            pair4<MODE, MASS>(b0, b1, xs, ys, zs, fc, ax, ay, az, rmin);
         } while (src < end);
     }
 }
@@ -179,8 +180,8 @@ __global__ void __launch_bounds__(256) k_encode(const float4 *__restrict__ pos, 
     for (uint64_t s = s0 + lane; s < s1; s += 32) {
         const float4 o = pos[s];
         const float x = o.x * scale, y = o.y * scale;
-        enc[s] = make_float4(x, y, fmaf(o.z, scale, ez), 0.f);
-        enc_h[s] = make_float4(x, y, fmaf(o.z, scale, eh), 0.f);
+        enc[s] = make_float4(x, y, fmaf(o.z, scale, ez), o.w);      // .w: the particle's mass (0 when none was given)
+        enc_h[s] = make_float4(x, y, fmaf(o.z, scale, eh), o.w);
     }
 }
 
@@ -194,7 +195,20 @@ __global__ void __launch_bounds__(256) k_encode(const float4 *__restrict__ pos, 
 // Poisson(64) cells against ~91 % for an even split.
 // ------------------------------------------------------------------------------------------
 constexpr int SPLIT_MAX = 4;       // tasks per remainder (< 128 sinks) at most
-constexpr int HEAVY_N = 256;       // cells with at least this many sinks are scheduled first
+constexpr int XB = 8;              // sink planes per block of the task order (see task_slot)
+
+// Position of sink cell (plane ix of n_sink_planes, cyz) in the task order: blocks of XB planes,
+// inside a block y is the slow index, then the plane, then z.  The warps working at any moment then
+// share (XB + 2R) x (2R + 1) rows of source cells per step in y instead of (2R + 1)^2 rows per plane:
+// with planes larger than the L2 (C4: 67 MB each) this cuts the re-reads from DRAM threefold.
+__device__ __forceinline__ size_t task_slot(int ix, int cyz, int K, int n_sink_planes)
+{
+    const int b0 = ix / XB * XB;
+    const int bw = min(XB, n_sink_planes - b0);
+    const int cy = cyz / K, cz = cyz - cy * K;
+    return ((size_t)b0 * K + (size_t)cy * bw + (size_t)(ix - b0)) * K + cz;
+}
+constexpr int HEAVY_N = 1024;         // cells with at least this many sinks are scheduled first
 
 struct Task {
     uint32_t cyz;     // cell index within the plane, cy*K + cz
@@ -214,7 +228,7 @@ __global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restr
     const int cyz = blockIdx.x * blockDim.x + threadIdx.x;
     const int KK = p.K * p.K;
     if (cyz >= KK) return;
-    const size_t nc = (size_t)gridDim.y * KK, c = (size_t)blockIdx.y * KK + cyz;
+    const size_t nc = (size_t)gridDim.y * KK, c = task_slot((int)blockIdx.y, cyz, p.K, (int)gridDim.y);
     const uint64_t *off = planes[p.sink_lo + blockIdx.y].off;
     const uint64_t n = off[cyz + 1] - off[cyz];
     const uint32_t nt = (uint32_t)(n >> 7) + c_split.nt[n & 127];
@@ -231,7 +245,7 @@ __global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restri
     const int cyz = blockIdx.x * blockDim.x + threadIdx.x;
     const int KK = p.K * p.K;
     if (cyz >= KK) return;
-    const size_t nc = (size_t)gridDim.y * KK, c = (size_t)blockIdx.y * KK + cyz;
+    const size_t nc = (size_t)gridDim.y * KK, c = task_slot((int)blockIdx.y, cyz, p.K, (int)gridDim.y);
     const uint64_t *off = planes[p.sink_lo + blockIdx.y].off;
     const uint64_t n = off[cyz + 1] - off[cyz];
     const size_t e = n >= HEAVY_N ? c : nc + c;
@@ -298,7 +312,7 @@ struct TileDesc {
     uint32_t start, n, meta;                // n == 0: no more tiles
 };
 
-template <int R>
+template <int R, bool MASS>
 __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_view *__restrict__ planes, const nf_force_params p,
                                                                const ForceConsts fc, const Task *__restrict__ tasks,
                                                                uint32_t *__restrict__ ctl)
@@ -485,14 +499,14 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             else if (sticky_col == col || (d0.meta >> 24) != 0) mode = 0;
             else if ((fc.flags & FC_FAR_OK) && max(abs(dxi - R), abs(dyi - R)) >= 2) mode = 2;
             if (active) {
-                if (mode == 1) sweep<1>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-                else if (mode == 2) sweep<2>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-                else sweep<0>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                if (mode == 1) sweep<1, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                else if (mode == 2) sweep<2, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                else sweep<0, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
             }
             if (mode == 1 && __any_sync(0xffffffffu, rmin < fc.eps2_test)) {
                 sticky_col = col;
                 ax[0] = ax[1] = ay[0] = ay[1] = az[0] = az[1] = 0;
-                if (active) sweep<0>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                if (active) sweep<0, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
             }
 #pragma unroll
             for (int h = 0; h < 2; h++) {
@@ -520,6 +534,7 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             }
         }
         __syncwarp();
+        float a2max = 0.f;
         for (int i = lane; i < n; i += 32) {
             const int l = i >> 2, h = (i & 3) * 3;
             double sx = 0.0, sy = 0.0, sz = 0.0;
@@ -527,13 +542,23 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                 const double *d = red + (size_t)(pp * L + l) * 12 + h;
                 sx += d[0]; sy += d[1]; sz += d[2];
             }
+            const float fx = (float)(sx * (double)fc.out_scale), fy = (float)(sy * (double)fc.out_scale),
+                        fz = (float)(sz * (double)fc.out_scale);
+            a2max = fmaxf(a2max, fx * fx + fy * fy + fz * fz);
             if (sp.acc) {
                 const uint64_t si = s0 + (uint64_t)i;
                 const uint64_t o = sp.perm ? (uint64_t)sp.perm[si] : si;
-                sp.acc[3 * o + 0] = (float)(sx * (double)fc.out_scale);
-                sp.acc[3 * o + 1] = (float)(sy * (double)fc.out_scale);
-                sp.acc[3 * o + 2] = (float)(sz * (double)fc.out_scale);
+                sp.acc[3 * o + 0] = fx;
+                sp.acc[3 * o + 1] = fy;
+                sp.acc[3 * o + 2] = fz;
             }
+        }
+        if (sp.amax) {
+            // per-cell maximum of |a| for the time-step criterion: the order of
+            // non-negative floats is the order of their bit patterns, so an integer atomicMax is exact
+            // and independent of the order in which a cell's tasks arrive
+            for (int d = 16; d > 0; d >>= 1) a2max = fmaxf(a2max, __shfl_xor_sync(0xffffffffu, a2max, d));
+            if (lane == 0) atomicMax(reinterpret_cast<unsigned int *>(sp.amax) + task.cyz, __float_as_uint(sqrtf(a2max)));
         }
         __syncwarp();
     }
@@ -566,7 +591,7 @@ __global__ void __launch_bounds__(256) k_interactions(const uint32_t *__restrict
 }
 
 __global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
-                              const uint64_t *off, const uint32_t *perm, float *acc)
+                              const uint64_t *off, const uint32_t *perm, float *acc, float *amax)
 {
     int cx = blockIdx.x * blockDim.x + threadIdx.x;
     if (cx >= K) return;
@@ -577,6 +602,7 @@ __global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, c
     v.off = off + (size_t)cx * K * K;
     v.perm = perm;
     v.acc = acc;
+    v.amax = amax ? amax + (size_t)cx * K * K : nullptr;
     planes[cx] = v;
 }
 
@@ -621,7 +647,7 @@ ForceConsts make_consts(const nf_force_params &p)
     float scale = ldexpf(1.0f, -e);    // eps*scale in [0.5, 1)
     if (p.eps * scale < 0.70710678f) scale *= 2.0f;  // -> [0.7071, 1.4142)
     const double es = (double)p.eps * (double)scale;
-    const bool plummer = p.softening == NF_SOFT_PLUMMER;
+    const bool plummer = (p.softening & NF_SOFT_LAW_MASK) == NF_SOFT_PLUMMER;
     fc.scale = scale;
     fc.ws = (p.box / (float)p.K) * scale;
     fc.A = (float)(10.0 / (es * es * es));
@@ -705,9 +731,9 @@ int nf_forces_init(nf_ctx *ctx)
 }
 
 int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
-                        const uint64_t *off, const uint32_t *perm, float *acc, cudaStream_t st)
+                        const uint64_t *off, const uint32_t *perm, float *acc, float *cell_amax, cudaStream_t st)
 {
-    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, enc, enc_h, off, perm, acc);
+    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, enc, enc_h, off, perm, acc, cell_amax);
     NF_LAUNCHED(ctx);
     return NF_OK;
 }
@@ -732,19 +758,19 @@ int nf_interactions_planes(nf_ctx *ctx, const nf_force_params &p, const nf_plane
     return NF_OK;
 }
 
-template <int R>
+template <int R, bool MASS>
 static int launch_warp(nf_ctx *ctx, const nf_force_params &p, const ForceConsts &fc, const nf_plane_view *d_planes,
                        const Task *tasks, uint32_t *ctl, cudaStream_t st)
 {
     const size_t smem = sizeof(WarpShared<R>) * WARPS;
-    NF_CUDA(ctx, cudaFuncSetAttribute(k_forces_warp<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NF_CUDA(ctx, cudaFuncSetAttribute(k_forces_warp<R, MASS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    NF_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_forces_warp<R>, WARPS * 32, smem));
+    NF_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_forces_warp<R, MASS>, WARPS * 32, smem));
     if (occ < 1) occ = 1;
     const size_t want = (max_tasks(p) + WARPS - 1) / WARPS;
     size_t blocks = (size_t)ctx->sm_count * occ;
     if (blocks > want) blocks = want;
-    k_forces_warp<R><<<(unsigned)blocks, WARPS * 32, smem, st>>>(d_planes, p, fc, tasks, ctl);
+    k_forces_warp<R, MASS><<<(unsigned)blocks, WARPS * 32, smem, st>>>(d_planes, p, fc, tasks, ctl);
     NF_LAUNCHED(ctx);
     return NF_OK;
 }
@@ -776,11 +802,16 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
     }
     if (record_timing) NF_CUDA(ctx, cudaEventRecord(ctx->ev_kern0, st));
     if (n_sink_planes > 0) {
-        switch (p.R) {
-        case 0: NF_TRY(launch_warp<0>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
-        case 1: NF_TRY(launch_warp<1>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
-        case 2: NF_TRY(launch_warp<2>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
-        default: NF_TRY(launch_warp<3>(ctx, p, fc, d_planes, tasks, ctl, st)); break;
+        const bool mass = (p.softening & NF_MASS_W) != 0;
+        switch (p.R * 2 + (mass ? 1 : 0)) {
+        case 0: NF_TRY((launch_warp<0, false>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
+        case 1: NF_TRY((launch_warp<0, true>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
+        case 2: NF_TRY((launch_warp<1, false>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
+        case 3: NF_TRY((launch_warp<1, true>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
+        case 4: NF_TRY((launch_warp<2, false>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
+        case 5: NF_TRY((launch_warp<2, true>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
+        case 6: NF_TRY((launch_warp<3, false>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
+        default: NF_TRY((launch_warp<3, true>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
         }
     }
     if (record_timing) {

@@ -78,7 +78,7 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
     NF_ARG(ctx, P + 2 * R <= K, "P + 2R = %d planes exceed K = %d", P + 2 * R, K);
     NF_ARG(ctx, eps > 0.0f && eps < 3.0e38f, "eps must be positive and finite");
     NF_ARG(ctx, box > 0.0f && box < 3.0e38f, "box must be positive and finite");
-    NF_ARG(ctx, softening == NF_SOFT_SPLINE || softening == NF_SOFT_PLUMMER, "unknown softening %d", softening);
+    NF_ARG(ctx, softening == NF_SOFT_SPLINE || softening == NF_SOFT_PLUMMER, "unknown softening %d (the slab stream carries no masses)", softening);
     const int NP = P + 2 * R;
     int64_t max_n = 1;
     for (int q = 0; q < NP; q++) {
@@ -169,6 +169,7 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         S->h_views[q].off = sl.off;
         S->h_views[q].perm = sl.perm;
         S->h_views[q].acc = sl.acc;
+        S->h_views[q].amax = nullptr;
     }
     NF_CUDA(ctx, cudaMemcpyAsync(S->d_views, S->h_views, sizeof(nf_plane_view) * NP, cudaMemcpyHostToDevice, st));
     NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st));
@@ -206,7 +207,7 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         nf_scratch_reset(ctx);
         const int cx = ((plane0 + q) % K + K) % K;
         // counters[0] accumulates out-of-range / wrong-plane particles over all planes
-        NF_TRY(nf_bin_impl(ctx, sl.raw, plane_n[q], K, box, cx, sl.sorted, sl.perm, sl.count, sl.off, st));
+        NF_TRY(nf_bin_impl(ctx, sl.raw, nullptr, plane_n[q], K, box, cx, sl.sorted, sl.perm, sl.count, sl.off, st));
         NF_TRY(nf_encode_impl(ctx, fp, (const float4 *)sl.sorted, sl.off, ncell, (float4 *)sl.enc, (float4 *)sl.enc_h, st));
         NF_CUDA(ctx, cudaEventRecord(bin1[q], st));
 
