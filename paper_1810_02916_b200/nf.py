@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libnf.so")
 
 NF_OK, NF_ERR_ARG, NF_ERR_NOMEM, NF_ERR_CUDA, NF_ERR_RANGE = 0, 1, 2, 3, 4
 SOFT_SPLINE, SOFT_PLUMMER = 0, 1
+NF_MASS_W = 0x100
 _SOFT = {"spline": SOFT_SPLINE, "plummer": SOFT_PLUMMER}
 
 # every symbol include/nf.h declares
@@ -69,6 +70,10 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.nf_reserve.argtypes = [vp, i64, i32]
     lib.nf_bin.restype = i32
     lib.nf_bin.argtypes = [vp, vp, i64, i32, f32, vp, vp, vp, vp, vp]
+    lib.nf_bin_m.restype = i32
+    lib.nf_bin_m.argtypes = [vp, vp, vp, i64, i32, f32, vp, vp, vp, vp, vp]
+    lib.nf_forces_ex.restype = i32
+    lib.nf_forces_ex.argtypes = [vp, vp, vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp, vp]
     lib.nf_out_of_range.restype = i32
     lib.nf_out_of_range.argtypes = [vp, ctypes.POINTER(i64), vp]
     lib.nf_forces.restype = i32
@@ -147,9 +152,11 @@ class Context:
     def reserve(self, maxN: int, K: int):
         self._check(self.lib.nf_reserve(self._h, int(maxN), int(K)))
 
-    def bin(self, pos: torch.Tensor, K: int, box: float, out: Optional[Binned] = None, stream=None) -> Binned:
-        """nf_bin: pos float32 [N, 3] on the device -> cell-contiguous arrays (written into
-        ``out`` if given, so repeated calls reuse the same device buffers)."""
+    def bin(self, pos: torch.Tensor, K: int, box: float, out: Optional[Binned] = None, stream=None,
+            mass: Optional[torch.Tensor] = None) -> Binned:
+        """nf_bin (nf_bin_m when ``mass`` float32 [N] is given: it lands in pos_sorted[:, 3]): pos float32
+        [N, 3] on the device -> cell-contiguous arrays (written into ``out`` if given, so repeated
+        calls reuse the same device buffers)."""
         assert pos.is_cuda and pos.dtype == torch.float32 and pos.dim() == 2 and pos.shape[1] == 3 and pos.is_contiguous()
         N = pos.shape[0]
         dev = pos.device
@@ -160,6 +167,11 @@ class Context:
                          torch.empty(ncell, dtype=torch.int32, device=dev),
                          torch.empty(ncell + 1, dtype=torch.int64, device=dev), N, int(K), float(box))
         assert out.N == N and out.K == int(K) and out.box == float(box)
+        if mass is not None:
+            assert mass.is_cuda and mass.dtype == torch.float32 and mass.shape == (N,) and mass.is_contiguous()
+            self._check(self.lib.nf_bin_m(self._h, _ptr(pos), _ptr(mass), N, int(K), float(box), _ptr(out.pos_sorted),
+                                          _ptr(out.perm), _ptr(out.cell_count), _ptr(out.cell_offset), self._stream(stream)))
+            return out
         self._check(self.lib.nf_bin(self._h, _ptr(pos), N, int(K), float(box), _ptr(out.pos_sorted), _ptr(out.perm),
                                     _ptr(out.cell_count), _ptr(out.cell_offset), self._stream(stream)))
         return out
@@ -170,10 +182,21 @@ class Context:
         return int(n.value)
 
     def forces(self, b: Binned, R: int, eps: float, Gm: float, softening: str = "spline",
-               original_order: bool = True, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
-        """nf_forces: accelerations float32 [N, 3] (caller's order if original_order)."""
+               original_order: bool = True, out: Optional[torch.Tensor] = None, stream=None,
+               use_mass: bool = False, cell_amax: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """nf_forces: accelerations float32 [N, 3] (caller's order if original_order).
+        use_mass: sources carry their masses in pos_sorted[:, 3] (NF_MASS_W; Gm is then G).
+        cell_amax: float32 [K^3] device tensor to receive the per-cell max |a| (nf_forces_ex)."""
         acc = out if out is not None else torch.empty(b.N, 3, dtype=torch.float32, device=b.pos_sorted.device)
         assert acc.is_cuda and acc.dtype == torch.float32 and acc.shape == (b.N, 3) and acc.is_contiguous()
+        if use_mass or cell_amax is not None:
+            if cell_amax is not None:
+                assert cell_amax.is_cuda and cell_amax.dtype == torch.float32 and cell_amax.numel() == b.K ** 3 and cell_amax.is_contiguous()
+            self._check(self.lib.nf_forces_ex(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset), _ptr(b.cell_count),
+                                              _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
+                                              float(b.box), float(Gm), _SOFT[softening] | (NF_MASS_W if use_mass else 0),
+                                              _ptr(acc), _ptr(cell_amax), self._stream(stream)))
+            return acc
         self._check(self.lib.nf_forces(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset), _ptr(b.cell_count),
                                        _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
                                        float(b.box), float(Gm), _SOFT[softening], _ptr(acc), self._stream(stream)))

@@ -224,3 +224,63 @@ def test_stream_slabs_small(ctx):
     assert stats["particles_in"] == allpos.shape[0] and stats["particles_out"] == sink_idx.size
     cnt = oracle.bin_particles(allpos, cfg.K, cfg.box)["cell_count"]
     assert stats["interactions"] == oracle.interactions(cnt, cfg.K, R, cfg.plane0 + R, cfg.plane0 + R + P)
+
+
+# ------------------------------------------------- next rows: masses, a_max
+@pytest.mark.parametrize("softening", ["spline", "plummer"])
+def test_forces_per_particle_masses(ctx, softening):
+    """nf_bin_m + NF_MASS_W: a_i = G sum_j m_j f d against the oracle with the same float32 masses;
+    the mass lane is carried through the sort bit for bit (pos_sorted.w = mass[perm])."""
+    cfg = inputs.scaled(inputs.config(3), 64 ** 3, 16)
+    cfg = inputs.dataclasses.replace(cfg, n_halos=24)
+    pos = inputs.make_positions(cfg).numpy()
+    rng = np.random.default_rng(5)
+    mass = np.exp(rng.normal(0.0, 1.0, cfg.N)).astype(np.float32)
+    eps = cfg.eps * (2.0 if softening == "plummer" else 1.0)
+    b = ctx.bin(torch.from_numpy(pos).cuda(), cfg.K, cfg.box, mass=torch.from_numpy(mass).cuda())
+    ref_b = oracle.bin_particles(pos, cfg.K, cfg.box)
+    assert np.array_equal(u32(b.perm), ref_b["perm"])
+    ps = b.pos_sorted.cpu().numpy()
+    assert np.array_equal(ps[:, 3].view(np.uint32), mass[ref_b["perm"]].view(np.uint32))
+    assert np.array_equal(ps[:, :3].view(np.uint32), ref_b["pos_sorted"][:, :3].view(np.uint32))
+    G = 1.0 / cfg.N
+    acc = ctx.forces(b, cfg.R, eps, G, softening=softening, use_mass=True).cpu().numpy()
+    sink_idx = np.sort(rng.choice(cfg.N, 40_000, replace=False))
+    ref = oracle.forces(pos, cfg.K, cfg.R, eps, cfg.box, G, sink_idx=sink_idx, softening=softening, mass=mass)
+    err = oracle.parity_error(acc[sink_idx], ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (np.median(err), err.max())
+    # unit masses through the mass path == the scalar-Gm path, bit for bit
+    b1 = ctx.bin(torch.from_numpy(pos).cuda(), cfg.K, cfg.box, mass=torch.ones(cfg.N, device="cuda"))
+    a1 = ctx.forces(b1, cfg.R, eps, G, softening=softening, use_mass=True)
+    a0 = ctx.forces(b1, cfg.R, eps, G, softening=softening)
+    assert torch.equal(a1, a0)
+
+
+def test_cell_amax(ctx):
+    """nf_forces_ex: per-cell max |a| from the kernel's epilogue.  It must equal, bit for bit, the
+    maximum over the cell of the float32 norm of the accelerations the same call wrote (the
+    reduction is an integer atomicMax: exact, order-independent), and match the oracle's per-cell
+    maximum of its own double accelerations within the force tolerance."""
+    cfg = inputs.scaled(inputs.config(3), 64 ** 3, 16)
+    cfg = inputs.dataclasses.replace(cfg, n_halos=24)
+    pos = inputs.make_positions(cfg).numpy()
+    b = ctx.bin(torch.from_numpy(pos).cuda(), cfg.K, cfg.box)
+    amax = torch.full((cfg.K ** 3,), -1.0, device="cuda")
+    acc = ctx.forces(b, cfg.R, cfg.eps, cfg.Gm, cell_amax=amax)
+    acc0 = ctx.forces(b, cfg.R, cfg.eps, cfg.Gm)
+    assert torch.equal(acc, acc0)
+    key, _ = oracle.keys(pos, cfg.K, cfg.box)
+    a_ref = oracle.forces(pos, cfg.K, cfg.R, cfg.eps, cfg.box, cfg.Gm)
+    ref = oracle.cell_amax(a_ref, key, cfg.K ** 3)
+    got = amax.cpu().numpy().astype(np.float64)
+    cnt = np.bincount(key, minlength=cfg.K ** 3)
+    assert (got[cnt == 0] == 0).all() and (got >= 0).all()
+    rms = np.sqrt((a_ref ** 2).sum(axis=1).mean())
+    assert (np.abs(got - ref) <= 1e-4 * np.maximum(ref, rms)).all()
+    assert np.median(np.abs(got - ref)[cnt > 0] / ref[cnt > 0]) < 1e-5
+    # consistency with the accelerations of the same call: max over the cell of the float32 norm
+    a = acc.cpu().numpy()
+    n32 = np.sqrt((a[:, 0] * a[:, 0] + a[:, 1] * a[:, 1] + a[:, 2] * a[:, 2]).astype(np.float32))
+    own = np.zeros(cfg.K ** 3, np.float32)
+    np.maximum.at(own, key, n32)
+    assert np.allclose(got, own, rtol=3e-7, atol=0)

@@ -384,3 +384,86 @@ def test_parity_metric():
     rms = np.sqrt((25 + 0.01) / 2)
     e = oracle.parity_error(tst, ref)
     assert e[0] == pytest.approx(0.05 / 5.0) and e[1] == pytest.approx(0.01 / rms)
+
+
+# ------------------------------------------------- next rows: masses, a_max
+def test_masses_two_particle_and_momentum():
+    """Unequal masses: the pair force is G m_i m_j F (PAPER.md:37 with Eq. 2), so a_i carries m_j.
+    Two particles: |a_0| / |a_1| = m_1 / m_0 and each is m_other times the closed form; many
+    particles: total momentum change sum_i m_i a_i = 0 on a fully periodic box."""
+    eps, box, K = 0.01, 1.0, 8
+    d = np.array([0.3, -0.4, 0.5]) / np.sqrt(0.5) * 0.5 * eps        # |d| = eps/2: u s(u) = 2 (golden value)
+    pos = np.array([[0.51, 0.52, 0.53], [0.51, 0.52, 0.53] + d], dtype=np.float32)
+    m = np.array([3.0, 0.25], dtype=np.float32)
+    a = oracle.forces(pos, K, 2, eps, box, 1.0, mass=m)
+    sep = pos[1].astype(np.float64) - pos[0].astype(np.float64)
+    r = np.sqrt((sep ** 2).sum())
+    u = r / eps
+    closed = (10 - 15 * u + 6 * u * u) * r / eps ** 3
+    assert np.allclose(a[0], 0.25 * closed * sep / r, rtol=1e-12)
+    assert np.allclose(a[1], -3.0 * closed * sep / r, rtol=1e-12)
+    rng = np.random.default_rng(11)
+    pos = _clustered(4000, 1.0, rng)
+    pos = np.minimum(pos, np.nextafter(np.float32(1), np.float32(0)))
+    m = rng.uniform(0.1, 5.0, 4000).astype(np.float32)
+    a = oracle.forces(pos, 8, 2, 2e-3, 1.0, 1.0, mass=m)
+    p = (m.astype(np.float64)[:, None] * a)
+    assert np.abs(p.sum(axis=0)).max() < 1e-11 * np.sqrt((p ** 2).sum(axis=1)).sum()
+
+
+def test_masses_against_brute_force_and_superposition():
+    """Brute force with masses (no cell lists), equal masses == the scalar-Gm path, and linearity
+    in the source masses: a[m1 + m2] = a[m1] + a[m2]."""
+    rng = np.random.default_rng(12)
+    n, K, R, eps, box = 300, 6, 2, 0.05, 1.0
+    pos = rng.random((n, 3)).astype(np.float32)
+    m1 = rng.uniform(0.0, 2.0, n).astype(np.float32)
+    m2 = rng.uniform(0.0, 2.0, n).astype(np.float32)
+    x = pos.astype(np.float64)
+    c = cells_f32(pos, K, box)
+    ref = np.zeros((n, 3))
+    for i in range(n):
+        for j in range(n):
+            dl = []
+            for ax in range(3):
+                df = (c[j, ax] - c[i, ax]) % K
+                dl.append(df if df <= R else (df - K if df >= K - R else None))
+            if None in dl:
+                continue
+            img = [(c[i, ax] + dl[ax] - c[j, ax]) // K for ax in range(3)]
+            dv = x[j] + np.array(img) * box - x[i]
+            r = np.sqrt((dv ** 2).sum())
+            if r == 0:
+                continue
+            u = r / eps
+            f = (10 - 15 * u + 6 * u * u) / eps ** 3 if u < 1 else 1 / r ** 3
+            ref[i] += float(m1[j]) * f * dv
+    a1 = oracle.forces(pos, K, R, eps, box, 1.0, mass=m1)
+    assert np.allclose(a1, ref, rtol=1e-10, atol=1e-10 * np.abs(ref).max())
+    a2 = oracle.forces(pos, K, R, eps, box, 1.0, mass=m2)
+    a12 = oracle.forces(pos, K, R, eps, box, 1.0, mass=(m1.astype(np.float64) + m2).astype(np.float32))
+    # m1 + m2 is rounded to float32 once: compare with the same rounded masses split exactly
+    m12 = (m1.astype(np.float64) + m2).astype(np.float32)
+    a2x = oracle.forces(pos, K, R, eps, box, 1.0, mass=(m12.astype(np.float64) - m1).astype(np.float32))
+    assert np.allclose(a12, a1 + a2x, rtol=1e-6, atol=1e-6 * np.abs(a12).max())
+    assert np.abs(a2).max() > 0
+    eq = oracle.forces(pos, K, R, eps, box, 1.0, mass=np.full(n, 0.5, np.float32))
+    assert np.allclose(eq, oracle.forces(pos, K, R, eps, box, 0.5), rtol=1e-13, atol=0)
+
+
+def test_cell_amax_definition():
+    """Per-cell max |a| against a python loop; empty cells are 0; the maximum
+    over cells is the global maximum."""
+    rng = np.random.default_rng(13)
+    n, K = 500, 5
+    pos = rng.random((n, 3)).astype(np.float32)
+    a = oracle.forces(pos, K, 2, 0.02, 1.0, 1.0 / n)
+    key, _ = oracle.keys(pos, K, 1.0)
+    got = oracle.cell_amax(a, key, K ** 3)
+    mag = np.sqrt((a ** 2).sum(axis=1))
+    ref = np.zeros(K ** 3)
+    for i in range(n):
+        ref[key[i]] = max(ref[key[i]], mag[i])
+    assert np.array_equal(got, ref)
+    assert got.max() == mag.max()
+    assert (got[np.bincount(key, minlength=K ** 3) == 0] == 0).all()
