@@ -24,7 +24,8 @@ _SOFT = {"spline": SOFT_SPLINE, "plummer": SOFT_PLUMMER}
 # every symbol include/nf.h declares
 EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve", "nf_bin",
            "nf_out_of_range", "nf_forces", "nf_interactions", "nf_spline_equivalent_eps",
-           "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host"]
+           "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host",
+           "nf_bin_m", "nf_forces_ex"]
 
 
 class NFError(RuntimeError):
