@@ -162,6 +162,37 @@ int nf_forces_ex(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offs
                  float *cell_amax, void *stream);
 
 /*
+ * nf_kick_drift -- the leapfrog updates that follow the force in the slab pipeline (Table 1
+ * "Kick", "Drift").  The paper gives no formula, so the
+ * factors are the caller's (they absorb the cosmological prefactors of the time step):
+ *
+ *   v <- v + a * kick ;   x <- x + v * drift  (with the NEW v), wrapped once into [0, box)
+ *
+ * float32 contract, bit-reproducible: v1 = fma(a, kick, v) and x1 = fma(v1, drift, x), each a single
+ * rounding; then x1 >= box: x1 - box; x1 < 0: x1 + box; a result equal to box becomes 0.  One wrap only:
+ * the third time-step criterion keeps |v * drift| below 80 % of a cell width.
+ *
+ *   pos_xyz, vel_xyz   dev in/out  N x 3 float32 (updated in place)
+ *   acc_xyz            dev in      N x 3 float32, same order
+ */
+int nf_kick_drift(nf_ctx *ctx, float *pos_xyz, float *vel_xyz, const float *acc_xyz, int64_t N,
+                  float kick, float drift, float box, void *stream);
+
+/*
+ * nf_cell_vrms -- velocity reductions of the time-step criteria: the rms speed
+ * within each cell (criterion 2 pairs it with the a_max of nf_forces_ex) and the largest velocity
+ * component of any particle (criterion 3: "the step size times the maximum velocity must be less
+ * than 80% of a cell width").
+ *
+ *   vel_xyz      dev in   N x 3 float32 in the caller's order (perm given) or in sorted order (perm NULL)
+ *   perm, cell_offset     dev in   as written by nf_bin for the same particles
+ *   cell_vrms    dev out, nullable  K^3 float32: sqrt(mean |v|^2) over the cell's particles, 0 if empty
+ *   vmax         dev out, nullable  1 float32: max over particles and axes of |v_axis|
+ */
+int nf_cell_vrms(nf_ctx *ctx, const float *vel_xyz, const uint32_t *perm, const uint64_t *cell_offset,
+                 int64_t N, int K, float *cell_vrms, float *vmax, void *stream);
+
+/*
  * nf_forces_host -- the whole path from HOST buffers: H2D copy of the positions, nf_bin,
  * nf_forces, D2H copy of the accelerations (the paper's GPU rate "includes
  * PCIe bus transfer overheads").  All device buffers come from the context's scratch arena

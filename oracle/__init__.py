@@ -10,6 +10,8 @@ from .nf_oracle import (  # noqa: F401
     bin_particles,
     forces,
     cell_amax,
+    kick_drift,
+    cell_vrms,
     interactions,
     spline_over_r,
     plummer_over_r,

@@ -273,6 +273,50 @@ int64_t nfo_interactions(const uint32_t *cell_count, int K, int R, int sink_plan
     return total;
 }
 
+/* ---- kick and drift (Table 1 "Kick", "Drift") -----------------------------
+ * The paper names the two leapfrog updates but prints no formula; the factors are the caller's
+ * (DESIGN.md "Kick and drift").  float32 contract, written out: v1 = fmaf(a, kick, v) -- velocity
+ * first -- then x1 = fmaf(v1, drift, x) with the NEW velocity, each a single rounding (C99 fmaf),
+ * then one periodic wrap into [0, box): x1 >= box -> x1 - box; x1 < 0 -> x1 + box; a result that
+ * is not below box after that (x1 + box rounded up to box) -> 0.  Elementwise over the 3N
+ * coordinates, in place. */
+void nfo_kick_drift(float *pos, float *vel, const float *acc, int64_t N, float kick, float drift, float box)
+{
+    for (int64_t i = 0; i < 3 * N; i++) {
+        float v1 = fmaf(acc[i], kick, vel[i]);
+        float x1 = fmaf(v1, drift, pos[i]);
+        if (x1 >= box) x1 = x1 - box;
+        else if (x1 < 0.0f) x1 = x1 + box;
+        if (!(x1 < box)) x1 = 0.0f;
+        vel[i] = v1;
+        pos[i] = x1;
+    }
+}
+
+/* ---- velocity reductions of the time-step criteria -----------------------
+ * vrms[c] = sqrt(mean over the particles of cell c of |v|^2), 0 for empty cells (criterion 2 uses
+ * "v_rms/a_max computed within each cell"); *vmax = the largest |v_axis| of any particle
+ * (criterion 3: "the step size times the maximum velocity must be less than 80% of a cell width";
+ * cells are axis-aligned, so the component is what crosses a face -- DESIGN.md reading c18).
+ * vel: N x 3 float32 in input order; key: the particles' cell keys.  All in double. */
+void nfo_cell_vrms(const float *vel, const uint32_t *key, int64_t N, int64_t ncell, double *vrms, double *vmax)
+{
+    int64_t *cnt = (int64_t *)calloc((size_t)ncell, sizeof(int64_t));
+    double m = 0.0;
+    for (int64_t c = 0; c < ncell; c++) vrms[c] = 0.0;
+    for (int64_t i = 0; i < N; i++) {
+        double vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+        vrms[key[i]] += vx * vx + vy * vy + vz * vz;
+        cnt[key[i]]++;
+        if (fabs(vx) > m) m = fabs(vx);
+        if (fabs(vy) > m) m = fabs(vy);
+        if (fabs(vz) > m) m = fabs(vz);
+    }
+    for (int64_t c = 0; c < ncell; c++) vrms[c] = cnt[c] ? sqrt(vrms[c] / (double)cnt[c]) : 0.0;
+    *vmax = m;
+    free(cnt);
+}
+
 int nfo_max_threads(void)
 {
 #ifdef _OPENMP

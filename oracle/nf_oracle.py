@@ -56,6 +56,10 @@ def _load():
                                      ctypes.c_int, ctypes.c_int, c_f64p]
         lib.nfo_cell_amax.restype = None
         lib.nfo_cell_amax.argtypes = [c_f64p, c_u32p, ctypes.c_int64, ctypes.c_int64, c_f64p]
+        lib.nfo_kick_drift.restype = None
+        lib.nfo_kick_drift.argtypes = [c_f32p, c_f32p, c_f32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float, ctypes.c_float]
+        lib.nfo_cell_vrms.restype = None
+        lib.nfo_cell_vrms.argtypes = [c_f32p, c_u32p, ctypes.c_int64, ctypes.c_int64, c_f64p, c_f64p]
         lib.nfo_interactions.restype = ctypes.c_int64
         lib.nfo_interactions.argtypes = [c_u32p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
         lib.nfo_spline_over_r.restype = ctypes.c_double
@@ -142,6 +146,32 @@ def cell_amax(acc, key, ncell: int):
     lib.nfo_cell_amax(acc.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), key.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)),
                       acc.shape[0], int(ncell), out.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
     return out
+
+
+def kick_drift(pos, vel, acc, kick: float, drift: float, box: float):
+    """v <- v + a*kick; x <- wrap(x + v*drift) with the new v (Table 1 "Kick", "Drift"),
+    in the float32 contract of DESIGN.md.  Returns new (pos, vel) float32 arrays; inputs are not modified."""
+    lib = _load()
+    pos = np.array(pos, dtype=np.float32, order="C", copy=True)
+    vel = np.array(vel, dtype=np.float32, order="C", copy=True)
+    acc = np.ascontiguousarray(acc, dtype=np.float32)
+    assert pos.shape == vel.shape == acc.shape and pos.ndim == 2 and pos.shape[1] == 3
+    f = ctypes.POINTER(ctypes.c_float)
+    lib.nfo_kick_drift(pos.ctypes.data_as(f), vel.ctypes.data_as(f), acc.ctypes.data_as(f), pos.shape[0],
+                       float(kick), float(drift), float(box))
+    return pos, vel
+
+
+def cell_vrms(vel, key, ncell: int):
+    """(per-cell rms speed float64[ncell], max |v_axis|) -- PAPER.md:193-195."""
+    lib = _load()
+    vel = np.ascontiguousarray(vel, dtype=np.float32)
+    key = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.zeros(int(ncell), dtype=np.float64)
+    vmax = ctypes.c_double(0.0)
+    lib.nfo_cell_vrms(vel.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), key.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)),
+                      vel.shape[0], int(ncell), out.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), ctypes.byref(vmax))
+    return out, float(vmax.value)
 
 
 def interactions(cell_count, K: int, R: int, sink_plane_lo: int = 0, sink_plane_hi=None) -> int:

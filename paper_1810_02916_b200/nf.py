@@ -25,7 +25,7 @@ _SOFT = {"spline": SOFT_SPLINE, "plummer": SOFT_PLUMMER}
 EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve", "nf_bin",
            "nf_out_of_range", "nf_forces", "nf_interactions", "nf_spline_equivalent_eps",
            "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host",
-           "nf_bin_m", "nf_forces_ex"]
+           "nf_bin_m", "nf_forces_ex", "nf_kick_drift", "nf_cell_vrms"]
 
 
 class NFError(RuntimeError):
@@ -75,6 +75,10 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.nf_bin_m.argtypes = [vp, vp, vp, i64, i32, f32, vp, vp, vp, vp, vp]
     lib.nf_forces_ex.restype = i32
     lib.nf_forces_ex.argtypes = [vp, vp, vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp, vp]
+    lib.nf_kick_drift.restype = i32
+    lib.nf_kick_drift.argtypes = [vp, vp, vp, vp, i64, f32, f32, f32, vp]
+    lib.nf_cell_vrms.restype = i32
+    lib.nf_cell_vrms.argtypes = [vp, vp, vp, vp, i64, i32, vp, vp, vp]
     lib.nf_out_of_range.restype = i32
     lib.nf_out_of_range.argtypes = [vp, ctypes.POINTER(i64), vp]
     lib.nf_forces.restype = i32
@@ -202,6 +206,25 @@ class Context:
                                        _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
                                        float(b.box), float(Gm), _SOFT[softening], _ptr(acc), self._stream(stream)))
         return acc
+
+    def kick_drift(self, pos: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, kick: float, drift: float,
+                   box: float, stream=None):
+        """nf_kick_drift: v += a*kick; x = wrap(x + v*drift), in place on float32 [N, 3] device tensors."""
+        for t in (pos, vel, acc):
+            assert t.is_cuda and t.dtype == torch.float32 and t.dim() == 2 and t.shape[1] == 3 and t.is_contiguous()
+        assert pos.shape == vel.shape == acc.shape
+        self._check(self.lib.nf_kick_drift(self._h, _ptr(pos), _ptr(vel), _ptr(acc), pos.shape[0], float(kick),
+                                           float(drift), float(box), self._stream(stream)))
+
+    def cell_vrms(self, vel: torch.Tensor, b: Binned, original_order: bool = True, stream=None):
+        """nf_cell_vrms: (per-cell rms speed float32 [K^3], max |v_axis| float32 [1]) for velocities in the
+        caller's order (or in nf_bin's sorted order if not original_order)."""
+        assert vel.is_cuda and vel.dtype == torch.float32 and vel.shape == (b.N, 3) and vel.is_contiguous()
+        vrms = torch.empty(b.K ** 3, dtype=torch.float32, device=vel.device)
+        vmax = torch.empty(1, dtype=torch.float32, device=vel.device)
+        self._check(self.lib.nf_cell_vrms(self._h, _ptr(vel), _ptr(b.perm) if original_order else None, _ptr(b.cell_offset),
+                                          b.N, b.K, _ptr(vrms), _ptr(vmax), self._stream(stream)))
+        return vrms, vmax
 
     def reserve_host(self, maxN: int, K: int):
         self._check(self.lib.nf_reserve_host(self._h, int(maxN), int(K)))

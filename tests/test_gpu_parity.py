@@ -284,3 +284,83 @@ def test_cell_amax(ctx):
     own = np.zeros(cfg.K ** 3, np.float32)
     np.maximum.at(own, key, n32)
     assert np.allclose(got, own, rtol=3e-7, atol=0)
+
+
+# ------------------------------------------------- next rows: kick, drift, v_rms
+@pytest.mark.parametrize("n", [0, 1, 100_003, 3_000_017])
+def test_kick_drift_bit_exact(ctx, n):
+    """nf_kick_drift against the oracle on the same seeded float32 inputs, bit for bit (two
+    single-rounded FMAs and one wrap per coordinate); speeds large enough that ~10 % of the
+    coordinates wrap, in both directions, plus planted edge values."""
+    rng = np.random.default_rng(100 + n % 97)
+    box = 500.0
+    pos = (rng.random((n, 3)) * box).astype(np.float32)
+    pos = np.minimum(pos, np.nextafter(np.float32(box), np.float32(0)))
+    vel = (rng.standard_normal((n, 3)) * 300.0).astype(np.float32)
+    acc = (rng.standard_normal((n, 3)) * 50.0).astype(np.float32)
+    if n >= 100:
+        pos[:4, 0] = [0.0, np.nextafter(np.float32(box), np.float32(0)), 1e-30, 250.0]
+        vel[:4, 0] = [-1e-12, 1e-3, -1e-20, 0.0]
+        acc[:4, 0] = 0.0
+    kick, drift = 0.37, 0.21
+    x_ref, v_ref = oracle.kick_drift(pos, vel, acc, kick, drift, box)
+    p, v, a = (torch.from_numpy(t).cuda() for t in (pos, vel, acc))
+    ctx.kick_drift(p, v, a, kick, drift, box)
+    assert np.array_equal(v.cpu().numpy().view(np.uint32), v_ref.view(np.uint32))
+    assert np.array_equal(p.cpu().numpy().view(np.uint32), x_ref.view(np.uint32))
+    if n:
+        assert (x_ref >= 0).all() and (x_ref < np.float32(box)).all()
+    if n > 1000:
+        moved = x_ref != np.float32(pos + v_ref * np.float32(drift))
+        assert 0.02 < moved.mean() < 0.5          # a fair share of wraps was exercised
+
+
+def test_cell_vrms_and_vmax(ctx):
+    cfg = inputs.scaled(inputs.config(3), 64 ** 3, 16)
+    cfg = inputs.dataclasses.replace(cfg, n_halos=24)
+    pos = inputs.make_positions(cfg).numpy()
+    rng = np.random.default_rng(9)
+    vel = (rng.standard_normal((cfg.N, 3)) * np.exp(rng.normal(0, 1, (cfg.N, 1)))).astype(np.float32)
+    b = ctx.bin(torch.from_numpy(pos).cuda(), cfg.K, cfg.box)
+    vrms, vmax = ctx.cell_vrms(torch.from_numpy(vel).cuda(), b)
+    key, _ = oracle.keys(pos, cfg.K, cfg.box)
+    ref, ref_max = oracle.cell_vrms(vel, key, cfg.K ** 3)
+    got = vrms.cpu().numpy().astype(np.float64)
+    assert (got[ref == 0] == 0).all()
+    assert np.allclose(got, ref, rtol=2e-6, atol=0)
+    assert float(vmax.item()) == np.float32(ref_max)     # a maximum of float32 inputs: exact
+    # sorted-order input gives the same bits
+    vs = torch.from_numpy(vel).cuda()[b.perm.long()].contiguous()
+    vrms2, vmax2 = ctx.cell_vrms(vs, b, original_order=False)
+    assert torch.equal(vrms2, vrms) and torch.equal(vmax2, vmax)
+
+
+def test_step_cycle_force_kick_drift_rebin(ctx):
+    """One slab-pipeline cycle on the device -- nf_bin, nf_forces_ex, nf_kick_drift, nf_bin again --
+    against the same cycle on the oracle side.  The two sides' accelerations differ by rounding, so
+    the drifted positions are compared within that rounding; the second binning is compared bit for
+    bit on the oracle's drifted positions."""
+    cfg = inputs.scaled(inputs.config(2), 32 ** 3, 8)
+    pos = inputs.make_positions(cfg).numpy()
+    vel = np.zeros_like(pos)
+    b = ctx.bin(torch.from_numpy(pos).cuda(), cfg.K, cfg.box)
+    acc = ctx.forces(b, cfg.R, cfg.eps, cfg.Gm)
+    a_ref = oracle.forces(pos, cfg.K, cfg.R, cfg.eps, cfg.box, cfg.Gm)
+    amax = float(np.sqrt((a_ref ** 2).sum(axis=1)).max())
+    w = cfg.box / cfg.K
+    dt = np.sqrt(0.5 * w / amax)                         # the fastest particle moves about a quarter cell
+    p, v = torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda()
+    ctx.kick_drift(p, v, acc, dt, dt, cfg.box)
+    x_ref, v_ref = oracle.kick_drift(pos, vel, a_ref.astype(np.float32), dt, dt, cfg.box)
+    dx = np.abs(p.cpu().numpy().astype(np.float64) - x_ref)
+    dx = np.minimum(dx, cfg.box - dx)
+    assert dx.max() < 1e-3 * 0.25 * w                     # MAX_TOL of the force times the largest displacement
+    # re-bin: both sides bin the ORACLE's drifted positions (no oracle input comes from the CUDA path)
+    b2 = ctx.bin(torch.from_numpy(x_ref).cuda(), cfg.K, cfg.box)
+    assert ctx.out_of_range() == 0
+    ref2 = oracle.bin_particles(x_ref, cfg.K, cfg.box)
+    assert np.array_equal(u32(b2.perm), ref2["perm"]) and np.array_equal(u32(b2.cell_count), ref2["cell_count"])
+    assert not np.array_equal(u32(b2.cell_count), u32(b.cell_count))   # particles did change cells
+    # and the device's own drifted positions are valid input for the next step
+    ctx.bin(p, cfg.K, cfg.box)
+    assert ctx.out_of_range() == 0

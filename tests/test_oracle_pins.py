@@ -467,3 +467,60 @@ def test_cell_amax_definition():
     assert np.array_equal(got, ref)
     assert got.max() == mag.max()
     assert (got[np.bincount(key, minlength=K ** 3) == 0] == 0).all()
+
+
+# ------------------------------------------------- next rows: kick, drift
+def test_kick_drift_closed_forms_and_wrap():
+    """Exactly representable cases worked by hand (box = 1): the velocity is updated FIRST and the
+    drift uses the new velocity; one periodic wrap either way; x + box rounding up to box gives 0."""
+    pos = np.array([[0.25, 0.875, 0.125]], np.float32)
+    vel = np.array([[0.5, 1.0, -1.0]], np.float32)
+    acc = np.array([[1.0, 0.0, 0.0]], np.float32)
+    x, v = oracle.kick_drift(pos, vel, acc, 0.5, 0.25, 1.0)
+    # x: v1 = 0.5 + 1*0.5 = 1.0, x1 = 0.25 + 1.0*0.25 = 0.5 (an update with the OLD v would give 0.375)
+    # y: 0.875 + 0.25 = 1.125 -> 0.125;  z: 0.125 - 0.25 = -0.125 -> 0.875
+    assert np.array_equal(v, np.array([[1.0, 1.0, -1.0]], np.float32))
+    assert np.array_equal(x, np.array([[0.5, 0.125, 0.875]], np.float32))
+    tiny = np.array([[-1e-12, 0.0, 0.0]], np.float32)
+    x, _ = oracle.kick_drift(tiny, np.zeros((1, 3), np.float32), np.zeros((1, 3), np.float32), 0.0, 0.0, 1.0)
+    assert x[0, 0] == 0.0                      # -1e-12 + 1 rounds to 1.0f == box -> 0
+    assert (x >= 0).all() and (x < 1).all()
+
+
+def test_kick_drift_is_symplectic_leapfrog():
+    """Harmonic oscillator a = -x stepped with (kick h, drift h): the leapfrog map conserves the
+    modified energy v^2 + x^2 - h x v exactly in real arithmetic (textbook), so over 10^4 steps it
+    stays within float32 rounding drift, while x^2 + v^2 oscillates by O(h).  A drift with the old
+    velocity (explicit Euler) would grow by (1 + h^2) per step."""
+    h, box = 0.05, 8.0
+    x = np.array([[4.0 + 1.0, 4.0, 4.0]], np.float32)      # oscillate about the box centre
+    v = np.zeros((1, 3), np.float32)
+    inv0 = None
+    for _ in range(10000):
+        a = -(x - np.float32(4.0))
+        x, v = oracle.kick_drift(x, v, a, h, h, box)
+        q = float(x[0, 0]) - 4.0
+        inv = float(v[0, 0]) ** 2 + q * q - h * q * float(v[0, 0])
+        inv0 = inv if inv0 is None else inv0
+        assert abs(inv - inv0) < 2e-3 * inv0
+    assert abs(inv0 - 1.0) < 0.01
+
+
+def test_cell_vrms_definition():
+    rng = np.random.default_rng(21)
+    n, K = 700, 4
+    pos = rng.random((n, 3)).astype(np.float32)
+    vel = rng.standard_normal((n, 3)).astype(np.float32)
+    key, _ = oracle.keys(pos, K, 1.0)
+    got, vmax = oracle.cell_vrms(vel, key, K ** 3)
+    v64 = vel.astype(np.float64)
+    for c in range(K ** 3):
+        sel = key == c
+        ref = np.sqrt((v64[sel] ** 2).sum(axis=1).mean()) if sel.any() else 0.0
+        assert abs(got[c] - ref) <= 1e-14 * max(ref, 1.0)
+    assert vmax == np.abs(v64).max()
+    # equal speeds in every direction: v_rms is that speed
+    u = rng.standard_normal((n, 3))
+    u = (3.0 * u / np.sqrt((u ** 2).sum(axis=1))[:, None]).astype(np.float32)
+    got, _ = oracle.cell_vrms(u, key, K ** 3)
+    assert np.allclose(got[np.bincount(key, minlength=K ** 3) > 0], 3.0, rtol=1e-6)
