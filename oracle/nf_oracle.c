@@ -28,7 +28,11 @@
  * Pins (tests/test_oracle_pins.py): pair-centric brute force on tiny inputs, two-particle
  * closed forms inside and outside eps, C2 continuity at r = eps, the min identity of
  * footnote 4, antisymmetry / zero net force, symmetric lattice, power-of-two
- * rescaling, whole-cell translation, all-pairs direct sum for K = 2R+1.
+ * rescaling, whole-cell translation, all-pairs direct sum for K = 2R+1.  Next rows: masses (mass-ratio
+ * closed form, momentum, brute force with masses, linearity), per-cell a_max / v_rms (python-loop
+ * definition), kick + drift (hand-worked exact cases, leapfrog invariant of the harmonic oscillator).
+ * nfo_kick_drift: the paper names Kick and Drift but prints no formula, so its
+ * parity is UNPINNED AGAINST THE PAPER; it is pinned to the textbook leapfrog only (reading c20).
  */
 #include <math.h>
 #include <stdint.h>
