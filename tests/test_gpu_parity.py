@@ -364,3 +364,50 @@ def test_step_cycle_force_kick_drift_rebin(ctx):
     # and the device's own drifted positions are valid input for the next step
     ctx.bin(p, cfg.K, cfg.box)
     assert ctx.out_of_range() == 0
+
+
+# ------------------------------------------------------------------- degenerate force cases
+@pytest.mark.parametrize("eps_over_w", [0.6, 1.0, 1.7, 4.0])
+def test_forces_eps_comparable_to_cell(ctx, eps_over_w):
+    """Softening length of the order of the cell width or larger: cells two apart CAN then hold pairs
+    inside eps, so the kernel must not skip the close-pair tracking there (FC_FAR_OK off), and whole
+    neighbourhoods sit on the polynomial branch of Eq. 2."""
+    rng = np.random.default_rng(int(10 * eps_over_w))
+    K, R, box, n = 8, 2, 1.0, 20_000
+    pos = rng.random((n, 3)).astype(np.float32)
+    pos = np.minimum(pos, np.nextafter(np.float32(1), np.float32(0)))
+    check_forces(ctx, pos, K, R, eps_over_w * box / K, box, 1.0 / n)
+
+
+def test_forces_one_huge_cell_and_empty_box(ctx):
+    """Everything in one cell (5000 particles, many tasks of one cell, listed first) beside an
+    otherwise almost empty box; then N = 1 and N = 0."""
+    rng = np.random.default_rng(77)
+    K, R, box = 9, 2, 3.0
+    w = box / K
+    blob = (np.array([4.5, 4.5, 4.5]) * w + 0.2 * w * rng.standard_normal((5000, 3))).clip(4.01 * w, 4.99 * w)
+    few = rng.random((40, 3)) * box
+    pos = np.concatenate([blob, few]).astype(np.float32)
+    pos = np.minimum(pos, np.nextafter(np.float32(box), np.float32(0)))
+    check_forces(ctx, pos, K, R, 0.01 * w, box, 1.0 / len(pos))
+    one = np.array([[0.3, 1.7, 2.9]], np.float32)
+    b = ctx.bin(torch.from_numpy(one).cuda(), K, box)
+    assert (ctx.forces(b, R, 0.01, 1.0).cpu().numpy() == 0).all()          # only the self pair: exactly zero
+    empty = torch.empty(0, 3, device="cuda")
+    b = ctx.bin(empty, K, box)
+    amax = torch.full((K ** 3,), 7.0, device="cuda")
+    assert ctx.forces(b, R, 0.01, 1.0, cell_amax=amax).shape == (0, 3)
+    assert (amax == 0).all() and int(b.cell_count.sum()) == 0
+
+
+@pytest.mark.parametrize("eps", [1e-7, 3e-3, 2.5e2])
+def test_forces_extreme_eps_and_units(ctx, eps):
+    """The internal power-of-two rescaling (positions times 2^k ~ 1/eps) must keep every constant in
+    range from a softening far below float32 resolution of the box to one far above the box, in a box
+    of 10^3 length units."""
+    rng = np.random.default_rng(3)
+    K, R, box, n = 10, 2, 1000.0, 8000
+    pos = (rng.random((n, 3)) * box).astype(np.float32)
+    pos[:200] = (pos[0] + 0.05 * rng.standard_normal((200, 3))).astype(np.float32) % np.float32(box)
+    pos = np.clip(pos, 0, np.nextafter(np.float32(box), np.float32(0)))
+    check_forces(ctx, pos, K, R, eps, box, 1.0 / n)
