@@ -483,7 +483,9 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                 zs[h] = sub2(zi[h], pk(sz, sz));
             }
             float4 *buf = S.buf[b];
-            for (int i = tn + lane; i < P * q; i += 32) buf[i] = SENT;     // slots the bulk copy does not write
+            // slots the bulk copy does not write: P*q - tn < 2P <= 64 of them, two predicated stores
+            if (tn + lane < P * q) buf[tn + lane] = SENT;
+            if (tn + 32 + lane < P * q) buf[tn + 32 + lane] = SENT;
             mbar_wait(b ? bar1 : bar0, (parity >> b) & 1u);
             parity ^= 1u << b;
             __syncwarp();
