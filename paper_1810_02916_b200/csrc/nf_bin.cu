@@ -19,11 +19,11 @@
 
 namespace {
 
-constexpr int RS_THREADS = 256;
+constexpr int RS_THREADS = 512;
 constexpr int RS_WARPS = RS_THREADS / 32;
 constexpr int RS_ROUNDS = 16;                       // rounds of 32 elements per warp
 constexpr int RS_WARP_ELEMS = RS_ROUNDS * 32;       // 512
-constexpr int RS_TILE = RS_WARPS * RS_WARP_ELEMS;   // 4096
+constexpr int RS_TILE = RS_WARPS * RS_WARP_ELEMS;   // 8192
 
 // float32 cell index, include/nf.h contract: c = (int)floorf(x * invw) clamped to [0, K-1].
 // __fmul_rn is never contracted into an FMA.
@@ -66,39 +66,54 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pos, int
     if (m && (threadIdx.x & 31) == 0) atomicAdd(n_bad, (unsigned long long)__popc(m));
 }
 
-__device__ __forceinline__ uint32_t digit_of(uint32_t key, uint32_t div, uint32_t K) { return (key / div) % K; }
+// digit of a key: (key / div) % K, by shift and mask when K is a power of two (sh < 32)
+struct Digit {
+    uint32_t div, K, sh, mask;     // sh = 32: general K
+    __device__ __forceinline__ uint32_t operator()(uint32_t key) const { return sh < 32 ? (key >> sh) & mask : (key / div) % K; }
+};
 
 // per-tile digit histogram -> hist[digit * ntiles + tile]
-__global__ void __launch_bounds__(RS_THREADS) k_radix_hist(const uint32_t *__restrict__ keys, int64_t N, uint32_t div, uint32_t K,
+__global__ void __launch_bounds__(RS_THREADS) k_radix_hist(const uint32_t *__restrict__ keys, int64_t N, Digit dg,
                                                            uint32_t *__restrict__ hist, uint32_t ntiles)
 {
     extern __shared__ uint32_t sh[];
+    const uint32_t K = dg.K;
     for (uint32_t d = threadIdx.x; d < K; d += RS_THREADS) sh[d] = 0;
     __syncthreads();
     int64_t base = (int64_t)blockIdx.x * RS_TILE;
 #pragma unroll 4
     for (int k = 0; k < RS_TILE / RS_THREADS; k++) {
         int64_t i = base + (int64_t)k * RS_THREADS + threadIdx.x;
-        if (i < N) atomicAdd(&sh[digit_of(keys[i], div, K)], 1u);
+        if (i < N) atomicAdd(&sh[dg(keys[i])], 1u);
     }
     __syncthreads();
     for (uint32_t d = threadIdx.x; d < K; d += RS_THREADS) hist[(size_t)d * ntiles + blockIdx.x] = sh[d];
 }
 
-// stable scatter.  Warp w of the tile owns elements [tile*4096 + w*512, +512) in index order.
-// idx_in == nullptr means "identity" (first pass).
+// Stable scatter of one tile of RS_TILE elements.  Warp w owns elements [tile*RS_TILE + w*512, +512)
+// in index order.  Ranks come from warp match/ballot (no atomic decides a slot), the tile is first
+// sorted by digit INTO SHARED MEMORY, and only then written out, so that every digit's run of the
+// tile (RS_TILE / K elements on average) leaves as one contiguous, coalesced burst instead of
+// 4-byte stores scattered over the whole array.  idx_in == nullptr means "identity" (first pass).
+// shared: cnt[RS_WARPS][K] | gdelta[K] | wsum[RS_WARPS] | skey[RS_TILE] | sidx[RS_TILE]
 __global__ void __launch_bounds__(RS_THREADS) k_radix_scatter(const uint32_t *__restrict__ keys_in, const uint32_t *__restrict__ idx_in,
-                                                              int64_t N, uint32_t div, uint32_t K,
+                                                              int64_t N, Digit dg,
                                                               const uint32_t *__restrict__ hist_scanned, uint32_t ntiles,
                                                               uint32_t *__restrict__ keys_out, uint32_t *__restrict__ idx_out)
 {
-    extern __shared__ uint32_t sh[];  // [RS_WARPS][K]
+    extern __shared__ uint32_t sh[];
+    const uint32_t K = dg.K;
+    uint32_t *gdelta = sh + (size_t)RS_WARPS * K;
+    uint32_t *wsum = gdelta + K;
+    uint32_t *skey = wsum + 32;
+    uint32_t *sidx = skey + RS_TILE;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const unsigned lt = (1u << lane) - 1u;
     for (uint32_t d = threadIdx.x; d < K * RS_WARPS; d += RS_THREADS) sh[d] = 0;
     __syncthreads();
     uint32_t *cnt = sh + (size_t)w * K;
-    const int64_t wbase = (int64_t)blockIdx.x * RS_TILE + (int64_t)w * RS_WARP_ELEMS;
+    const int64_t tbase = (int64_t)blockIdx.x * RS_TILE;
+    const int64_t wbase = tbase + (int64_t)w * RS_WARP_ELEMS;
     uint32_t key[RS_ROUNDS];
     // count pass
 #pragma unroll
@@ -108,32 +123,60 @@ __global__ void __launch_bounds__(RS_THREADS) k_radix_scatter(const uint32_t *__
         key[r] = valid ? keys_in[i] : 0u;
         unsigned act = __ballot_sync(0xffffffffu, valid);
         if (valid) {
-            uint32_t d = digit_of(key[r], div, K);
+            uint32_t d = dg(key[r]);
             unsigned peers = __match_any_sync(act, d);
             if ((peers & lt) == 0) cnt[d] += __popc(peers);  // leader = lowest lane of the group
         }
         __syncwarp();
     }
     __syncthreads();
-    // exclusive scan across warps for every digit, seeded with the tile's global base
-    for (uint32_t d = threadIdx.x; d < K; d += RS_THREADS) {
-        uint32_t run = hist_scanned[(size_t)d * ntiles + blockIdx.x];
+    // For every digit: exclusive scan across warps, then across digits (block scan of the digit
+    // totals, RS_THREADS digits per sweep) -> cnt[w][d] = first slot of (warp, digit) within the
+    // sorted tile; gdelta[d] = (global slot of the tile's first element of digit d) - (its tile slot).
+    uint32_t carry = 0;
+    for (uint32_t d0 = 0; d0 < K; d0 += RS_THREADS) {
+        const uint32_t d = d0 + threadIdx.x;
+        uint32_t tot = 0;
+        if (d < K) {
+#pragma unroll
+            for (int ww = 0; ww < RS_WARPS; ww++) {
+                uint32_t t = sh[(size_t)ww * K + d];
+                sh[(size_t)ww * K + d] = tot;
+                tot += t;
+            }
+        }
+        uint32_t incl = tot;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        if (lane == 31) wsum[w] = incl;
+        __syncthreads();
+        uint32_t woff = 0, all = 0;
 #pragma unroll
         for (int ww = 0; ww < RS_WARPS; ww++) {
-            uint32_t t = sh[(size_t)ww * K + d];
-            sh[(size_t)ww * K + d] = run;
-            run += t;
+            uint32_t t = wsum[ww];
+            if (ww < w) woff += t;
+            all += t;
         }
+        const uint32_t dstart = carry + woff + incl - tot;
+        if (d < K) {
+#pragma unroll
+            for (int ww = 0; ww < RS_WARPS; ww++) sh[(size_t)ww * K + d] += dstart;
+            gdelta[d] = hist_scanned[(size_t)d * ntiles + blockIdx.x] - dstart;
+        }
+        carry += all;
+        __syncthreads();
     }
-    __syncthreads();
-    // rank + scatter pass
+    // rank pass: stable slot within the sorted tile, staged in shared memory
 #pragma unroll
     for (int r = 0; r < RS_ROUNDS; r++) {
         int64_t i = wbase + r * 32 + lane;
         bool valid = i < N;
         unsigned act = __ballot_sync(0xffffffffu, valid);
         if (valid) {
-            uint32_t d = digit_of(key[r], div, K);
+            uint32_t d = dg(key[r]);
             unsigned peers = __match_any_sync(act, d);
             int leader = __ffs(peers) - 1;
             uint32_t base = 0;
@@ -142,11 +185,21 @@ __global__ void __launch_bounds__(RS_THREADS) k_radix_scatter(const uint32_t *__
                 cnt[d] = base + __popc(peers);
             }
             base = __shfl_sync(peers, base, leader);
-            uint32_t dst = base + __popc(peers & lt);
-            keys_out[dst] = key[r];
-            idx_out[dst] = idx_in ? idx_in[i] : (uint32_t)i;
+            uint32_t slot = base + __popc(peers & lt);
+            skey[slot] = key[r];
+            sidx[slot] = idx_in ? idx_in[i] : (uint32_t)i;
         }
         __syncwarp();
+    }
+    __syncthreads();
+    // write out: consecutive tile slots of one digit go to consecutive global slots
+    const int64_t rem = N - tbase;
+    const uint32_t tile_n = rem < RS_TILE ? (uint32_t)rem : (uint32_t)RS_TILE;
+    for (uint32_t s = threadIdx.x; s < tile_n; s += RS_THREADS) {
+        const uint32_t k = skey[s];
+        const uint32_t dst = s + gdelta[dg(k)];
+        keys_out[dst] = k;
+        idx_out[dst] = sidx[s];
     }
 }
 
@@ -228,11 +281,15 @@ int nf_bin_impl(nf_ctx *ctx, const float *pos, const float *mass, int64_t N, int
         uint32_t *kout = (kin == keysA) ? keysB : keysA;
         uint32_t *iout = to_perm ? perm : idxB;
         size_t sh_hist = (size_t)K * sizeof(uint32_t);
-        size_t sh_scat = (size_t)K * RS_WARPS * sizeof(uint32_t);
-        k_radix_hist<<<(unsigned)ntiles, RS_THREADS, sh_hist, st>>>(kin, N, div, (uint32_t)K, hist, (uint32_t)ntiles);
+        size_t sh_scat = ((size_t)K * RS_WARPS + (size_t)K + 32 + 2 * (size_t)RS_TILE) * sizeof(uint32_t);
+        Digit dg;
+        dg.div = div; dg.K = (uint32_t)K; dg.sh = 32; dg.mask = (uint32_t)K - 1;
+        if ((K & (K - 1)) == 0) { dg.sh = 0; while ((1u << dg.sh) < div) dg.sh++; }
+        k_radix_hist<<<(unsigned)ntiles, RS_THREADS, sh_hist, st>>>(kin, N, dg, hist, (uint32_t)ntiles);
         NF_LAUNCHED(ctx);
         NF_TRY(nf_exclusive_scan_u32(ctx, hist, hist, (size_t)K * ntiles, tmp32, st));
-        k_radix_scatter<<<(unsigned)ntiles, RS_THREADS, sh_scat, st>>>(kin, iin, N, div, (uint32_t)K, hist, (uint32_t)ntiles, kout, iout);
+        NF_CUDA(ctx, cudaFuncSetAttribute(k_radix_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh_scat));
+        k_radix_scatter<<<(unsigned)ntiles, RS_THREADS, sh_scat, st>>>(kin, iin, N, dg, hist, (uint32_t)ntiles, kout, iout);
         NF_LAUNCHED(ctx);
         kin = kout;
         iin = iout;
