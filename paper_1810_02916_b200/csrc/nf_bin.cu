@@ -115,6 +115,7 @@ __global__ void __launch_bounds__(RS_THREADS) k_radix_scatter(const uint32_t *__
     const int64_t tbase = (int64_t)blockIdx.x * RS_TILE;
     const int64_t wbase = tbase + (int64_t)w * RS_WARP_ELEMS;
     uint32_t key[RS_ROUNDS];
+    unsigned peers[RS_ROUNDS];       // lanes of the round holding the same digit (0: element past N)
     // count pass
 #pragma unroll
     for (int r = 0; r < RS_ROUNDS; r++) {
@@ -122,10 +123,11 @@ __global__ void __launch_bounds__(RS_THREADS) k_radix_scatter(const uint32_t *__
         bool valid = i < N;
         key[r] = valid ? keys_in[i] : 0u;
         unsigned act = __ballot_sync(0xffffffffu, valid);
+        peers[r] = 0u;
         if (valid) {
             uint32_t d = dg(key[r]);
-            unsigned peers = __match_any_sync(act, d);
-            if ((peers & lt) == 0) cnt[d] += __popc(peers);  // leader = lowest lane of the group
+            peers[r] = __match_any_sync(act, d);
+            if ((peers[r] & lt) == 0) cnt[d] += __popc(peers[r]);  // leader = lowest lane of the group
         }
         __syncwarp();
     }
@@ -173,19 +175,17 @@ __global__ void __launch_bounds__(RS_THREADS) k_radix_scatter(const uint32_t *__
 #pragma unroll
     for (int r = 0; r < RS_ROUNDS; r++) {
         int64_t i = wbase + r * 32 + lane;
-        bool valid = i < N;
-        unsigned act = __ballot_sync(0xffffffffu, valid);
-        if (valid) {
+        if (peers[r]) {
+            const unsigned pr = peers[r];
             uint32_t d = dg(key[r]);
-            unsigned peers = __match_any_sync(act, d);
-            int leader = __ffs(peers) - 1;
+            int leader = __ffs(pr) - 1;
             uint32_t base = 0;
             if (lane == leader) {
                 base = cnt[d];
-                cnt[d] = base + __popc(peers);
+                cnt[d] = base + __popc(pr);
             }
-            base = __shfl_sync(peers, base, leader);
-            uint32_t slot = base + __popc(peers & lt);
+            base = __shfl_sync(pr, base, leader);
+            uint32_t slot = base + __popc(pr & lt);
             skey[slot] = key[r];
             sidx[slot] = idx_in ? idx_in[i] : (uint32_t)i;
         }
