@@ -267,6 +267,28 @@ int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const int64
                     int softening, float *const *plane_acc_host, nf_stream_stats *stats,
                     void *stream);
 
+/*
+ * nf_stream_step_slabs -- nf_stream_slabs with the Kick and Drift of the slab pipeline (Table 1,
+ * PAPER.md:149-150) as a streaming epilogue: after the forces of a sink plane its particles are
+ * kicked and drifted on the device (nf_kick_drift's float32 contract) and the NEW positions and
+ * velocities are copied back instead of (or beside) the accelerations -- one pass over the chunk
+ * per time step.
+ *
+ *   plane_vel_host       host in   P pointers (pinned): velocities of sink plane p, plane_n[R+p] x 3
+ *   kick, drift          as for nf_kick_drift
+ *   plane_pos_out_host   host out  P pointers (pinned): drifted positions of sink plane p, input order,
+ *                                  wrapped into [0, box) -- a particle may have left its plane; filing it
+ *                                  under its new plane for the next step is the caller's regrouping
+ *   plane_vel_out_host   host out  P pointers (pinned): kicked velocities
+ *   plane_acc_host       host out, nullable table: the accelerations, as nf_stream_slabs writes them
+ *   everything else as for nf_stream_slabs.
+ */
+int nf_stream_step_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const float *const *plane_vel_host,
+                         const int64_t *plane_n, int P, int K, int R, float eps, float box, int plane0,
+                         float Gm, int softening, float kick, float drift, float *const *plane_pos_out_host,
+                         float *const *plane_vel_out_host, float *const *plane_acc_host,
+                         nf_stream_stats *stats, void *stream);
+
 /* Timing of the kernels of the last nf_forces call on this context (CUDA events recorded on
  * the call's stream around the interaction kernel).  Synchronises on the end event.
  * *kernel_ms = duration of the interaction kernel alone; *total_ms = whole nf_forces call

@@ -131,4 +131,7 @@ int nf_forces_init(nf_ctx *ctx);
 // ordered pairs evaluated for the sink planes of a plane table (device result added to ctx->counters[1])
 int nf_interactions_planes(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d_planes, cudaStream_t st);
 void nf_slab_state_free(nf_ctx *ctx);
+// kick + drift launcher (nf_step.cu), also the epilogue of nf_stream_step_slabs
+int nf_kick_drift_impl(nf_ctx *ctx, float *pos, float *vel, const float *acc, int64_t N, float kick, float drift, float box,
+                       cudaStream_t st);
 int nf_interactions_impl(nf_ctx *ctx, const uint32_t *cell_count, int K, int R, int64_t *out, cudaStream_t st);

@@ -55,6 +55,16 @@ __global__ void __launch_bounds__(256) k_cell_vrms(const float *__restrict__ vel
 
 }  // namespace
 
+int nf_kick_drift_impl(nf_ctx *ctx, float *pos, float *vel, const float *acc, int64_t N, float kick, float drift, float box,
+                       cudaStream_t st)
+{
+    if (N <= 0) return NF_OK;
+    const size_t n3 = 3 * (size_t)N;
+    k_kick_drift<<<(unsigned)((n3 + 255) / 256), 256, 0, st>>>(pos, vel, acc, n3, kick, drift, box);
+    NF_LAUNCHED(ctx);
+    return NF_OK;
+}
+
 int nf_kick_drift(nf_ctx *ctx, float *pos_xyz, float *vel_xyz, const float *acc_xyz, int64_t N, float kick, float drift,
                   float box, void *stream)
 {
@@ -64,11 +74,7 @@ int nf_kick_drift(nf_ctx *ctx, float *pos_xyz, float *vel_xyz, const float *acc_
     NF_ARG(ctx, box > 0.0f && box < 3.0e38f, "box must be positive and finite");
     NF_ARG(ctx, kick == kick && drift == drift && fabsf(kick) < 3.0e38f && fabsf(drift) < 3.0e38f, "kick and drift must be finite");
     NF_CUDA(ctx, cudaSetDevice(ctx->device));
-    if (N == 0) return NF_OK;
-    const size_t n3 = 3 * (size_t)N;
-    k_kick_drift<<<(unsigned)((n3 + 255) / 256), 256, 0, (cudaStream_t)stream>>>(pos_xyz, vel_xyz, acc_xyz, n3, kick, drift, box);
-    NF_LAUNCHED(ctx);
-    return NF_OK;
+    return nf_kick_drift_impl(ctx, pos_xyz, vel_xyz, acc_xyz, N, kick, drift, box, (cudaStream_t)stream);
 }
 
 int nf_cell_vrms(nf_ctx *ctx, const float *vel_xyz, const uint32_t *perm, const uint64_t *cell_offset, int64_t N, int K,

@@ -25,6 +25,15 @@ struct Slot {
     uint32_t *count;   // K*K
     uint64_t *off;     // K*K + 1
     float *acc;        // n x 3
+    float *vel;        // n x 3 (nf_stream_step_slabs only)
+};
+
+// the kick + drift epilogue of nf_stream_step_slabs (null pointers: plain nf_stream_slabs)
+struct StepArgs {
+    const float *const *vel_host;     // P
+    float *const *pos_out_host;       // P
+    float *const *vel_out_host;       // P
+    float kick, drift;
 };
 
 struct SlabState {
@@ -64,13 +73,21 @@ void nf_slab_state_free(nf_ctx *ctx)
     ctx->slab_state = nullptr;
 }
 
-extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,
-                               int P, int K, int R, float eps, float box, int plane0, float Gm,
-                               int softening, float *const *plane_acc_host, nf_stream_stats *stats,
-                               void *stream)
+static bool is_pinned(const void *p)
+{
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeHost || at.type == cudaMemoryTypeManaged;
+}
+
+static int stream_impl(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,
+                       int P, int K, int R, float eps, float box, int plane0, float Gm,
+                       int softening, float *const *plane_acc_host, const StepArgs *step, nf_stream_stats *stats,
+                       void *stream)
 {
     if (!ctx) return NF_ERR_ARG;
-    NF_ARG(ctx, plane_pos_host && plane_n && plane_acc_host, "nf_stream_slabs: null pointer table");
+    NF_ARG(ctx, plane_pos_host && plane_n && (plane_acc_host || step), "nf_stream_slabs: null pointer table");
     NF_ARG(ctx, P >= 1, "nf_stream_slabs: P must be >= 1");
     NF_ARG(ctx, K >= 1 && K <= NF_MAX_K, "K = %d out of range [1, %d]", K, NF_MAX_K);
     NF_ARG(ctx, R >= 0 && R <= NF_MAX_R, "R = %d out of range [0, %d]", R, NF_MAX_R);
@@ -86,7 +103,15 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         NF_ARG(ctx, plane_n[q] == 0 || plane_pos_host[q], "plane_pos_host[%d] is null", q);
         if (plane_n[q] > max_n) max_n = plane_n[q];
     }
-    for (int p = 0; p < P; p++) NF_ARG(ctx, plane_n[R + p] == 0 || plane_acc_host[p], "plane_acc_host[%d] is null", p);
+    for (int p = 0; p < P; p++) {
+        if (plane_n[R + p] == 0) continue;
+        NF_ARG(ctx, !plane_acc_host || (plane_acc_host[p] && is_pinned(plane_acc_host[p])), "plane_acc_host[%d] is null or not pinned host memory", p);
+        if (step) {
+            NF_ARG(ctx, step->vel_host[p] && is_pinned(step->vel_host[p]), "plane_vel_host[%d] is null or not pinned host memory", p);
+            NF_ARG(ctx, step->pos_out_host[p] && is_pinned(step->pos_out_host[p]), "plane_pos_out_host[%d] is null or not pinned host memory", p);
+            NF_ARG(ctx, step->vel_out_host[p] && is_pinned(step->vel_out_host[p]), "plane_vel_out_host[%d] is null or not pinned host memory", p);
+        }
+    }
     NF_CUDA(ctx, cudaSetDevice(ctx->device));
     // host pointers must be pinned (page-locked): "Pinning memory"
     for (int q = 0; q < NP; q++) {
@@ -96,16 +121,6 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         if (e != cudaSuccess || (at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged)) {
             cudaGetLastError();
             NF_SET_ERR(ctx, "plane_pos_host[%d] is not pinned host memory", q);
-            return NF_ERR_ARG;
-        }
-    }
-    for (int p = 0; p < P; p++) {
-        if (plane_n[R + p] == 0) continue;
-        cudaPointerAttributes at;
-        cudaError_t e = cudaPointerGetAttributes(&at, plane_acc_host[p]);
-        if (e != cudaSuccess || (at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged)) {
-            cudaGetLastError();
-            NF_SET_ERR(ctx, "plane_acc_host[%d] is not pinned host memory", p);
             return NF_ERR_ARG;
         }
     }
@@ -123,7 +138,8 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
     }
     const size_t n = (size_t)max_n;
     const size_t slot_bytes = nf_align_up(n * 12, 256) + 3 * nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
-                              nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256) + nf_align_up(n * 12, 256);
+                              nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256) + nf_align_up(n * 12, 256) +
+                              (step ? nf_align_up(n * 12, 256) : 0);
     const size_t need = slot_bytes * W;
     if (need > S->mem_bytes) {
         NF_CUDA(ctx, cudaDeviceSynchronize());
@@ -158,7 +174,8 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         slots[s].perm = (uint32_t *)b;            b += nf_align_up(n * 4, 256);
         slots[s].count = (uint32_t *)b;           b += nf_align_up(ncell * 4, 256);
         slots[s].off = (uint64_t *)b;             b += nf_align_up((ncell + 1) * 8, 256);
-        slots[s].acc = (float *)b;
+        slots[s].acc = (float *)b;                b += nf_align_up(n * 12, 256);
+        slots[s].vel = step ? (float *)b : nullptr;
     }
     // plane views (device pointers are fixed by the slot assignment q % W)
     for (int q = 0; q < NP; q++) {
@@ -181,6 +198,7 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
     cudaEvent_t ev_begin = pool.get(true), ev_end = pool.get(true), ev_ready = pool.get(false);
     for (auto e : pool.ev) if (!e) { NF_SET_ERR(ctx, "cudaEventCreate failed"); return NF_ERR_CUDA; }
 
+    double vel_bytes = 0.0;
     NF_CUDA(ctx, cudaEventRecord(ev_ready, st));        // order the whole call after prior work on `stream`
     NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, ev_ready, 0));
     NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_d2h, ev_ready, 0));
@@ -200,6 +218,10 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         NF_CUDA(ctx, cudaEventRecord(h2d0[q], ctx->s_h2d));
         if (plane_n[q] > 0)
             NF_CUDA(ctx, cudaMemcpyAsync(sl.raw, plane_pos_host[q], (size_t)plane_n[q] * 12, cudaMemcpyHostToDevice, ctx->s_h2d));
+        if (step && q >= R && q < R + P && plane_n[q] > 0) {
+            NF_CUDA(ctx, cudaMemcpyAsync(sl.vel, step->vel_host[q - R], (size_t)plane_n[q] * 12, cudaMemcpyHostToDevice, ctx->s_h2d));
+            vel_bytes += (double)plane_n[q] * 12.0;
+        }
         NF_CUDA(ctx, cudaEventRecord(h2d1[q], ctx->s_h2d));
 
         NF_CUDA(ctx, cudaStreamWaitEvent(st, h2d1[q], 0));
@@ -218,11 +240,22 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
             NF_CUDA(ctx, cudaEventRecord(frc0[p], st));
             NF_TRY(nf_forces_impl(ctx, fp, S->d_views, st, false));
             NF_TRY(nf_interactions_planes(ctx, fp, S->d_views, st));
+            const Slot &ss = slots[sp % W];
+            // kick + drift of the sink plane in place: its raw positions were only the input of its own
+            // binning (the later sink planes read the sorted / encoded copies), so they can move now
+            if (step && plane_n[sp] > 0)
+                NF_TRY(nf_kick_drift_impl(ctx, ss.raw, ss.vel, ss.acc, plane_n[sp], step->kick, step->drift, box, st));
             NF_CUDA(ctx, cudaEventRecord(frc1[p], st));
             NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_d2h, frc1[p], 0));
             NF_CUDA(ctx, cudaEventRecord(d2h0[p], ctx->s_d2h));
-            if (plane_n[sp] > 0)
-                NF_CUDA(ctx, cudaMemcpyAsync(plane_acc_host[p], slots[sp % W].acc, (size_t)plane_n[sp] * 12, cudaMemcpyDeviceToHost, ctx->s_d2h));
+            if (plane_n[sp] > 0) {
+                const size_t nb = (size_t)plane_n[sp] * 12;
+                if (plane_acc_host) NF_CUDA(ctx, cudaMemcpyAsync(plane_acc_host[p], ss.acc, nb, cudaMemcpyDeviceToHost, ctx->s_d2h));
+                if (step) {
+                    NF_CUDA(ctx, cudaMemcpyAsync(step->pos_out_host[p], ss.raw, nb, cudaMemcpyDeviceToHost, ctx->s_d2h));
+                    NF_CUDA(ctx, cudaMemcpyAsync(step->vel_out_host[p], ss.vel, nb, cudaMemcpyDeviceToHost, ctx->s_d2h));
+                }
+            }
             NF_CUDA(ctx, cudaEventRecord(d2h1[p], ctx->s_d2h));
         }
     }
@@ -247,8 +280,8 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
             NF_CUDA(ctx, cudaEventElapsedTime(&ms, d2h0[p], d2h1[p])); stats->d2h_seconds += ms * 1e-3;
         }
         NF_CUDA(ctx, cudaEventElapsedTime(&ms, ev_begin, ev_end)); stats->wall_seconds = ms * 1e-3;
-        stats->h2d_bytes = 12.0 * (double)stats->particles_in;
-        stats->d2h_bytes = 12.0 * (double)stats->particles_out;
+        stats->h2d_bytes = 12.0 * (double)stats->particles_in + vel_bytes;
+        stats->d2h_bytes = 12.0 * (double)stats->particles_out * ((plane_acc_host ? 1.0 : 0.0) + (step ? 2.0 : 0.0));
         stats->h2d_gbps = stats->h2d_seconds > 0 ? stats->h2d_bytes / stats->h2d_seconds * 1e-9 : 0.0;
         stats->d2h_gbps = stats->d2h_seconds > 0 ? stats->d2h_bytes / stats->d2h_seconds * 1e-9 : 0.0;
         stats->interactions = (int64_t)ctx->h_counters[1];
@@ -258,4 +291,27 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
         stats->overlap_fraction = hidden < 0 ? 0.0 : (hidden > 1 ? 1.0 : hidden);
     }
     return NF_OK;
+}
+
+extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,
+                               int P, int K, int R, float eps, float box, int plane0, float Gm,
+                               int softening, float *const *plane_acc_host, nf_stream_stats *stats,
+                               void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, plane_acc_host != nullptr, "nf_stream_slabs: null pointer table");
+    return stream_impl(ctx, plane_pos_host, plane_n, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, nullptr, stats, stream);
+}
+
+extern "C" int nf_stream_step_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const float *const *plane_vel_host,
+                                    const int64_t *plane_n, int P, int K, int R, float eps, float box, int plane0,
+                                    float Gm, int softening, float kick, float drift, float *const *plane_pos_out_host,
+                                    float *const *plane_vel_out_host, float *const *plane_acc_host,
+                                    nf_stream_stats *stats, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, plane_vel_host && plane_pos_out_host && plane_vel_out_host, "nf_stream_step_slabs: null pointer table");
+    NF_ARG(ctx, kick == kick && drift == drift && fabsf(kick) < 3.0e38f && fabsf(drift) < 3.0e38f, "kick and drift must be finite");
+    StepArgs a{plane_vel_host, plane_pos_out_host, plane_vel_out_host, kick, drift};
+    return stream_impl(ctx, plane_pos_host, plane_n, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, &a, stats, stream);
 }

@@ -411,3 +411,50 @@ def test_forces_extreme_eps_and_units(ctx, eps):
     pos[:200] = (pos[0] + 0.05 * rng.standard_normal((200, 3))).astype(np.float32) % np.float32(box)
     pos = np.clip(pos, 0, np.nextafter(np.float32(box), np.float32(0)))
     check_forces(ctx, pos, K, R, eps, box, 1.0 / n)
+
+
+def test_stream_step_slabs_small(ctx):
+    """nf_stream_step_slabs (forces + kick + drift as a streaming epilogue) on a thin C5-recipe chunk:
+    against the oracle's forces followed by the oracle's kick/drift (velocities and positions agree
+    within the force tolerance times the factors), and -- CUDA-side consistency, not parity -- bit for
+    bit against nf_stream_slabs followed by nf_kick_drift."""
+    cfg = inputs.dataclasses.replace(inputs.config(5), K=32, planes=6, plane0=3, n_halos=4096,
+                                     r_trunc=2 * 500.0 / 32 / 2, a_lo=0.3, a_hi=2.0, eps=0.15)
+    planes = inputs.make_slab_planes(cfg, density_scale=(32 * 4) ** 3 / 2048 ** 3)
+    R, P = cfg.R, cfg.planes
+    rng = np.random.default_rng(4)
+    vels = [torch.from_numpy((rng.standard_normal((planes[R + p].shape[0], 3)) * 3.0).astype(np.float32)) for p in range(P)]
+    pinned = [p.pin_memory() for p in planes]
+    pv = [v.pin_memory() for v in vels]
+    Gm = 1.0 / sum(p.shape[0] for p in planes)
+    allpos = torch.cat(planes).numpy()
+    starts = np.cumsum([0] + [p.shape[0] for p in planes])
+    sink_idx = np.arange(starts[R], starts[R + P])
+    a_ref = oracle.forces(allpos, cfg.K, R, cfg.eps, cfg.box, Gm, sink_idx=sink_idx)
+    amax = np.sqrt((a_ref ** 2).sum(axis=1)).max()
+    kick = 2.0 / amax                       # the largest kick is 2 velocity units, comparable to the velocities
+    drift = 0.3 * (cfg.box / cfg.K) / 12.0  # the fastest particles move ~0.3 cell widths
+    x_ref, v_ref = oracle.kick_drift(allpos[sink_idx], torch.cat(vels).numpy(), a_ref.astype(np.float32), kick, drift, cfg.box)
+    pos_out, vel_out, acc, stats = ctx.stream_step_slabs(pinned, pv, P, cfg.K, R, cfg.eps, cfg.box, cfg.plane0, Gm,
+                                                         kick, drift, want_acc=True)
+    got_v, got_x, got_a = torch.cat(vel_out).numpy(), torch.cat(pos_out).numpy(), torch.cat(acc).numpy()
+    err = oracle.parity_error(got_a, a_ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
+    rms = np.sqrt((a_ref ** 2).sum(axis=1).mean())
+    dv = np.abs(got_v.astype(np.float64) - v_ref).max(axis=1)
+    tol_v = MAX_TOL * kick * np.maximum(np.sqrt((a_ref ** 2).sum(axis=1)), rms) + 1e-6 * np.abs(v_ref).max(axis=1)
+    assert (dv <= tol_v).all()
+    dx = np.abs(got_x.astype(np.float64) - x_ref)
+    dx = np.minimum(dx, cfg.box - dx).max(axis=1)
+    assert (dx <= tol_v * drift + 1e-6 * cfg.box).all()
+    assert (got_x >= 0).all() and (got_x < np.float32(cfg.box)).all()
+    assert stats["d2h_bytes"] == 36.0 * sink_idx.size and stats["h2d_bytes"] == 12.0 * (allpos.shape[0] + sink_idx.size)
+    # consistency with the separate calls
+    out, _ = ctx.stream_slabs(pinned, P, cfg.K, R, cfg.eps, cfg.box, cfg.plane0, Gm)
+    assert torch.equal(torch.cat(out), torch.cat(acc))
+    x2, v2 = torch.cat(planes[R:R + P]).cuda(), torch.cat(vels).cuda()
+    ctx.kick_drift(x2, v2, torch.cat(out).cuda(), kick, drift, cfg.box)
+    assert torch.equal(x2.cpu(), torch.cat(pos_out)) and torch.equal(v2.cpu(), torch.cat(vel_out))
+    # without the acceleration table
+    p3, v3, a3, st3 = ctx.stream_step_slabs(pinned, pv, P, cfg.K, R, cfg.eps, cfg.box, cfg.plane0, Gm, kick, drift)
+    assert a3 is None and torch.equal(torch.cat(p3), torch.cat(pos_out)) and st3["d2h_bytes"] == 24.0 * sink_idx.size
