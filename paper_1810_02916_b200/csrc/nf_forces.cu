@@ -35,6 +35,7 @@ struct ForceConsts {
     float scale;        // 2^k
     float ws;           // cell width in internal units, (box / K) * scale
     float out_scale;    // Gm * scale^2: a = out_scale * sum f' d'
+    float near_lo;      // -(ws/2 - eps' - margin): a sink offset below it (above its negative) is "near" that face of its cell
     int flags;          // FC_FAR_OK: a cell width exceeds eps, so cells two or more apart hold no pair inside eps;  FC_PLUMMER
 };
 constexpr int FC_FAR_OK = 1, FC_PLUMMER = 2;
@@ -408,7 +409,8 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                     if (cn[s] == 0) continue;
                     if (newp[s]) {
                         slot++;
-                        const uint32_t self = (col == NR / 2 && s == R) ? 1u << 24 : 0u;
+                        // bit 24: the sinks' own cell; bits 25 / 26: a piece of the own column below / above it
+                        const uint32_t self = col != NR / 2 ? 0u : (s == R ? 1u << 24 : (s < R ? 1u << 25 : 1u << 26));
                         S.piece[slot] = make_uint4(st[s], cn[s], (uint32_t)col | ((uint32_t)(kz[s] + 128) << 8) | ((uint32_t)dxi << 16) | self, 0u);
                     } else {
                         S.piece[slot].y += cn[s];
@@ -420,13 +422,23 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
 
         // ---- the lane's four sinks (slots past n repeat the last sink; they are never written) ----
         u64 xi[2], yi[2], zi[2];
+        unsigned near = 0;
 #pragma unroll
         for (int h = 0; h < 2; h++) {
             const int j0 = min(4 * sl + 2 * h, n - 1), j1 = min(4 * sl + 2 * h + 1, n - 1);
             const float4 *se = zphi ? sp.enc_h : sp.enc;
             const float4 m0 = se[s0 + j0], m1 = se[s0 + j1];
             xi[h] = pk(m0.x, m1.x); yi[h] = pk(m0.y, m1.y); zi[h] = pk(m0.z, m1.z);
+            // which faces of the own cell does a sink of this task come within eps of?  (bit 0/1: x-/x+,
+            // 2/3: y-/y+, 4/5: z-/z+.)  Only then can a source of the cell beyond that face be inside eps.
+            const float ezs = ((float)((cz + zphi) % ZB) - 0.5f * (float)(ZB - 1)) * fc.ws;
+            const float lo = fc.near_lo, hi = -fc.near_lo;
+            const float z0 = m0.z - ezs, z1 = m1.z - ezs;
+            near |= (fminf(m0.x, m1.x) < lo ? 1u : 0u) | (fmaxf(m0.x, m1.x) > hi ? 2u : 0u) |
+                    (fminf(m0.y, m1.y) < lo ? 4u : 0u) | (fmaxf(m0.y, m1.y) > hi ? 8u : 0u) |
+                    (fminf(z0, z1) < lo ? 16u : 0u) | (fmaxf(z0, z1) > hi ? 32u : 0u);
         }
+        near = __reduce_or_sync(0xffffffffu, near);
         __syncwarp();
 
         // balanced tile length of every piece (no division on the per-tile path)
@@ -498,8 +510,16 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             // hold a pair inside eps (FC_FAR_OK), and Plummer has no second branch: nothing to track.
             int mode = 1;
             if (fc.flags & FC_PLUMMER) mode = 2;
-            else if (sticky_col == col || (d0.meta >> 24) != 0) mode = 0;
+            else if (sticky_col == col || ((d0.meta >> 24) & 1u) != 0) mode = 0;
             else if ((fc.flags & FC_FAR_OK) && max(abs(dxi - R), abs(dyi - R)) >= 2) mode = 2;
+            else {
+                // an adjacent column: a pair inside eps needs a sink within eps of every face that
+                // separates the own cell from the piece's cells
+                const int ddx = dxi - R, ddy = dyi - R;
+                unsigned need = (ddx < 0 ? 1u : 0u) | (ddx > 0 ? 2u : 0u) | (ddy < 0 ? 4u : 0u) | (ddy > 0 ? 8u : 0u) |
+                                ((d0.meta >> 25) & 1u ? 16u : 0u) | ((d0.meta >> 26) & 1u ? 32u : 0u);
+                if ((near & need) != need) mode = 2;
+            }
             if (active) {
                 if (mode == 1) sweep<1, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
                 else if (mode == 2) sweep<2, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
@@ -659,6 +679,9 @@ ForceConsts make_consts(const nf_force_params &p)
     fc.eps2_test = plummer ? 0.0f : (float)(es * es * 1.0001);
     fc.out_scale = (float)((double)p.Gm * (double)scale * (double)scale);
     // sources two or more cells away are at least one cell width (minus rounding) from every sink of the cell
+    // margin: 1e-3 of a cell for the float32 rounding of the cell assignment (a particle may sit a few ulp of
+    // its coordinate outside its nominal cell) and of the encoding
+    fc.near_lo = -(float)(0.5 * (double)fc.ws - es * 1.0001 - 1e-3 * (double)fc.ws);
     fc.flags = (plummer ? FC_PLUMMER : 0) | ((double)fc.ws * 0.999 > es * 1.0001 ? FC_FAR_OK : 0);
     return fc;
 }
