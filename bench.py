@@ -42,7 +42,7 @@ FP32_LANES_PER_SM = 128
 ORACLE_BLOCK = 44                  # the oracle's sample is drawn from the sinks of a 44^3-cell block (~5 M sinks at 64 per cell)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_forces_warp launch, from the `ncu --set full`
 # captures summarised under profiles/ (the file named there gives the command); None = not captured
-NCU_TRAFFIC_BYTES = {"C4-clustered-1024^3": 169.98e9}   # profiles/r01_interaction_kernel_c4_dram.md
+NCU_TRAFFIC_BYTES = {"C4-clustered-1024^3": 169.60e9}   # profiles/r01_interaction_kernel_c4_dram.md
 
 
 def read_peaks():
