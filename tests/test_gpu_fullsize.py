@@ -75,6 +75,7 @@ def test_full_box_sampled_sinks(ctx, which):
     a_ref = oracle.forces(pos_np, cfg.K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=sink_idx)
     # the metric's rms is taken over the sampled sinks
     err = oracle.parity_error(acc[torch.from_numpy(sink_idx).cuda()].cpu().numpy(), a_ref)
+    print(f"[parity] {cfg.name}: {sink_idx.size} sinks, median {np.median(err):.2e}, 99.9 % {np.quantile(err, 0.999):.2e}, max {err.max():.2e}")
     assert np.median(err) <= MEDIAN_TOL, f"median error {np.median(err):.3e}"
     assert err.max() <= MAX_TOL, f"max error {err.max():.3e}"
 
@@ -129,6 +130,7 @@ def test_c4_full_size_blocks(ctx):
         a_ref = oracle.forces(sub, K, R, cfg.eps, cfg.box, cfg.Gm, sink_idx=sink_local)
         got = acc[idx[torch.from_numpy(sink_local).cuda()]].cpu().numpy()
         err = oracle.parity_error(got, a_ref)
+        print(f"[parity] {cfg.name} block {c0}: {sink_local.size} sinks, median {np.median(err):.2e}, 99.9 % {np.quantile(err, 0.999):.2e}, max {err.max():.2e}")
         assert np.median(err) <= MEDIAN_TOL, f"median error {np.median(err):.3e} at block {c0}"
         assert err.max() <= MAX_TOL, f"max error {err.max():.3e} at block {c0}"
 
@@ -183,6 +185,7 @@ def test_c5_stream_full_size(ctx):
         a_ref = oracle.forces(sub, K, R, cfg.eps, cfg.box, Gm, sink_idx=sink_local)
         got = np.stack([out[q - R][r].numpy() for q, r in where[sink_local]])
         err = oracle.parity_error(got, a_ref)
+        print(f"[parity] {cfg.name} block {c0}: {sink_local.size} sinks, median {np.median(err):.2e}, 99.9 % {np.quantile(err, 0.999):.2e}, max {err.max():.2e}")
         assert np.median(err) <= MEDIAN_TOL, f"median error {np.median(err):.3e} at block {c0}"
         assert err.max() <= MAX_TOL, f"max error {err.max():.3e} at block {c0}"
         n_inter += 1
