@@ -394,6 +394,10 @@ def main():
     e2e = None
     if not args.no_e2e:
         try:
+            import psutil
+            need = 24 * N * world * 1.15            # pinned host input + output of every rank on this node
+            if psutil.virtual_memory().available < need:
+                raise MemoryError(f"host leg needs {need / 2**30:.0f} GiB of pinned memory for {world} rank(s)")
             del b, acc
             torch.cuda.empty_cache()
             hpos = torch.empty(N, 3, dtype=torch.float32).pin_memory()
