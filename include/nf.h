@@ -29,7 +29,9 @@
  *   - nf_bin and nf_forces are asynchronous: they enqueue work on `stream` and return.
  *     They may synchronise only when scratch memory has to grow (avoid with nf_reserve).
  *   - There is no CPU fallback anywhere in this library.
- *   - A context must not be used from two threads at once.
+ *   - A context must not be used from two threads at once.  Its scratch arena is reused from call
+ *     to call in stream order: issue the calls of one context on ONE stream (or order the streams
+ *     yourself with events); use one context per concurrent stream.
  */
 #ifndef NF_H
 #define NF_H
