@@ -3,6 +3,8 @@ element by element on the same seeded inputs.  Bars (BASELINE.json north_star): 
 assignment and sort bit-exact; accelerations within a per-particle relative error
 |a_gpu - a_ref| / max(|a_ref|, rms|a_ref|) of 1e-5 at the median and 1e-3 at the maximum.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -521,3 +523,48 @@ def test_stream_slabs_other_shapes(ctx, K, R, P, softening):
     err = oracle.parity_error(got, ref)
     assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (np.median(err), err.max())
     assert stats["particles_out"] == sink_idx.size
+
+
+@pytest.mark.parametrize("seed", list(range(int(os.environ.get("NF_FUZZ_CASES", "40")))))
+def test_forces_randomised_configurations(ctx, seed):
+    """Differential fuzz against the oracle: random K, R, box, N, softening law and length (from 2e-3
+    to 4 cell widths), masses or not, uniform or clumped input with clumps planted on cell corners."""
+    rng = np.random.default_rng(9000 + seed)
+    R = int(rng.integers(0, 4))
+    K = int(rng.integers(2 * R + 1, 2 * R + 14))
+    box = float(10.0 ** rng.uniform(-2, 3))
+    n = int(rng.integers(1, 9000))
+    w = box / K
+    eps = float(w * 10.0 ** rng.uniform(-2.4, 0.6))        # >= 4e-3 w: inside the float32 envelope, see below and DESIGN.md Sec. 7
+    softening = "plummer" if rng.random() < 0.3 else "spline"
+    pos = rng.random((n, 3)) * box
+    n_clumps = int(rng.integers(0, 6))
+    for c in range(n_clumps):
+        m = int(rng.integers(1, max(2, n // 4)))
+        idx = rng.choice(n, m, replace=False)
+        centre = np.round(rng.random(3) * K) * w if rng.random() < 0.6 else rng.random(3) * box   # on a cell corner / anywhere
+        # clump widths stay above 5e-3 cell widths: pairs that straddle a cell face are formed from offsets
+        # shifted by whole cells in float32 (resolution ~1e-7 w in x, y, ~2.4e-7 w in z and more for R = 3,
+        # DESIGN.md Sec. 7), so a clump on a cell corner narrower than that is only good to ~3e-7 w / width
+        sigma = max(eps * 10.0 ** rng.uniform(-1, 1.5), 5e-3 * w)
+        pos[idx] = centre + sigma * rng.standard_normal((m, 3))
+    pos = np.mod(pos, box).astype(np.float32)
+    pos = np.clip(pos, 0, np.nextafter(np.float32(box), np.float32(0)))
+    if n > 3:
+        pos[1] = pos[0]                                   # coincident pair
+    G = float(10.0 ** rng.uniform(-3, 1))
+    use_mass = rng.random() < 0.4
+    mass = rng.uniform(0.0, 3.0, n).astype(np.float32) if use_mass else None
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box, mass=torch.from_numpy(mass).cuda() if use_mass else None)
+    assert ctx.out_of_range() == 0
+    amax = torch.empty(K ** 3, device="cuda")
+    acc = ctx.forces(b, R, eps, G, softening=softening, use_mass=use_mass, cell_amax=amax).cpu().numpy()
+    assert np.isfinite(acc).all()
+    ref = oracle.forces(pos, K, R, eps, box, G, softening=softening, mass=mass)
+    err = oracle.parity_error(acc, ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (seed, K, R, n, eps / w, softening, float(np.median(err)), float(err.max()))
+    key, _ = oracle.keys(pos, K, box)
+    ref_amax = oracle.cell_amax(ref, key, K ** 3)
+    rms = np.sqrt((ref ** 2).sum(axis=1).mean()) if n else 0.0
+    assert (np.abs(amax.cpu().numpy() - ref_amax) <= MAX_TOL * np.maximum(ref_amax, rms) + 1e-30).all()
+    assert ctx.interactions(b, R) == oracle.interactions(u32(b.cell_count), K, R)
