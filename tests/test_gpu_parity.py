@@ -568,3 +568,64 @@ def test_forces_randomised_configurations(ctx, seed):
     rms = np.sqrt((ref ** 2).sum(axis=1).mean()) if n else 0.0
     assert (np.abs(amax.cpu().numpy() - ref_amax) <= MAX_TOL * np.maximum(ref_amax, rms) + 1e-30).all()
     assert ctx.interactions(b, R) == oracle.interactions(u32(b.cell_count), K, R)
+
+
+@pytest.mark.parametrize("seed", list(range(30)))
+def test_bin_randomised(ctx, seed):
+    """nf_bin bit for bit on random K (incl. 1 and non powers of two), box, N around the tile sizes of
+    the radix sort, with particles on cell faces, at 0 and just below the box, out of range and NaN."""
+    rng = np.random.default_rng(500 + seed)
+    K = int(rng.choice([1, 2, 3, 5, 8, 13, 16, 31, 32, 37, 64, 100]))
+    box = float(10.0 ** rng.uniform(-3, 3))
+    n = int(rng.choice([1, 31, 32, 33, 511, 512, 513, 8191, 8192, 8193, 16385, 50_000, 200_003]))
+    pos = (rng.random((n, 3)) * box).astype(np.float32)
+    m = min(n, 64)
+    faces = (rng.integers(0, K + 1, (m, 3)) * (box / K)).astype(np.float32)       # exactly on cell faces (incl. 0 and box)
+    pos[:m] = faces
+    if n > 200:
+        pos[100] = [np.nan, 0.5 * box, 0.5 * box]
+        pos[101] = [-1e-3 * box, 0.5 * box, 2.0 * box]
+        pos[102] = np.nextafter(np.float32(box), np.float32(0))
+        pos[103] = [0.0, -0.0, 1e-38]
+    check_bin(ctx, pos, K, box)
+
+
+@pytest.mark.parametrize("seed", list(range(12)))
+def test_stream_slabs_randomised(ctx, seed):
+    """nf_stream_slabs on random chunk shapes that do not wrap in x (the periodic oracle then sees
+    the same neighbourhoods), uneven planes including empty ones."""
+    rng = np.random.default_rng(700 + seed)
+    R = int(rng.integers(0, 4))
+    P = int(rng.integers(1, 7))
+    K = P + 2 * R + int(rng.integers(1, 6))
+    K = max(K, 2 * R + 1)
+    box = float(10.0 ** rng.uniform(-1, 2))
+    w = box / K
+    plane0 = int(rng.integers(0, K - (P + 2 * R) + 1))
+    eps = float(w * 10.0 ** rng.uniform(-2.2, 0.3))
+    planes = []
+    for q in range(P + 2 * R):
+        n = 0 if rng.random() < 0.15 else int(rng.integers(1, 1500))
+        x = np.empty((n, 3), np.float32)
+        x[:, 0] = ((plane0 + q) + rng.uniform(0.01, 0.99, n)) * w
+        x[:, 1:] = rng.random((n, 2)) * box
+        if n > 50:
+            x[:40, 1:] = np.mod(x[0, 1:] + 0.02 * box * rng.standard_normal((40, 2)), box)
+        planes.append(torch.from_numpy(np.minimum(x, np.nextafter(np.float32(box), np.float32(0)))))
+    pinned = [p.pin_memory() if p.shape[0] else p for p in planes]
+    Gm = float(10.0 ** rng.uniform(-2, 1))
+    softening = "plummer" if rng.random() < 0.3 else "spline"
+    out, stats = ctx.stream_slabs(pinned, P, K, R, eps, box, plane0, Gm, softening=softening)
+    assert stats["out_of_range"] == 0
+    allpos = torch.cat(planes).numpy()
+    starts = np.cumsum([0] + [p.shape[0] for p in planes])
+    sink_idx = np.arange(starts[R], starts[R + P])
+    got = torch.cat(out).numpy()
+    assert got.shape[0] == sink_idx.size
+    if sink_idx.size == 0:
+        return
+    ref = oracle.forces(allpos, K, R, eps, box, Gm, sink_idx=sink_idx, softening=softening)
+    err = oracle.parity_error(got, ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (seed, K, R, P, float(np.median(err)), float(err.max()))
+    cnt = oracle.bin_particles(allpos, K, box)["cell_count"]
+    assert stats["interactions"] == oracle.interactions(cnt, K, R, plane0 + R, plane0 + R + P)
