@@ -203,3 +203,34 @@ def test_c5_stream_full_size(ctx):
     for p in range(P):
         tot += int((cnt[R + p] * nb[p:p + 2 * R + 1].sum(dim=0)).sum())
     assert stats["interactions"] == tot
+
+
+def test_maximum_K(ctx):
+    """K = NF_MAX_K = 1024 (2^30 cells, keys up to 2^30 - 1, 3 radix digits of 1024 bins): binning bit
+    for bit, forces of a sample, interaction count -- on a sparse box with a few dense clumps, so that
+    almost every cell is empty."""
+    import psutil
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90 * (1 << 30) or psutil.virtual_memory().available < 48 * (1 << 30):
+        pytest.skip("needs ~90 GB of device and ~48 GB of host memory for 2^30 cells")
+    K, R, box, n = 1024, 2, 1.0, 300_000
+    rng = np.random.default_rng(1)
+    pos = rng.random((n, 3)).astype(np.float32)
+    c = rng.random((20, 3))
+    pos[:100_000] = np.mod(c[rng.integers(0, 20, 100_000)] + 2e-3 * rng.standard_normal((100_000, 3)), 1.0).astype(np.float32)
+    pos = np.minimum(pos, np.nextafter(np.float32(1), np.float32(0)))
+    eps = 1e-5
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box)
+    assert ctx.out_of_range() == 0
+    acc = ctx.forces(b, R, eps, 1.0 / n).cpu().numpy()
+    assert np.isfinite(acc).all()
+    rb = oracle.bin_particles(pos, K, box)
+    assert np.array_equal(u32(b.perm), rb["perm"]) and np.array_equal(u32(b.cell_count), rb["cell_count"])
+    assert np.array_equal(b.cell_offset.cpu().numpy().view(np.uint64), rb["cell_offset"])
+    assert np.array_equal(b.pos_sorted.cpu().numpy().view(np.uint32), rb["pos_sorted"].view(np.uint32))
+    assert ctx.interactions(b, R) == oracle.interactions(rb["cell_count"], K, R)
+    sink = np.sort(rng.choice(100_000, 20_000, replace=False))          # clump members: they have neighbours
+    ref = oracle.forces(pos, K, R, eps, box, 1.0 / n, sink_idx=sink)
+    err = oracle.parity_error(acc[sink], ref)
+    print(f"[parity] K = 1024: {sink.size} sinks, median {np.median(err):.2e}, max {err.max():.2e}")
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
