@@ -222,9 +222,10 @@ struct SplitTable {
     uint8_t nt[128];
     uint8_t L[128][SPLIT_MAX];
 };
-__constant__ SplitTable c_split;
+__constant__ SplitTable c_split[2];   // [0]: L <= 32;  [1]: L <= 8, for problems too small to fill the GPU with full-width tasks
 
-__global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restrict__ planes, nf_force_params p, uint32_t *__restrict__ tc)
+__global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restrict__ planes, nf_force_params p, int small,
+                                                    uint32_t *__restrict__ tc)
 {
     const int cyz = blockIdx.x * blockDim.x + threadIdx.x;
     const int KK = p.K * p.K;
@@ -232,7 +233,7 @@ __global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restr
     const size_t nc = (size_t)gridDim.y * KK, c = task_slot((int)blockIdx.y, cyz, p.K, (int)gridDim.y);
     const uint64_t *off = planes[p.sink_lo + blockIdx.y].off;
     const uint64_t n = off[cyz + 1] - off[cyz];
-    const uint32_t nt = (uint32_t)(n >> 7) + c_split.nt[n & 127];
+    const uint32_t nt = (uint32_t)(n >> 7) + c_split[small].nt[n & 127];
     const bool heavy = n >= HEAVY_N;
     tc[c] = heavy ? nt : 0u;            // first half of the list: dense cells
     tc[nc + c] = heavy ? 0u : nt;
@@ -240,8 +241,8 @@ __global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restr
 
 // ctl[0] = work cursor (zeroed here), ctl[1] = number of tasks
 __global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restrict__ planes, const uint32_t *__restrict__ tc,
-                                                   const uint32_t *__restrict__ to, nf_force_params p, Task *__restrict__ tasks,
-                                                   uint32_t *__restrict__ ctl)
+                                                   const uint32_t *__restrict__ to, nf_force_params p, int small,
+                                                   Task *__restrict__ tasks, uint32_t *__restrict__ ctl)
 {
     const int cyz = blockIdx.x * blockDim.x + threadIdx.x;
     const int KK = p.K * p.K;
@@ -262,9 +263,9 @@ __global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restri
         first += 128;
     }
     const int rem = (int)(n & 127);
-    for (int k = 0; k < c_split.nt[rem]; k++) {
+    for (int k = 0; k < c_split[small].nt[rem]; k++) {
         t.first = first;
-        t.L = c_split.L[rem][k];
+        t.L = c_split[small].L[rem][k];
         tasks[o++] = t;
         first += 4u * t.L;
     }
@@ -687,7 +688,7 @@ ForceConsts make_consts(const nf_force_params &p)
 }
 
 // split of a remainder of n < 128 sinks into tasks of 4L sinks: minimise sum(1/P + C0), P = floor(32/L)
-void make_split_table(SplitTable &t)
+void make_split_table(SplitTable &t, int Lmax)
 {
     const double C0 = 0.045, INF = 1e30;
     static double dp[SPLIT_MAX + 1][128];
@@ -698,7 +699,7 @@ void make_split_table(SplitTable &t)
         for (int m = 1; m < 128; m++) {
             dp[k][m] = dp[k - 1][m];
             ch[k][m] = 0;                                  // 0: use the (k-1)-task solution
-            for (int L = 1; L <= 32; L++) {
+            for (int L = 1; L <= Lmax; L++) {
                 const int prev = m - 4 * L > 0 ? m - 4 * L : 0;
                 const double c = dp[k - 1][prev] + 1.0 / (32 / L) + C0;
                 if (c < dp[k][m] - 1e-12) { dp[k][m] = c; ch[k][m] = L; }
@@ -749,9 +750,10 @@ size_t nf_forces_scratch_bytes(const nf_force_params &p)
 
 int nf_forces_init(nf_ctx *ctx)
 {
-    SplitTable t;
-    make_split_table(t);
-    NF_CUDA(ctx, cudaMemcpyToSymbol(c_split, &t, sizeof(t)));
+    static SplitTable t[2];
+    make_split_table(t[0], 32);
+    make_split_table(t[1], 8);        // 4 tasks of 32 sinks still cover any remainder below 128
+    NF_CUDA(ctx, cudaMemcpyToSymbol(c_split, t, sizeof(t)));
     return NF_OK;
 }
 
@@ -819,10 +821,13 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
     if (n_sink_planes > 0) {
         // work list
         dim3 grid((unsigned)((p.K * p.K + 255) / 256), (unsigned)n_sink_planes);
-        k_task_count<<<grid, 256, 0, st>>>(d_planes, p, tc);
+        // A problem with fewer tasks than resident warps (3 blocks of 4 per SM) is bound by the length of
+        // one task: narrower tasks (L <= 8, so P >= 4 phases share every tile) halve it.  ~40 sinks per task.
+        const int small = p.max_sinks < 40LL * ctx->sm_count * 3 * WARPS ? 1 : 0;
+        k_task_count<<<grid, 256, 0, st>>>(d_planes, p, small, tc);
         NF_LAUNCHED(ctx);
         NF_TRY(nf_exclusive_scan_u32(ctx, tc, to, 2 * nc, tmp, st));
-        k_task_fill<<<grid, 256, 0, st>>>(d_planes, tc, to, p, tasks, ctl);
+        k_task_fill<<<grid, 256, 0, st>>>(d_planes, tc, to, p, small, tasks, ctl);
         NF_LAUNCHED(ctx);
     }
     if (record_timing) NF_CUDA(ctx, cudaEventRecord(ctx->ev_kern0, st));

@@ -81,6 +81,7 @@ def test_full_box_sampled_sinks(ctx, which):
 
 
 def test_c4_full_size_blocks(ctx):
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 90 * (1 << 30):
         pytest.skip("needs ~90 GB of free device memory")
@@ -210,6 +211,7 @@ def test_maximum_K(ctx):
     for bit, forces of a sample, interaction count -- on a sparse box with a few dense clumps, so that
     almost every cell is empty."""
     import psutil
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 90 * (1 << 30) or psutil.virtual_memory().available < 48 * (1 << 30):
         pytest.skip("needs ~90 GB of device and ~48 GB of host memory for 2^30 cells")
