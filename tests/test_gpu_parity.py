@@ -629,3 +629,33 @@ def test_stream_slabs_randomised(ctx, seed):
     assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (seed, K, R, P, float(np.median(err)), float(err.max()))
     cnt = oracle.bin_particles(allpos, K, box)["cell_count"]
     assert stats["interactions"] == oracle.interactions(cnt, K, R, plane0 + R, plane0 + R + P)
+
+
+@pytest.mark.parametrize("seed", list(range(6)))
+def test_forces_dense_cells_randomised(ctx, seed):
+    """Few cells, many particles (cells of 10^3 - 6x10^4): full 128-sink tasks, the dense-cells-first
+    part of the work list, columns cut into many tiles, K down to 2R+1; sampled sinks against the oracle."""
+    rng = np.random.default_rng(4000 + seed)
+    R = int(rng.integers(1, 4))
+    K = int(rng.integers(2 * R + 1, 2 * R + 5))
+    box = float(10 ** rng.uniform(-1, 2))
+    n = int(rng.integers(50_000, 250_000))
+    w = box / K
+    eps = float(w * 10 ** rng.uniform(-2.3, -0.5))
+    softening = "plummer" if rng.random() < 0.3 else "spline"
+    pos = rng.random((n, 3)) * box
+    for c in range(int(rng.integers(1, 5))):
+        m = int(rng.integers(1000, n // 3))
+        idx = rng.choice(n, m, replace=False)
+        pos[idx] = rng.random(3) * box + w * 10 ** rng.uniform(-1.5, 0.3) * rng.standard_normal((m, 3))
+    pos = np.clip(np.mod(pos, box).astype(np.float32), 0, np.nextafter(np.float32(box), np.float32(0)))
+    use_mass = rng.random() < 0.4
+    mass = rng.uniform(0, 3, n).astype(np.float32) if use_mass else None
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box, mass=torch.from_numpy(mass).cuda() if use_mass else None)
+    acc = ctx.forces(b, R, eps, 1.0 / n, softening=softening, use_mass=use_mass).cpu().numpy()
+    sink = np.sort(rng.choice(n, 3000, replace=False))
+    ref = oracle.forces(pos, K, R, eps, box, 1.0 / n, sink_idx=sink, softening=softening, mass=mass)
+    err = oracle.parity_error(acc[sink], ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (seed, K, R, n, float(np.median(err)), float(err.max()))
+    assert ctx.interactions(b, R) == oracle.interactions(u32(b.cell_count), K, R)
+    assert int(u32(b.cell_count).max()) > 1000
