@@ -286,29 +286,25 @@ class Context:
                                              self._stream(stream)))
         return out, stats.as_dict()
 
-
-def _stream_step(self, planes, vels, P, K, R, eps, box, plane0, Gm, kick, drift, softening="spline", want_acc=False, stream=None):
-    """nf_stream_step_slabs: planes = P + 2R pinned float32 [n_q, 3] position tensors, vels = P pinned
-    velocity tensors of the sink planes; returns (new positions, new velocities, accelerations or None,
-    stats), each a list of P pinned host tensors."""
-    NP = P + 2 * R
-    assert len(planes) == NP and len(vels) == P
-    for t in list(planes) + list(vels):
-        assert (not t.is_cuda) and t.dtype == torch.float32 and t.dim() == 2 and t.shape[1] == 3 and t.is_contiguous()
-        assert t.shape[0] == 0 or t.is_pinned(), "plane tensors must be pinned host memory"
-    mk = lambda: [torch.empty(planes[R + p].shape[0], 3, dtype=torch.float32).pin_memory() for p in range(P)]
-    pos_out, vel_out, acc = mk(), mk(), (mk() if want_acc else None)
-    tab = lambda ts: (ctypes.c_void_p * len(ts))(*[t.data_ptr() if t.shape[0] else None for t in ts])
-    ns = (ctypes.c_int64 * NP)(*[t.shape[0] for t in planes])
-    stats = StreamStats()
-    self._check(self.lib.nf_stream_step_slabs(self._h, tab(planes), tab(vels), ns, int(P), int(K), int(R), float(eps), float(box),
-                                              int(plane0), float(Gm), _SOFT[softening], float(kick), float(drift),
-                                              tab(pos_out), tab(vel_out), tab(acc) if acc is not None else None,
-                                              ctypes.byref(stats), self._stream(stream)))
-    return pos_out, vel_out, acc, stats.as_dict()
-
-
-Context.stream_step_slabs = _stream_step
+    def stream_step_slabs(self, planes, vels, P, K, R, eps, box, plane0, Gm, kick, drift, softening="spline", want_acc=False, stream=None):
+        """nf_stream_step_slabs: planes = P + 2R pinned float32 [n_q, 3] position tensors, vels = P pinned
+        velocity tensors of the sink planes; returns (new positions, new velocities, accelerations or None,
+        stats), each a list of P pinned host tensors."""
+        NP = P + 2 * R
+        assert len(planes) == NP and len(vels) == P
+        for t in list(planes) + list(vels):
+            assert (not t.is_cuda) and t.dtype == torch.float32 and t.dim() == 2 and t.shape[1] == 3 and t.is_contiguous()
+            assert t.shape[0] == 0 or t.is_pinned(), "plane tensors must be pinned host memory"
+        mk = lambda: [torch.empty(planes[R + p].shape[0], 3, dtype=torch.float32).pin_memory() for p in range(P)]
+        pos_out, vel_out, acc = mk(), mk(), (mk() if want_acc else None)
+        tab = lambda ts: (ctypes.c_void_p * len(ts))(*[t.data_ptr() if t.shape[0] else None for t in ts])
+        ns = (ctypes.c_int64 * NP)(*[t.shape[0] for t in planes])
+        stats = StreamStats()
+        self._check(self.lib.nf_stream_step_slabs(self._h, tab(planes), tab(vels), ns, int(P), int(K), int(R), float(eps), float(box),
+                                                  int(plane0), float(Gm), _SOFT[softening], float(kick), float(drift),
+                                                  tab(pos_out), tab(vel_out), tab(acc) if acc is not None else None,
+                                                  ctypes.byref(stats), self._stream(stream)))
+        return pos_out, vel_out, acc, stats.as_dict()
 
 
 def spline_equivalent_eps(eps_plummer: float) -> float:
