@@ -139,8 +139,10 @@ int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream);
  *   softening    NF_SOFT_SPLINE or NF_SOFT_PLUMMER, optionally | NF_MASS_W
  *   acc_xyz      dev out  N x 3 float32
  *
- * float32 in, float32 accumulate (per source tile, with a compensated outer sum), float32
- * out.  Deterministic: no floating-point atomics; the same inputs give the same bits.
+ * float32 in, float32 accumulate (per-tile partial sums formed from zero, added to a running
+ * float32 sum over tiles visited in mirror-paired column order; the partial sums of the lanes that
+ * share a sink are combined in double), float32 out.  Deterministic: no floating-point atomics;
+ * the same inputs give the same bits.
  */
 int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
               const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
