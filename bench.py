@@ -40,9 +40,35 @@ from paper_1810_02916_b200 import inputs  # noqa: E402
 FLOP_PER_INTERACTION = 20          # BASELINE.json convention (the paper counts 23)
 FP32_LANES_PER_SM = 128
 ORACLE_BLOCK = 44                  # the oracle's sample is drawn from the sinks of a 44^3-cell block (~5 M sinks at 64 per cell)
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_forces_warp launch, from the `ncu --set full`
-# captures summarised under profiles/ (the file named there gives the command); None = not captured
-NCU_TRAFFIC_BYTES = {"C4-clustered-1024^3": 169.60e9}   # profiles/r01_interaction_kernel_c4_dram.md
+ORACLE_SINKS = 1 << 21             # ... a seeded choice of this many of them, the SAME in both arms (cpu_baseline and --impl reference)
+ORACLE_SEED = 1
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "interaction_kernel_traffic.json")
+KERNEL_SOURCES = ["paper_1810_02916_b200/csrc/nf_forces.cu", "paper_1810_02916_b200/csrc/nf_common.cuh"]
+
+
+def kernel_source_hash() -> str:
+    """sha256 over the interaction kernel's sources: what a stored ncu counter is valid for (the GPU box
+    has no .git, so a commit id cannot be checked there)."""
+    import hashlib
+    h = hashlib.sha256()
+    for rel in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, rel), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
+def ncu_traffic(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one interaction-kernel launch on `workload`, from
+    the ncu capture recorded in profiles/interaction_kernel_traffic.json -- or None when that capture was
+    taken from other kernel sources than the ones in this tree (the number would be stale)."""
+    try:
+        with open(TRAFFIC_JSON) as fh:
+            rec = json.load(fh).get(workload)
+    except (OSError, ValueError):
+        return None
+    if not rec or rec.get("kernel_source_sha256") != kernel_source_hash():
+        return None
+    return float(rec["dram_bytes_read"]) + float(rec["dram_bytes_write"])
 
 
 def read_peaks():
@@ -114,46 +140,67 @@ def oracle_sample(pos_dev: torch.Tensor, cfg, m: int, c0=(3, 5, 7)):
     return sub, idx
 
 
-def time_oracle(sub, cfg, m, c0, budget_s=20.0):
-    """Oracle forces for the sinks in the inner m^3 block; returns (interactions, seconds, cores, n_sinks)."""
+def time_oracle(sub, cfg, m, c0, n_sinks=ORACLE_SINKS):
+    """The oracle, as it stands, on a seeded sample of `n_sinks` sinks of the inner m^3 block (all their
+    sources are in `sub`).  The SAME sample in both arms of the bench.  One oracle.forces call does its own
+    cell assignment and sort of `sub` first (a fixed cost that does not scale with the sample); that part is
+    timed by itself with oracle.bin_particles and reported beside the rate, which is pairs / (call - binning).
+    Returns a dict: interactions, seconds (force part), seconds_binning, seconds_call, cores, n_sinks, sinks
+    (indices into sub), acc (float64 [n_sinks, 3])."""
     import numpy as np
     import oracle
-    keys, _ = oracle.keys(sub, cfg.K, cfg.box)
-    K = cfg.K
+    K, R = cfg.K, cfg.R
+    keys, _ = oracle.keys(sub, K, cfg.box)
     cz, cy, cx = keys % K, (keys // K) % K, keys // (K * K)
     inner = np.ones(len(keys), bool)
     for c, lo in ((cx, c0[0]), (cy, c0[1]), (cz, c0[2])):
-        if K > m + 2 * (cfg.R + 1):
+        if K > m + 2 * (R + 1):
             inner &= ((c.astype(np.int64) - lo) % K) < m
     sink_idx = np.nonzero(inner)[0]
-    # interactions of those sinks: count neighbours through the oracle's own cell counts
-    cnt = np.bincount(keys, minlength=K ** 3).astype(np.uint32)
-    # two pilots (2 000 and 20 000 sinks) separate the call's fixed cost (its own binning of `sub`)
-    # from the per-sink cost; the timed sample is then sized to ~budget_s of CPU work
-    rng = np.random.default_rng(1)
-    tp = []
-    for n_p in (2000, 20000):
-        pilot = np.sort(rng.choice(sink_idx, min(len(sink_idx), n_p), replace=False))
-        t0 = time.perf_counter()
-        oracle.forces(sub, K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=pilot)
-        tp.append((len(pilot), max(time.perf_counter() - t0, 1e-4)))
-    per_sink = max((tp[1][1] - tp[0][1]) / max(tp[1][0] - tp[0][0], 1), 1e-9)
-    n_timed = int(min(len(sink_idx), max(tp[1][0], budget_s / per_sink)))
-    timed = np.sort(rng.choice(sink_idx, n_timed, replace=False))
+    rng = np.random.default_rng(ORACLE_SEED)
+    timed = np.sort(rng.choice(sink_idx, min(len(sink_idx), n_sinks), replace=False))
     t0 = time.perf_counter()
-    acc = oracle.forces(sub, K, cfg.R, cfg.eps, cfg.box, cfg.Gm, sink_idx=timed)
-    dt = time.perf_counter() - t0
-    # ordered pairs evaluated for the timed sinks
+    oracle.bin_particles(sub, K, cfg.box)
+    t_bin = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    acc = oracle.forces(sub, K, R, cfg.eps, cfg.box, cfg.Gm, sink_idx=timed)
+    t_call = time.perf_counter() - t0
+    # ordered pairs evaluated for the timed sinks, from the oracle's own cell counts
+    cnt3 = np.bincount(keys, minlength=K ** 3).reshape(K, K, K).astype(np.int64)
     kk = keys[timed].astype(np.int64)
     tz, ty, tx = kk % K, (kk // K) % K, kk // (K * K)
-    cnt3 = cnt.reshape(K, K, K).astype(np.int64)
     inter = 0
-    R = cfg.R
     for dx in range(-R, R + 1):
         for dy in range(-R, R + 1):
             for dz in range(-R, R + 1):
                 inter += int(cnt3[(tx + dx) % K, (ty + dy) % K, (tz + dz) % K].sum())
-    return inter, dt, oracle.max_threads(), n_timed, timed, acc
+    return {"interactions": inter, "seconds": max(t_call - t_bin, 1e-9), "seconds_binning": t_bin, "seconds_call": t_call,
+            "cores": oracle.max_threads(), "n_sinks": len(timed), "sinks": timed, "acc": acc}
+
+
+def cpu_baseline_block(o, cfg, m):
+    return {"value": o["interactions"] / o["seconds"], "unit": "interactions/s", "cores": o["cores"], "kind": "oracle",
+            "seconds": o["seconds"], "seconds_binning": o["seconds_binning"],
+            "sample": f"{o['n_sinks']} seeded sinks of a {m}^3-cell block of {cfg.name} with all their sources "
+                      f"({o['interactions']} pairs, float64); the oracle's own binning of the block ({o['seconds_binning']:.2f} s) "
+                      f"is timed separately and not in the rate"}
+
+
+def parity_block(a_gpu, a_ref):
+    """GPU accelerations of the timed run against the oracle's, on the cpu_baseline sample: the north_star
+    metric e = |da| / max(|a_ref|, rms |a_ref|) and the paper's own statistic, the fractional error
+    |da| / |a| (median 7.5e-7, 0.038 % of particles above 1e-4 on the S2016 z = 0 state)."""
+    import numpy as np
+    import oracle
+    a_gpu = np.asarray(a_gpu, dtype=np.float64)
+    e = oracle.parity_error(a_gpu, a_ref)
+    mag = np.sqrt((a_ref ** 2).sum(axis=1))
+    fe = np.sqrt(((a_gpu - a_ref) ** 2).sum(axis=1)) / np.where(mag > 0, mag, 1.0)
+    return {"n_sinks": int(e.size), "median": float(np.median(e)), "p999": float(np.quantile(e, 0.999)), "max": float(e.max()),
+            "frac_err_median": float(np.median(fe)), "frac_gt_1e-4": float(np.mean(fe > 1e-4)),
+            "tolerance": {"median": 1e-5, "max": 1e-3},
+            "pass": bool(np.median(e) <= 1e-5 and e.max() <= 1e-3),
+            "metric": "|a_gpu - a_ref| / max(|a_ref|, rms|a_ref|) over the sampled sinks; frac_err = |da|/|a| (PAPER.md:264)"}
 
 
 def run_reference(args, cfg):
@@ -170,23 +217,21 @@ def run_reference(args, cfg):
     pos = inputs.make_positions(cfg, device=dev)
     sub, _ = oracle_sample(pos, cfg, m)
     del pos
-    per_step = []
-    inter_step = 0
-    budget = 8.0
+    per_step, o = [], None
     for it in range(args.warmup + args.steps):
-        inter, dt, cores, n_sinks, _, _ = time_oracle(sub, cfg, m, (3, 5, 7), budget_s=budget)
+        o = time_oracle(sub, cfg, m, (3, 5, 7))
         if it >= args.warmup:
-            per_step.append(dt)
-            inter_step = inter
+            per_step.append(o["seconds"])
     ms = 1e3 * sum(per_step) / len(per_step)
-    value = inter_step / (ms * 1e-3)
+    value = o["interactions"] / (ms * 1e-3)
+    cb = cpu_baseline_block(o, cfg, m)
+    cb["value"] = value
     line = {"impl": "reference", "metric": "near_field_pairwise_interactions_per_s", "value": value,
             "unit": "interactions/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "N": cfg.N, "K": cfg.K, "R": cfg.R, "sample": f"{n_sinks} sinks of a {m}^3-cell block, all their sources"},
-            "cpu_baseline": {"value": value, "unit": "interactions/s", "cores": cores, "kind": "oracle",
-                             "sample": f"{n_sinks} sinks of a {m}^3-cell block with all their sources, {inter_step} pairs per step"},
+            "config": {"workload": cfg.name, "N": cfg.N, "K": cfg.K, "R": cfg.R, "eps": cfg.eps, "box": cfg.box},
+            "cpu_baseline": cb,
             "e2e": {"value": value, "unit": "interactions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -212,7 +257,10 @@ def run_stream(args, cfg):
         torch.cuda.synchronize()
 
     rcfg = cfg if rank == 0 else inputs.dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
-    planes_dev = inputs.make_slab_planes(rcfg, device=dev)
+    ctx = nf.Context(local)
+    # particles are filed under the x-plane the library's own cell assignment gives them (nf_keys / K^2)
+    plane_of = lambda x: ctx.keys(x.contiguous(), rcfg.K, rcfg.box).long() // (rcfg.K * rcfg.K)
+    planes_dev = inputs.make_slab_planes(rcfg, device=dev, plane_of=plane_of)
     planes = []
     for t in planes_dev:
         h = torch.empty(t.shape, dtype=torch.float32).pin_memory()
@@ -224,7 +272,6 @@ def run_stream(args, cfg):
     n_in = sum(t.shape[0] for t in planes)
     n_out = sum(planes[R + p].shape[0] for p in range(P))
     Gm = 1.0 / float(rcfg.density_n) ** 3
-    ctx = nf.Context(local)
     out = [torch.empty(planes[R + p].shape[0], 3, dtype=torch.float32).pin_memory() for p in range(P)]
     stats = None
     for _ in range(max(args.warmup, 1)):
@@ -265,7 +312,7 @@ def run_stream(args, cfg):
     achieved = FLOP_PER_INTERACTION * I / (f_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "interaction kernel (16 launches, one per sink plane, with their work-list kernels)",
                 "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                "traffic": NCU_TRAFFIC_BYTES.get(rcfg.name),
+                "traffic": ncu_traffic(rcfg.name),
                 "peak_source": f"{sms} SMs x {sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz) x 2 x {FP32_LANES_PER_SM} FP32 lanes",
                 "flop_per_interaction": FLOP_PER_INTERACTION, "frac_at_paper_23_flop": achieved / peak_tflops * 23.0 / FLOP_PER_INTERACTION,
                 "kernel_ms": f_ms,
@@ -293,6 +340,44 @@ def run_stream(args, cfg):
         dist.destroy_process_group()
 
 
+def sweep_small_configs(ctx, dev, steps=3, warmup=3):
+    """Interaction-kernel roofline fraction of C1, C2 and C3 in the same process (milliseconds each): the
+    other single-GPU configs of BASELINE.json beside the headline workload.  Same timing rules as the main
+    line: W warm-up steps, the L2 flushed between timed steps (inputs smaller than the L2), CUDA events
+    around the kernel inside nf_forces."""
+    sm_max_mhz, _, _ = read_peaks()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak = sms * sm_max_mhz * 1e6 * 2 * FP32_LANES_PER_SM
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    out = {}
+    for which in (1, 2, 3):
+        cfg = inputs.config(which)
+        pos = inputs.make_positions(cfg, device=dev)
+        b = ctx.bin(pos, cfg.K, cfg.box)
+        acc = torch.empty(cfg.N, 3, dtype=torch.float32, device=dev)
+        I = ctx.interactions(b, cfg.R)
+        k_ms, s_ms = [], []
+        for it in range(warmup + steps):
+            flush.fill_(it)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.bin(pos, cfg.K, cfg.box, out=b)
+            ctx.forces(b, cfg.R, cfg.eps, cfg.Gm, out=acc)
+            e1.record()
+            k = ctx.last_forces_timing()[0]
+            if it >= warmup:
+                k_ms.append(k)
+                s_ms.append(e0.elapsed_time(e1))
+        k = sum(k_ms) / len(k_ms)
+        out[cfg.name] = {"kernel_ms": k, "step_ms": sum(s_ms) / len(s_ms), "interactions": I,
+                         "frac": FLOP_PER_INTERACTION * I / (k * 1e-3) / peak,
+                         "interactions_per_s_step": I / (sum(s_ms) / len(s_ms) * 1e-3)}
+        del pos, b, acc
+    del flush
+    torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -302,6 +387,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the C1-C3 kernel sweep of the default line")
     ap.add_argument("--n-side", type=int, default=0,
                     help="profiling aid: the same recipe at n_side^3 particles and K = n_side/4 (not the bench workload)")
     args = ap.parse_args()
@@ -339,9 +425,12 @@ def main():
 
     # every rank owns an independently seeded box of the same recipe (weak scaling)
     rcfg = cfg if rank == 0 else inputs.dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    ctx = nf.Context(local)
+    sweep = None
+    if args.config == 4 and not args.n_side and not args.no_sweep and world == 1:
+        sweep = sweep_small_configs(ctx, dev)
     pos = inputs.make_positions(rcfg, device=dev)
     N, K, R = rcfg.N, rcfg.K, rcfg.R
-    ctx = nf.Context(local)
     ctx.reserve(N, K)
     b = ctx.bin(pos, K, rcfg.box)
     acc = torch.empty(N, 3, dtype=torch.float32, device=dev)
@@ -385,10 +474,13 @@ def main():
     value = float(I_all.item()) / (ms_per_step * 1e-3)
     k_ms = sum(kern_ms) / len(kern_ms)
 
-    # sample for the CPU oracle (taken now, while the positions are still on the device)
-    cpu_sub = None
+    # sample for the CPU oracle (taken now, while the positions and the accelerations of the last timed
+    # step are still on the device): the block's particles, and the GPU's accelerations of the same rows
+    cpu_sub, acc_sub = None, None
     if not args.no_cpu and world == 1 and rank == 0:
-        cpu_sub, _ = oracle_sample(pos, rcfg, ORACLE_BLOCK)
+        cpu_sub, sub_idx = oracle_sample(pos, rcfg, ORACLE_BLOCK)
+        acc_sub = (acc if sub_idx is None else acc[sub_idx]).cpu().numpy()
+        del sub_idx
 
     # ---- end to end through nf_forces_host (pinned host buffers, copies inside the timing) ----
     e2e = None
@@ -439,7 +531,7 @@ def main():
     peak_tflops = sms * sm_max_mhz * 1e6 * 2 * FP32_LANES_PER_SM / 1e12
     achieved = FLOP_PER_INTERACTION * I / (k_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "interaction kernel (nf_forces)", "achieved": achieved,
-                "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": NCU_TRAFFIC_BYTES.get(rcfg.name),
+                "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": ncu_traffic(rcfg.name),
                 "peak_source": f"{sms} SMs x {sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz) x 2 x {FP32_LANES_PER_SM} FP32 lanes",
                 "flop_per_interaction": FLOP_PER_INTERACTION, "frac_at_paper_23_flop": achieved / peak_tflops * 23.0 / FLOP_PER_INTERACTION,
                 "kernel_ms": k_ms,
@@ -447,13 +539,12 @@ def main():
                 "frac_at_sampled_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max_mhz)
                                           if clocks and clocks.get("sm_mhz") else None)}
 
-    cpu = None
+    cpu, parity = None, None
     if cpu_sub is not None:
-        m = ORACLE_BLOCK
-        inter, dt, cores, n_sinks, _, _ = time_oracle(cpu_sub, rcfg, m, (3, 5, 7), budget_s=15.0)
-        cpu = {"value": inter / dt, "unit": "interactions/s", "cores": cores, "kind": "oracle",
-               "sample": f"{n_sinks} sinks drawn from a {m}^3-cell block of {rcfg.name} with all their sources: "
-                         f"{inter} pairs in {dt:.2f} s, float64"}
+        o = time_oracle(cpu_sub, rcfg, ORACLE_BLOCK, (3, 5, 7))
+        cpu = cpu_baseline_block(o, rcfg, ORACLE_BLOCK)
+        # the oracle's accelerations of the timed sample against the GPU's from the last TIMED step
+        parity = parity_block(acc_sub[o["sinks"]], o["acc"])
 
     line = {"metric": "near_field_pairwise_interactions_per_s", "value": value, "unit": "interactions/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
@@ -463,7 +554,8 @@ def main():
                        "l2": "flushed between timed steps (256 MiB write)" if small else "inputs larger than L2",
                        "parallelism": f"{world} independent boxes, one per GPU" if world > 1 else "1 GPU"},
             "particles_per_s": float(N_all.item()) / (ms_per_step * 1e-3),
-            "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu}
+            "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+            "parity": parity, "sweep": sweep}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -115,6 +115,13 @@ int nf_bin_m(nf_ctx *ctx, const float *pos_xyz, const float *mass, int64_t N, in
              float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,
              void *stream);
 
+/* nf_keys -- the cell assignment alone: keys[i] =
+ * (cx*K + cy)*K + cz of particle i by the bit-exact float32 formula of nf_bin, no histogram, no sort.
+ * The x-plane ("slab") a particle is filed under is keys[i] / K^2.
+ *   pos_xyz  dev in   N x 3 float32;   keys  dev out  N uint32.
+ * Out-of-range particles are clamped and counted as for nf_bin (read with nf_out_of_range). */
+int nf_keys(nf_ctx *ctx, const float *pos_xyz, int64_t N, int K, float box, uint32_t *keys, void *stream);
+
 /* Synchronises `stream`, stores the number of out-of-range particles seen by the last nf_bin
  * (or nf_stream_slabs) on this context in *n, and returns NF_ERR_RANGE if it is non-zero. */
 int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream);
@@ -128,7 +135,9 @@ int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream);
  *   or the Plummer law.  Pairs with r = 0 (self, coincident particles) contribute zero.
  *   The periodic image of a source is fixed by the cell offset (reading c8).
  *
- *   pos_sorted, cell_offset, cell_count   dev in   as written by nf_bin
+ *   pos_sorted, cell_offset   dev in   as written by nf_bin
+ *   cell_count   dev in, may be NULL: kept in the signature beside nf_bin's other outputs; the
+ *                current implementation derives every count from cell_offset and never reads it
  *   perm         dev in, nullable: if given, accelerations are written in the caller's
  *                original order (acc[perm[s]] = a of sorted slot s), else in sorted order
  *   N, K, box    as for nf_bin;  requires K >= 2R+1 (else a cell would be listed twice)
@@ -142,7 +151,23 @@ int nf_out_of_range(nf_ctx *ctx, int64_t *n, void *stream);
  * float32 in, float32 accumulate (per-tile partial sums formed from zero, added to a running
  * float32 sum over tiles visited in mirror-paired column order; the partial sums of the lanes that
  * share a sink are combined in double), float32 out.  Deterministic: no floating-point atomics;
- * the same inputs give the same bits.
+ * the same inputs give the same bits.  Denormal float32 values are flushed to zero inside the
+ * interaction kernel (not in nf_bin / nf_kick_drift, whose contracts are IEEE).
+ *
+ * Accuracy envelope ("Float32 envelope").  A pair inside one cell is formed from
+ * exact differences of cell-centred offsets.  A pair that straddles a cell face is
+ * formed from offsets shifted by whole cells in float32, which rounds at ~1e-7 w (w = box/K; up to
+ * 2.4e-7 w in z), so such a pair at separation r carries a relative error of up to ~3e-7 w/r in its
+ * force.  The north_star bar (1e-5 median, 1e-3 maximum of |da| / max(|a|, rms|a|)) therefore holds
+ * when eps >= 4e-3 w and no structure narrower than ~5e-3 w sits on a cell face or corner; below
+ * that the maximum error of face-straddling close pairs grows like 3e-7 w / min(r, eps) (an unsoftened
+ * clump 1e-4 w wide planted on a corner reaches ~5e-3), while pairs inside one cell stay exact.
+ * All five BASELINE configs (eps/w = 5e-3 .. 1e-2) and the paper's run (eps/w ~ 1.4e-2) are inside.
+ * The library accepts any eps > 0; results outside the envelope are bounded as stated, not refused.
+ *
+ * If nf_out_of_range() reports clamped particles for the arrays passed here, accelerations of
+ * particles in the edge cells are unspecified (the pruning of close-pair tests assumes every offset
+ * lies within its cell): treat NF_ERR_RANGE as an error of the input, not as a warning.
  */
 int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
               const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
@@ -164,6 +189,25 @@ int nf_forces_ex(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offs
                  const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
                  float eps, float box, float Gm, int softening, float *acc_xyz,
                  float *cell_amax, void *stream);
+
+/*
+ * nf_forces_chunk -- nf_forces_ex for a device-resident CHUNK of the box: the multi-GPU slab
+ * decomposition (PAPER.md:41 slabs, :81 "a parallel version of Abacus based on the existing slab
+ * decomposition").  The arrays describe whatever particles this GPU holds,
+ * binned by nf_bin over the full K^3 grid: its own x-planes [x_lo, x_hi) plus the R ghost planes
+ * received from each x-neighbour; all other planes are simply empty.  Only particles of planes
+ * [x_lo, x_hi) are sinks (acc_xyz rows of ghost particles are not written); every particle present is
+ * a source for the sinks within R cells of it, with the usual periodic wrap in x, y and z -- so a
+ * chunk touching the box edge takes its wrapped ghost planes with their stored coordinates.
+ * Missing planes contribute nothing: x is open at the ends of what was supplied.
+ *
+ *   x_lo, x_hi   sink plane range, 0 <= x_lo <= x_hi <= K (ranges that wrap are two calls)
+ *   cell_amax    nullable, K^3 float32 as for nf_forces_ex (zero outside the sink planes)
+ *   everything else as for nf_forces_ex.  nf_forces_ex is nf_forces_chunk with [0, K).
+ */
+int nf_forces_chunk(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset, const uint32_t *perm,
+                    int64_t N, int K, int R, float eps, float box, float Gm, int softening, int x_lo, int x_hi,
+                    float *acc_xyz, float *cell_amax, void *stream);
 
 /*
  * nf_kick_drift -- the leapfrog updates that follow the force in the slab pipeline (Table 1
@@ -210,9 +254,14 @@ int nf_cell_vrms(nf_ctx *ctx, const float *vel_xyz, const uint32_t *perm, const 
  *
  * The call returns after the D2H copy has completed (it synchronises `stream`).  Returns
  * NF_ERR_RANGE (after completing the computation) if positions outside [0, box) were clamped.
+ * nf_forces_host takes equal masses only (NF_MASS_W is an NF_ERR_ARG here);
+ * nf_forces_host_m adds   mass_host  host in, N float32 source masses in the caller's order, and
+ * wants NF_MASS_W set in `softening` exactly when mass_host is non-NULL (Gm is then G).
  */
 int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, float eps,
                    float box, float Gm, int softening, float *acc_host, void *stream);
+int nf_forces_host_m(nf_ctx *ctx, const float *pos_host, const float *mass_host, int64_t N, int K, int R,
+                     float eps, float box, float Gm, int softening, float *acc_host, void *stream);
 int nf_reserve_host(nf_ctx *ctx, int64_t maxN, int K);
 
 /* Number of ordered (sink, source) pairs nf_forces evaluates for these cell counts:
@@ -246,7 +295,8 @@ typedef struct nf_stream_stats {
  * cells, from pinned host memory, with H2D / D2H copies on side streams overlapping the
  * kernels.
  *
- *   plane_pos_host  host in   P + 2R pointers (pinned memory); plane q holds plane_n[q] x 3
+ *   plane_pos_host  host in   P + 2R pointers (pinned = page-locked host memory, cudaMemoryTypeHost;
+ *                             pageable or managed memory is refused with NF_ERR_ARG); plane q holds plane_n[q] x 3
  *                             float32 global positions of the particles whose x-cell index
  *                             is (plane0 + q) mod K; the first and last R planes are ghosts
  *                             (sources only)
@@ -263,8 +313,14 @@ typedef struct nf_stream_stats {
  *   stats           host out, nullable
  *
  * x is open inside the chunk: only the P + 2R supplied planes act as sources.  Requires
- * K >= 2R+1 and P + 2R <= K.  Returns after the last D2H copy has completed (the call
- * synchronises); `stream` orders the call after prior work on that stream.
+ * K >= 2R+1 and P <= K (with P + 2R > K the ghost planes repeat sink planes of the other end of
+ * the periodic box: pass the same arrays again).  Returns after the last D2H copy has completed
+ * (the call synchronises, also on every error path, so no caller buffer is in use after it
+ * returns); `stream` orders the call after prior work on that stream.
+ * A particle outside [0, box) or filed under a plane other than the one its x coordinate maps to
+ * (nf_keys / K^2) is clamped into its plane's edge cells and counted in stats->out_of_range; the
+ * call then completes and returns NF_ERR_RANGE, and the accelerations of that pass are unspecified
+ * near those particles (see the envelope note of nf_forces).
  */
 int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,
                     int P, int K, int R, float eps, float box, int plane0, float Gm,

@@ -164,30 +164,24 @@ static int check_force_args(nf_ctx *ctx, int K, int R, float eps, float Gm, int 
     return NF_OK;
 }
 
-int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
-              const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
-              float eps, float box, float Gm, int softening, float *acc_xyz, void *stream)
+// nf_forces / nf_forces_ex / nf_forces_chunk: sinks are the particles of the x-planes [x_lo, x_hi)
+static int forces_common(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset, const uint32_t *perm, int64_t N, int K,
+                         int R, float eps, float box, float Gm, int softening, int x_lo, int x_hi, float *acc_xyz, float *cell_amax,
+                         void *stream)
 {
-    return nf_forces_ex(ctx, pos_sorted, cell_offset, cell_count, perm, N, K, R, eps, box, Gm, softening, acc_xyz, nullptr, stream);
-}
-
-int nf_forces_ex(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
-                 const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
-                 float eps, float box, float Gm, int softening, float *acc_xyz, float *cell_amax, void *stream)
-{
-    if (!ctx) return NF_ERR_ARG;
     NF_TRY(check_common(ctx, N, K, box));
     NF_TRY(check_force_args(ctx, K, R, eps, Gm, softening));
-    NF_ARG(ctx, cell_offset && cell_count, "nf_forces: cell_offset / cell_count must not be null");
+    NF_ARG(ctx, cell_offset != nullptr, "nf_forces: cell_offset must not be null");
     NF_ARG(ctx, N == 0 || (pos_sorted && acc_xyz), "nf_forces: null particle array with N > 0");
     NF_ARG(ctx, ((uintptr_t)pos_sorted & 15) == 0, "nf_forces: pos_sorted must be 16-byte aligned");
+    NF_ARG(ctx, 0 <= x_lo && x_lo <= x_hi && x_hi <= K, "sink plane range [%d, %d) is not inside [0, %d]", x_lo, x_hi, K);
     NF_CUDA(ctx, cudaSetDevice(ctx->device));
-    if (N == 0) {
+    if (N == 0 || x_lo == x_hi) {
         if (cell_amax) NF_CUDA(ctx, cudaMemsetAsync(cell_amax, 0, sizeof(float) * (size_t)K * K * K, (cudaStream_t)stream));
         return NF_OK;
     }
     nf_force_params p{};
-    p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
+    p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = x_lo; p.sink_hi = x_hi;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
     nf_scratch_reset(ctx);
     NF_TRY(nf_scratch_reserve(ctx, forces_scratch_full(N, K)));
@@ -203,10 +197,44 @@ int nf_forces_ex(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offs
     return nf_forces_impl(ctx, p, d_planes, st, true);
 }
 
+int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
+              const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
+              float eps, float box, float Gm, int softening, float *acc_xyz, void *stream)
+{
+    return nf_forces_ex(ctx, pos_sorted, cell_offset, cell_count, perm, N, K, R, eps, box, Gm, softening, acc_xyz, nullptr, stream);
+}
+
+int nf_forces_ex(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,
+                 const uint32_t *cell_count, const uint32_t *perm, int64_t N, int K, int R,
+                 float eps, float box, float Gm, int softening, float *acc_xyz, float *cell_amax, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    (void)cell_count;     // accepted for symmetry with nf_bin's outputs; everything is derived from cell_offset
+    return forces_common(ctx, pos_sorted, cell_offset, perm, N, K, R, eps, box, Gm, softening, 0, K, acc_xyz, cell_amax, stream);
+}
+
+int nf_forces_chunk(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset, const uint32_t *perm, int64_t N, int K,
+                    int R, float eps, float box, float Gm, int softening, int x_lo, int x_hi, float *acc_xyz, float *cell_amax,
+                    void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    return forces_common(ctx, pos_sorted, cell_offset, perm, N, K, R, eps, box, Gm, softening, x_lo, x_hi, acc_xyz, cell_amax, stream);
+}
+
+int nf_keys(nf_ctx *ctx, const float *pos_xyz, int64_t N, int K, float box, uint32_t *keys, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_TRY(check_common(ctx, N, K, box));
+    NF_ARG(ctx, N == 0 || (pos_xyz && keys), "nf_keys: null array with N > 0");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, sizeof(unsigned long long), (cudaStream_t)stream));
+    return nf_keys_impl(ctx, pos_xyz, N, K, box, keys, (cudaStream_t)stream);
+}
+
 static size_t host_path_bytes(int64_t N, int K)
 {
     const size_t n = (size_t)(N > 0 ? N : 1), ncell = (size_t)K * K * K;
-    size_t b = nf_align_up(n * 12, 256) * 2 + nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
+    size_t b = nf_align_up(n * 12, 256) * 2 + nf_align_up(n * 16, 256) + 2 * nf_align_up(n * 4, 256) +
                nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256);
     return b + nf_bin_scratch_bytes(N, K, false) + forces_scratch_full(N, K) + 4096;
 }
@@ -223,10 +251,18 @@ int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, 
                    float box, float Gm, int softening, float *acc_host, void *stream)
 {
     if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, (softening & NF_MASS_W) == 0, "nf_forces_host takes no masses (NF_MASS_W): use nf_forces_host_m");
+    return nf_forces_host_m(ctx, pos_host, nullptr, N, K, R, eps, box, Gm, softening, acc_host, stream);
+}
+
+int nf_forces_host_m(nf_ctx *ctx, const float *pos_host, const float *mass_host, int64_t N, int K, int R, float eps,
+                     float box, float Gm, int softening, float *acc_host, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
     NF_TRY(check_common(ctx, N, K, box));
     NF_TRY(check_force_args(ctx, K, R, eps, Gm, softening));
     NF_ARG(ctx, N == 0 || (pos_host && acc_host), "nf_forces_host: null particle array with N > 0");
-    NF_ARG(ctx, (softening & NF_MASS_W) == 0, "nf_forces_host takes no masses: NF_MASS_W is not accepted");
+    NF_ARG(ctx, ((softening & NF_MASS_W) != 0) == (mass_host != nullptr) || N == 0, "nf_forces_host_m: NF_MASS_W must be set exactly when mass_host is given");
     NF_CUDA(ctx, cudaSetDevice(ctx->device));
     if (N == 0) return NF_OK;
     NF_TRY(nf_scratch_reserve(ctx, host_path_bytes(N, K)));
@@ -236,19 +272,21 @@ int nf_forces_host(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, 
     float *acc = nf_scratch_take<float>(ctx, n * 3);
     float *sorted = nf_scratch_take<float>(ctx, n * 4);
     uint32_t *perm = nf_scratch_take<uint32_t>(ctx, n);
+    float *mass = mass_host ? nf_scratch_take<float>(ctx, n) : nullptr;
     uint32_t *count = nf_scratch_take<uint32_t>(ctx, ncell);
     uint64_t *off = nf_scratch_take<uint64_t>(ctx, ncell + 1);
     nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
     float4 *enc = nf_scratch_take<float4>(ctx, n);
     float4 *enc_h = nf_scratch_take<float4>(ctx, n);
-    if (!raw || !acc || !sorted || !perm || !count || !off || !d_planes || !enc || !enc_h) {
+    if (!raw || !acc || !sorted || !perm || !count || !off || !d_planes || !enc || !enc_h || (mass_host && !mass)) {
         NF_SET_ERR(ctx, "nf_forces_host: internal scratch arena too small");
         return NF_ERR_NOMEM;
     }
     cudaStream_t st = (cudaStream_t)stream;
     NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, sizeof(unsigned long long), st));
     NF_CUDA(ctx, cudaMemcpyAsync(raw, pos_host, n * 12, cudaMemcpyHostToDevice, st));
-    NF_TRY(nf_bin_impl(ctx, raw, nullptr, N, K, box, -1, sorted, perm, count, off, st));
+    if (mass) NF_CUDA(ctx, cudaMemcpyAsync(mass, mass_host, n * 4, cudaMemcpyHostToDevice, st));
+    NF_TRY(nf_bin_impl(ctx, raw, mass, N, K, box, -1, sorted, perm, count, off, st));
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;

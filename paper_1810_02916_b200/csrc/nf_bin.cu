@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pos, int
             key = ((uint32_t)cx * (uint32_t)K + (uint32_t)cy) * (uint32_t)K + (uint32_t)cz;
         }
         keys[i] = key;
-        atomicAdd(&cell_count[key], 1u);
+        if (cell_count) atomicAdd(&cell_count[key], 1u);
     }
     unsigned m = __ballot_sync(0xffffffffu, bad);
     if (m && (threadIdx.x & 31) == 0) atomicAdd(n_bad, (unsigned long long)__popc(m));
@@ -239,6 +239,16 @@ size_t nf_bin_scratch_bytes(int64_t N, int K, bool plane)
     b += nf_align_up(nf_scan_temp_elems((size_t)K * ntiles) * sizeof(uint32_t), 256);
     b += nf_align_up(nf_scan_temp_elems(ncell) * sizeof(uint64_t), 256);
     return b + 4096;
+}
+
+// a1 alone: keys (cx*K+cy)*K+cz of N positions, no histogram; out-of-range particles counted in counters[0]
+int nf_keys_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, uint32_t *keys, cudaStream_t st)
+{
+    if (N <= 0) return NF_OK;
+    const float invw = (float)K / box;
+    k_keys<<<(unsigned)(((size_t)N + 255) / 256), 256, 0, st>>>(pos, N, K, invw, box, -1, keys, nullptr, ctx->counters);
+    NF_LAUNCHED(ctx);
+    return NF_OK;
 }
 
 int nf_bin_impl(nf_ctx *ctx, const float *pos, const float *mass, int64_t N, int K, float box, int plane_cx,

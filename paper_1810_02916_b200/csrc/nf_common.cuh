@@ -94,6 +94,8 @@ int nf_bin_impl(nf_ctx *ctx, const float *pos, const float *mass /* nullable */,
                 float *pos_sorted, uint32_t *perm, uint32_t *cell_count, uint64_t *cell_offset,
                 cudaStream_t st);
 
+int nf_keys_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, uint32_t *keys, cudaStream_t st);
+
 // forces (nf_forces.cu).  A "plane table" describes the x-planes available as sources and
 // sinks: plane p (0 <= p < n_planes) has its own cell-contiguous arrays.
 struct nf_plane_view {

@@ -294,8 +294,9 @@ __global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restri
 // a pair inside eps the tile is redone with the min form of Eq. 2 (and the rest of that column
 // uses the min form directly).  Exact, because the two laws agree for r >= eps.  Columns two or
 // more cells away in x or y are at least a cell width from the sinks: no pair inside eps, nothing tracked.
-// float32 partial sums per tile, double outer sum over tiles and phases in a fixed order:
-// deterministic, no floating-point atomics.
+// float32 partial sums per tile (formed from zero), a running float32 sum over the task's tiles, and
+// a double sum over the phases that share a sink, all in a fixed order: deterministic, no
+// floating-point atomics.
 // ------------------------------------------------------------------------------------------
 constexpr int WARPS = 4;                    // warps per block (independent workers)
 constexpr int TILE_CAP = 512;               // float4 slots per tile buffer (8 KiB)
@@ -468,7 +469,6 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
         };
         auto issue = [&](const TileDesc &d, int b) {
             if (d.n && lane == 0) {
-                fence_proxy_async();          // earlier generic accesses to the buffer (sentinels, reduction scratch) come first
                 const uint32_t bar = b ? bar1 : bar0;
                 mbar_expect_tx(bar, d.n * 16u);
                 bulk_g2s(smem_u32(&S.buf[b][0]), S.enc[(d.meta >> 16) & 0xff] + d.start, d.n * 16u, bar);
@@ -537,7 +537,10 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
                 gy[h] = add2(gy[h], ay[h]);
                 gz[h] = add2(gz[h], az[h]);
             }
-            __syncwarp();                                  // every lane is done with buf
+            // every lane is done with buf; each lane orders its own generic-proxy accesses to it (the
+            // sentinel stores, the sweep's loads) before the bulk copy that refills it (async proxy)
+            fence_proxy_async();
+            __syncwarp();
             const TileDesc d2 = next_tile();
             issue(d2, b);
             d0 = d1;
@@ -583,6 +586,7 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             for (int d = 16; d > 0; d >>= 1) a2max = fmaxf(a2max, __shfl_xor_sync(0xffffffffu, a2max, d));
             if (lane == 0) atomicMax(reinterpret_cast<unsigned int *>(sp.amax) + task.cyz, __float_as_uint(sqrtf(a2max)));
         }
+        fence_proxy_async();      // the reduction scratch in buf[0] (generic proxy) before the next task's bulk copies
         __syncwarp();
     }
 }

@@ -78,13 +78,13 @@ static bool is_pinned(const void *p)
     cudaPointerAttributes at;
     cudaError_t e = cudaPointerGetAttributes(&at, p);
     if (e != cudaSuccess) { cudaGetLastError(); return false; }
-    return at.type == cudaMemoryTypeHost || at.type == cudaMemoryTypeManaged;
+    return at.type == cudaMemoryTypeHost;      // page-locked host memory; managed memory migrates and is refused
 }
 
-static int stream_impl(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,
-                       int P, int K, int R, float eps, float box, int plane0, float Gm,
-                       int softening, float *const *plane_acc_host, const StepArgs *step, nf_stream_stats *stats,
-                       void *stream)
+static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_pos_host, const int64_t *plane_n,
+                      int P, int K, int R, float eps, float box, int plane0, float Gm,
+                      int softening, float *const *plane_acc_host, const StepArgs *step, nf_stream_stats *stats,
+                      void *stream)
 {
     if (!ctx) return NF_ERR_ARG;
     NF_ARG(ctx, plane_pos_host && plane_n && (plane_acc_host || step), "nf_stream_slabs: null pointer table");
@@ -92,7 +92,7 @@ static int stream_impl(nf_ctx *ctx, const float *const *plane_pos_host, const in
     NF_ARG(ctx, K >= 1 && K <= NF_MAX_K, "K = %d out of range [1, %d]", K, NF_MAX_K);
     NF_ARG(ctx, R >= 0 && R <= NF_MAX_R, "R = %d out of range [0, %d]", R, NF_MAX_R);
     NF_ARG(ctx, K >= 2 * R + 1, "K = %d < 2R+1", K);
-    NF_ARG(ctx, P + 2 * R <= K, "P + 2R = %d planes exceed K = %d", P + 2 * R, K);
+    NF_ARG(ctx, P <= K, "P = %d sink planes exceed K = %d", P, K);
     NF_ARG(ctx, eps > 0.0f && eps < 3.0e38f, "eps must be positive and finite");
     NF_ARG(ctx, box > 0.0f && box < 3.0e38f, "box must be positive and finite");
     NF_ARG(ctx, softening == NF_SOFT_SPLINE || softening == NF_SOFT_PLUMMER, "unknown softening %d (the slab stream carries no masses)", softening);
@@ -116,13 +116,7 @@ static int stream_impl(nf_ctx *ctx, const float *const *plane_pos_host, const in
     // host pointers must be pinned (page-locked): "Pinning memory"
     for (int q = 0; q < NP; q++) {
         if (plane_n[q] == 0) continue;
-        cudaPointerAttributes at;
-        cudaError_t e = cudaPointerGetAttributes(&at, plane_pos_host[q]);
-        if (e != cudaSuccess || (at.type != cudaMemoryTypeHost && at.type != cudaMemoryTypeManaged)) {
-            cudaGetLastError();
-            NF_SET_ERR(ctx, "plane_pos_host[%d] is not pinned host memory", q);
-            return NF_ERR_ARG;
-        }
+        NF_ARG(ctx, is_pinned(plane_pos_host[q]), "plane_pos_host[%d] is not pinned host memory", q);
     }
 
     cudaStream_t st = (cudaStream_t)stream;
@@ -191,7 +185,6 @@ static int stream_impl(nf_ctx *ctx, const float *const *plane_pos_host, const in
     NF_CUDA(ctx, cudaMemcpyAsync(S->d_views, S->h_views, sizeof(nf_plane_view) * NP, cudaMemcpyHostToDevice, st));
     NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st));
 
-    EventPool pool;
     std::vector<cudaEvent_t> h2d0(NP), h2d1(NP), bin0(NP), bin1(NP), frc0(P), frc1(P), d2h0(P), d2h1(P);
     for (int q = 0; q < NP; q++) { h2d0[q] = pool.get(true); h2d1[q] = pool.get(true); bin0[q] = pool.get(true); bin1[q] = pool.get(true); }
     for (int p = 0; p < P; p++) { frc0[p] = pool.get(true); frc1[p] = pool.get(true); d2h0[p] = pool.get(true); d2h1[p] = pool.get(true); }
@@ -290,7 +283,34 @@ static int stream_impl(nf_ctx *ctx, const float *const *plane_pos_host, const in
         double hidden = copy_s > 0 ? 1.0 - (stats->wall_seconds - stats->kernel_seconds) / copy_s : 0.0;
         stats->overlap_fraction = hidden < 0 ? 0.0 : (hidden > 1 ? 1.0 : hidden);
     }
+    if (ctx->h_counters[0]) {
+        NF_SET_ERR(ctx, "%lld particle(s) outside [0, box) or filed under the wrong plane were clamped into edge cells",
+                   (long long)ctx->h_counters[0]);
+        return NF_ERR_RANGE;
+    }
     return NF_OK;
+}
+
+// Every path out of the pass -- also an error in the middle of it -- first waits for the three
+// streams: copies already queued still read and write the caller's pinned buffers, and the events of
+// the pool must not be destroyed while work that records or waits on them is pending (include/nf.h:
+// "the library never retains a caller buffer past the call").
+static int stream_impl(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,
+                       int P, int K, int R, float eps, float box, int plane0, float Gm,
+                       int softening, float *const *plane_acc_host, const StepArgs *step, nf_stream_stats *stats,
+                       void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    EventPool pool;
+    const int rc = stream_run(ctx, pool, plane_pos_host, plane_n, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, step,
+                              stats, stream);
+    if (rc != NF_OK && rc != NF_ERR_ARG) {
+        cudaStreamSynchronize((cudaStream_t)stream);
+        if (ctx->s_h2d) cudaStreamSynchronize(ctx->s_h2d);
+        if (ctx->s_d2h) cudaStreamSynchronize(ctx->s_d2h);
+        if (rc != NF_ERR_RANGE) cudaGetLastError();
+    }
+    return rc;
 }
 
 extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,

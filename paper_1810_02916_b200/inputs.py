@@ -17,7 +17,7 @@ from __future__ import annotations
 
 import dataclasses
 import math
-from typing import List, Optional
+from typing import Callable, List, Optional
 
 import torch
 
@@ -172,12 +172,20 @@ def make_positions(cfg: Config, device="cpu", out: Optional[torch.Tensor] = None
 
 
 def make_slab_planes(cfg: Config, device="cpu", n_planes_total: Optional[int] = None,
-                     density_scale: float = 1.0) -> List[torch.Tensor]:
+                     density_scale: float = 1.0, plane_of: Optional[Callable[[torch.Tensor], torch.Tensor]] = None
+                     ) -> List[torch.Tensor]:
     """C5: the particles of P + 2R consecutive x-planes (plane0 .. plane0+P+2R-1; the outer R on
     each side are ghosts) of a density_n^3-particle periodic box with the C4-style halo
     catalogue.  Returns one float32 [n_p, 3] tensor per plane (global coordinates, arbitrary
-    in-plane order).  density_scale < 1 thins the box for small tests."""
+    in-plane order).  density_scale < 1 thins the box for small tests.
+
+    ``plane_of(x)`` maps float32 [n, 3] positions to the int64 x-plane (x-cell index) each particle
+    is filed under.  Which plane a particle on or next to a plane face belongs to is decided by the
+    float32 cell-assignment formula of the method, which this module must not restate: the caller
+    passes the method's own answer (tests: the oracle's keys // K^2; bench.py: the library's nf_keys
+    // K^2).  Particles filed outside the chunk's planes are left out; nothing else is dropped."""
     assert cfg.kind == "slab"
+    assert plane_of is not None, "make_slab_planes needs plane_of (the method's cell assignment); see the docstring"
     device = torch.device(device)
     P2 = n_planes_total if n_planes_total is not None else cfg.planes + 2 * cfg.R
     w = cfg.box / cfg.K
@@ -207,19 +215,17 @@ def make_slab_planes(cfg: Config, device="cpu", n_planes_total: Optional[int] = 
         hid = hid_all[lo:lo + CHUNK]
         gg = _gen(cfg.seed, 2000 + c, device)
         off = _plummer_offsets(hid.numel(), scales[hid], cfg.r_trunc, gg, device)
-        parts.append((centres[hid] + off).float())
+        xh = (centres[hid] + off).float()
+        # a coarse geometric pre-cut one cell wider than the chunk (halo members far outside it are of no
+        # use); the filing below decides which plane, if any, every survivor belongs to
+        xh = xh[(xh[:, 0] >= x0 - w) & (xh[:, 0] < x1 + w)]
+        parts.append(xh)
     x = torch.cat(parts, dim=0) if parts else torch.empty(0, 3, dtype=torch.float32, device=device)
     x[:, 1:] = _wrap_(x[:, 1:].contiguous(), cfg.box)
-    # plane index: assigned here only to split the input into per-plane arrays; clamp guards
-    # the float32 rounding of x at plane faces so that every particle lies inside its plane.
-    # Particles within 1e-4 of a cell width of a plane face are dropped (2 in 10^4): which plane
-    # such a particle belongs to depends on the float32 rounding of the cell-assignment formula,
-    # and the per-plane interface wants every particle filed under the plane it will be binned to.
-    t = x[:, 0].double() / w
-    frac = t - torch.floor(t)
-    keep = (x[:, 0] >= x0) & (x[:, 0] < x1) & (frac > 1e-4) & (frac < 1.0 - 1e-4)
-    x = x[keep]
-    p = torch.clamp(torch.floor(x[:, 0].double() / w).long() - cfg.plane0, 0, P2 - 1)
+    x = x[(x[:, 0] >= 0) & (x[:, 0] < cfg.box)]
+    p = plane_of(x).to(device=device, dtype=torch.int64) - cfg.plane0
+    keep = (p >= 0) & (p < P2)
+    x, p = x[keep], p[keep]
     # shuffle so in-plane order carries no structure, then split
     perm = torch.randperm(x.shape[0], generator=g, device=device)
     x, p = x[perm], p[perm]

@@ -25,7 +25,8 @@ _SOFT = {"spline": SOFT_SPLINE, "plummer": SOFT_PLUMMER}
 EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve", "nf_bin",
            "nf_out_of_range", "nf_forces", "nf_interactions", "nf_spline_equivalent_eps",
            "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host",
-           "nf_bin_m", "nf_forces_ex", "nf_kick_drift", "nf_cell_vrms", "nf_stream_step_slabs"]
+           "nf_bin_m", "nf_forces_ex", "nf_kick_drift", "nf_cell_vrms", "nf_stream_step_slabs",
+           "nf_keys", "nf_forces_chunk", "nf_forces_host_m"]
 
 
 class NFError(RuntimeError):
@@ -100,6 +101,12 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.nf_forces_host.argtypes = [vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp]
     lib.nf_reserve_host.restype = i32
     lib.nf_reserve_host.argtypes = [vp, i64, i32]
+    lib.nf_forces_host_m.restype = i32
+    lib.nf_forces_host_m.argtypes = [vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp]
+    lib.nf_keys.restype = i32
+    lib.nf_keys.argtypes = [vp, vp, i64, i32, f32, vp, vp]
+    lib.nf_forces_chunk.restype = i32
+    lib.nf_forces_chunk.argtypes = [vp, vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, i32, i32, vp, vp, vp]
     lib.nf_launch_count.restype = i32
     lib.nf_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     _lib = lib
@@ -190,6 +197,26 @@ class Context:
         self._check(self.lib.nf_out_of_range(self._h, ctypes.byref(n), self._stream(stream)), allow=(NF_ERR_RANGE,))
         return int(n.value)
 
+    def keys(self, pos: torch.Tensor, K: int, box: float, stream=None) -> torch.Tensor:
+        """nf_keys: cell key (cx*K+cy)*K+cz per particle as an int32 view of uint32 [N]; the x-plane is key // K^2."""
+        assert pos.is_cuda and pos.dtype == torch.float32 and pos.dim() == 2 and pos.shape[1] == 3 and pos.is_contiguous()
+        out = torch.empty(pos.shape[0], dtype=torch.int32, device=pos.device)
+        self._check(self.lib.nf_keys(self._h, _ptr(pos), pos.shape[0], int(K), float(box), _ptr(out), self._stream(stream)))
+        return out
+
+    def forces_chunk(self, b: Binned, R: int, eps: float, Gm: float, x_lo: int, x_hi: int, softening: str = "spline",
+                     original_order: bool = True, out: Optional[torch.Tensor] = None, stream=None,
+                     use_mass: bool = False, cell_amax: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """nf_forces_chunk: accelerations of the particles in x-planes [x_lo, x_hi) only (rows of the other
+        particles -- ghosts -- are left untouched); every particle of ``b`` acts as a source."""
+        acc = out if out is not None else torch.zeros(b.N, 3, dtype=torch.float32, device=b.pos_sorted.device)
+        assert acc.is_cuda and acc.dtype == torch.float32 and acc.shape == (b.N, 3) and acc.is_contiguous()
+        self._check(self.lib.nf_forces_chunk(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset),
+                                             _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
+                                             float(b.box), float(Gm), _SOFT[softening] | (NF_MASS_W if use_mass else 0),
+                                             int(x_lo), int(x_hi), _ptr(acc), _ptr(cell_amax), self._stream(stream)))
+        return acc
+
     def forces(self, b: Binned, R: int, eps: float, Gm: float, softening: str = "spline",
                original_order: bool = True, out: Optional[torch.Tensor] = None, stream=None,
                use_mass: bool = False, cell_amax: Optional[torch.Tensor] = None) -> torch.Tensor:
@@ -234,18 +261,26 @@ class Context:
         self._check(self.lib.nf_reserve_host(self._h, int(maxN), int(K)))
 
     def forces_host(self, pos_host: torch.Tensor, K: int, R: int, eps: float, box: float, Gm: float,
-                    softening: str = "spline", out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
-        """nf_forces_host: the whole path from a HOST float32 [N, 3] tensor (pinned recommended) to
-        a host float32 [N, 3] acceleration tensor; H2D, binning, forces and D2H all inside the call."""
+                    softening: str = "spline", out: Optional[torch.Tensor] = None, stream=None,
+                    mass_host: Optional[torch.Tensor] = None, strict: bool = False) -> torch.Tensor:
+        """nf_forces_host (nf_forces_host_m when ``mass_host`` float32 [N] is given): the whole path from a
+        HOST float32 [N, 3] tensor (pinned recommended) to a host float32 [N, 3] acceleration tensor; H2D,
+        binning, forces and D2H all inside the call.  strict: raise on NF_ERR_RANGE instead of returning."""
         assert (not pos_host.is_cuda) and pos_host.dtype == torch.float32 and pos_host.dim() == 2 \
             and pos_host.shape[1] == 3 and pos_host.is_contiguous()
         N = pos_host.shape[0]
         if out is None:
             out = torch.empty(N, 3, dtype=torch.float32).pin_memory()
         assert (not out.is_cuda) and out.dtype == torch.float32 and out.shape == (N, 3) and out.is_contiguous()
+        allow = () if strict else (NF_ERR_RANGE,)
+        if mass_host is not None:
+            assert (not mass_host.is_cuda) and mass_host.dtype == torch.float32 and mass_host.shape == (N,) and mass_host.is_contiguous()
+            self._check(self.lib.nf_forces_host_m(self._h, _ptr(pos_host), _ptr(mass_host), N, int(K), int(R), float(eps),
+                                                  float(box), float(Gm), _SOFT[softening] | NF_MASS_W, _ptr(out),
+                                                  self._stream(stream)), allow=allow)
+            return out
         self._check(self.lib.nf_forces_host(self._h, _ptr(pos_host), N, int(K), int(R), float(eps), float(box),
-                                            float(Gm), _SOFT[softening], _ptr(out), self._stream(stream)),
-                    allow=(NF_ERR_RANGE,))
+                                            float(Gm), _SOFT[softening], _ptr(out), self._stream(stream)), allow=allow)
         return out
 
     def interactions(self, b: Binned, R: int, stream=None) -> int:
@@ -267,9 +302,11 @@ class Context:
 
     def stream_slabs(self, planes: Sequence[torch.Tensor], P: int, K: int, R: int, eps: float, box: float,
                      plane0: int, Gm: float, softening: str = "spline",
-                     out: Optional[List[torch.Tensor]] = None, stream=None):
+                     out: Optional[List[torch.Tensor]] = None, stream=None, strict: bool = True):
         """nf_stream_slabs: planes = P + 2R pinned host float32 [n_q, 3] tensors; returns
-        (list of P pinned host float32 [n, 3] acceleration tensors, stats dict)."""
+        (list of P pinned host float32 [n, 3] acceleration tensors, stats dict).  NF_ERR_RANGE
+        (mis-filed or out-of-range particles, counted in stats["out_of_range"]) raises unless
+        strict is False."""
         NP = P + 2 * R
         assert len(planes) == NP
         for t in planes:
@@ -283,7 +320,7 @@ class Context:
         stats = StreamStats()
         self._check(self.lib.nf_stream_slabs(self._h, pos_ptrs, ns, int(P), int(K), int(R), float(eps), float(box),
                                              int(plane0), float(Gm), _SOFT[softening], acc_ptrs, ctypes.byref(stats),
-                                             self._stream(stream)))
+                                             self._stream(stream)), allow=() if strict else (NF_ERR_RANGE,))
         return out, stats.as_dict()
 
     def stream_step_slabs(self, planes, vels, P, K, R, eps, box, plane0, Gm, kick, drift, softening="spline", want_acc=False, stream=None):

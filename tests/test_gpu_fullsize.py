@@ -6,9 +6,10 @@ can compute one by one, plus properties that hold at any size (SURVEY.md Sec. 8(
     a seeded sample of sinks (random particles + every particle of the fullest cells) against the
     oracle run on the full input.
   - C4 (1024^3 clustered, the config the roofline target is quoted on): the oracle cannot hold
-    2^30 particles, so it gets the particles of two padded blocks of cells (one interior, one
-    wrapping around the box corner) cut out by a plain coordinate filter; every sink of the inner
-    blocks then has all of its sources.  Binning is compared bit for bit on those cells.
+    2^30 particles, so it gets the particles of the (2R+1)^3 neighbourhoods of a seeded sample of
+    cells (>= 4096 random cells + the 256 fullest + a 5^3 block wrapping around the box corner,
+    >= 10^6 sinks); every sampled sink then has all of its sources.  Binning is compared bit for bit
+    on a stride of those cells.
   - everywhere: no NaN/Inf, zero net force, interaction count from the cell counts.
 """
 import numpy as np
@@ -16,6 +17,7 @@ import pytest
 import torch
 
 import oracle
+from helpers import frac_error, oracle_plane_of
 from paper_1810_02916_b200 import inputs
 
 pytestmark = pytest.mark.gpu
@@ -80,11 +82,31 @@ def test_full_box_sampled_sinks(ctx, which):
     assert err.max() <= MAX_TOL, f"max error {err.max():.3e}"
 
 
-def test_c4_full_size_blocks(ctx):
+FRAC_MEDIAN_TOL = 2e-6      # the paper's own float32-vs-double median is 7.5e-7; measured here: see DESIGN.md Sec. 5
+
+
+def torch_cell_keys(pos: torch.Tensor, K: int, box: float) -> torch.Tensor:
+    """Cell key per particle with plain torch ops, in chunks: a SAMPLER for this test (which cells are the
+    fullest, which particles lie near the sampled cells), not an authority -- sink membership and every
+    expected value come from the oracle."""
+    invw = float(np.float32(K) / np.float32(box))
+    out = torch.empty(pos.shape[0], dtype=torch.int64, device=pos.device)
+    for lo in range(0, pos.shape[0], 1 << 26):
+        c = torch.clamp(torch.floor(pos[lo:lo + (1 << 26)] * invw).long(), 0, K - 1)
+        out[lo:lo + (1 << 26)] = (c[:, 0] * K + c[:, 1]) * K + c[:, 2]
+    return out
+
+
+def test_c4_full_size_sampled_cells(ctx):
+    """C4 at full size (the config the 60 % target is quoted on), in bench.py's launch configuration,
+    on the sample SURVEY.md Sec. 8(d) asks for: >= 4096 random cells + the 256 fullest cells + every cell
+    of a 5^3 block around the box corner (wrap paths), >= 10^6 sinks in all, each with ALL its sources
+    (the particles of the sampled cells' (2R+1)^3 neighbourhoods go to the oracle).  Bars: the north_star
+    metric (rms over the sampled sinks) and the paper's fractional error |da|/|a|."""
     torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
-    if free < 90 * (1 << 30):
-        pytest.skip("needs ~90 GB of free device memory")
+    if free < 110 * (1 << 30):
+        pytest.skip("needs ~110 GB of free device memory")
     cfg = inputs.config(4)
     K, R, m = cfg.K, cfg.R, 5
     pos = inputs.make_positions(cfg, device="cuda")
@@ -104,36 +126,86 @@ def test_c4_full_size_blocks(ctx):
             for dz in range(-R, R + 1):
                 nb += torch.roll(c3, shifts=(dx, dy, dz), dims=(0, 1, 2))
     assert ctx.interactions(b, R) == int((c3 * nb).sum())
-    w = cfg.box / K
+    del nb
+    # ---- the sample ----
+    keys_t = torch_cell_keys(pos, K, cfg.box)
+    cnt_t = torch.bincount(keys_t, minlength=K ** 3)
+    assert torch.equal(cnt_t, cnt)                                   # 2^30 cell assignments agree with plain float32 torch
+    g = torch.Generator(device="cpu")
+    g.manual_seed(cfg.seed)
+    order = torch.randperm(K ** 3, generator=g).cuda()
+    chosen = torch.zeros(K ** 3, dtype=torch.bool, device="cuda")
+    chosen[torch.topk(cnt_t, 256).indices] = True                   # the 256 fullest cells
+    cc = torch.tensor([(K - 2 + i) % K for i in range(m)], device="cuda")
+    corner = ((cc[:, None, None] * K + cc[None, :, None]) * K + cc[None, None, :]).flatten()
+    chosen[corner] = True                                           # 5^3 block wrapping around the box corner
+    n_rand = 4096
+    while True:                                                      # >= 4096 random cells, more until >= 10^6 sinks
+        ch = chosen.clone()
+        ch[order[:n_rand]] = True
+        if int(cnt_t[ch].sum()) >= 1_050_000:
+            break
+        n_rand += 1024
+    chosen = ch
+    # every particle of the chosen cells' neighbourhoods (Chebyshev distance <= R, periodic)
+    need = torch.zeros(K, K, K, dtype=torch.bool, device="cuda")
+    ch3 = chosen.view(K, K, K)
+    for dx in range(-R, R + 1):
+        for dy in range(-R, R + 1):
+            for dz in range(-R, R + 1):
+                need |= torch.roll(ch3, shifts=(dx, dy, dz), dims=(0, 1, 2))
+    idx = torch.nonzero(need.view(-1)[keys_t]).flatten()            # increasing original indices
+    del keys_t, need
+    sub = pos[idx].cpu().numpy()
+    keys, nbad = oracle.keys(sub, K, cfg.box)
+    assert nbad == 0
+    sink_local = np.nonzero(chosen.cpu().numpy()[keys])[0]
+    assert sink_local.size >= 1_000_000 and n_rand >= 4096
+    # binning of a stride of the sampled cells, bit for bit (the sub-sample keeps the input order, so
+    # the stable order inside a cell is the same)
+    ref = oracle.bin_particles(sub, K, cfg.box)
     off = b.cell_offset.cpu().numpy()
-    for c0 in [(3, 5, 7), (K - 2, K - 3, K - 1)]:          # interior block; block wrapping around the box corner
-        lo = [(c - R - 1) * w for c in c0]
-        hi = [(c + m + R + 1) * w for c in c0]
-        idx = inputs.select_box(pos, lo, hi, cfg.box)       # increasing original indices
-        sub = pos[idx].cpu().numpy()
-        idx_np = idx.cpu().numpy()
-        ref = oracle.bin_particles(sub, K, cfg.box)
-        keys, nbad = oracle.keys(sub, K, cfg.box)
-        assert nbad == 0
-        cx, cy, cz = keys // (K * K), (keys // K) % K, keys % K
-        inner = np.ones(len(keys), bool)
-        for c, l0 in ((cx, c0[0]), (cy, c0[1]), (cz, c0[2])):
-            inner &= ((c.astype(np.int64) - l0) % K) < m
-        # binning of the inner cells, bit for bit (the sub-sample keeps the input order, so the
-        # stable order inside a cell is the same)
-        for key in np.unique(keys[inner])[:: 7]:
-            g0, g1 = int(off[key]), int(off[key + 1])
-            r0, r1 = int(ref["cell_offset"][key]), int(ref["cell_offset"][key + 1])
-            assert g1 - g0 == r1 - r0
-            assert np.array_equal(u32(b.perm[g0:g1]), idx_np[ref["perm"][r0:r1]].astype(np.uint32))
-            assert np.array_equal(b.pos_sorted[g0:g1].cpu().numpy().view(np.uint32), ref["pos_sorted"][r0:r1].view(np.uint32))
-        sink_local = np.nonzero(inner)[0]
-        a_ref = oracle.forces(sub, K, R, cfg.eps, cfg.box, cfg.Gm, sink_idx=sink_local)
-        got = acc[idx[torch.from_numpy(sink_local).cuda()]].cpu().numpy()
-        err = oracle.parity_error(got, a_ref)
-        print(f"[parity] {cfg.name} block {c0}: {sink_local.size} sinks, median {np.median(err):.2e}, 99.9 % {np.quantile(err, 0.999):.2e}, max {err.max():.2e}")
-        assert np.median(err) <= MEDIAN_TOL, f"median error {np.median(err):.3e} at block {c0}"
-        assert err.max() <= MAX_TOL, f"max error {err.max():.3e} at block {c0}"
+    idx_np = idx.cpu().numpy()
+    for key in np.unique(keys[sink_local])[:: 23]:
+        g0, g1 = int(off[key]), int(off[key + 1])
+        r0, r1 = int(ref["cell_offset"][key]), int(ref["cell_offset"][key + 1])
+        assert g1 - g0 == r1 - r0
+        assert np.array_equal(u32(b.perm[g0:g1]), idx_np[ref["perm"][r0:r1]].astype(np.uint32))
+        assert np.array_equal(b.pos_sorted[g0:g1].cpu().numpy().view(np.uint32), ref["pos_sorted"][r0:r1].view(np.uint32))
+    a_ref = oracle.forces(sub, K, R, cfg.eps, cfg.box, cfg.Gm, sink_idx=sink_local)
+    got = acc[idx[torch.from_numpy(sink_local).cuda()]].cpu().numpy()
+    err = oracle.parity_error(got, a_ref)
+    fe = frac_error(got, a_ref)
+    print(f"[parity] {cfg.name}: {sink_local.size} sinks in {int(chosen.sum())} cells ({n_rand} random + 256 fullest + corner block), "
+          f"{sub.shape[0]} particles to the oracle; metric median {np.median(err):.2e}, 99.9 % {np.quantile(err, 0.999):.2e}, "
+          f"max {err.max():.2e}; fractional error median {np.median(fe):.2e}, share > 1e-4: {np.mean(fe > 1e-4):.2e}")
+    assert np.median(err) <= MEDIAN_TOL, f"median error {np.median(err):.3e}"
+    assert err.max() <= MAX_TOL, f"max error {err.max():.3e}"
+    assert np.median(fe) <= FRAC_MEDIAN_TOL, f"median fractional error {np.median(fe):.3e}"
+
+
+def test_one_dense_cell(ctx):
+    """The other end of the range: one cell of ~4x10^5 particles (sigma = 0.08 w, eps = 0.01 w) in an
+    otherwise almost empty K = 5 box -- the shape of the paper's late-time "largest cell has over 200,000
+    particles": thousands of full tasks of one cell, every tile holding pairs inside eps.
+    Sampled sinks against the oracle, interaction count, determinism."""
+    rng = np.random.default_rng(5)
+    K, R, box, n = 5, 2, 1.0, 400_000
+    w = box / K
+    pos = (np.array([2.5, 2.5, 2.5]) * w + 0.08 * w * rng.standard_normal((n, 3))).clip(2.01 * w, 2.99 * w)
+    pos[:1000] = rng.random((1000, 3)) * box
+    pos = pos.astype(np.float32)
+    eps = 0.01 * w
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box)
+    assert int(b.cell_count.max()) >= 200_000
+    acc = ctx.forces(b, R, eps, 1.0 / n)
+    assert torch.equal(acc, ctx.forces(b, R, eps, 1.0 / n))
+    assert ctx.interactions(b, R) == oracle.interactions(u32(b.cell_count), K, R)
+    sink = np.sort(rng.choice(n, 4000, replace=False))
+    ref = oracle.forces(pos, K, R, eps, box, 1.0 / n, sink_idx=sink)
+    err = oracle.parity_error(acc.cpu().numpy()[sink], ref)
+    print(f"[parity] one dense cell ({int(b.cell_count.max())} particles): median {np.median(err):.2e}, max {err.max():.2e}")
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
 
 
 def test_c5_stream_full_size(ctx):
@@ -148,7 +220,7 @@ def test_c5_stream_full_size(ctx):
         pytest.skip("needs ~24 GB of host memory (8 GB of it pinned)")
     cfg = inputs.config(5)
     K, R, P, m = cfg.K, cfg.R, cfg.planes, 4
-    planes_dev = inputs.make_slab_planes(cfg, device="cuda")
+    planes_dev = inputs.make_slab_planes(cfg, device="cuda", plane_of=oracle_plane_of(cfg.K, cfg.box))
     planes = []
     for t in planes_dev:
         h = torch.empty(t.shape, dtype=torch.float32).pin_memory()

@@ -10,6 +10,7 @@ import pytest
 import torch
 
 import oracle
+from helpers import oracle_plane_of
 from paper_1810_02916_b200 import inputs
 
 pytestmark = pytest.mark.gpu
@@ -85,6 +86,9 @@ def test_bin_edge_cases(ctx):
     check_bin(ctx, rng.random((1000, 3)).astype(np.float32), 1, 1.0)           # a single cell
     top = np.nextafter(np.float32(500.0), np.float32(0))                         # 499.99997 * 0.512f rounds to 256.0f: valid, cell K-1
     check_bin(ctx, np.array([[top, top, 1.0], [500.0, 1.0, 1.0], [3.0, top, 499.0]], np.float32), 256, 500.0)
+    # a box so small that half a cell width and the offsets are float32 DENORMALS: the contract is IEEE (no flush to zero)
+    tiny = np.float32(1e-37)
+    check_bin(ctx, np.minimum((rng.random((2000, 3)) * tiny).astype(np.float32), np.nextafter(tiny, np.float32(0))), 4, float(tiny))
 
 
 def test_bin_is_deterministic(ctx):
@@ -210,7 +214,7 @@ def test_stream_slabs_small(ctx):
     cfg = inputs.dataclasses.replace(inputs.config(5), K=32, planes=6, plane0=29 - 32, n_halos=4096,
                                      r_trunc=2 * 500.0 / 32 / 2, a_lo=0.3, a_hi=2.0, eps=0.15)
     cfg = inputs.dataclasses.replace(cfg, plane0=3)
-    planes = inputs.make_slab_planes(cfg, density_scale=(32 * 4) ** 3 / 2048 ** 3)
+    planes = inputs.make_slab_planes(cfg, density_scale=(32 * 4) ** 3 / 2048 ** 3, plane_of=oracle_plane_of(cfg.K, cfg.box))
     R, P = cfg.R, cfg.planes
     pinned = [p.pin_memory() for p in planes]
     Gm = 1.0 / sum(p.shape[0] for p in planes)
@@ -304,6 +308,10 @@ def test_kick_drift_bit_exact(ctx, n):
         pos[:4, 0] = [0.0, np.nextafter(np.float32(box), np.float32(0)), 1e-30, 250.0]
         vel[:4, 0] = [-1e-12, 1e-3, -1e-20, 0.0]
         acc[:4, 0] = 0.0
+        # denormal operands and results: the float32 contract is IEEE, nothing is flushed to zero
+        pos[4:7, 0] = [1e-40, 3e-39, 0.0]
+        vel[4:7, 0] = [1e-41, -2e-39, 1e-39]
+        acc[4:7, 0] = [1e-38, 1e-39, -2e-39]
     kick, drift = 0.37, 0.21
     x_ref, v_ref = oracle.kick_drift(pos, vel, acc, kick, drift, box)
     p, v, a = (torch.from_numpy(t).cuda() for t in (pos, vel, acc))
@@ -422,7 +430,7 @@ def test_stream_step_slabs_small(ctx):
     bit against nf_stream_slabs followed by nf_kick_drift."""
     cfg = inputs.dataclasses.replace(inputs.config(5), K=32, planes=6, plane0=3, n_halos=4096,
                                      r_trunc=2 * 500.0 / 32 / 2, a_lo=0.3, a_hi=2.0, eps=0.15)
-    planes = inputs.make_slab_planes(cfg, density_scale=(32 * 4) ** 3 / 2048 ** 3)
+    planes = inputs.make_slab_planes(cfg, density_scale=(32 * 4) ** 3 / 2048 ** 3, plane_of=oracle_plane_of(cfg.K, cfg.box))
     R, P = cfg.R, cfg.planes
     rng = np.random.default_rng(4)
     vels = [torch.from_numpy((rng.standard_normal((planes[R + p].shape[0], 3)) * 3.0).astype(np.float32)) for p in range(P)]
@@ -659,3 +667,234 @@ def test_forces_dense_cells_randomised(ctx, seed):
     assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (seed, K, R, n, float(np.median(err)), float(err.max()))
     assert ctx.interactions(b, R) == oracle.interactions(u32(b.cell_count), K, R)
     assert int(u32(b.cell_count).max()) > 1000
+
+
+# ------------------------------------------------- slab stream: plane faces and error paths
+def _face_planes(rng, K, R, P, box, plane0, n_per_plane=400):
+    """P + 2R planes whose particles sit ON plane faces, one float32 ulp either side of them, and at
+    random places, filed under the plane the ORACLE's cell assignment gives (keys // K^2)."""
+    w = box / K
+    NP = P + 2 * R
+    xs = []
+    for q in range(NP + 1):
+        face = np.float32((plane0 + q) * w)
+        xs += [face, np.nextafter(face, np.float32(0)), np.nextafter(face, np.float32(2 * box))] * 12
+    x = np.empty((len(xs) + NP * n_per_plane, 3), np.float32)
+    x[:len(xs), 0] = xs
+    x[len(xs):, 0] = (plane0 + rng.random(NP * n_per_plane) * NP) * w
+    x[:, 1:] = rng.random((x.shape[0], 2)) * box
+    x[: len(xs) // 2, 1] = np.round(x[: len(xs) // 2, 1] / w) * w           # on y faces as well, incl. 0 and box
+    x = np.minimum(np.mod(x, np.float32(box)), np.nextafter(np.float32(box), np.float32(0))).astype(np.float32)
+    x = x[rng.permutation(x.shape[0])]
+    keys, nbad = oracle.keys(x, K, box)
+    assert nbad == 0
+    cx = (keys // (K * K)).astype(np.int64)
+    planes = []
+    for q in range(NP):
+        planes.append(torch.from_numpy(x[cx == (plane0 + q) % K].copy()))
+    return planes
+
+
+@pytest.mark.parametrize("K,R,P,plane0", [(16, 2, 5, 3), (12, 1, 6, 0), (9, 2, 3, 1)])
+def test_stream_slabs_particles_on_plane_faces(ctx, K, R, P, plane0):
+    """Particles on and within one ulp of plane faces: the plane a particle is filed under is the
+    oracle's cell assignment, and the library must agree with it bit for bit (out_of_range == 0) and
+    give the oracle's forces."""
+    rng = np.random.default_rng(K * 31 + R)
+    box = 500.0 if K == 16 else 3.0
+    planes = _face_planes(rng, K, R, P, box, plane0)
+    pinned = [p.pin_memory() for p in planes]
+    eps, Gm = 0.02 * box / K, 0.5
+    out, stats = ctx.stream_slabs(pinned, P, K, R, eps, box, plane0, Gm)
+    assert stats["out_of_range"] == 0
+    allpos = torch.cat(planes).numpy()
+    starts = np.cumsum([0] + [p.shape[0] for p in planes])
+    sink_idx = np.arange(starts[R], starts[R + P])
+    ref = oracle.forces(allpos, K, R, eps, box, Gm, sink_idx=sink_idx)
+    err = oracle.parity_error(torch.cat(out).numpy(), ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (np.median(err), err.max())
+
+
+def test_stream_slabs_misfiled_particles(ctx):
+    """k particles deliberately filed under the wrong plane, plus one outside the box: the pass completes,
+    reports exactly those in stats["out_of_range"], returns NF_ERR_RANGE, and every output is finite."""
+    from paper_1810_02916_b200 import nf
+    rng = np.random.default_rng(11)
+    K, R, P, plane0, box = 12, 2, 4, 2, 6.0
+    w = box / K
+    planes = []
+    for q in range(P + 2 * R):
+        x = np.empty((500, 3), np.float32)
+        x[:, 0] = (plane0 + q + rng.uniform(0.05, 0.95, 500)) * w
+        x[:, 1:] = rng.random((500, 2)) * box
+        planes.append(x)
+    k = 7
+    for j in range(k):                       # wrong plane: one cell width off, either side
+        planes[R + j % P][j, 0] += w if j % 2 else -w
+    planes[R][100, 1] = box * 1.5            # outside the box in y
+    pinned = [torch.from_numpy(p).pin_memory() for p in planes]
+    with pytest.raises(nf.NFError) as e:
+        ctx.stream_slabs(pinned, P, K, R, 0.02, box, plane0, 1.0)
+    assert e.value.status == nf.NF_ERR_RANGE
+    out, stats = ctx.stream_slabs(pinned, P, K, R, 0.02, box, plane0, 1.0, strict=False)
+    assert stats["out_of_range"] == k + 1
+    assert all(torch.isfinite(o).all() for o in out)
+    # the same planes without the planted particles are clean
+    for j in range(k):
+        planes[R + j % P][j, 0] -= w if j % 2 else -w
+    planes[R][100, 1] = 0.5 * box
+    out, stats = ctx.stream_slabs([torch.from_numpy(p).pin_memory() for p in planes], P, K, R, 0.02, box, plane0, 1.0)
+    assert stats["out_of_range"] == 0
+
+
+def test_stream_slabs_rejects_pageable_memory(ctx):
+    """The C function itself (not the binding's assert) refuses host pointers that are not page-locked."""
+    import ctypes
+    from paper_1810_02916_b200 import nf
+    K, R, P = 8, 1, 2
+    NP = P + 2 * R
+    rng = np.random.default_rng(0)
+    pageable = [np.ascontiguousarray(rng.random((50, 3)).astype(np.float32)) for _ in range(NP)]
+    pinned = [torch.from_numpy(p).pin_memory() for p in pageable]
+    acc_pinned = [torch.empty(50, 3).pin_memory() for _ in range(P)]
+    acc_pageable = [np.empty((50, 3), np.float32) for _ in range(P)]
+    ns = (ctypes.c_int64 * NP)(*[50] * NP)
+    stats = nf.StreamStats()
+
+    def call(pos_ptrs, acc_ptrs):
+        return ctx.lib.nf_stream_slabs(ctx._h, (ctypes.c_void_p * NP)(*pos_ptrs), ns, P, K, R, 0.01, 1.0, 0, 1.0, 0,
+                                       (ctypes.c_void_p * P)(*acc_ptrs), ctypes.byref(stats), None)
+    pin_pos = [t.data_ptr() for t in pinned]
+    pin_acc = [t.data_ptr() for t in acc_pinned]
+    assert call([p.ctypes.data for p in pageable], pin_acc) == nf.NF_ERR_ARG
+    assert b"not pinned" in ctx.lib.nf_last_error(ctx._h)
+    assert call(pin_pos, [a.ctypes.data for a in acc_pageable]) == nf.NF_ERR_ARG
+    assert call(pin_pos[:1] + [pageable[1].ctypes.data] + pin_pos[2:], pin_acc) == nf.NF_ERR_ARG
+    assert call(pin_pos, pin_acc) in (nf.NF_OK, nf.NF_ERR_RANGE)        # the pinned version of the same call goes through
+
+
+def test_forces_host_range_error_and_masses(ctx):
+    """nf_forces_host returns NF_ERR_RANGE (after completing) when a position lies outside [0, box);
+    nf_forces_host_m carries per-particle masses and matches the device-buffer path bit for bit."""
+    from paper_1810_02916_b200 import nf
+    rng = np.random.default_rng(21)
+    K, R, box, n = 8, 2, 2.0, 5000
+    pos = (rng.random((n, 3)) * box).astype(np.float32)
+    hp = torch.from_numpy(pos).pin_memory()
+    a_ok = ctx.forces_host(hp, K, R, 0.01, box, 1.0 / n, strict=True)
+    bad = pos.copy()
+    bad[17, 2] = box
+    bad[18, 0] = -1e-3
+    hb = torch.from_numpy(bad).pin_memory()
+    with pytest.raises(nf.NFError) as e:
+        ctx.forces_host(hb, K, R, 0.01, box, 1.0 / n, strict=True)
+    assert e.value.status == nf.NF_ERR_RANGE and "2 particle" in str(e.value)
+    a_bad = ctx.forces_host(hb, K, R, 0.01, box, 1.0 / n)
+    assert torch.isfinite(a_bad).all()
+    mass = rng.uniform(0.1, 3.0, n).astype(np.float32)
+    a_m = ctx.forces_host(hp, K, R, 0.01, box, 1.0 / n, mass_host=torch.from_numpy(mass).pin_memory())
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box, mass=torch.from_numpy(mass).cuda())
+    assert torch.equal(a_m, ctx.forces(b, R, 0.01, 1.0 / n, use_mass=True).cpu())
+    ref = oracle.forces(pos, K, R, 0.01, box, 1.0 / n, mass=mass)
+    err = oracle.parity_error(a_m.numpy(), ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
+    with pytest.raises(nf.NFError):
+        ctx._check(ctx.lib.nf_forces_host(ctx._h, hp.data_ptr(), n, K, R, 0.01, box, 1.0, nf.NF_MASS_W, a_ok.data_ptr(), None))
+
+
+# ------------------------------------------------- the float32 envelope, pinned from outside
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_forces_outside_float32_envelope(ctx, seed):
+    """include/nf.h "Accuracy envelope": a pair that straddles a cell face is formed from cell-centred
+    offsets shifted by whole cells in float32, so its separation vector is only good to dd ~ 3e-7 w and its
+    force to a relative ~ dd / r.  An unsoftened clump 1e-4 w wide planted ON a cell corner (eps = 1e-6 w)
+    is far outside the 1e-3 bar's envelope; what is pinned here is the documented bound itself: per
+    particle |a_gpu - a_ref| <= sum over its pairs of 4 dd Gm / r^3 with dd = 3e-7 w (the derivative of
+    d / r^3 has norm <= 4 / r^3), and pairs INSIDE one cell stay exact to float32 summation."""
+    rng = np.random.default_rng(300 + seed)
+    K, R, box, n = 8, 2, 1.0, 160
+    w = box / K
+    corner = np.array([3, 5, 2]) * w
+    width = 1e-4 * w
+    pos = np.mod(corner + width * rng.standard_normal((n, 3)), box).astype(np.float32)
+    eps, Gm = 1e-6 * w, 1.0 / n
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box)
+    acc = ctx.forces(b, R, eps, Gm).cpu().numpy().astype(np.float64)
+    ref = oracle.forces(pos, K, R, eps, box, Gm)
+    x = pos.astype(np.float64)
+    d = x[None, :, :] - x[:, None, :]
+    d -= np.round(d / box) * box
+    r = np.sqrt((d ** 2).sum(axis=2))
+    np.fill_diagonal(r, np.inf)
+    dd = 3e-7 * w
+    bound = (4.0 * dd * Gm / r ** 3).sum(axis=1)
+    err = np.sqrt(((acc - ref) ** 2).sum(axis=1))
+    mag = np.sqrt((ref ** 2).sum(axis=1))
+    assert (err <= bound + 1e-5 * mag).all(), float((err / (bound + 1e-5 * mag)).max())
+    # (the metric itself may exceed the 1e-3 bar here: this input is outside the stated envelope)
+    # the same clump moved to a cell centre is inside one cell: exact differences, full accuracy
+    pos_c = (pos.astype(np.float64) - corner + (np.array([3, 5, 2]) + 0.5) * w).astype(np.float32)
+    b = ctx.bin(torch.from_numpy(pos_c).cuda(), K, box)
+    acc_c = ctx.forces(b, R, eps, Gm).cpu().numpy()
+    e_c = oracle.parity_error(acc_c, oracle.forces(pos_c, K, R, eps, box, Gm))
+    assert np.median(e_c) <= MEDIAN_TOL and e_c.max() <= MAX_TOL
+
+
+# ------------------------------------------------- nf_keys, nf_forces_chunk (the sharded path on a device)
+@pytest.mark.parametrize("K,box,n", [(8, 1.0, 40_000), (37, 500.0, 100_003), (256, 500.0, 70_000), (1, 2.0, 100)])
+def test_keys_bit_exact(ctx, K, box, n):
+    rng = np.random.default_rng(K + n)
+    pos = (rng.random((n, 3)) * box).astype(np.float32)
+    m = min(n, 90)
+    pos[:m] = (rng.integers(0, K + 1, (m, 3)) * (box / K)).astype(np.float32)        # on cell faces, incl. 0 and box
+    pos[m:2 * m] = np.nextafter(pos[:m], np.float32(-1))
+    if n > 1000:
+        pos[500] = [np.nan, 0.1, 0.1]
+        pos[501] = [-1.0, 0.1, box * 2]
+    ref, nbad = oracle.keys(pos, K, box)
+    got = ctx.keys(torch.from_numpy(pos).cuda(), K, box)
+    assert np.array_equal(u32(got), ref)
+    assert ctx.out_of_range() == nbad
+
+
+@pytest.mark.parametrize("world,K,R", [(2, 16, 2), (3, 13, 2), (4, 12, 1), (2, 9, 3)])
+def test_forces_chunk_ranks_on_one_device(ctx, world, K, R):
+    """The sharded path of SURVEY.md Sec. 8(e) with every "rank" run back to back on one device: plan the
+    x-slab ranges by work, give each rank its own planes plus R ghost planes from either side (wrapped at
+    the box edge), nf_bin + nf_forces_chunk per rank, and compare EVERY particle with the oracle on the
+    whole box.  No rank sees more than its own planes and ghosts."""
+    from paper_1810_02916_b200 import shard
+    cfg = inputs.scaled(inputs.config(3), 60_000, K)
+    cfg = inputs.dataclasses.replace(cfg, n_halos=12)
+    pos = inputs.make_positions(cfg).numpy()
+    keys, _ = oracle.keys(pos, K, cfg.box)
+    cx = (keys // (K * K)).astype(np.int64)
+    cnt = np.bincount(keys, minlength=K ** 3).astype(np.uint32)
+    work = [oracle.interactions(cnt, K, R, p, p + 1) for p in range(K)]
+    ranges = shard.plan_x_slabs(work, world)
+    ref = oracle.forces(pos, K, R, cfg.eps, cfg.box, cfg.Gm)
+    got = np.full((cfg.N, 3), np.nan, np.float32)
+    total_I = 0
+    for lo, hi in ranges:
+        need_l, need_r = shard.ghost_sources(lo, hi, R, K)
+        ghosts = [p for p in dict.fromkeys(need_l + need_r) if not lo <= p < hi]      # a plane at most once, never an own plane
+        own = np.nonzero((cx >= lo) & (cx < hi))[0]
+        gh = np.nonzero(np.isin(cx, ghosts))[0]
+        local = np.concatenate([pos[own], pos[gh]])
+        b = ctx.bin(torch.from_numpy(local).cuda(), K, cfg.box)
+        acc = torch.full((local.shape[0], 3), float("nan"), device="cuda")
+        ctx.forces_chunk(b, R, cfg.eps, cfg.Gm, lo, hi, out=acc)
+        acc = acc.cpu().numpy()
+        assert np.isfinite(acc[:own.size]).all() and np.isnan(acc[own.size:]).all()       # ghosts are sources only
+        got[own] = acc[:own.size]
+        total_I += oracle.interactions(u32(b.cell_count), K, R, lo, hi)
+    assert np.isfinite(got).all()
+    err = oracle.parity_error(got, ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (np.median(err), err.max())
+    if all(hi - lo + 2 * R <= K for lo, hi in ranges):
+        assert total_I == oracle.interactions(cnt, K, R)
+    # the whole box as one chunk is nf_forces, bit for bit
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, cfg.box)
+    assert torch.equal(ctx.forces_chunk(b, R, cfg.eps, cfg.Gm, 0, K), ctx.forces(b, R, cfg.eps, cfg.Gm))
+    with pytest.raises(Exception):
+        ctx.forces_chunk(b, R, cfg.eps, cfg.Gm, 3, K + 1)
