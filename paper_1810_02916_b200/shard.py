@@ -46,6 +46,13 @@ def ghost_sources(lo: int, hi: int, R: int, K: int) -> Tuple[List[int], List[int
     return [(lo - R + j) % K for j in range(R)], [(hi + j) % K for j in range(R)]
 
 
+def ghost_planes(lo: int, hi: int, R: int, K: int) -> List[int]:
+    """The planes a rank owning [lo, hi) holds as ghosts: the left and right neighbours' planes in the
+    order of ghost_sources, each plane once, never one of its own (short periodic boxes alias them)."""
+    need_l, need_r = ghost_sources(lo, hi, R, K)
+    return [p for p in dict.fromkeys(need_l + need_r) if not lo <= p < hi]
+
+
 def _owner(plane: int, ranges: Sequence[Tuple[int, int]]) -> int:
     for r, (lo, hi) in enumerate(ranges):
         if lo <= plane < hi:
@@ -54,13 +61,20 @@ def _owner(plane: int, ranges: Sequence[Tuple[int, int]]) -> int:
 
 
 def exchange_ghosts(my_planes: List[torch.Tensor], ranges: Sequence[Tuple[int, int]], R: int, K: int, dist,
-                    rank: Optional[int] = None) -> Tuple[List[torch.Tensor], List[torch.Tensor]]:
+                    rank: Optional[int] = None, alloc=None, via_host: bool = False
+                    ) -> Tuple[List[torch.Tensor], List[torch.Tensor]]:
     """The one exchange step.  `my_planes[i]` is the float32 [n, 3] array of plane ranges[rank][0] + i.
     Returns (left ghosts, right ghosts), each a list of R arrays in increasing plane order.
-    Counts travel first (one int64 per plane), then the positions, all as isend/irecv pairs
-    keyed by the plane index so that any mix of neighbours (including a rank that is its own
-    neighbour when world == 1, or a neighbour two ranks away when ranges are shorter than R)
-    is served."""
+    Counts travel first (one int64 per plane), then the positions, as batched isend/irecv pairs, so that
+    any mix of neighbours (including a rank that is its own neighbour when world == 1, or a neighbour
+    two ranks away when ranges are shorter than R) is served.
+
+    Matching does NOT rely on message tags (NCCL ignores them): for every ordered pair of ranks the sender
+    and the receiver enumerate the planes in the same order -- the receiver's need list (left ghosts, then
+    right ghosts, increasing slot) -- and the operations of one pair are issued in that order on both sides.
+    Empty planes send their count only.  `alloc(slot, n)` may supply the receive buffer of ghost slot
+    `slot` (e.g. a slice at the tail of the rank's particle array); `via_host` stages CUDA tensors through
+    host memory (for the gloo backend on a GPU box)."""
     rank = dist.get_rank() if rank is None else rank
     world = len(ranges)
     lo, hi = ranges[rank]
@@ -85,27 +99,53 @@ def exchange_ghosts(my_planes: List[torch.Tensor], ranges: Sequence[Tuple[int, i
         else:
             remote_recv.append((src, slot))
     remote_send = [(dst, slot, pl) for dst, slot, pl in sends if dst != rank]
+    # per-pair order: sends to `dst` follow dst's slot order (the loop above enumerates them so); receives
+    # from `src` follow my own slot order.  Both are "the receiver's need list in increasing slot".
+    remote_send.sort(key=lambda t: (t[0], t[1]))
+    remote_recv.sort(key=lambda t: (t[0], t[1]))
+    xdev = torch.device("cpu") if via_host else dev
     # 1) counts
     ops, cnt_bufs = [], {}
     for dst, slot, pl in remote_send:
-        t = torch.tensor([my_planes[pl - lo].shape[0]], dtype=torch.int64, device=dev)
-        ops.append(dist.P2POp(dist.isend, t, dst, tag=slot))
+        t = torch.tensor([my_planes[pl - lo].shape[0]], dtype=torch.int64, device=xdev)
+        ops.append(dist.P2POp(dist.isend, t, dst))
     for src, slot in remote_recv:
-        cnt_bufs[slot] = torch.zeros(1, dtype=torch.int64, device=dev)
-        ops.append(dist.P2POp(dist.irecv, cnt_bufs[slot], src, tag=slot))
+        cnt_bufs[slot] = torch.zeros(1, dtype=torch.int64, device=xdev)
+        ops.append(dist.P2POp(dist.irecv, cnt_bufs[slot], src))
     if ops:
         for w in dist.batch_isend_irecv(ops):
             w.wait()
-    # 2) positions
-    ops = []
+    # 2) positions (nothing travels for an empty plane: both sides know its count)
+    ops, staged = [], []
     for dst, slot, pl in remote_send:
-        ops.append(dist.P2POp(dist.isend, my_planes[pl - lo].contiguous(), dst, tag=100 + slot))
+        t = my_planes[pl - lo]
+        if t.shape[0] == 0:
+            continue
+        t = t.contiguous()
+        ops.append(dist.P2POp(dist.isend, t.cpu() if via_host else t, dst))
     for src, slot in remote_recv:
-        out[slot] = torch.empty(int(cnt_bufs[slot].item()), 3, dtype=torch.float32, device=dev)
-        ops.append(dist.P2POp(dist.irecv, out[slot], src, tag=100 + slot))
+        n = int(cnt_bufs[slot].item())
+        out[slot] = alloc(slot, n) if alloc is not None else torch.empty(n, 3, dtype=torch.float32, device=dev)
+        assert out[slot].shape == (n, 3) and out[slot].is_contiguous()
+        if n == 0:
+            continue
+        if via_host:
+            h = torch.empty(n, 3, dtype=torch.float32)
+            staged.append((out[slot], h))
+            ops.append(dist.P2POp(dist.irecv, h, src))
+        else:
+            ops.append(dist.P2POp(dist.irecv, out[slot], src))
     if ops:
         for w in dist.batch_isend_irecv(ops):
             w.wait()
+    for dst_t, h in staged:
+        dst_t.copy_(h)
+    if alloc is not None:                       # ghosts that are my own planes (periodic wrap onto myself) are copied in
+        for slot, pl in enumerate(needs):
+            if _owner(pl, ranges) == rank:
+                buf = alloc(slot, my_planes[pl - lo].shape[0])
+                buf.copy_(my_planes[pl - lo])
+                out[slot] = buf
     return out[:R], out[R:]
 
 

@@ -845,7 +845,7 @@ def test_forces_outside_float32_envelope(ctx, seed):
 def test_keys_bit_exact(ctx, K, box, n):
     rng = np.random.default_rng(K + n)
     pos = (rng.random((n, 3)) * box).astype(np.float32)
-    m = min(n, 90)
+    m = min(n // 2, 90)
     pos[:m] = (rng.integers(0, K + 1, (m, 3)) * (box / K)).astype(np.float32)        # on cell faces, incl. 0 and box
     pos[m:2 * m] = np.nextafter(pos[:m], np.float32(-1))
     if n > 1000:
