@@ -340,6 +340,196 @@ def run_stream(args, cfg):
         dist.destroy_process_group()
 
 
+def run_sharded(args, cfg):
+    """N > 1 GPUs: ONE box of the named config cut into N contiguous x-slab ranges balanced by pairwise
+    interactions (SURVEY.md Sec. 8(e); PAPER.md:41 slabs, :81 "a parallel version of Abacus based on the
+    existing slab decomposition").  A rank holds the particles of its planes, filed by plane.  One step =
+    ONE exchange of R ghost planes with each x-neighbour (point-to-point, no all-reduce, no output
+    exchange) + nf_bin + nf_forces_chunk on (own + ghost) particles; all of it inside the timed region.
+    Strong scaling: the total work is fixed as N grows.  Also runs with N = 1 (`--shard`), where the
+    single range is the whole periodic box and there is nothing to exchange."""
+    from paper_1810_02916_b200 import nf, shard
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    same_gpu = args.shard_backend == "gloo"          # debugging aid: every rank on cuda:0, ghosts staged through the host
+    local = 0 if same_gpu else local
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        if same_gpu:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K, R, N = cfg.K, cfg.R, cfg.N
+    KK = K * K
+    ctx = nf.Context(local)
+    n_chunks = (N + inputs.CHUNK - 1) // inputs.CHUNK
+    # ---- the plan: per-plane work from the box's cell counts (each rank counts 1/world of the chunks)
+    cnt = torch.zeros(K ** 3, dtype=torch.int64, device=dev)
+    for c in range(rank, n_chunks, world):
+        x = inputs.make_positions_chunk(cfg, c, device=dev)
+        cnt += torch.bincount(ctx.keys(x, K, cfg.box).long(), minlength=K ** 3)
+    if world > 1:
+        if same_gpu:
+            h = cnt.cpu()
+            dist.all_reduce(h)
+            cnt.copy_(h)
+        else:
+            dist.all_reduce(cnt)
+    c3 = cnt.view(K, K, K)
+    nb = torch.zeros_like(c3)
+    for dx in range(-R, R + 1):
+        for dy in range(-R, R + 1):
+            for dz in range(-R, R + 1):
+                nb += torch.roll(c3, shifts=(dx, dy, dz), dims=(0, 1, 2))
+    work = (c3 * nb).sum(dim=(1, 2)).tolist()          # ordered pairs whose sink lies in plane p
+    I_total = int(sum(work))
+    ranges = shard.plan_x_slabs(work, world)
+    lo, hi = ranges[rank]
+    ghosts = shard.ghost_planes(lo, hi, R, K) if world > 1 else []
+    if world > 1 and any(h - l + 2 * R > K for l, h in ranges):
+        raise SystemExit("bench.py: a rank's planes plus ghosts exceed the box (K too small for this many ranks)")
+    plane_n = c3.sum(dim=(1, 2)).tolist()
+    n_own = int(sum(plane_n[lo:hi]))
+    n_ghost = int(sum(plane_n[p] for p in ghosts))
+    del cnt, c3, nb
+    # ---- this rank's particles, filed by plane (stable), with room for the ghosts behind them
+    local_pos = torch.empty(n_own + n_ghost, 3, dtype=torch.float32, device=dev)
+    plane_id = torch.empty(n_own, dtype=torch.int64, device=dev)
+    fill = 0
+    for c in range(n_chunks):
+        x = inputs.make_positions_chunk(cfg, c, device=dev)
+        p = ctx.keys(x, K, cfg.box).long() // KK
+        keep = (p >= lo) & (p < hi)
+        m = int(keep.sum())
+        local_pos[fill:fill + m] = x[keep]
+        plane_id[fill:fill + m] = p[keep]
+        fill += m
+    assert fill == n_own
+    order = torch.argsort(plane_id, stable=True)
+    local_pos[:n_own] = local_pos[:n_own][order]
+    del order, plane_id, x, p, keep
+    starts = [0]
+    for q in range(lo, hi):
+        starts.append(starts[-1] + int(plane_n[q]))
+    my_planes = [local_pos[starts[i]:starts[i + 1]] for i in range(hi - lo)]
+    need_l, need_r = shard.ghost_sources(lo, hi, R, K)
+    slot_plane = need_l + need_r
+    goff, o = {}, n_own
+    for pl in ghosts:
+        goff[pl] = o
+        o += int(plane_n[pl])
+
+    def alloc(slot, n):
+        pl = slot_plane[slot]
+        assert n == int(plane_n[pl])
+        return local_pos[goff[pl]:goff[pl] + n]
+
+    torch.cuda.empty_cache()
+    ctx.reserve(n_own + n_ghost, K)
+    b = None
+    acc = torch.empty(n_own + n_ghost, 3, dtype=torch.float32, device=dev)
+
+    def step():
+        nonlocal b
+        if world > 1:
+            shard.exchange_ghosts(my_planes, ranges, R, K, dist, rank=rank, alloc=alloc, via_host=same_gpu)
+        b = ctx.bin(local_pos, K, cfg.box, out=b)
+        ctx.forces_chunk(b, R, cfg.eps, cfg.Gm, lo, hi, out=acc)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    launches0 = ctx.launch_count()
+    kern_ms = []
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    e0.record()
+    for s_ in range(args.steps):
+        step()
+        kern_ms.append(ctx.last_forces_timing()[0])
+    e1.record()
+    barrier()
+    wall = time.perf_counter() - t0
+    launches = ctx.launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    k_ms = sum(kern_ms) / len(kern_ms)
+    red = lambda v, op: v
+    t = torch.tensor([max(wall, e0.elapsed_time(e1) * 1e-3), k_ms * 1e-3], dtype=torch.float64)
+    if world > 1:
+        t = t if same_gpu else t.to(dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_per_step = 1e3 * float(t[0]) / args.steps
+    k_ms_max = 1e3 * float(t[1])
+
+    # ---- end to end: own particles from pinned host memory, accelerations back to it, every step
+    e2e = None
+    if not args.no_e2e:
+        h_own = torch.empty(n_own, 3, dtype=torch.float32).pin_memory()
+        h_own.copy_(local_pos[:n_own])
+        h_acc = torch.empty(n_own, 3, dtype=torch.float32).pin_memory()
+        n_e2e = max(1, min(args.steps, 3))
+
+        def e2e_step():
+            local_pos[:n_own].copy_(h_own, non_blocking=True)
+            step()
+            h_acc.copy_(acc[:n_own], non_blocking=True)
+            torch.cuda.synchronize()
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_step()
+        barrier()
+        te = torch.tensor([(time.perf_counter() - t0) / n_e2e], dtype=torch.float64)
+        if world > 1:
+            te = te if same_gpu else te.to(dev)
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": I_total / float(te[0]), "unit": "interactions/s", "h2d_bytes_per_step": 12 * N, "d2h_bytes_per_step": 12 * N,
+               "ms_per_step": 1e3 * float(te[0]), "api": "H2D own planes + ghost exchange + nf_bin + nf_forces_chunk + D2H", "steps": n_e2e,
+               "result_checksum": float(h_acc[:: max(1, n_own // 4096)].double().abs().sum())}
+
+    # parity of rank 0's sinks against the oracle on a block inside its range (N = 1: --shard only)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    value = I_total / (ms_per_step * 1e-3)
+    sm_max_mhz, hbm_gbs, peak_src = read_peaks()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak_tflops = world * sms * sm_max_mhz * 1e6 * 2 * FP32_LANES_PER_SM / 1e12
+    achieved = FLOP_PER_INTERACTION * I_total / (k_ms_max * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "interaction kernel (nf_forces_chunk), slowest rank", "achieved": achieved, "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
+                "peak_source": f"{world} x {sms} SMs x {sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz) x 2 x {FP32_LANES_PER_SM} FP32 lanes",
+                "flop_per_interaction": FLOP_PER_INTERACTION, "kernel_ms": k_ms_max, "kernel_share_of_step": k_ms_max / ms_per_step}
+    line = {"metric": "near_field_pairwise_interactions_per_s", "value": value, "unit": "interactions/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg.name, "N": N, "K": K, "R": R, "eps": cfg.eps, "box": cfg.box,
+                       "interactions_per_step": I_total, "interactions_per_particle": I_total / N,
+                       "l2": "inputs larger than L2",
+                       "parallelism": f"x-slab sharding over {world} GPU(s), R ghost planes from each x-neighbour, ranges balanced by interactions",
+                       "ranges": ranges, "rank0_particles": n_own, "rank0_ghost_particles": n_ghost,
+                       "ghost_bytes_per_step_rank0": 12 * n_ghost},
+            "particles_per_s": N / (ms_per_step * 1e-3),
+            "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": None}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def sweep_small_configs(ctx, dev, steps=3, warmup=3):
     """Interaction-kernel roofline fraction of C1, C2 and C3 in the same process (milliseconds each): the
     other single-GPU configs of BASELINE.json beside the headline workload.  Same timing rules as the main
@@ -388,6 +578,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the C1-C3 kernel sweep of the default line")
+    ap.add_argument("--shard", action="store_true", help="use the x-slab sharded path (the default for --gpus N > 1) even on one GPU")
+    ap.add_argument("--shard-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="gloo: debugging aid, every rank on cuda:0 with ghosts staged through host memory")
     ap.add_argument("--n-side", type=int, default=0,
                     help="profiling aid: the same recipe at n_side^3 particles and K = n_side/4 (not the bench workload)")
     args = ap.parse_args()
@@ -405,6 +598,9 @@ def main():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     if cfg.kind == "slab":
         run_stream(args, cfg)
+        return
+    if args.shard or int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        run_sharded(args, cfg)
         return
     from paper_1810_02916_b200 import nf
 

@@ -144,31 +144,40 @@ def make_positions(cfg: Config, device="cpu", out: Optional[torch.Tensor] = None
     if out is None:
         out = torch.empty(N, 3, dtype=torch.float32, device=device)
     assert out.shape == (N, 3) and out.dtype == torch.float32
-    if cfg.kind == "clustered":
-        centres, scales = _halo_catalogue(cfg, device)
+    cat = _halo_catalogue(cfg, device) if cfg.kind == "clustered" else None
     for c, lo in enumerate(range(0, N, CHUNK)):
-        hi = min(N, lo + CHUNK)
-        n = hi - lo
-        g = _gen(cfg.seed, c, device)
-        if cfg.kind == "uniform":
-            x = torch.rand(n, 3, generator=g, device=device, dtype=torch.float32) * cfg.box
-        elif cfg.kind == "lattice":
-            m = cfg.lattice_n
-            idx = torch.arange(lo, hi, device=device, dtype=torch.int64)
-            ijk = torch.stack([idx // (m * m), (idx // m) % m, idx % m], dim=1).double()
-            x = (ijk + 0.5) * (cfg.box / m)
-            x = x + torch.randn(n, 3, generator=g, device=device, dtype=torch.float64) * cfg.lattice_sigma
-            x = x.float()
-        elif cfg.kind == "clustered":
-            x = torch.rand(n, 3, generator=g, device=device, dtype=torch.float64) * cfg.box
-            is_halo = torch.rand(n, generator=g, device=device, dtype=torch.float64) < cfg.frac_halo
-            hid = torch.randint(0, cfg.n_halos, (n,), generator=g, device=device)
-            off = _plummer_offsets(n, scales[hid], cfg.r_trunc, g, device)
-            x = torch.where(is_halo[:, None], centres[hid] + off, x).float()
-        else:
-            raise ValueError(f"make_positions: kind {cfg.kind!r} not supported (use make_slab_planes)")
-        out[lo:hi] = _wrap_(x, cfg.box)
+        out[lo:min(N, lo + CHUNK)] = make_positions_chunk(cfg, c, device, cat)
     return out
+
+
+def make_positions_chunk(cfg: Config, c: int, device="cpu", catalogue=None) -> torch.Tensor:
+    """Chunk c (particles [c*CHUNK, min(N, (c+1)*CHUNK))) of make_positions: every chunk has its own
+    generator, so a rank of a sharded run can produce any part of the box without the rest."""
+    device = torch.device(device)
+    lo = c * CHUNK
+    assert 0 <= lo < cfg.N
+    hi = min(cfg.N, lo + CHUNK)
+    n = hi - lo
+    g = _gen(cfg.seed, c, device)
+    if cfg.kind == "uniform":
+        x = torch.rand(n, 3, generator=g, device=device, dtype=torch.float32) * cfg.box
+    elif cfg.kind == "lattice":
+        m = cfg.lattice_n
+        idx = torch.arange(lo, hi, device=device, dtype=torch.int64)
+        ijk = torch.stack([idx // (m * m), (idx // m) % m, idx % m], dim=1).double()
+        x = (ijk + 0.5) * (cfg.box / m)
+        x = x + torch.randn(n, 3, generator=g, device=device, dtype=torch.float64) * cfg.lattice_sigma
+        x = x.float()
+    elif cfg.kind == "clustered":
+        centres, scales = catalogue if catalogue is not None else _halo_catalogue(cfg, device)
+        x = torch.rand(n, 3, generator=g, device=device, dtype=torch.float64) * cfg.box
+        is_halo = torch.rand(n, generator=g, device=device, dtype=torch.float64) < cfg.frac_halo
+        hid = torch.randint(0, cfg.n_halos, (n,), generator=g, device=device)
+        off = _plummer_offsets(n, scales[hid], cfg.r_trunc, g, device)
+        x = torch.where(is_halo[:, None], centres[hid] + off, x).float()
+    else:
+        raise ValueError(f"make_positions: kind {cfg.kind!r} not supported (use make_slab_planes)")
+    return _wrap_(x, cfg.box)
 
 
 def make_slab_planes(cfg: Config, device="cpu", n_planes_total: Optional[int] = None,

@@ -47,6 +47,28 @@ def _worker(rank, world, port, q):
         need_l, need_r = shard.ghost_sources(lo, hi, R, K)
         for got, pl in zip(left + right, need_l + need_r):            # the exchange delivered the right planes
             assert np.array_equal(got.numpy(), pos[plane_idx[pl]])
+        # the same exchange straight into the tail of the rank's particle array (what bench.py's sharded step
+        # does): one slot per distinct ghost plane behind the own particles
+        ghosts = shard.ghost_planes(lo, hi, R, K)
+        n_own = sum(t.shape[0] for t in mine)
+        goff, o = {}, n_own
+        for pl in ghosts:
+            goff[pl] = o
+            o += plane_idx[pl].size
+        buf = torch.zeros(o, 3)
+        buf[:n_own] = torch.cat(mine)
+        slot_plane = need_l + need_r
+        scratch = {}
+
+        def alloc(slot, n):
+            pl = slot_plane[slot]
+            if pl in goff:
+                return buf[goff[pl]:goff[pl] + n]
+            scratch[slot] = torch.empty(n, 3)            # a ghost that is one of my own planes (short periodic box)
+            return scratch[slot]
+        shard.exchange_ghosts(mine, ranges, R, K, dist, alloc=alloc)
+        for pl in ghosts:
+            assert np.array_equal(buf[goff[pl]:goff[pl] + plane_idx[pl].size].numpy(), pos[plane_idx[pl]])
         # a plane can be both an own plane and a ghost (short periodic box): use each plane once
         have = {}
         for pl, t in zip(need_l, left):
