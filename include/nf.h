@@ -337,8 +337,8 @@ int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const int64
  *   plane_vel_host       host in   P pointers (pinned): velocities of sink plane p, plane_n[R+p] x 3
  *   kick, drift          as for nf_kick_drift
  *   plane_pos_out_host   host out  P pointers (pinned): drifted positions of sink plane p, input order,
- *                                  wrapped into [0, box) -- a particle may have left its plane; filing it
- *                                  under its new plane for the next step is the caller's regrouping
+ *                                  wrapped into [0, box) -- a particle may have left its plane; this call
+ *                                  leaves the filing to the caller, nf_stream_step_regroup does it in the stream
  *   plane_vel_out_host   host out  P pointers (pinned): kicked velocities
  *   plane_acc_host       host out, nullable table: the accelerations, as nf_stream_slabs writes them
  *   everything else as for nf_stream_slabs.
@@ -348,6 +348,52 @@ int nf_stream_step_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const 
                          float Gm, int softening, float kick, float drift, float *const *plane_pos_out_host,
                          float *const *plane_vel_out_host, float *const *plane_acc_host,
                          nf_stream_stats *stats, void *stream);
+
+/*
+ * nf_regroup_plane -- regrouping after the drift, one plane ("update particles on the central
+ * slab, write out the trailing slab"; :195, :209 "particles drift by at most one slab per time step";
+ * SURVEY.md Sec. 8(f) rank 3).  The drifted particles of x-plane plane_cx are rewritten as three STABLE
+ * segments by the plane their new x coordinate maps to (the bit-exact cell formula of nf_bin / nf_keys):
+ *
+ *     [ now in plane_cx - 1 | still in plane_cx | now in plane_cx + 1 ]      (periodic in K; input order kept
+ *                                                                             inside each segment)
+ *   pos_xyz, vel_xyz   dev in   N x 3 float32, positions already wrapped into [0, box) (nf_kick_drift)
+ *   pos_out, vel_out   dev out  N x 3 float32, must not alias the inputs
+ *   seg_n              host out 3 segment lengths (they sum to N)
+ *
+ * The new content of plane d is then [ third segment of d-1 | second of d | first of d+1 ].  A particle that
+ * moved further than one plane breaks time-step criterion 3: it is filed under the nearer neighbour and
+ * counted, and the call returns NF_ERR_RANGE after completing.  Synchronises `stream` (it returns counts).
+ */
+int nf_regroup_plane(nf_ctx *ctx, const float *pos_xyz, const float *vel_xyz, int64_t N, int K, float box,
+                     int plane_cx, float *pos_out, float *vel_out, int64_t *seg_n, void *stream);
+
+/*
+ * nf_stream_step_regroup -- nf_stream_step_slabs with the regrouping done in the stream as well, so that one
+ * call is one whole time step of the slab pipeline and its output is directly the input of the
+ * next call -- no host-side filing in between.
+ *
+ *   seg_pos_host   host in  (P + 2R) x 3 pinned pointers: plane q is the concatenation, in this order, of the
+ *                           segments seg_pos_host[3q + 0..2] with seg_n[3q + 0..2] particles (empty segments
+ *                           may be NULL).  A first step passes whole planes as {NULL, plane, NULL}; a later
+ *                           step passes, for plane d, the three segments the previous step wrote:
+ *                           {third segment of plane d-1's output, second of d's, first of d+1's}.
+ *   seg_vel_host   host in  P x 3 pinned pointers: velocities of the sink planes, same segmentation
+ *   seg_n          host in  (P + 2R) x 3 counts
+ *   plane_pos_out_host, plane_vel_out_host
+ *                  host out P pinned pointers, each with room for the plane's particles (sum of its 3 input
+ *                           segments): the kicked and drifted particles of sink plane p as the three stable
+ *                           segments of nf_regroup_plane
+ *   out_seg_n      host out P x 3 segment lengths
+ *   plane_acc_host host out, nullable table: accelerations in the plane's INPUT order (before regrouping)
+ *   everything else as for nf_stream_step_slabs.  With P = K (ghost planes = the sink planes of the other end
+ *   of the periodic box, passed again) the call steps the whole box.
+ */
+int nf_stream_step_regroup(nf_ctx *ctx, const float *const *seg_pos_host, const float *const *seg_vel_host,
+                           const int64_t *seg_n, int P, int K, int R, float eps, float box, int plane0, float Gm,
+                           int softening, float kick, float drift, float *const *plane_pos_out_host,
+                           float *const *plane_vel_out_host, int64_t *out_seg_n, float *const *plane_acc_host,
+                           nf_stream_stats *stats, void *stream);
 
 /* Timing of the kernels of the last nf_forces call on this context (CUDA events recorded on
  * the call's stream around the interaction kernel).  Synchronises on the end event.

@@ -137,3 +137,7 @@ void nf_slab_state_free(nf_ctx *ctx);
 int nf_kick_drift_impl(nf_ctx *ctx, float *pos, float *vel, const float *acc, int64_t N, float kick, float drift, float box,
                        cudaStream_t st);
 int nf_interactions_impl(nf_ctx *ctx, const uint32_t *cell_count, int K, int R, int64_t *out, cudaStream_t st);
+// regrouping after the drift (nf_regroup.cu): [to plane-1 | stay | to plane+1], stable; scratch from the arena
+size_t nf_regroup_scratch_bytes(int64_t N);
+int nf_regroup_impl(nf_ctx *ctx, const float *pos, const float *vel, int64_t n, int K, float box, int plane_cx, float *pos_out,
+                    float *vel_out, unsigned long long *seg_n, cudaStream_t st);

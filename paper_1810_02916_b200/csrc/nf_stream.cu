@@ -26,19 +26,31 @@ struct Slot {
     uint64_t *off;     // K*K + 1
     float *acc;        // n x 3
     float *vel;        // n x 3 (nf_stream_step_slabs only)
+    float *part_pos;   // n x 3, n x 3 (nf_stream_step_regroup only): the drifted plane as [to plane-1 | stay | to plane+1]
+    float *part_vel;
 };
 
 // the kick + drift epilogue of nf_stream_step_slabs (null pointers: plain nf_stream_slabs)
 struct StepArgs {
-    const float *const *vel_host;     // P
+    const float *const *vel_host;     // P x nseg
     float *const *pos_out_host;       // P
     float *const *vel_out_host;       // P
     float kick, drift;
+    int64_t *out_seg_n;               // non-null: regroup after the drift (nf_stream_step_regroup), P x 3 counts (host out)
+};
+
+// the planes of a pass: plane q is the concatenation of nseg host segments pos[q*nseg + k] of n[q*nseg + k] particles
+struct PlaneIn {
+    const float *const *pos;
+    const int64_t *n;
+    int nseg;
 };
 
 struct SlabState {
     char *mem = nullptr;
     size_t mem_bytes = 0;
+    unsigned long long *d_segn = nullptr, *h_segn = nullptr;   // [P][3] segment lengths of the regrouped planes
+    int segn_cap = 0;
     nf_plane_view *h_views = nullptr;  // pinned, [P+2R]
     nf_plane_view *d_views = nullptr;
     int views_cap = 0;
@@ -50,6 +62,8 @@ void free_state(SlabState *s)
     if (s->mem) cudaFree(s->mem);
     if (s->h_views) cudaFreeHost(s->h_views);
     if (s->d_views) cudaFree(s->d_views);
+    if (s->d_segn) cudaFree(s->d_segn);
+    if (s->h_segn) cudaFreeHost(s->h_segn);
     delete s;
 }
 
@@ -81,13 +95,13 @@ static bool is_pinned(const void *p)
     return at.type == cudaMemoryTypeHost;      // page-locked host memory; managed memory migrates and is refused
 }
 
-static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_pos_host, const int64_t *plane_n,
+static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
                       int P, int K, int R, float eps, float box, int plane0, float Gm,
                       int softening, float *const *plane_acc_host, const StepArgs *step, nf_stream_stats *stats,
                       void *stream)
 {
     if (!ctx) return NF_ERR_ARG;
-    NF_ARG(ctx, plane_pos_host && plane_n && (plane_acc_host || step), "nf_stream_slabs: null pointer table");
+    NF_ARG(ctx, in.pos && in.n && (plane_acc_host || step), "nf_stream_slabs: null pointer table");
     NF_ARG(ctx, P >= 1, "nf_stream_slabs: P must be >= 1");
     NF_ARG(ctx, K >= 1 && K <= NF_MAX_K, "K = %d out of range [1, %d]", K, NF_MAX_K);
     NF_ARG(ctx, R >= 0 && R <= NF_MAX_R, "R = %d out of range [0, %d]", R, NF_MAX_R);
@@ -96,27 +110,35 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
     NF_ARG(ctx, eps > 0.0f && eps < 3.0e38f, "eps must be positive and finite");
     NF_ARG(ctx, box > 0.0f && box < 3.0e38f, "box must be positive and finite");
     NF_ARG(ctx, softening == NF_SOFT_SPLINE || softening == NF_SOFT_PLUMMER, "unknown softening %d (the slab stream carries no masses)", softening);
-    const int NP = P + 2 * R;
+    const int NP = P + 2 * R, NS = in.nseg;
+    const bool regroup = step && step->out_seg_n;
+    NF_ARG(ctx, NS >= 1 && NS <= 3, "a plane has 1 to 3 host segments");
+    std::vector<int64_t> plane_n_v(NP, 0);
     int64_t max_n = 1;
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
     for (int q = 0; q < NP; q++) {
-        NF_ARG(ctx, plane_n[q] >= 0 && plane_n[q] < ((int64_t)1 << 32), "plane_n[%d] out of range", q);
-        NF_ARG(ctx, plane_n[q] == 0 || plane_pos_host[q], "plane_pos_host[%d] is null", q);
-        if (plane_n[q] > max_n) max_n = plane_n[q];
+        for (int k = 0; k < NS; k++) {
+            const int64_t nk = in.n[q * NS + k];
+            NF_ARG(ctx, nk >= 0 && nk < ((int64_t)1 << 32), "plane %d, segment %d: particle count out of range", q, k);
+            // host pointers must be pinned (page-locked): "Pinning memory"
+            NF_ARG(ctx, nk == 0 || (in.pos[q * NS + k] && is_pinned(in.pos[q * NS + k])),
+                   "plane_pos_host[%d] (segment %d) is null or not pinned host memory", q, k);
+            plane_n_v[q] += nk;
+        }
+        NF_ARG(ctx, plane_n_v[q] < ((int64_t)1 << 32), "plane_n[%d] out of range", q);
+        if (plane_n_v[q] > max_n) max_n = plane_n_v[q];
     }
+    const int64_t *plane_n = plane_n_v.data();
     for (int p = 0; p < P; p++) {
         if (plane_n[R + p] == 0) continue;
         NF_ARG(ctx, !plane_acc_host || (plane_acc_host[p] && is_pinned(plane_acc_host[p])), "plane_acc_host[%d] is null or not pinned host memory", p);
         if (step) {
-            NF_ARG(ctx, step->vel_host[p] && is_pinned(step->vel_host[p]), "plane_vel_host[%d] is null or not pinned host memory", p);
+            for (int k = 0; k < NS; k++)
+                NF_ARG(ctx, in.n[(R + p) * NS + k] == 0 || (step->vel_host[p * NS + k] && is_pinned(step->vel_host[p * NS + k])),
+                       "plane_vel_host[%d] (segment %d) is null or not pinned host memory", p, k);
             NF_ARG(ctx, step->pos_out_host[p] && is_pinned(step->pos_out_host[p]), "plane_pos_out_host[%d] is null or not pinned host memory", p);
             NF_ARG(ctx, step->vel_out_host[p] && is_pinned(step->vel_out_host[p]), "plane_vel_out_host[%d] is null or not pinned host memory", p);
         }
-    }
-    NF_CUDA(ctx, cudaSetDevice(ctx->device));
-    // host pointers must be pinned (page-locked): "Pinning memory"
-    for (int q = 0; q < NP; q++) {
-        if (plane_n[q] == 0) continue;
-        NF_ARG(ctx, is_pinned(plane_pos_host[q]), "plane_pos_host[%d] is not pinned host memory", q);
     }
 
     cudaStream_t st = (cudaStream_t)stream;
@@ -133,7 +155,7 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
     const size_t n = (size_t)max_n;
     const size_t slot_bytes = nf_align_up(n * 12, 256) + 3 * nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
                               nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256) + nf_align_up(n * 12, 256) +
-                              (step ? nf_align_up(n * 12, 256) : 0);
+                              (step ? nf_align_up(n * 12, 256) : 0) + (regroup ? 2 * nf_align_up(n * 12, 256) : 0);
     const size_t need = slot_bytes * W;
     if (need > S->mem_bytes) {
         NF_CUDA(ctx, cudaDeviceSynchronize());
@@ -155,8 +177,18 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
     nf_force_params fp{};
     fp.K = K; fp.n_planes = NP; fp.periodic_x = 0; fp.R = R; fp.eps = eps; fp.box = box; fp.Gm = Gm; fp.softening = softening;
     fp.sink_lo = 0; fp.sink_hi = 1; fp.max_sinks = max_n;     // one sink plane per nf_forces_impl call
-    // binning and the force work list of a plane take their scratch one after the other
-    NF_TRY(nf_scratch_reserve(ctx, nf_bin_scratch_bytes(max_n, K, true) + nf_forces_scratch_bytes(fp)));
+    if (regroup && P > S->segn_cap) {
+        NF_CUDA(ctx, cudaDeviceSynchronize());
+        if (S->d_segn) NF_CUDA(ctx, cudaFree(S->d_segn));
+        if (S->h_segn) NF_CUDA(ctx, cudaFreeHost(S->h_segn));
+        S->d_segn = nullptr; S->h_segn = nullptr; S->segn_cap = 0;
+        NF_CUDA(ctx, cudaMalloc((void **)&S->d_segn, sizeof(unsigned long long) * 3 * P));
+        NF_CUDA(ctx, cudaMallocHost((void **)&S->h_segn, sizeof(unsigned long long) * 3 * P));
+        S->segn_cap = P;
+    }
+    // binning, the force work list and the regrouping of a plane take their scratch one after the other
+    NF_TRY(nf_scratch_reserve(ctx, nf_bin_scratch_bytes(max_n, K, true) + nf_forces_scratch_bytes(fp) +
+                                       (regroup ? nf_regroup_scratch_bytes(max_n) : 0)));
 
     std::vector<Slot> slots(W);
     for (int s = 0; s < W; s++) {
@@ -170,6 +202,10 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
         slots[s].off = (uint64_t *)b;             b += nf_align_up((ncell + 1) * 8, 256);
         slots[s].acc = (float *)b;                b += nf_align_up(n * 12, 256);
         slots[s].vel = step ? (float *)b : nullptr;
+        if (step) b += nf_align_up(n * 12, 256);
+        slots[s].part_pos = regroup ? (float *)b : nullptr;
+        if (regroup) b += nf_align_up(n * 12, 256);
+        slots[s].part_vel = regroup ? (float *)b : nullptr;
     }
     // plane views (device pointers are fixed by the slot assignment q % W)
     for (int q = 0; q < NP; q++) {
@@ -209,11 +245,16 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
             if (own_sink >= 0 && own_sink < P) NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, d2h1[own_sink], 0));
         }
         NF_CUDA(ctx, cudaEventRecord(h2d0[q], ctx->s_h2d));
-        if (plane_n[q] > 0)
-            NF_CUDA(ctx, cudaMemcpyAsync(sl.raw, plane_pos_host[q], (size_t)plane_n[q] * 12, cudaMemcpyHostToDevice, ctx->s_h2d));
-        if (step && q >= R && q < R + P && plane_n[q] > 0) {
-            NF_CUDA(ctx, cudaMemcpyAsync(sl.vel, step->vel_host[q - R], (size_t)plane_n[q] * 12, cudaMemcpyHostToDevice, ctx->s_h2d));
-            vel_bytes += (double)plane_n[q] * 12.0;
+        size_t at = 0;
+        for (int k = 0; k < NS; k++) {
+            const size_t nk = (size_t)in.n[q * NS + k];
+            if (nk == 0) continue;
+            NF_CUDA(ctx, cudaMemcpyAsync(sl.raw + 3 * at, in.pos[q * NS + k], nk * 12, cudaMemcpyHostToDevice, ctx->s_h2d));
+            if (step && q >= R && q < R + P) {
+                NF_CUDA(ctx, cudaMemcpyAsync(sl.vel + 3 * at, step->vel_host[(q - R) * NS + k], nk * 12, cudaMemcpyHostToDevice, ctx->s_h2d));
+                vel_bytes += (double)nk * 12.0;
+            }
+            at += nk;
         }
         NF_CUDA(ctx, cudaEventRecord(h2d1[q], ctx->s_h2d));
 
@@ -238,6 +279,10 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
             // binning (the later sink planes read the sorted / encoded copies), so they can move now
             if (step && plane_n[sp] > 0)
                 NF_TRY(nf_kick_drift_impl(ctx, ss.raw, ss.vel, ss.acc, plane_n[sp], step->kick, step->drift, box, st));
+            // ... and be filed by the plane they now belong to (three stable segments + their lengths)
+            if (regroup)
+                NF_TRY(nf_regroup_impl(ctx, ss.raw, ss.vel, plane_n[sp], K, box, ((plane0 + sp) % K + K) % K, ss.part_pos, ss.part_vel,
+                                       S->d_segn + 3 * p, st));
             NF_CUDA(ctx, cudaEventRecord(frc1[p], st));
             NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_d2h, frc1[p], 0));
             NF_CUDA(ctx, cudaEventRecord(d2h0[p], ctx->s_d2h));
@@ -245,8 +290,8 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
                 const size_t nb = (size_t)plane_n[sp] * 12;
                 if (plane_acc_host) NF_CUDA(ctx, cudaMemcpyAsync(plane_acc_host[p], ss.acc, nb, cudaMemcpyDeviceToHost, ctx->s_d2h));
                 if (step) {
-                    NF_CUDA(ctx, cudaMemcpyAsync(step->pos_out_host[p], ss.raw, nb, cudaMemcpyDeviceToHost, ctx->s_d2h));
-                    NF_CUDA(ctx, cudaMemcpyAsync(step->vel_out_host[p], ss.vel, nb, cudaMemcpyDeviceToHost, ctx->s_d2h));
+                    NF_CUDA(ctx, cudaMemcpyAsync(step->pos_out_host[p], regroup ? ss.part_pos : ss.raw, nb, cudaMemcpyDeviceToHost, ctx->s_d2h));
+                    NF_CUDA(ctx, cudaMemcpyAsync(step->vel_out_host[p], regroup ? ss.part_vel : ss.vel, nb, cudaMemcpyDeviceToHost, ctx->s_d2h));
                 }
             }
             NF_CUDA(ctx, cudaEventRecord(d2h1[p], ctx->s_d2h));
@@ -255,10 +300,13 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
     NF_CUDA(ctx, cudaStreamWaitEvent(st, d2h1[P - 1], 0));
     NF_CUDA(ctx, cudaEventRecord(ev_end, st));
     NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->counters, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    if (regroup) NF_CUDA(ctx, cudaMemcpyAsync(S->h_segn, S->d_segn, sizeof(unsigned long long) * 3 * P, cudaMemcpyDeviceToHost, st));
     NF_CUDA(ctx, cudaStreamSynchronize(st));
     NF_CUDA(ctx, cudaStreamSynchronize(ctx->s_d2h));
     NF_CUDA(ctx, cudaStreamSynchronize(ctx->s_h2d));
 
+    if (regroup)
+        for (int i = 0; i < 3 * P; i++) step->out_seg_n[i] = (int64_t)S->h_segn[i];
     if (stats) {
         memset(stats, 0, sizeof(*stats));
         float ms = 0.f;
@@ -284,7 +332,7 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
         stats->overlap_fraction = hidden < 0 ? 0.0 : (hidden > 1 ? 1.0 : hidden);
     }
     if (ctx->h_counters[0]) {
-        NF_SET_ERR(ctx, "%lld particle(s) outside [0, box) or filed under the wrong plane were clamped into edge cells",
+        NF_SET_ERR(ctx, "%lld particle(s) outside [0, box), filed under the wrong plane (clamped into edge cells), or drifted further than one plane",
                    (long long)ctx->h_counters[0]);
         return NF_ERR_RANGE;
     }
@@ -295,15 +343,14 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const float *const *plane_po
 // streams: copies already queued still read and write the caller's pinned buffers, and the events of
 // the pool must not be destroyed while work that records or waits on them is pending (include/nf.h:
 // "the library never retains a caller buffer past the call").
-static int stream_impl(nf_ctx *ctx, const float *const *plane_pos_host, const int64_t *plane_n,
+static int stream_impl(nf_ctx *ctx, const PlaneIn &in,
                        int P, int K, int R, float eps, float box, int plane0, float Gm,
                        int softening, float *const *plane_acc_host, const StepArgs *step, nf_stream_stats *stats,
                        void *stream)
 {
     if (!ctx) return NF_ERR_ARG;
     EventPool pool;
-    const int rc = stream_run(ctx, pool, plane_pos_host, plane_n, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, step,
-                              stats, stream);
+    const int rc = stream_run(ctx, pool, in, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, step, stats, stream);
     if (rc != NF_OK && rc != NF_ERR_ARG) {
         cudaStreamSynchronize((cudaStream_t)stream);
         if (ctx->s_h2d) cudaStreamSynchronize(ctx->s_h2d);
@@ -320,7 +367,8 @@ extern "C" int nf_stream_slabs(nf_ctx *ctx, const float *const *plane_pos_host, 
 {
     if (!ctx) return NF_ERR_ARG;
     NF_ARG(ctx, plane_acc_host != nullptr, "nf_stream_slabs: null pointer table");
-    return stream_impl(ctx, plane_pos_host, plane_n, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, nullptr, stats, stream);
+    const PlaneIn in{plane_pos_host, plane_n, 1};
+    return stream_impl(ctx, in, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, nullptr, stats, stream);
 }
 
 extern "C" int nf_stream_step_slabs(nf_ctx *ctx, const float *const *plane_pos_host, const float *const *plane_vel_host,
@@ -332,6 +380,21 @@ extern "C" int nf_stream_step_slabs(nf_ctx *ctx, const float *const *plane_pos_h
     if (!ctx) return NF_ERR_ARG;
     NF_ARG(ctx, plane_vel_host && plane_pos_out_host && plane_vel_out_host, "nf_stream_step_slabs: null pointer table");
     NF_ARG(ctx, kick == kick && drift == drift && fabsf(kick) < 3.0e38f && fabsf(drift) < 3.0e38f, "kick and drift must be finite");
-    StepArgs a{plane_vel_host, plane_pos_out_host, plane_vel_out_host, kick, drift};
-    return stream_impl(ctx, plane_pos_host, plane_n, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, &a, stats, stream);
+    StepArgs a{plane_vel_host, plane_pos_out_host, plane_vel_out_host, kick, drift, nullptr};
+    const PlaneIn in{plane_pos_host, plane_n, 1};
+    return stream_impl(ctx, in, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, &a, stats, stream);
+}
+
+extern "C" int nf_stream_step_regroup(nf_ctx *ctx, const float *const *seg_pos_host, const float *const *seg_vel_host,
+                                      const int64_t *seg_n, int P, int K, int R, float eps, float box, int plane0, float Gm,
+                                      int softening, float kick, float drift, float *const *plane_pos_out_host,
+                                      float *const *plane_vel_out_host, int64_t *out_seg_n, float *const *plane_acc_host,
+                                      nf_stream_stats *stats, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, seg_vel_host && plane_pos_out_host && plane_vel_out_host && out_seg_n, "nf_stream_step_regroup: null pointer table");
+    NF_ARG(ctx, kick == kick && drift == drift && fabsf(kick) < 3.0e38f && fabsf(drift) < 3.0e38f, "kick and drift must be finite");
+    StepArgs a{seg_vel_host, plane_pos_out_host, plane_vel_out_host, kick, drift, out_seg_n};
+    const PlaneIn in{seg_pos_host, seg_n, 3};
+    return stream_impl(ctx, in, P, K, R, eps, box, plane0, Gm, softening, plane_acc_host, &a, stats, stream);
 }

@@ -26,7 +26,7 @@ EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve
            "nf_out_of_range", "nf_forces", "nf_interactions", "nf_spline_equivalent_eps",
            "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host",
            "nf_bin_m", "nf_forces_ex", "nf_kick_drift", "nf_cell_vrms", "nf_stream_step_slabs",
-           "nf_keys", "nf_forces_chunk", "nf_forces_host_m"]
+           "nf_keys", "nf_forces_chunk", "nf_forces_host_m", "nf_regroup_plane", "nf_stream_step_regroup"]
 
 
 class NFError(RuntimeError):
@@ -103,6 +103,12 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.nf_reserve_host.argtypes = [vp, i64, i32]
     lib.nf_forces_host_m.restype = i32
     lib.nf_forces_host_m.argtypes = [vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp]
+    lib.nf_regroup_plane.restype = i32
+    lib.nf_regroup_plane.argtypes = [vp, vp, vp, i64, i32, f32, i32, vp, vp, ctypes.POINTER(i64), vp]
+    lib.nf_stream_step_regroup.restype = i32
+    lib.nf_stream_step_regroup.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64), i32, i32, i32, f32, f32,
+                                           i32, f32, i32, f32, f32, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64),
+                                           ctypes.POINTER(vp), ctypes.POINTER(StreamStats), vp]
     lib.nf_keys.restype = i32
     lib.nf_keys.argtypes = [vp, vp, i64, i32, f32, vp, vp]
     lib.nf_forces_chunk.restype = i32
@@ -342,6 +348,63 @@ class Context:
                                                   tab(pos_out), tab(vel_out), tab(acc) if acc is not None else None,
                                                   ctypes.byref(stats), self._stream(stream)))
         return pos_out, vel_out, acc, stats.as_dict()
+
+
+    def regroup_plane(self, pos: torch.Tensor, vel: torch.Tensor, K: int, box: float, plane_cx: int, stream=None, strict: bool = True):
+        """nf_regroup_plane: (positions, velocities) of one drifted plane as [to plane-1 | stay | to plane+1]
+        and the three segment lengths."""
+        for t in (pos, vel):
+            assert t.is_cuda and t.dtype == torch.float32 and t.dim() == 2 and t.shape[1] == 3 and t.is_contiguous()
+        assert pos.shape == vel.shape
+        po, vo = torch.empty_like(pos), torch.empty_like(vel)
+        seg = (ctypes.c_int64 * 3)()
+        self._check(self.lib.nf_regroup_plane(self._h, _ptr(pos), _ptr(vel), pos.shape[0], int(K), float(box), int(plane_cx),
+                                              _ptr(po), _ptr(vo), seg, self._stream(stream)), allow=() if strict else (NF_ERR_RANGE,))
+        return po, vo, [int(x) for x in seg]
+
+    def stream_step_regroup(self, seg_pos, seg_vel, P, K, R, eps, box, plane0, Gm, kick, drift, softening="spline",
+                            out_pos=None, out_vel=None, want_acc=False, stream=None, strict: bool = True):
+        """nf_stream_step_regroup.  seg_pos: P + 2R planes, each a list of up to 3 pinned float32 [n, 3]
+        segments (None or empty = nothing); seg_vel: the same for the P sink planes.  Returns (out_pos, out_vel:
+        P pinned tensors holding each sink plane's drifted particles as [to plane-1 | stay | to plane+1],
+        seg_n: P lists of 3 lengths, accelerations or None, stats)."""
+        NP = P + 2 * R
+        assert len(seg_pos) == NP and len(seg_vel) == P
+
+        def table(planes):
+            ptrs, ns = [], []
+            for segs in planes:
+                segs = list(segs) + [None] * (3 - len(segs))
+                assert len(segs) == 3
+                for t in segs:
+                    if t is None or t.shape[0] == 0:
+                        ptrs.append(None); ns.append(0)
+                        continue
+                    assert (not t.is_cuda) and t.dtype == torch.float32 and t.dim() == 2 and t.shape[1] == 3 and t.is_contiguous()
+                    assert t.is_pinned(), "plane segments must be pinned host memory"
+                    ptrs.append(t.data_ptr()); ns.append(t.shape[0])
+            return (ctypes.c_void_p * len(ptrs))(*ptrs), ns
+        pos_ptrs, pos_ns = table(seg_pos)
+        vel_ptrs, vel_ns = table(seg_vel)
+        assert vel_ns == pos_ns[3 * R:3 * (R + P)], "velocity segments must match the sink planes' position segments"
+        n_sink = [sum(pos_ns[3 * (R + p):3 * (R + p) + 3]) for p in range(P)]
+        mk = lambda: [torch.empty(n, 3, dtype=torch.float32).pin_memory() for n in n_sink]
+        out_pos = out_pos if out_pos is not None else mk()
+        out_vel = out_vel if out_vel is not None else mk()
+        acc = mk() if want_acc else None
+        for p in range(P):
+            assert out_pos[p].shape[0] >= n_sink[p] and out_vel[p].shape[0] >= n_sink[p]
+        tab = lambda ts: (ctypes.c_void_p * len(ts))(*[t.data_ptr() if t.shape[0] else None for t in ts])
+        ns = (ctypes.c_int64 * len(pos_ns))(*pos_ns)
+        out_n = (ctypes.c_int64 * (3 * P))()
+        stats = StreamStats()
+        self._check(self.lib.nf_stream_step_regroup(self._h, pos_ptrs, vel_ptrs, ns, int(P), int(K), int(R), float(eps), float(box),
+                                                    int(plane0), float(Gm), _SOFT[softening], float(kick), float(drift),
+                                                    tab(out_pos), tab(out_vel), out_n, tab(acc) if acc is not None else None,
+                                                    ctypes.byref(stats), self._stream(stream)),
+                    allow=() if strict else (NF_ERR_RANGE,))
+        seg_n = [[int(out_n[3 * p + k]) for k in range(3)] for p in range(P)]
+        return out_pos, out_vel, seg_n, acc, stats.as_dict()
 
 
 def spline_equivalent_eps(eps_plummer: float) -> float:

@@ -898,3 +898,125 @@ def test_forces_chunk_ranks_on_one_device(ctx, world, K, R):
     assert torch.equal(ctx.forces_chunk(b, R, cfg.eps, cfg.Gm, 0, K), ctx.forces(b, R, cfg.eps, cfg.Gm))
     with pytest.raises(Exception):
         ctx.forces_chunk(b, R, cfg.eps, cfg.Gm, 3, K + 1)
+
+
+# ------------------------------------------------- regrouping after the drift
+def _oracle_partition(x, v, K, box, plane_cx):
+    """Stable partition of one drifted plane by the ORACLE's cell assignment: [to plane-1 | stay | to plane+1]."""
+    keys, _ = oracle.keys(x, K, box)
+    rel = ((keys // (K * K)).astype(np.int64) - plane_cx) % K
+    seg = [np.nonzero(rel == (K - 1) % K)[0] if K > 2 else np.zeros(0, np.int64), np.nonzero(rel == 0)[0], np.nonzero(rel == 1)[0]]
+    if K <= 2:
+        seg[0] = np.zeros(0, np.int64)
+    order = np.concatenate(seg)
+    return x[order], v[order], [len(t) for t in seg], order
+
+
+@pytest.mark.parametrize("K,plane_cx,n", [(16, 5, 100_003), (8, 0, 40_000), (8, 7, 40_000), (37, 36, 9000), (3, 1, 5000), (12, 4, 0), (12, 4, 1)])
+def test_regroup_plane_bit_exact(ctx, K, plane_cx, n):
+    from paper_1810_02916_b200 import nf
+    rng = np.random.default_rng(K * 100 + plane_cx)
+    box = 500.0 if K == 16 else 3.0
+    w = box / K
+    x = np.empty((n, 3), np.float32)
+    x[:, 0] = np.mod((plane_cx + rng.uniform(-0.79, 1.79, n)) * w, box)
+    x[:, 1:] = rng.random((n, 2)) * box
+    if n > 100:                                                      # exactly on the plane's faces and one ulp either side
+        lo, hi = np.float32(plane_cx * w), np.float32(((plane_cx + 1) % K) * w)
+        x[:6, 0] = [lo, np.nextafter(lo, np.float32(-1)) % np.float32(box), np.nextafter(lo, np.float32(box)),
+                    hi, np.nextafter(hi, np.float32(-1)) % np.float32(box), np.nextafter(hi, np.float32(box))]
+    x = np.minimum(x, np.nextafter(np.float32(box), np.float32(0))).astype(np.float32)
+    v = rng.standard_normal((n, 3)).astype(np.float32)
+    ex, ev, en, _ = _oracle_partition(x, v, K, box, plane_cx)
+    po, vo, seg = ctx.regroup_plane(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda(), K, box, plane_cx)
+    assert seg == en and sum(seg) == n
+    assert np.array_equal(po.cpu().numpy().view(np.uint32), ex.view(np.uint32))
+    assert np.array_equal(vo.cpu().numpy().view(np.uint32), ev.view(np.uint32))
+    if n > 100 and K >= 5:
+        x[50, 0] = np.float32(((plane_cx + 2) % K + 0.5) * w)        # two planes away: time-step criterion 3 broken
+        with pytest.raises(nf.NFError) as e:
+            ctx.regroup_plane(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda(), K, box, plane_cx)
+        assert e.value.status == nf.NF_ERR_RANGE
+        po, vo, seg = ctx.regroup_plane(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda(), K, box, plane_cx, strict=False)
+        assert sum(seg) == n and torch.isfinite(po).all()            # no particle is lost: it is filed under the nearer neighbour
+
+
+def test_stream_two_steps_with_regroup(ctx):
+    """Two whole time steps of a periodic box through nf_stream_step_regroup (P = K: every plane is a sink, the
+    ghost planes are the sink planes of the other end passed again), the SECOND step fed directly from the
+    segments the first one wrote -- no host-side filing in between -- against two oracle steps (forces, kick,
+    drift, stable partition by the oracle's cell assignment)."""
+    cfg = inputs.scaled(inputs.config(3), 24_000, 8)
+    cfg = inputs.dataclasses.replace(cfg, n_halos=5)
+    K, R, box, P = cfg.K, cfg.R, cfg.box, cfg.K
+    w = box / K
+    pos = inputs.make_positions(cfg).numpy()
+    rng = np.random.default_rng(3)
+    vel = (rng.standard_normal(pos.shape) * 1.0).astype(np.float32)
+    keys, _ = oracle.keys(pos, K, box)
+    cx = (keys // (K * K)).astype(np.int64)
+    planes_x = [pos[cx == p] for p in range(K)]
+    planes_v = [vel[cx == p] for p in range(K)]
+    a0 = oracle.forces(pos, K, R, cfg.eps, box, cfg.Gm)
+    kick = 0.5 / np.sqrt((a0 ** 2).sum(axis=1)).max()
+    drift = 0.7 * w / (np.abs(vel).max() + 0.5)                       # the fastest particle moves ~0.7 cell widths
+
+    def oracle_step(px, pv):
+        allx = np.concatenate(px)
+        a = oracle.forces(allx, K, R, cfg.eps, box, cfg.Gm)
+        x1, v1 = oracle.kick_drift(allx, np.concatenate(pv), a.astype(np.float32), kick, drift, box)
+        starts = np.cumsum([0] + [t.shape[0] for t in px])
+        parts = [_oracle_partition(x1[starts[p]:starts[p + 1]], v1[starts[p]:starts[p + 1]], K, box, p) for p in range(K)]
+        nx, nv = [], []
+        for d in range(K):
+            segs = []
+            for src, k in (((d - 1) % K, 2), (d, 1), ((d + 1) % K, 0)):
+                ex, ev, en, _ = parts[src]
+                o = sum(en[:k])
+                segs.append((ex[o:o + en[k]], ev[o:o + en[k]]))
+            nx.append(np.concatenate([s[0] for s in segs]))
+            nv.append(np.concatenate([s[1] for s in segs]))
+        return nx, nv, [p[2] for p in parts], a
+
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    chunk = lambda seq: [seq[(q - R) % K] for q in range(P + 2 * R)]          # sink plane p is chunk plane R + p; ghosts wrap
+    # ---- step 1: whole planes as the middle segment
+    hx, hv = [pin(t) for t in planes_x], [pin(t) for t in planes_v]
+    seg_pos = chunk([[None, t, None] for t in hx])
+    seg_vel = [[None, t, None] for t in hv]
+    o_pos, o_vel, seg_n, acc, stats = ctx.stream_step_regroup(seg_pos, seg_vel, P, K, R, cfg.eps, box, -R, cfg.Gm, kick, drift, want_acc=True)
+    rx, rv, rn, ra = oracle_step(planes_x, planes_v)
+    assert seg_n == rn                                                          # the same particles crossed the same faces
+    assert sum(n[0] + n[2] for n in seg_n) > 0.1 * cfg.N                      # and many did
+    err = oracle.parity_error(torch.cat(acc).numpy(), ra)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
+
+    def new_plane_segments(out, n):
+        segs = []
+        for d in range(K):
+            s = []
+            for src, k in (((d - 1) % K, 2), (d, 1), ((d + 1) % K, 0)):
+                o = sum(n[src][:k])
+                s.append(out[src][o:o + n[src][k]])
+            segs.append(s)
+        return segs
+    # ---- step 2: straight from the segments step 1 wrote
+    sp2, sv2 = new_plane_segments(o_pos, seg_n), new_plane_segments(o_vel, seg_n)
+    for d in range(K):                                                          # they are the oracle's new planes, within the force rounding
+        gx = torch.cat(sp2[d]).numpy().astype(np.float64)
+        dxx = np.abs(gx - rx[d])
+        assert np.minimum(dxx, box - dxx).max() < 1e-3 * drift * kick * np.sqrt((ra ** 2).sum(axis=1)).max() + 1e-6 * box
+    o_pos2, o_vel2, seg_n2, acc2, stats2 = ctx.stream_step_regroup(chunk(sp2), sv2, P, K, R, cfg.eps, box, -R, cfg.Gm, kick, drift, want_acc=True)
+    rx2, rv2, rn2, ra2 = oracle_step(rx, rv)
+    assert stats2["out_of_range"] == 0 and stats2["particles_out"] == cfg.N
+    err2 = oracle.parity_error(torch.cat(acc2).numpy(), ra2)
+    assert np.median(err2) <= MEDIAN_TOL and err2.max() <= MAX_TOL
+    assert seg_n2 == rn2
+    sp3, sv3 = new_plane_segments(o_pos2, seg_n2), new_plane_segments(o_vel2, seg_n2)
+    amax = np.sqrt((ra2 ** 2).sum(axis=1)).max()
+    for d in range(K):
+        gx, gv = torch.cat(sp3[d]).numpy().astype(np.float64), torch.cat(sv3[d]).numpy().astype(np.float64)
+        assert gx.shape == rx2[d].shape
+        assert np.abs(gv - rv2[d]).max() <= 2 * MAX_TOL * kick * amax + 2e-6 * np.abs(rv2[d]).max()
+        dxx = np.abs(gx - rx2[d])
+        assert np.minimum(dxx, box - dxx).max() <= drift * (2 * MAX_TOL * kick * amax + 2e-6 * np.abs(rv2[d]).max()) + 2e-6 * box
