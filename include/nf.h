@@ -264,6 +264,27 @@ int nf_forces_host_m(nf_ctx *ctx, const float *pos_host, const float *mass_host,
                      float eps, float box, float Gm, int softening, float *acc_host, void *stream);
 int nf_reserve_host(nf_ctx *ctx, int64_t maxN, int K);
 
+/*
+ * nf_forces_host_begin / nf_forces_host_end -- nf_forces_host as a two-deep pipeline, for callers with a
+ * sequence of independent batches (or with step n+1's positions ready while step n is still running): the
+ * H2D copy of step n+1 and the D2H copy of step n run on the context's copy streams BEHIND the kernels of the
+ * step in between (PAPER.md:69 GPU work overlapped with the transfers; :111 the paper's rate "includes PCIe
+ * bus transfer overheads"), so a steady stream of steps runs at the speed of the kernels alone.
+ *
+ *   begin  enqueues one whole step (H2D, nf_bin, nf_forces, D2H into acc_host) and returns at once; at most
+ *          two steps may be in flight (a third begin is an NF_ERR_ARG).  pos_host and acc_host must be pinned
+ *          for the copies to be asynchronous, and must stay valid and untouched until the matching end.
+ *          Equal masses only.  N and K must not change while a step is in flight.
+ *   end    waits for the OLDEST step in flight (its accelerations are then in its acc_host) and returns its
+ *          status: NF_ERR_RANGE if positions outside [0, box) were clamped.
+ *
+ * Between a begin and its end no other call may be made on this context (the scratch arena is in use).
+ * Device memory: about 112 bytes per particle (input and output buffers doubled).
+ */
+int nf_forces_host_begin(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, float eps, float box,
+                         float Gm, int softening, float *acc_host, void *stream);
+int nf_forces_host_end(nf_ctx *ctx);
+
 /* Number of ordered (sink, source) pairs nf_forces evaluates for these cell counts:
  * I = sum_c n_c * sum_{c' in N(c)} n_c'  (self pairs included, padding excluded; the
  * "pairwise interactions" of PAPER.md:107).  Computed on the device, synchronises `stream`,

@@ -6,6 +6,32 @@
 
 static const char *const k_no_ctx = "nf: null context";
 
+struct HostPipe {                    // state of nf_forces_host_begin / _end
+    int active, next;                // steps in flight (0..2); buffer pair of the next begin
+    int64_t N;
+    int K;
+    size_t shared_at;                // arena offset where the part shared by all steps starts
+    float *raw[2], *acc[2];          // doubled input / output buffers (arena)
+    bool used[2];
+    cudaEvent_t ev_h2d[2], ev_raw_free[2], ev_done[2], ev_d2h[2];
+    unsigned long long *h_bad;       // pinned [2]: out-of-range count of each step
+};
+
+void nf_host_pipe_free(nf_ctx *ctx)
+{
+    HostPipe *hp = static_cast<HostPipe *>(ctx->host_pipe);
+    if (!hp) return;
+    for (int i = 0; i < 2; i++) {
+        if (hp->ev_h2d[i]) cudaEventDestroy(hp->ev_h2d[i]);
+        if (hp->ev_raw_free[i]) cudaEventDestroy(hp->ev_raw_free[i]);
+        if (hp->ev_done[i]) cudaEventDestroy(hp->ev_done[i]);
+        if (hp->ev_d2h[i]) cudaEventDestroy(hp->ev_d2h[i]);
+    }
+    if (hp->h_bad) cudaFreeHost(hp->h_bad);
+    delete hp;
+    ctx->host_pipe = nullptr;
+}
+
 int nf_scratch_reserve(nf_ctx *ctx, size_t bytes)
 {
     if (bytes <= ctx->scratch_bytes) return NF_OK;
@@ -79,6 +105,7 @@ int nf_destroy(nf_ctx *ctx)
     if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
     if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
     nf_slab_state_free(ctx);
+    nf_host_pipe_free(ctx);
     cudaGetLastError();
     delete ctx;
     return NF_OK;
@@ -298,6 +325,122 @@ int nf_forces_host_m(nf_ctx *ctx, const float *pos_host, const float *mass_host,
     NF_CUDA(ctx, cudaStreamSynchronize(st));
     if (ctx->h_counters[0]) {
         NF_SET_ERR(ctx, "%lld particle(s) outside [0, box) were clamped into edge cells", (long long)ctx->h_counters[0]);
+        return NF_ERR_RANGE;
+    }
+    return NF_OK;
+}
+
+// ---- pipelined host path: two steps in flight -----------------------------------------------------
+// Step s+1's H2D copy runs on the context's copy stream while step s computes, and step s's D2H copy runs
+// while step s+1 computes (PAPER.md:69: the GPU work is overlapped with the transfers; :111 the paper's
+// rate "includes PCIe bus transfer overheads").  Input and output buffers are doubled; everything else in
+// the scratch arena is shared, because the compute parts of consecutive steps are ordered on one stream.
+int nf_forces_host_begin(nf_ctx *ctx, const float *pos_host, int64_t N, int K, int R, float eps, float box, float Gm,
+                         int softening, float *acc_host, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_TRY(check_common(ctx, N, K, box));
+    NF_TRY(check_force_args(ctx, K, R, eps, Gm, softening));
+    NF_ARG(ctx, N > 0 && pos_host && acc_host, "nf_forces_host_begin: needs N > 0 and non-null host arrays");
+    NF_ARG(ctx, (softening & NF_MASS_W) == 0, "nf_forces_host_begin takes no masses");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    HostPipe *hp = static_cast<HostPipe *>(ctx->host_pipe);
+    if (!hp) {
+        hp = new (std::nothrow) HostPipe();
+        if (!hp) { NF_SET_ERR(ctx, "host allocation failed"); return NF_ERR_NOMEM; }
+        memset(hp, 0, sizeof(*hp));
+        ctx->host_pipe = hp;
+        for (int i = 0; i < 2; i++) {
+            NF_CUDA(ctx, cudaEventCreateWithFlags(&hp->ev_h2d[i], cudaEventDisableTiming));
+            NF_CUDA(ctx, cudaEventCreateWithFlags(&hp->ev_raw_free[i], cudaEventDisableTiming));
+            NF_CUDA(ctx, cudaEventCreateWithFlags(&hp->ev_done[i], cudaEventDisableTiming));
+            NF_CUDA(ctx, cudaEventCreateWithFlags(&hp->ev_d2h[i], cudaEventDisableTiming));
+        }
+        NF_CUDA(ctx, cudaMallocHost((void **)&hp->h_bad, 2 * sizeof(unsigned long long)));
+    }
+    NF_ARG(ctx, hp->active < 2, "nf_forces_host_begin: two steps are already in flight (call nf_forces_host_end)");
+    const size_t n = (size_t)N, ncell = (size_t)K * K * K;
+    if (hp->active == 0) {
+        // doubled input / output + sorted, perm, cells, the two encoded copies + the larger of the binning scratch
+        // and the work list (the work list overlays the binning scratch: same stream, binning is done by then)
+        nf_force_params fp{};
+        fp.K = K; fp.n_planes = K; fp.sink_lo = 0; fp.sink_hi = K; fp.max_sinks = N;
+        const size_t wl = nf_forces_scratch_bytes(fp), bs = nf_bin_scratch_bytes(N, K, false);
+        const size_t need = 4 * nf_align_up(n * 12, 256) + 3 * nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
+                            nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256) + (wl > bs ? wl : bs) + 8192;
+        NF_TRY(nf_scratch_reserve(ctx, need));
+        nf_scratch_reset(ctx);
+        for (int i = 0; i < 2; i++) {
+            hp->raw[i] = nf_scratch_take<float>(ctx, n * 3);
+            hp->acc[i] = nf_scratch_take<float>(ctx, n * 3);
+            hp->used[i] = false;
+        }
+        hp->shared_at = ctx->scratch_used;
+        hp->N = N; hp->K = K; hp->next = 0;
+        if (!hp->raw[1] || !hp->acc[1]) { NF_SET_ERR(ctx, "nf_forces_host_begin: internal scratch arena too small"); return NF_ERR_NOMEM; }
+    } else {
+        NF_ARG(ctx, hp->N == N && hp->K == K, "nf_forces_host_begin: N and K must not change while a step is in flight");
+    }
+    const int i = hp->next;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the shared part of the arena, carved the same way every step
+    ctx->scratch_used = hp->shared_at;
+    float *sorted = nf_scratch_take<float>(ctx, n * 4);
+    uint32_t *perm = nf_scratch_take<uint32_t>(ctx, n);
+    uint32_t *count = nf_scratch_take<uint32_t>(ctx, ncell);
+    uint64_t *off = nf_scratch_take<uint64_t>(ctx, ncell + 1);
+    nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
+    float4 *enc = nf_scratch_take<float4>(ctx, n);
+    float4 *enc_h = nf_scratch_take<float4>(ctx, n);
+    if (!sorted || !perm || !count || !off || !d_planes || !enc || !enc_h) {
+        NF_SET_ERR(ctx, "nf_forces_host_begin: internal scratch arena too small");
+        return NF_ERR_NOMEM;
+    }
+    // H2D on the copy stream, as soon as the binning that last read this input buffer is done
+    if (hp->used[i]) NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, hp->ev_raw_free[i], 0));
+    else {                                         // first use: order after prior work on the caller's stream
+        NF_CUDA(ctx, cudaEventRecord(hp->ev_raw_free[i], st));
+        NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_h2d, hp->ev_raw_free[i], 0));
+    }
+    NF_CUDA(ctx, cudaMemcpyAsync(hp->raw[i], pos_host, n * 12, cudaMemcpyHostToDevice, ctx->s_h2d));
+    NF_CUDA(ctx, cudaEventRecord(hp->ev_h2d[i], ctx->s_h2d));
+    // compute on the caller's stream
+    NF_CUDA(ctx, cudaStreamWaitEvent(st, hp->ev_h2d[i], 0));
+    if (hp->used[i]) NF_CUDA(ctx, cudaStreamWaitEvent(st, hp->ev_d2h[i], 0));     // acc[i] has been copied out
+    NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, sizeof(unsigned long long), st));
+    const size_t mark = ctx->scratch_used;
+    NF_TRY(nf_bin_impl(ctx, hp->raw[i], nullptr, N, K, box, -1, sorted, perm, count, off, st));
+    NF_CUDA(ctx, cudaEventRecord(hp->ev_raw_free[i], st));
+    ctx->scratch_used = mark;                       // the work list may overlay the binning scratch
+    nf_force_params p{};
+    p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
+    p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
+    NF_TRY(nf_encode_impl(ctx, p, reinterpret_cast<const float4 *>(sorted), off, ncell, enc, enc_h, st));
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, hp->acc[i], nullptr, st));
+    NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
+    NF_CUDA(ctx, cudaMemcpyAsync(hp->h_bad + i, ctx->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    NF_CUDA(ctx, cudaEventRecord(hp->ev_done[i], st));
+    // D2H on the other copy stream
+    NF_CUDA(ctx, cudaStreamWaitEvent(ctx->s_d2h, hp->ev_done[i], 0));
+    NF_CUDA(ctx, cudaMemcpyAsync(acc_host, hp->acc[i], n * 12, cudaMemcpyDeviceToHost, ctx->s_d2h));
+    NF_CUDA(ctx, cudaEventRecord(hp->ev_d2h[i], ctx->s_d2h));
+    hp->used[i] = true;
+    hp->next = i ^ 1;
+    hp->active++;
+    return NF_OK;
+}
+
+int nf_forces_host_end(nf_ctx *ctx)
+{
+    if (!ctx) return NF_ERR_ARG;
+    HostPipe *hp = static_cast<HostPipe *>(ctx->host_pipe);
+    NF_ARG(ctx, hp && hp->active > 0, "nf_forces_host_end: no step in flight");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    const int j = hp->active == 2 ? hp->next : (hp->next ^ 1);      // the oldest step in flight
+    NF_CUDA(ctx, cudaEventSynchronize(hp->ev_d2h[j]));
+    hp->active--;
+    if (hp->h_bad[j]) {
+        NF_SET_ERR(ctx, "%lld particle(s) outside [0, box) were clamped into edge cells", (long long)hp->h_bad[j]);
         return NF_ERR_RANGE;
     }
     return NF_OK;

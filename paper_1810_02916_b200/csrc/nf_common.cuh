@@ -28,6 +28,7 @@ struct nf_ctx {
     // slab streaming resources (created lazily)
     cudaStream_t s_h2d, s_d2h;
     void *slab_state;
+    void *host_pipe;     // nf_forces_host_begin / _end (created lazily)
 };
 
 #define NF_SET_ERR(ctx, ...)                                        \
@@ -133,6 +134,7 @@ int nf_forces_init(nf_ctx *ctx);
 // ordered pairs evaluated for the sink planes of a plane table (device result added to ctx->counters[1])
 int nf_interactions_planes(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d_planes, cudaStream_t st);
 void nf_slab_state_free(nf_ctx *ctx);
+void nf_host_pipe_free(nf_ctx *ctx);
 // kick + drift launcher (nf_step.cu), also the epilogue of nf_stream_step_slabs
 int nf_kick_drift_impl(nf_ctx *ctx, float *pos, float *vel, const float *acc, int64_t N, float kick, float drift, float box,
                        cudaStream_t st);

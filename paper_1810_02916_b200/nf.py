@@ -26,7 +26,8 @@ EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve
            "nf_out_of_range", "nf_forces", "nf_interactions", "nf_spline_equivalent_eps",
            "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host",
            "nf_bin_m", "nf_forces_ex", "nf_kick_drift", "nf_cell_vrms", "nf_stream_step_slabs",
-           "nf_keys", "nf_forces_chunk", "nf_forces_host_m", "nf_regroup_plane", "nf_stream_step_regroup"]
+           "nf_keys", "nf_forces_chunk", "nf_forces_host_m", "nf_regroup_plane", "nf_stream_step_regroup",
+           "nf_forces_host_begin", "nf_forces_host_end"]
 
 
 class NFError(RuntimeError):
@@ -109,6 +110,10 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.nf_stream_step_regroup.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64), i32, i32, i32, f32, f32,
                                            i32, f32, i32, f32, f32, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64),
                                            ctypes.POINTER(vp), ctypes.POINTER(StreamStats), vp]
+    lib.nf_forces_host_begin.restype = i32
+    lib.nf_forces_host_begin.argtypes = [vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp]
+    lib.nf_forces_host_end.restype = i32
+    lib.nf_forces_host_end.argtypes = [vp]
     lib.nf_keys.restype = i32
     lib.nf_keys.argtypes = [vp, vp, i64, i32, f32, vp, vp]
     lib.nf_forces_chunk.restype = i32
@@ -288,6 +293,20 @@ class Context:
         self._check(self.lib.nf_forces_host(self._h, _ptr(pos_host), N, int(K), int(R), float(eps), float(box),
                                             float(Gm), _SOFT[softening], _ptr(out), self._stream(stream)), allow=allow)
         return out
+
+    def forces_host_begin(self, pos_host: torch.Tensor, K: int, R: int, eps: float, box: float, Gm: float, out: torch.Tensor,
+                          softening: str = "spline", stream=None):
+        """nf_forces_host_begin: enqueue one whole step from pinned host positions into the pinned host tensor
+        ``out``; returns at once (at most two steps in flight).  Pair with forces_host_end()."""
+        for t in (pos_host, out):
+            assert (not t.is_cuda) and t.dtype == torch.float32 and t.dim() == 2 and t.shape[1] == 3 and t.is_contiguous() and t.is_pinned()
+        assert out.shape == pos_host.shape
+        self._check(self.lib.nf_forces_host_begin(self._h, _ptr(pos_host), pos_host.shape[0], int(K), int(R), float(eps), float(box),
+                                                  float(Gm), _SOFT[softening], _ptr(out), self._stream(stream)))
+
+    def forces_host_end(self, strict: bool = False):
+        """nf_forces_host_end: wait for the oldest step in flight; its ``out`` tensor is then complete."""
+        return self._check(self.lib.nf_forces_host_end(self._h), allow=() if strict else (NF_ERR_RANGE,))
 
     def interactions(self, b: Binned, R: int, stream=None) -> int:
         n = ctypes.c_int64(0)

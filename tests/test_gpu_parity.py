@@ -1020,3 +1020,38 @@ def test_stream_two_steps_with_regroup(ctx):
         assert np.abs(gv - rv2[d]).max() <= 2 * MAX_TOL * kick * amax + 2e-6 * np.abs(rv2[d]).max()
         dxx = np.abs(gx - rx2[d])
         assert np.minimum(dxx, box - dxx).max() <= drift * (2 * MAX_TOL * kick * amax + 2e-6 * np.abs(rv2[d]).max()) + 2e-6 * box
+
+
+def test_forces_host_pipeline(ctx):
+    """nf_forces_host_begin / _end: five independent batches through the two-deep pipeline give, batch by batch,
+    the bits nf_forces_host gives; a third begin and an end with nothing in flight are refused; an out-of-range
+    batch reports NF_ERR_RANGE at ITS end and does not disturb its neighbours."""
+    from paper_1810_02916_b200 import nf
+    K, R, box, n = 12, 2, 4.0, 30_000
+    rng = np.random.default_rng(8)
+    batches = [torch.from_numpy((rng.random((n, 3)) * box).astype(np.float32)).pin_memory() for _ in range(5)]
+    batches[3][7, 1] = box * 1.25                                       # batch 3 holds a particle outside the box
+    ref = [ctx.forces_host(b, K, R, 0.01, box, 1.0 / n).clone() for b in batches]
+    outs = [torch.empty(n, 3).pin_memory() for _ in batches]
+    with pytest.raises(nf.NFError):
+        ctx.forces_host_end()
+    status = []
+    ctx.forces_host_begin(batches[0], K, R, 0.01, box, 1.0 / n, outs[0])
+    ctx.forces_host_begin(batches[1], K, R, 0.01, box, 1.0 / n, outs[1])
+    with pytest.raises(nf.NFError) as e:
+        ctx.forces_host_begin(batches[2], K, R, 0.01, box, 1.0 / n, outs[2])
+    assert e.value.status == nf.NF_ERR_ARG
+    for s in range(2, 5):
+        status.append(ctx.forces_host_end())
+        ctx.forces_host_begin(batches[s], K, R, 0.01, box, 1.0 / n, outs[s])
+    status.append(ctx.forces_host_end())
+    status.append(ctx.forces_host_end())
+    assert status == [nf.NF_OK, nf.NF_OK, nf.NF_OK, nf.NF_ERR_RANGE, nf.NF_OK]
+    for s in range(5):
+        assert torch.equal(outs[s], ref[s]), s
+    a_ref = oracle.forces(batches[4].numpy(), K, R, 0.01, box, 1.0 / n)
+    err = oracle.parity_error(outs[4].numpy(), a_ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
+    # the context is usable for ordinary calls again
+    b = ctx.bin(batches[0].cuda(), K, box)
+    assert torch.equal(ctx.forces(b, R, 0.01, 1.0 / n).cpu(), ref[0])
