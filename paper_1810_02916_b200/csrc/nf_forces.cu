@@ -359,13 +359,34 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
 
         // which of the two encoded copies: the one whose z-blocks do not cut cz-R..cz+R (if any)
         const int zphi = ((cz - R + ZB * 4) / ZB != (cz + R + ZB * 4) / ZB) ? ZB / 2 : 0;
-        // ---- piece table: lane r builds the pieces of column r ----
         if (lane < W) {
             int px = sink_plane + lane - R;
             if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
             else if (px < 0 || px >= p.n_planes) px = -1;
             S.enc[lane] = px >= 0 ? (zphi ? planes[px].enc_h : planes[px].enc) : nullptr;
         }
+        // ---- the lane's four sinks (slots past n repeat the last sink; they are never written) ----
+        u64 xi[2], yi[2], zi[2];
+        unsigned near = 0;
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+            const int j0 = min(4 * sl + 2 * h, n - 1), j1 = min(4 * sl + 2 * h + 1, n - 1);
+            const float4 *se = zphi ? sp.enc_h : sp.enc;
+            const float4 m0 = se[s0 + j0], m1 = se[s0 + j1];
+            // (x - 0 through the packed adder: the pair is born in an aligned register pair, so the per-tile
+            // shifts below need no moves to assemble their 64-bit operands)
+            xi[h] = sub2(pk(m0.x, m1.x), 0ull); yi[h] = sub2(pk(m0.y, m1.y), 0ull); zi[h] = sub2(pk(m0.z, m1.z), 0ull);
+            // which faces of the own cell does a sink of this task come within eps of?  (bit 0/1: x-/x+,
+            // 2/3: y-/y+, 4/5: z-/z+.)  Only then can a source of the cell beyond that face be inside eps.
+            const float ezs = ((float)((cz + zphi) % ZB) - 0.5f * (float)(ZB - 1)) * fc.ws;
+            const float lo = fc.near_lo, hi = -fc.near_lo;
+            const float z0 = m0.z - ezs, z1 = m1.z - ezs;
+            near |= (fminf(m0.x, m1.x) < lo ? 1u : 0u) | (fmaxf(m0.x, m1.x) > hi ? 2u : 0u) |
+                    (fminf(m0.y, m1.y) < lo ? 4u : 0u) | (fmaxf(m0.y, m1.y) > hi ? 8u : 0u) |
+                    (fminf(z0, z1) < lo ? 16u : 0u) | (fmaxf(z0, z1) > hi ? 32u : 0u);
+        }
+        near = __reduce_or_sync(0xffffffffu, near);
+        // ---- piece table: lane r builds the pieces of column r ----
         int n_pieces = 0;
         for (int rb = 0; rb < NR; rb += 32) {
             const int r = rb + lane;
@@ -406,14 +427,28 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             }
             int slot = n_pieces + incl - np - 1;
             if (r < NR) {
+                // Which law the tiles of a piece need (bits 27-28 of meta).  The sinks' own cell holds every
+                // sink as a source (r = 0), which would always trip the close-pair test: it takes the min form
+                // (0) directly.  Columns two or more cells away in x or y cannot hold a pair inside eps
+                // (FC_FAR_OK), and Plummer has no second branch: nothing to track (2).  An adjacent column
+                // (or the own column above / below the own cell): a pair inside eps needs a sink within eps of
+                // every face that separates the own cell from the piece's cells; else nothing to track either.
+                const int ddx = dxi - R, ddy = dyi - R;
+                const unsigned need_xy = (ddx < 0 ? 1u : 0u) | (ddx > 0 ? 2u : 0u) | (ddy < 0 ? 4u : 0u) | (ddy > 0 ? 8u : 0u);
+                const bool far_col = (fc.flags & FC_FAR_OK) && max(abs(ddx), abs(ddy)) >= 2;
 #pragma unroll
                 for (int s = 0; s < W; s++) {
                     if (cn[s] == 0) continue;
                     if (newp[s]) {
                         slot++;
-                        // bit 24: the sinks' own cell; bits 25 / 26: a piece of the own column below / above it
-                        const uint32_t self = col != NR / 2 ? 0u : (s == R ? 1u << 24 : (s < R ? 1u << 25 : 1u << 26));
-                        S.piece[slot] = make_uint4(st[s], cn[s], (uint32_t)col | ((uint32_t)(kz[s] + 128) << 8) | ((uint32_t)dxi << 16) | self, 0u);
+                        const bool own_col = col == NR / 2;
+                        const unsigned need = need_xy | (own_col && s < R ? 16u : 0u) | (own_col && s > R ? 32u : 0u);
+                        uint32_t mode = 1u;
+                        if (fc.flags & FC_PLUMMER) mode = 2u;
+                        else if (own_col && s == R) mode = 0u;
+                        else if (far_col) mode = 2u;
+                        else if ((near & need) != need) mode = 2u;
+                        S.piece[slot] = make_uint4(st[s], cn[s], (uint32_t)col | ((uint32_t)(kz[s] + 128) << 8) | ((uint32_t)dxi << 16) | (mode << 27), 0u);
                     } else {
                         S.piece[slot].y += cn[s];
                     }
@@ -421,26 +456,6 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             }
             n_pieces += __shfl_sync(0xffffffffu, incl, 31);
         }
-
-        // ---- the lane's four sinks (slots past n repeat the last sink; they are never written) ----
-        u64 xi[2], yi[2], zi[2];
-        unsigned near = 0;
-#pragma unroll
-        for (int h = 0; h < 2; h++) {
-            const int j0 = min(4 * sl + 2 * h, n - 1), j1 = min(4 * sl + 2 * h + 1, n - 1);
-            const float4 *se = zphi ? sp.enc_h : sp.enc;
-            const float4 m0 = se[s0 + j0], m1 = se[s0 + j1];
-            xi[h] = pk(m0.x, m1.x); yi[h] = pk(m0.y, m1.y); zi[h] = pk(m0.z, m1.z);
-            // which faces of the own cell does a sink of this task come within eps of?  (bit 0/1: x-/x+,
-            // 2/3: y-/y+, 4/5: z-/z+.)  Only then can a source of the cell beyond that face be inside eps.
-            const float ezs = ((float)((cz + zphi) % ZB) - 0.5f * (float)(ZB - 1)) * fc.ws;
-            const float lo = fc.near_lo, hi = -fc.near_lo;
-            const float z0 = m0.z - ezs, z1 = m1.z - ezs;
-            near |= (fminf(m0.x, m1.x) < lo ? 1u : 0u) | (fmaxf(m0.x, m1.x) > hi ? 2u : 0u) |
-                    (fminf(m0.y, m1.y) < lo ? 4u : 0u) | (fmaxf(m0.y, m1.y) > hi ? 8u : 0u) |
-                    (fminf(z0, z1) < lo ? 16u : 0u) | (fmaxf(z0, z1) > hi ? 32u : 0u);
-        }
-        near = __reduce_or_sync(0xffffffffu, near);
         __syncwarp();
 
         // balanced tile length of every piece (no division on the per-tile path)
@@ -502,40 +517,36 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k_forces_warp(const nf_plane_vi
             mbar_wait(b ? bar1 : bar0, (parity >> b) & 1u);
             parity ^= 1u << b;
             __syncwarp();
-            u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
-            float rmin = 3.0e38f;
             const float4 *src = buf + ph * q;
-            // Which law the tile needs (warp-uniform).  The sinks' own cell holds every sink as a source
-            // (r = 0), which would always trip the close-pair test: it takes the min form directly, as
-            // does the rest of a column after a hit.  Columns two or more cells away in x or y cannot
-            // hold a pair inside eps (FC_FAR_OK), and Plummer has no second branch: nothing to track.
-            int mode = 1;
-            if (fc.flags & FC_PLUMMER) mode = 2;
-            else if (sticky_col == col || ((d0.meta >> 24) & 1u) != 0) mode = 0;
-            else if ((fc.flags & FC_FAR_OK) && max(abs(dxi - R), abs(dyi - R)) >= 2) mode = 2;
-            else {
-                // an adjacent column: a pair inside eps needs a sink within eps of every face that
-                // separates the own cell from the piece's cells
-                const int ddx = dxi - R, ddy = dyi - R;
-                unsigned need = (ddx < 0 ? 1u : 0u) | (ddx > 0 ? 2u : 0u) | (ddy < 0 ? 4u : 0u) | (ddy > 0 ? 8u : 0u) |
-                                ((d0.meta >> 25) & 1u ? 16u : 0u) | ((d0.meta >> 26) & 1u ? 32u : 0u);
-                if ((near & need) != need) mode = 2;
-            }
-            if (active) {
-                if (mode == 1) sweep<1, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-                else if (mode == 2) sweep<2, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-                else sweep<0, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-            }
-            if (mode == 1 && __any_sync(0xffffffffu, rmin < fc.eps2_test)) {
-                sticky_col = col;
-                ax[0] = ax[1] = ay[0] = ay[1] = az[0] = az[1] = 0;
-                if (active) sweep<0, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-            }
+            // The law the tile needs was decided when its piece was built (bits 27-28 of meta); the only
+            // run-time change: after a tile of a column really held a pair inside eps, the rest of that
+            // column takes the min form directly.  Every path forms the tile's sums from zero in its own
+            // registers and adds them to the running sums.
+            int mode = (int)((d0.meta >> 27) & 3u);
+            if (mode == 1 && sticky_col == col) mode = 0;
+            if (mode == 2) {
+                u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
+                float rmin = 0.f;
+                if (active) sweep<2, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
 #pragma unroll
-            for (int h = 0; h < 2; h++) {
-                gx[h] = add2(gx[h], ax[h]);
-                gy[h] = add2(gy[h], ay[h]);
-                gz[h] = add2(gz[h], az[h]);
+                for (int h = 0; h < 2; h++) { gx[h] = add2(gx[h], ax[h]); gy[h] = add2(gy[h], ay[h]); gz[h] = add2(gz[h], az[h]); }
+            } else if (mode == 0) {
+                u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
+                float rmin = 0.f;
+                if (active) sweep<0, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+#pragma unroll
+                for (int h = 0; h < 2; h++) { gx[h] = add2(gx[h], ax[h]); gy[h] = add2(gy[h], ay[h]); gz[h] = add2(gz[h], az[h]); }
+            } else {
+                u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
+                float rmin = 3.0e38f;
+                if (active) sweep<1, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                if (__any_sync(0xffffffffu, rmin < fc.eps2_test)) {        // a pair inside eps: redo with the min form
+                    sticky_col = col;
+                    ax[0] = ax[1] = ay[0] = ay[1] = az[0] = az[1] = 0;
+                    if (active) sweep<0, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                }
+#pragma unroll
+                for (int h = 0; h < 2; h++) { gx[h] = add2(gx[h], ax[h]); gy[h] = add2(gy[h], ay[h]); gz[h] = add2(gz[h], az[h]); }
             }
             // every lane is done with buf; each lane orders its own generic-proxy accesses to it (the
             // sentinel stores, the sweep's loads) before the bulk copy that refills it (async proxy)
