@@ -231,7 +231,9 @@ struct Task {
     uint32_t cyz;     // cell index within the plane, cy*K + cz
     uint32_t first;   // first sink of the task within the cell
     uint16_t plane;   // sink plane (index into the plane table)
-    uint16_t L;       // lanes holding sinks (1..32); the task covers min(4L, n - first) sinks
+    uint8_t L;        // lanes holding sinks (1..32); the task covers min(4L, n - first) sinks
+    uint8_t nparts;   // the task's tiles are shared between nparts entries of the work list (1: not split) ...
+    uint32_t part_slot;   // ... of which this is part (bits 0-7); bits 8-31: first partial-sum slot of the group
 };
 
 struct SplitTable {
@@ -255,7 +257,7 @@ __global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restr
     tc[nc + c] = heavy ? 0u : nt;
 }
 
-// ctl[0] = work cursor (zeroed here), ctl[1] = number of tasks
+// ctl[0] = work cursor (zeroed here), ctl[1] = number of entries of the work list the kernel reads, ctl[2] = number of tasks
 __global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restrict__ planes, const uint32_t *__restrict__ tc,
                                                    const uint32_t *__restrict__ to, nf_force_params p, int small,
                                                    Task *__restrict__ tasks, uint32_t *__restrict__ ctl)
@@ -269,6 +271,8 @@ __global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restri
     const size_t e = n >= HEAVY_N ? c : nc + c;
     uint32_t o = to[e];
     Task t;
+    t.nparts = 1;
+    t.part_slot = 0;
     t.cyz = (uint32_t)cyz;
     t.plane = (uint16_t)(p.sink_lo + blockIdx.y);
     uint32_t first = 0;
@@ -281,14 +285,94 @@ __global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restri
     const int rem = (int)(n & 127);
     for (int k = 0; k < c_split[small].nt[rem]; k++) {
         t.first = first;
-        t.L = c_split[small].L[rem][k];
+        t.L = (uint8_t)c_split[small].L[rem][k];
         tasks[o++] = t;
         first += 4u * t.L;
     }
     if (cyz == KK - 1 && blockIdx.y == gridDim.y - 1) {
         ctl[0] = 0;
-        ctl[1] = to[2 * nc - 1] + tc[2 * nc - 1];
+        ctl[1] = ctl[2] = to[2 * nc - 1] + tc[2 * nc - 1];
+        ctl[4] = ctl[5] = ctl[6] = 0;
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// Source split for problems with FEW, LONG tasks (one cell of 4x10^5 particles is ~3000 tasks of ~900
+// tiles each for 1776 consumer warps: without it the last wave runs three-quarters empty).  When the work
+// list is shorter than SPLIT_TARGET entries, a task whose source count S exceeds the fair share
+// max(sum S / SPLIT_TARGET, SPLIT_MIN_SRC) becomes nparts entries that take every nparts-th tile of
+// the task's tile sequence; each part leaves its float32 sums in a slot of a partial-sum buffer and the
+// part that arrives last adds the slots IN PART ORDER (double), scales and writes -- deterministic
+// whichever part that is.  Large problems (C2-C5) never split: the pass is not even launched for them.
+// ------------------------------------------------------------------------------------------
+constexpr uint32_t SPLIT_MIN_SRC = 8192;          // a part sweeps at least this many sources (~20 tiles)
+constexpr uint32_t SPLIT_MAX_PARTS = 255;
+
+// ctl[0] work cursor, ctl[1] number of entries, ctl[2] entries of the unsplit list, ctl[4..5] sum of S (u64), ctl[6] slot cursor
+template <int R>
+__global__ void __launch_bounds__(256) k_split_measure(const nf_plane_view *__restrict__ planes, nf_force_params p,
+                                                       const Task *__restrict__ tasks, uint32_t *__restrict__ ctl,
+                                                       uint32_t split_target, uint32_t *__restrict__ src_count)
+{
+    const uint32_t n_tasks = ctl[2];
+    if (n_tasks >= split_target) return;
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long S = 0;
+    if (i < n_tasks) {
+        const Task t = tasks[i];
+        const int K = p.K;
+        const int cy = (int)(t.cyz / (uint32_t)K), cz = (int)(t.cyz % (uint32_t)K);
+        for (int dx = -R; dx <= R; dx++) {
+            int px = (int)t.plane + dx;
+            if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
+            else if (px < 0 || px >= p.n_planes) continue;
+            const uint64_t *off = planes[px].off;
+            for (int dy = -R; dy <= R; dy++) {
+                const int qy = ((cy + dy) % K + K) % K;
+                for (int dz = -R; dz <= R; dz++) {
+                    const int qz = ((cz + dz) % K + K) % K;
+                    S += off[qy * K + qz + 1] - off[qy * K + qz];
+                }
+            }
+        }
+        src_count[i] = (uint32_t)min(S, 0xffffffffull);
+    }
+    for (int d = 16; d > 0; d >>= 1) S += __shfl_down_sync(0xffffffffu, S, d);
+    if ((threadIdx.x & 31) == 0 && S) atomicAdd(reinterpret_cast<unsigned long long *>(ctl + 4), S);   // integer: order-independent
+}
+
+__global__ void __launch_bounds__(256) k_split_parts(const uint32_t *__restrict__ ctl, uint32_t split_target,
+                                                     const uint32_t *__restrict__ src_count, uint32_t *__restrict__ parts, uint32_t n_max)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_max) return;
+    const uint32_t n_tasks = ctl[2];
+    uint32_t np = i < n_tasks ? 1u : 0u;
+    if (i < n_tasks && n_tasks < split_target) {
+        const unsigned long long total = *reinterpret_cast<const unsigned long long *>(ctl + 4);
+        const unsigned long long share = max(total / split_target, (unsigned long long)SPLIT_MIN_SRC);
+        np = (uint32_t)min((unsigned long long)SPLIT_MAX_PARTS, max(1ull, (src_count[i] + share / 2) / share));
+    }
+    parts[i] = np;
+}
+
+__global__ void __launch_bounds__(256) k_split_fill(const Task *__restrict__ tasks, const uint32_t *__restrict__ parts,
+                                                    const uint32_t *__restrict__ parts_off, uint32_t *__restrict__ ctl,
+                                                    Task *__restrict__ tasks2, uint32_t n_max)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t n_tasks = ctl[2];
+    if (i >= n_tasks) return;
+    Task t = tasks[i];
+    const uint32_t np = parts[i], o = parts_off[i];
+    uint32_t slot = 0;
+    if (np > 1) slot = atomicAdd(&ctl[6], np);      // which slots a group gets does not influence any result
+    t.nparts = (uint8_t)np;
+    for (uint32_t k = 0; k < np; k++) {
+        t.part_slot = k | (slot << 8);
+        tasks2[o + k] = t;
+    }
+    if (i == n_tasks - 1) ctl[1] = o + np;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -343,7 +427,8 @@ struct TaskHdr {                            // what a consumer needs to know abo
     const uint32_t *perm;
     float *amax;
     uint64_t s0;                            // first sink (slot in the plane's arrays)
-    uint32_t n, L, cyz, pad;
+    uint32_t n, L, cyz;
+    uint32_t part, nparts, slot;                // source split: this entry is part `part` of `nparts`, partial sums in slots slot..slot+nparts-1
 };
 
 template <int R>
@@ -351,12 +436,12 @@ struct ConsShared {
     static constexpr int W = 2 * R + 1, NR = W * W, TILE_CAP = tile_cap(R), PIECE_CAP = piece_cap(R);
     float4 buf[2][TILE_CAP];
     uint4 piece[PIECE_CAP];                 // x: first particle, y: count, z: meta, w: balanced tile length   (producer's)
-    uint4 desc[2];                          // per buffer: x = tn | q << 16, y = meta | flags, z = header slot
+    uint4 desc[2];                          // per buffer: x = tn | q << 16, y = meta | flags
     TaskHdr hdr[2];
     const float4 *enc[W];                   // encoded positions of the W source planes (by dx + R; null = outside the chunk)
     unsigned long long full[2], empty[2];
     // producer's cursor for this consumer
-    uint32_t p_npieces, p_cur_piece, p_cur_off, p_P, p_invP, p_seq, p_state;   // p_state 0: inside a task, 1: next tile starts a task, 2: stop
+    uint32_t p_npieces, p_cur_piece, p_j, p_nparts, p_P, p_invP, p_seq, p_state;   // p_state 0: inside a task, 1: next tile starts a task, 2: stop
 };
 
 // ---- producer: everything about task ti that does not need the FMA pipe -------------------------------
@@ -387,7 +472,8 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
     if (lane == 0) {
         TaskHdr h;
         h.se = se; h.acc = sp.acc; h.perm = sp.perm; h.amax = sp.amax; h.s0 = s0;
-        h.n = (uint32_t)n; h.L = (uint32_t)L; h.cyz = task.cyz; h.pad = 0;
+        h.n = (uint32_t)n; h.L = (uint32_t)L; h.cyz = task.cyz;
+        h.part = task.part_slot & 0xffu; h.nparts = task.nparts; h.slot = task.part_slot >> 8;
         S.hdr[seq & 1u] = h;
         S.p_P = (uint32_t)P;
         S.p_invP = (65536u + P - 1) / P;        // floor(x / P) == (x * inv_P) >> 16 for x < 1024
@@ -484,7 +570,18 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
         const uint32_t nt = (cnt + tile_max - 1) / tile_max;
         S.piece[i].w = (cnt + nt - 1) / nt;
     }
-    if (lane == 0) { S.p_npieces = (uint32_t)n_pieces; S.p_cur_piece = 0; S.p_cur_off = 0; }
+    __syncwarp();
+    // the entry's first tile: tile number `part` of the task's tile sequence (every nparts-th tile is its own)
+    uint32_t cp = 0, j = task.part_slot & 0xffu;
+    while (cp < (uint32_t)n_pieces) {
+        const uint4 pc = S.piece[cp];
+        const uint32_t nt = (pc.y + pc.w - 1) / pc.w;
+        if (j < nt) break;
+        j -= nt;
+        cp++;
+    }
+    __syncwarp();
+    if (lane == 0) { S.p_npieces = (uint32_t)n_pieces; S.p_cur_piece = cp; S.p_j = j; S.p_nparts = task.nparts; }
     __syncwarp();
 }
 
@@ -527,12 +624,25 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
         return false;
     }
     uint32_t flags = state == 1u ? (D_FIRST | (((S.p_seq - 1u) & 1u) << 26)) : 0u;      // bit 26: header slot
-    const uint32_t cur_piece = S.p_cur_piece, cur_off = S.p_cur_off;
+    const uint32_t cur_piece = S.p_cur_piece, cur_j = S.p_j, n_pieces = S.p_npieces;
     const uint4 pc = S.piece[cur_piece];
-    const uint32_t start = pc.x + cur_off;
-    const uint32_t tn = min(pc.w, pc.y - cur_off);
-    const bool piece_done = cur_off + tn >= pc.y;
-    const bool last = piece_done && cur_piece + 1 >= S.p_npieces;
+    const uint32_t start = pc.x + cur_j * pc.w;
+    const uint32_t tn = min(pc.w, pc.y - cur_j * pc.w);
+    // the entry's next tile: nparts tiles further along the task's tile sequence
+    const uint32_t nparts = S.p_nparts;
+    uint32_t np = cur_piece, nj = cur_j + nparts;
+    if (nparts == 1) {                          // not split (the usual case): no division
+        if (nj * pc.w >= pc.y) { np++; nj = 0; }
+    } else {
+        while (np < n_pieces) {
+            const uint4 qc = S.piece[np];
+            const uint32_t nt = (qc.y + qc.w - 1) / qc.w;
+            if (nj < nt) break;
+            nj -= nt;
+            np++;
+        }
+    }
+    const bool last = np >= n_pieces;
     if (last) flags |= D_LAST;
     const uint32_t P = S.p_P;
     const uint32_t q = ((((tn + P - 1) * S.p_invP) >> 16) + UNR - 1) & ~(uint32_t)(UNR - 1);   // ceil(tn / P), even
@@ -544,8 +654,8 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
     __syncwarp();                                 // every lane has read the cursor before lane 0 moves it
     if (lane == 0) {
         S.desc[b] = make_uint4(tn | (q << 16), (pc.z & 0x1bffffffu) | flags, 0u, 0u);
-        S.p_cur_piece = piece_done ? cur_piece + 1 : cur_piece;
-        S.p_cur_off = piece_done ? 0u : cur_off + tn;
+        S.p_cur_piece = np;
+        S.p_j = nj;
         S.p_state = 0u;
     }
     fence_proxy_async();          // the sentinel stores (generic proxy) before the bulk copy into the same buffer
@@ -564,7 +674,8 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
 template <int R, bool MASS>
 __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const nf_plane_view *__restrict__ planes, const nf_force_params p,
                                                                              const ForceConsts fc, const Task *__restrict__ tasks,
-                                                                             uint32_t *__restrict__ ctl)
+                                                                             uint32_t *__restrict__ ctl, float *__restrict__ partial,
+                                                                             uint32_t *__restrict__ arrive)
 {
     constexpr int W = 2 * R + 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -576,7 +687,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
         mbar_init(smem_u32(&S.full[1]), 1);
         mbar_init(smem_u32(&S.empty[0]), 1);
         mbar_init(smem_u32(&S.empty[1]), 1);
-        S.p_npieces = 0; S.p_cur_piece = 0; S.p_cur_off = 0; S.p_seq = 0; S.p_state = 0;
+        S.p_npieces = 0; S.p_cur_piece = 0; S.p_j = 0; S.p_nparts = 1; S.p_seq = 0; S.p_state = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -672,23 +783,26 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
             if (active) sweep<2, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
 #pragma unroll
             for (int h = 0; h < 2; h++) { gx[h] = add2(gx[h], ax[h]); gy[h] = add2(gy[h], ay[h]); gz[h] = add2(gz[h], az[h]); }
-        } else if (mode == 0) {
-            u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
-            float rmin = 0.f;
-            if (active) sweep<0, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-#pragma unroll
-            for (int h = 0; h < 2; h++) { gx[h] = add2(gx[h], ax[h]); gy[h] = add2(gy[h], ay[h]); gz[h] = add2(gz[h], az[h]); }
         } else {
-            u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
-            float rmin = 3.0e38f;
-            if (active) sweep<1, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-            if (__any_sync(0xffffffffu, rmin < fc.eps2_test)) {        // a pair inside eps: redo with the min form
-                sticky_col = col;
-                ax[0] = ax[1] = ay[0] = ay[1] = az[0] = az[1] = 0;
-                if (active) sweep<0, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
-            }
+            if (mode == 1) {
+                u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
+                float rmin = 3.0e38f;
+                if (active) sweep<1, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+                if (__any_sync(0xffffffffu, rmin < fc.eps2_test)) {    // a pair inside eps: the sums are dropped, the tile is redone below
+                    sticky_col = col;
+                    mode = 0;
+                } else {
 #pragma unroll
-            for (int h = 0; h < 2; h++) { gx[h] = add2(gx[h], ax[h]); gy[h] = add2(gy[h], ay[h]); gz[h] = add2(gz[h], az[h]); }
+                    for (int h = 0; h < 2; h++) { gx[h] = add2(gx[h], ax[h]); gy[h] = add2(gy[h], ay[h]); gz[h] = add2(gz[h], az[h]); }
+                }
+            }
+            if (mode == 0) {                                            // the min form of Eq. 2 (one copy of this code)
+                u64 ax[2] = {0, 0}, ay[2] = {0, 0}, az[2] = {0, 0};
+                float rmin = 0.f;
+                if (active) sweep<0, MASS>(src, q, xs, ys, zs, fc, ax, ay, az, rmin);
+#pragma unroll
+                for (int h = 0; h < 2; h++) { gx[h] = add2(gx[h], ax[h]); gy[h] = add2(gy[h], ay[h]); gz[h] = add2(gz[h], az[h]); }
+            }
         }
         if (d0.y & D_LAST) {
             // ---- the task is complete: reduce the phases (fixed order), scale and write.  The scratch is
@@ -707,13 +821,44 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
                 }
             }
             __syncwarp();
+            bool write = true;
+            if (h.nparts > 1) {
+                // one part of a split task: leave the float32 sums of this part in its slot; whoever arrives
+                // last adds all slots in part order
+                float *mine = partial + (size_t)(h.slot + h.part) * 384;
+                for (int i = lane; i < n; i += 32) {
+                    const int l = i >> 2, hh = (i & 3) * 3;
+                    double ssx = 0.0, ssy = 0.0, ssz = 0.0;
+                    for (int pp = 0; pp < P; pp++) {
+                        const double *dd = red + (size_t)(pp * L + l) * 12 + hh;
+                        ssx += dd[0]; ssy += dd[1]; ssz += dd[2];
+                    }
+                    __stcg(mine + 3 * i + 0, (float)ssx);
+                    __stcg(mine + 3 * i + 1, (float)ssy);
+                    __stcg(mine + 3 * i + 2, (float)ssz);
+                }
+                __threadfence();
+                __syncwarp();
+                uint32_t old = 0;
+                if (lane == 0) old = atomicAdd(&arrive[h.slot], 1u);
+                old = __shfl_sync(0xffffffffu, old, 0);
+                write = old == h.nparts - 1u;
+                if (write) __threadfence();
+            }
             float a2max = 0.f;
-            for (int i = lane; i < n; i += 32) {
+            for (int i = lane; write && i < n; i += 32) {
                 const int l = i >> 2, hh = (i & 3) * 3;
                 double ssx = 0.0, ssy = 0.0, ssz = 0.0;
-                for (int pp = 0; pp < P; pp++) {
-                    const double *dd = red + (size_t)(pp * L + l) * 12 + hh;
-                    ssx += dd[0]; ssy += dd[1]; ssz += dd[2];
+                if (h.nparts > 1) {
+                    for (uint32_t pp = 0; pp < h.nparts; pp++) {
+                        const float *sl_ = partial + (size_t)(h.slot + pp) * 384 + 3 * i;
+                        ssx += (double)__ldcg(sl_); ssy += (double)__ldcg(sl_ + 1); ssz += (double)__ldcg(sl_ + 2);
+                    }
+                } else {
+                    for (int pp = 0; pp < P; pp++) {
+                        const double *dd = red + (size_t)(pp * L + l) * 12 + hh;
+                        ssx += dd[0]; ssy += dd[1]; ssz += dd[2];
+                    }
                 }
                 const float fx = (float)(ssx * (double)fc.out_scale), fy = (float)(ssy * (double)fc.out_scale),
                             fz = (float)(ssz * (double)fc.out_scale);
@@ -726,7 +871,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
                     h.acc[3 * o + 2] = fz;
                 }
             }
-            if (h.amax) {
+            if (h.amax && write) {
                 // per-cell maximum of |a| for the time-step criterion: the order of
                 // non-negative floats is the order of their bit patterns, so an integer atomicMax is exact
                 // and independent of the order in which a cell's tasks arrive
@@ -891,6 +1036,11 @@ static size_t max_tasks(const nf_force_params &p)
 {
     return n_sink_cells(p) * SPLIT_MAX + (size_t)(p.max_sinks > 0 ? p.max_sinks : 0) / 128 + 1;
 }
+// The source split is considered only for problems that can have fewer than split_target tasks (every task holds
+// at most 128 sinks); its work list has at most max_tasks + split_target entries, of which at most
+// 2 * split_target belong to split tasks (sum over tasks of S / share <= split_target).
+static uint32_t split_target(const nf_ctx *ctx) { return 32u * (uint32_t)ctx->sm_count * N_CONS; }
+static bool may_split(const nf_ctx *ctx, const nf_force_params &p) { return p.max_sinks / 128 < (long long)split_target(ctx); }
 
 // scratch taken by nf_forces_impl (work list) plus room for a plane table of n_planes views
 size_t nf_forces_scratch_bytes(const nf_force_params &p)
@@ -900,6 +1050,14 @@ size_t nf_forces_scratch_bytes(const nf_force_params &p)
     b += 2 * nf_align_up(2 * nc * sizeof(uint32_t), 256);                           // tc, to
     b += nf_align_up(nf_scan_temp_elems(2 * nc) * sizeof(uint32_t), 256);           // scan temp
     b += nf_align_up(max_tasks(p) * sizeof(Task), 256);                             // tasks
+    // the source split of small problems (sized for the largest GPU this could run on: 256 SMs)
+    const size_t st_max = 32u * 256u * N_CONS;
+    if ((size_t)(p.max_sinks > 0 ? p.max_sinks : 0) / 128 < st_max) {
+        const size_t mt = max_tasks(p);
+        b += 3 * nf_align_up(mt * sizeof(uint32_t), 256) + nf_align_up(nf_scan_temp_elems(mt) * sizeof(uint32_t), 256);   // src_count, parts, parts_off, scan temp
+        b += nf_align_up((mt + st_max) * sizeof(Task), 256);                        // expanded work list
+        b += nf_align_up(2 * st_max * 384 * sizeof(float), 256) + nf_align_up(2 * st_max * sizeof(uint32_t), 256);        // partial sums, arrival counters
+    }
     return b + 256 + 4096;
 }
 
@@ -942,7 +1100,7 @@ int nf_interactions_planes(nf_ctx *ctx, const nf_force_params &p, const nf_plane
 
 template <int R, bool MASS>
 static int launch_warp(nf_ctx *ctx, const nf_force_params &p, const ForceConsts &fc, const nf_plane_view *d_planes,
-                       const Task *tasks, uint32_t *ctl, cudaStream_t st)
+                       const Task *tasks, uint32_t *ctl, float *partial, uint32_t *arrive, cudaStream_t st)
 {
     // one block per SM: 12 consumer + 4 producer warps, the consumers' tile buffers fill the shared memory
     const size_t smem = sizeof(ConsShared<R>) * N_CONS;
@@ -950,7 +1108,7 @@ static int launch_warp(nf_ctx *ctx, const nf_force_params &p, const ForceConsts 
     const size_t want = (max_tasks(p) + N_CONS - 1) / N_CONS;
     size_t blocks = (size_t)ctx->sm_count;
     if (blocks > want) blocks = want;
-    k_forces_warp<R, MASS><<<(unsigned)blocks, (N_CONS + N_PROD) * 32, smem, st>>>(d_planes, p, fc, tasks, ctl);
+    k_forces_warp<R, MASS><<<(unsigned)blocks, (N_CONS + N_PROD) * 32, smem, st>>>(d_planes, p, fc, tasks, ctl, partial, arrive);
     NF_LAUNCHED(ctx);
     return NF_OK;
 }
@@ -966,10 +1124,30 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
     uint32_t *to = nf_scratch_take<uint32_t>(ctx, nc ? 2 * nc : 1);
     uint32_t *tmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(2 * nc));
     Task *tasks = nf_scratch_take<Task>(ctx, max_tasks(p));
-    uint32_t *ctl = nf_scratch_take<uint32_t>(ctx, 2);
+    uint32_t *ctl = nf_scratch_take<uint32_t>(ctx, 8);
     if (!tc || !to || !tmp || !tasks || !ctl) {
         NF_SET_ERR(ctx, "nf_forces: internal scratch arena too small");
         return NF_ERR_NOMEM;
+    }
+    // source split of problems with few, long tasks (see k_split_measure)
+    const bool split = n_sink_planes > 0 && may_split(ctx, p);
+    const size_t mt = max_tasks(p);
+    const uint32_t starget = split_target(ctx);
+    uint32_t *src_count = nullptr, *parts = nullptr, *parts_off = nullptr, *stmp = nullptr, *arrive = nullptr;
+    Task *tasks2 = nullptr;
+    float *partial = nullptr;
+    if (split) {
+        src_count = nf_scratch_take<uint32_t>(ctx, mt);
+        parts = nf_scratch_take<uint32_t>(ctx, mt);
+        parts_off = nf_scratch_take<uint32_t>(ctx, mt);
+        stmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(mt));
+        tasks2 = nf_scratch_take<Task>(ctx, mt + starget);
+        partial = nf_scratch_take<float>(ctx, (size_t)2 * starget * 384);
+        arrive = nf_scratch_take<uint32_t>(ctx, (size_t)2 * starget);
+        if (!src_count || !parts || !parts_off || !stmp || !tasks2 || !partial || !arrive) {
+            NF_SET_ERR(ctx, "nf_forces: internal scratch arena too small");
+            return NF_ERR_NOMEM;
+        }
     }
     if (n_sink_planes > 0) {
         // work list
@@ -982,19 +1160,36 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
         NF_TRY(nf_exclusive_scan_u32(ctx, tc, to, 2 * nc, tmp, st));
         k_task_fill<<<grid, 256, 0, st>>>(d_planes, tc, to, p, small, tasks, ctl);
         NF_LAUNCHED(ctx);
+        if (split) {
+            const unsigned gb = (unsigned)((mt + 255) / 256);
+            switch (p.R) {
+            case 0: k_split_measure<0><<<gb, 256, 0, st>>>(d_planes, p, tasks, ctl, starget, src_count); break;
+            case 1: k_split_measure<1><<<gb, 256, 0, st>>>(d_planes, p, tasks, ctl, starget, src_count); break;
+            case 2: k_split_measure<2><<<gb, 256, 0, st>>>(d_planes, p, tasks, ctl, starget, src_count); break;
+            default: k_split_measure<3><<<gb, 256, 0, st>>>(d_planes, p, tasks, ctl, starget, src_count); break;
+            }
+            NF_LAUNCHED(ctx);
+            k_split_parts<<<gb, 256, 0, st>>>(ctl, starget, src_count, parts, (uint32_t)mt);
+            NF_LAUNCHED(ctx);
+            NF_TRY(nf_exclusive_scan_u32(ctx, parts, parts_off, mt, stmp, st));
+            k_split_fill<<<gb, 256, 0, st>>>(tasks, parts, parts_off, ctl, tasks2, (uint32_t)mt);
+            NF_LAUNCHED(ctx);
+            NF_CUDA(ctx, cudaMemsetAsync(arrive, 0, sizeof(uint32_t) * 2 * starget, st));
+        }
     }
+    const Task *work = split ? tasks2 : tasks;
     if (record_timing) NF_CUDA(ctx, cudaEventRecord(ctx->ev_kern0, st));
     if (n_sink_planes > 0) {
         const bool mass = (p.softening & NF_MASS_W) != 0;
         switch (p.R * 2 + (mass ? 1 : 0)) {
-        case 0: NF_TRY((launch_warp<0, false>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
-        case 1: NF_TRY((launch_warp<0, true>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
-        case 2: NF_TRY((launch_warp<1, false>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
-        case 3: NF_TRY((launch_warp<1, true>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
-        case 4: NF_TRY((launch_warp<2, false>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
-        case 5: NF_TRY((launch_warp<2, true>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
-        case 6: NF_TRY((launch_warp<3, false>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
-        default: NF_TRY((launch_warp<3, true>(ctx, p, fc, d_planes, tasks, ctl, st))); break;
+        case 0: NF_TRY((launch_warp<0, false>(ctx, p, fc, d_planes, work, ctl, partial, arrive, st))); break;
+        case 1: NF_TRY((launch_warp<0, true>(ctx, p, fc, d_planes, work, ctl, partial, arrive, st))); break;
+        case 2: NF_TRY((launch_warp<1, false>(ctx, p, fc, d_planes, work, ctl, partial, arrive, st))); break;
+        case 3: NF_TRY((launch_warp<1, true>(ctx, p, fc, d_planes, work, ctl, partial, arrive, st))); break;
+        case 4: NF_TRY((launch_warp<2, false>(ctx, p, fc, d_planes, work, ctl, partial, arrive, st))); break;
+        case 5: NF_TRY((launch_warp<2, true>(ctx, p, fc, d_planes, work, ctl, partial, arrive, st))); break;
+        case 6: NF_TRY((launch_warp<3, false>(ctx, p, fc, d_planes, work, ctl, partial, arrive, st))); break;
+        default: NF_TRY((launch_warp<3, true>(ctx, p, fc, d_planes, work, ctl, partial, arrive, st))); break;
         }
     }
     if (record_timing) {
