@@ -651,19 +651,16 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
     if (tn + lane < P * q) buf[tn + lane] = SENT;
     if (tn + 32 + lane < P * q) buf[tn + 32 + lane] = SENT;
     const float4 *src = S.enc[(pc.z >> 16) & 0xff] + start;
-    __syncwarp();                                 // every lane has read the cursor before lane 0 moves it
-    if (lane == 0) {
-        S.desc[b] = make_uint4(tn | (q << 16), (pc.z & 0x1bffffffu) | flags, 0u, 0u);
-        S.p_cur_piece = np;
-        S.p_j = nj;
-        S.p_state = 0u;
-    }
+    if (lane == 0) S.desc[b] = make_uint4(tn | (q << 16), (pc.z & 0x1bffffffu) | flags, 0u, 0u);
     fence_proxy_async();          // the sentinel stores (generic proxy) before the bulk copy into the same buffer
-    __syncwarp();
+    __syncwarp();                 // ... and every lane has read the cursor before lane 0 moves it
     if (lane == 0) {
         const uint32_t bar = smem_u32(&S.full[b]);
         mbar_expect_tx(bar, tn * 16u);
         bulk_g2s(smem_u32(buf), src, tn * 16u, bar);
+        S.p_cur_piece = np;
+        S.p_j = nj;
+        S.p_state = 0u;
     }
     __syncwarp();
     // the task's last tile is on its way and its piece table is dead: prepare the next task now
