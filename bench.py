@@ -40,35 +40,17 @@ from paper_1810_02916_b200 import inputs  # noqa: E402
 FLOP_PER_INTERACTION = 20          # BASELINE.json convention (the paper counts 23)
 FP32_LANES_PER_SM = 128
 ORACLE_BLOCK = 44                  # the oracle's sample is drawn from the sinks of a 44^3-cell block (~5 M sinks at 64 per cell)
-ORACLE_SINKS = 1 << 21             # ... a seeded choice of this many of them, the SAME in both arms (cpu_baseline and --impl reference)
+ORACLE_SINKS = 1 << 22             # ... a seeded choice of this many of them, the SAME in both arms (cpu_baseline and --impl reference)
 ORACLE_SEED = 1
-TRAFFIC_JSON = os.path.join(ROOT, "profiles", "interaction_kernel_traffic.json")
-KERNEL_SOURCES = ["paper_1810_02916_b200/csrc/nf_forces.cu", "paper_1810_02916_b200/csrc/nf_common.cuh"]
-
-
-def kernel_source_hash() -> str:
-    """sha256 over the interaction kernel's sources: what a stored ncu counter is valid for (the GPU box
-    has no .git, so a commit id cannot be checked there)."""
-    import hashlib
-    h = hashlib.sha256()
-    for rel in KERNEL_SOURCES:
-        with open(os.path.join(ROOT, rel), "rb") as fh:
-            h.update(fh.read())
-    return h.hexdigest()
+ORACLE_MAX_PAIRS = 4e10            # ... cut back (the same way in both arms) when those sinks would mean more pairs than this (dense cells)
 
 
 def ncu_traffic(workload: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one interaction-kernel launch on `workload`, from
-    the ncu capture recorded in profiles/interaction_kernel_traffic.json -- or None when that capture was
-    taken from other kernel sources than the ones in this tree (the number would be stale)."""
-    try:
-        with open(TRAFFIC_JSON) as fh:
-            rec = json.load(fh).get(workload)
-    except (OSError, ValueError):
-        return None
-    if not rec or rec.get("kernel_source_sha256") != kernel_source_hash():
-        return None
-    return float(rec["dram_bytes_read"]) + float(rec["dram_bytes_write"])
+    """roofline.traffic: dram bytes (read + write) of one interaction-kernel launch on `workload` from the ncu
+    capture recorded in profiles/interaction_kernel_traffic.json by `python -m paper_1810_02916_b200.profiling
+    traffic`, or None when that capture was taken from other kernel sources than the ones in this tree."""
+    from paper_1810_02916_b200 import profiling
+    return profiling.read_traffic(workload)
 
 
 def read_peaks():
@@ -158,22 +140,30 @@ def time_oracle(sub, cfg, m, c0, n_sinks=ORACLE_SINKS):
             inner &= ((c.astype(np.int64) - lo) % K) < m
     sink_idx = np.nonzero(inner)[0]
     rng = np.random.default_rng(ORACLE_SEED)
-    timed = np.sort(rng.choice(sink_idx, min(len(sink_idx), n_sinks), replace=False))
+    timed = rng.choice(sink_idx, min(len(sink_idx), n_sinks), replace=False)
+    cnt3 = np.bincount(keys, minlength=K ** 3).reshape(K, K, K).astype(np.int64)
+
+    def pairs_of(sel):       # ordered pairs evaluated for the sinks `sel`, from the oracle's own cell counts
+        kk = keys[sel].astype(np.int64)
+        tz, ty, tx = kk % K, (kk // K) % K, kk // (K * K)
+        tot = 0
+        for dx in range(-R, R + 1):
+            for dy in range(-R, R + 1):
+                for dz in range(-R, R + 1):
+                    tot += int(cnt3[(tx + dx) % K, (ty + dy) % K, (tz + dz) % K].sum())
+        return tot
+
+    inter = pairs_of(timed)
+    if inter > ORACLE_MAX_PAIRS:
+        timed = timed[: max(1, int(len(timed) * ORACLE_MAX_PAIRS / inter))]
+        inter = pairs_of(timed)
+    timed = np.sort(timed)
     t0 = time.perf_counter()
     oracle.bin_particles(sub, K, cfg.box)
     t_bin = time.perf_counter() - t0
     t0 = time.perf_counter()
     acc = oracle.forces(sub, K, R, cfg.eps, cfg.box, cfg.Gm, sink_idx=timed)
     t_call = time.perf_counter() - t0
-    # ordered pairs evaluated for the timed sinks, from the oracle's own cell counts
-    cnt3 = np.bincount(keys, minlength=K ** 3).reshape(K, K, K).astype(np.int64)
-    kk = keys[timed].astype(np.int64)
-    tz, ty, tx = kk % K, (kk // K) % K, kk // (K * K)
-    inter = 0
-    for dx in range(-R, R + 1):
-        for dy in range(-R, R + 1):
-            for dz in range(-R, R + 1):
-                inter += int(cnt3[(tx + dx) % K, (ty + dy) % K, (tz + dz) % K].sum())
     return {"interactions": inter, "seconds": max(t_call - t_bin, 1e-9), "seconds_binning": t_bin, "seconds_call": t_call,
             "cores": oracle.max_threads(), "n_sinks": len(timed), "sinks": timed, "acc": acc}
 
@@ -573,7 +563,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number 1..5 (default 4 = C4; 5 = slab streaming)")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number 1..5 (default 4 = C4; 5 = slab streaming); 6 = one dense cell of 4x10^5 particles (profiling workload)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

@@ -167,6 +167,17 @@ __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)     // 
                  : "memory");
     return ok != 0;
 }
+// try_wait with a suspend-time hint: the thread sleeps in hardware (no issue slots) until the phase completes or
+// about `ns` nanoseconds have passed
+__device__ __forceinline__ bool mbar_try_timed(uint32_t bar, uint32_t parity, uint32_t ns)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok)
+                 : "r"(bar), "r"(parity), "r"(ns)
+                 : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------
@@ -384,7 +395,8 @@ __global__ void __launch_bounds__(256) k_split_fill(const Task *__restrict__ tas
 // Producer, per consumer: pulls tasks from the work list, builds the task's piece table, cuts pieces into
 // tiles, pads the tile's tail with sentinels, writes the tile's descriptor and issues its bulk copy
 // (cp.async.bulk + mbarrier transaction count) into whichever of the consumer's two 8 KiB buffers is
-// free (an "empty" mbarrier the consumer arrives on).  Consumer, per tile: waits on the buffer's "full"
+// free (an "empty" mbarrier the consumer arrives on; a producer with nothing to do sleeps on a "doorbell"
+// mbarrier that its three consumers ring at every release).  Consumer, per tile: waits on the buffer's "full"
 // mbarrier, reads the descriptor, shifts its sinks into the tile's frame, sweeps, adds the tile's sums to
 // its running sums and releases the buffer.  Nothing on the consumer's path waits on a copy it issued
 // itself, reads the work list or touches the piece table (measured in isolation: 70.8 % -> 74.5 % of the
@@ -677,6 +689,8 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
     constexpr int W = 2 * R + 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     ConsShared<R> *CS = reinterpret_cast<ConsShared<R> *>(smem_raw);
+    // one "doorbell" mbarrier per producer: its consumers ring it whenever they release a buffer
+    unsigned long long *bells = reinterpret_cast<unsigned long long *>(smem_raw + sizeof(ConsShared<R>) * N_CONS);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp < N_CONS && lane == 0) {
         ConsShared<R> &S = CS[warp];
@@ -685,6 +699,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
         mbar_init(smem_u32(&S.empty[0]), 1);
         mbar_init(smem_u32(&S.empty[1]), 1);
         S.p_npieces = 0; S.p_cur_piece = 0; S.p_j = 0; S.p_nparts = 1; S.p_seq = 0; S.p_state = 0;
+        if (warp < N_PROD) mbar_init(smem_u32(&bells[warp]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -701,7 +716,10 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
         for (int i = 0; i < CONS_PER_PROD; i++)
             produce_next_task<R>(CS[pw * CONS_PER_PROD + i], planes, p, fc, tasks, ctl, n_tasks, lane);
         int remaining = CONS_PER_PROD;
+        const uint32_t bell = smem_u32(&bells[pw]);
+        uint32_t bq = 0;                            // doorbell phase this producer waits on next
         while (remaining > 0) {
+            while (mbar_test(bell, bq & 1u)) bq++;  // catch up with the rings so far (an even lag behaves like none)
             bool progress = false;
 #pragma unroll
             for (int i = 0; i < CONS_PER_PROD; i++) {
@@ -715,9 +733,11 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
                 if (produce_tile<R>(S, planes, p, fc, tasks, ctl, n_tasks, b, lane)) tt[i] = t + 1;
                 else { tt[i] = 1u << 31; remaining--; }
             }
-            // nothing to do: every buffer is full.  Sleep instead of spinning on the schedulers' issue slots
-            // (a tile takes a consumer several microseconds).
-            if (!progress) __nanosleep(1000);
+            // nothing to do: every buffer is full.  Sleep in hardware on the doorbell (no issue slots) until one of
+            // this producer's consumers releases a buffer.  Two rings between the scan above and this wait would
+            // look like none (parity); the time limit bounds that rare case to a few microseconds -- a consumer
+            // still holds a full buffer then.
+            if (!progress && remaining > 0 && mbar_try_timed(bell, bq & 1u, 4000u)) bq++;
         }
         return;
     }
@@ -727,6 +747,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
     ConsShared<R> &S = CS[warp];
     const uint32_t full0 = smem_u32(&S.full[0]), full1 = smem_u32(&S.full[1]);
     const uint32_t emp0 = smem_u32(&S.empty[0]), emp1 = smem_u32(&S.empty[1]);
+    const uint32_t bell = smem_u32(&bells[warp / CONS_PER_PROD]);
     u64 xi[2] = {0, 0}, yi[2] = {0, 0}, zi[2] = {0, 0};
     u64 gx[2] = {0, 0}, gy[2] = {0, 0}, gz[2] = {0, 0};
     int L = 32, P = 1, n = 0, sl = 0, ph = 0, hslot = 0, sticky_col = -1;
@@ -880,7 +901,10 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
         // scratch) are ordered before the producer's next bulk copy into it (async proxy), then it is released
         fence_proxy_async();
         __syncwarp();
-        if (lane == 0) mbar_arrive(b ? emp1 : emp0);
+        if (lane == 0) {
+            mbar_arrive(b ? emp1 : emp0);
+            mbar_arrive(bell);                      // wake the producer
+        }
     }
 }
 
@@ -1031,7 +1055,9 @@ static size_t n_sink_cells(const nf_force_params &p)
 }
 static size_t max_tasks(const nf_force_params &p)
 {
-    return n_sink_cells(p) * SPLIT_MAX + (size_t)(p.max_sinks > 0 ? p.max_sinks : 0) / 128 + 1;
+    // full tasks (128 sinks) plus at most SPLIT_MAX remainder tasks per cell, each holding at least one sink
+    const size_t ms = (size_t)(p.max_sinks > 0 ? p.max_sinks : 0), rem = n_sink_cells(p) * SPLIT_MAX;
+    return (rem < ms ? rem : ms) + ms / 128 + 1;
 }
 // The source split is considered only for problems that can have fewer than split_target tasks (every task holds
 // at most 128 sinks); its work list has at most max_tasks + split_target entries, of which at most
@@ -1100,7 +1126,7 @@ static int launch_warp(nf_ctx *ctx, const nf_force_params &p, const ForceConsts 
                        const Task *tasks, uint32_t *ctl, float *partial, uint32_t *arrive, cudaStream_t st)
 {
     // one block per SM: 12 consumer + 4 producer warps, the consumers' tile buffers fill the shared memory
-    const size_t smem = sizeof(ConsShared<R>) * N_CONS;
+    const size_t smem = sizeof(ConsShared<R>) * N_CONS + N_PROD * sizeof(unsigned long long);
     NF_CUDA(ctx, cudaFuncSetAttribute(k_forces_warp<R, MASS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const size_t want = (max_tasks(p) + N_CONS - 1) / N_CONS;
     size_t blocks = (size_t)ctx->sm_count;

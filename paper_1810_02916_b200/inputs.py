@@ -74,7 +74,12 @@ def config(which: int) -> Config:
         return Config("C5-slab-2048^3-density", N, 512, 2, 500.0, 0.01, 1.0 / N, s, "slab",
                       frac_halo=0.4, n_halos=1 << 20, a_lo=0.020, a_hi=0.300,
                       r_trunc=2.0 * 500.0 / 256, planes=16, plane0=100, density_n=2048)
-    raise ValueError("config number must be 1..5")
+    if which == 6:
+        # not a BASELINE.json config: the dense-cell end of the range ("the largest cell has
+        # over 200,000 particles"): one cell of ~4x10^5 particles in an otherwise almost empty K = 5 box
+        N = 400_000
+        return Config("D1-one-dense-cell-4e5", N, 5, 2, 1.0, 0.01 * 0.2, 1.0 / N, s, "onecell")
+    raise ValueError("config number must be 1..5 (6: the one-dense-cell profiling workload)")
 
 
 def scaled(cfg: Config, N: int, K: int, name: Optional[str] = None) -> Config:
@@ -175,6 +180,15 @@ def make_positions_chunk(cfg: Config, c: int, device="cpu", catalogue=None) -> t
         hid = torch.randint(0, cfg.n_halos, (n,), generator=g, device=device)
         off = _plummer_offsets(n, scales[hid], cfg.r_trunc, g, device)
         x = torch.where(is_halo[:, None], centres[hid] + off, x).float()
+    elif cfg.kind == "onecell":
+        # Normal(centre of the middle cell, 0.08 w) clipped into that cell; the first 1000 particles uniform in the box
+        w = cfg.box / cfg.K
+        mid = (cfg.K // 2 + 0.5) * w
+        x = mid + 0.08 * w * torch.randn(n, 3, generator=g, device=device, dtype=torch.float64)
+        x = x.clamp(mid - 0.49 * w, mid + 0.49 * w)
+        u = torch.rand(n, 3, generator=g, device=device, dtype=torch.float64) * cfg.box
+        first = (torch.arange(lo, hi, device=device) < 1000)[:, None]
+        x = torch.where(first, u, x).float()
     else:
         raise ValueError(f"make_positions: kind {cfg.kind!r} not supported (use make_slab_planes)")
     return _wrap_(x, cfg.box)
