@@ -178,6 +178,17 @@ __device__ __forceinline__ bool mbar_try_timed(uint32_t bar, uint32_t parity, ui
                  : "memory");
     return ok != 0;
 }
+__device__ __forceinline__ void st_release_shared(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint4 ld_volatile_shared_v4(uint32_t addr)
+{
+    uint4 v;
+    asm volatile("ld.volatile.shared::cta.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void fence_acq_rel_cta() { asm volatile("fence.acq_rel.cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------
@@ -395,8 +406,8 @@ __global__ void __launch_bounds__(256) k_split_fill(const Task *__restrict__ tas
 // Producer, per consumer: pulls tasks from the work list, builds the task's piece table, cuts pieces into
 // tiles, pads the tile's tail with sentinels, writes the tile's descriptor and issues its bulk copy
 // (cp.async.bulk + mbarrier transaction count) into whichever of the consumer's two 8 KiB buffers is
-// free (an "empty" mbarrier the consumer arrives on; a producer with nothing to do sleeps on a "doorbell"
-// mbarrier that its three consumers ring at every release).  Consumer, per tile: waits on the buffer's "full"
+// free (the consumer publishes the number of tiles it has released with a release store; a producer with nothing
+// to do sleeps on a "doorbell" mbarrier that its three consumers ring at every release).  Consumer, per tile: waits on the buffer's "full"
 // mbarrier, reads the descriptor, shifts its sinks into the tile's frame, sweeps, adds the tile's sums to
 // its running sums and releases the buffer.  Nothing on the consumer's path waits on a copy it issued
 // itself, reads the work list or touches the piece table (measured in isolation: 70.8 % -> 74.5 % of the
@@ -449,9 +460,9 @@ struct ConsShared {
     float4 buf[2][TILE_CAP];
     uint4 piece[PIECE_CAP];                 // x: first particle, y: count, z: meta, w: balanced tile length   (producer's)
     uint4 desc[2];                          // per buffer: x = tn | q << 16, y = meta | flags
-    TaskHdr hdr[2];
+    TaskHdr hdr[4];                         // by task sequence number & 3 (the consumer can be two tasks behind the one being prepared)
     const float4 *enc[W];                   // encoded positions of the W source planes (by dx + R; null = outside the chunk)
-    unsigned long long full[2], empty[2];
+    unsigned long long full[2];
     // producer's cursor for this consumer
     uint32_t p_npieces, p_cur_piece, p_j, p_nparts, p_P, p_invP, p_seq, p_state;   // p_state 0: inside a task, 1: next tile starts a task, 2: stop
 };
@@ -486,7 +497,7 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
         h.se = se; h.acc = sp.acc; h.perm = sp.perm; h.amax = sp.amax; h.s0 = s0;
         h.n = (uint32_t)n; h.L = (uint32_t)L; h.cyz = task.cyz;
         h.part = task.part_slot & 0xffu; h.nparts = task.nparts; h.slot = task.part_slot >> 8;
-        S.hdr[seq & 1u] = h;
+        S.hdr[seq & 3u] = h;
         S.p_P = (uint32_t)P;
         S.p_invP = (65536u + P - 1) / P;        // floor(x / P) == (x * inv_P) >> 16 for x < 1024
     }
@@ -635,7 +646,7 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
         __syncwarp();
         return false;
     }
-    uint32_t flags = state == 1u ? (D_FIRST | (((S.p_seq - 1u) & 1u) << 26)) : 0u;      // bit 26: header slot
+    uint32_t flags = state == 1u ? (D_FIRST | (((S.p_seq - 1u) & 3u) << 25)) : 0u;      // bits 25-26: header slot
     const uint32_t cur_piece = S.p_cur_piece, cur_j = S.p_j, n_pieces = S.p_npieces;
     const uint4 pc = S.piece[cur_piece];
     const uint32_t start = pc.x + cur_j * pc.w;
@@ -663,7 +674,7 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
     if (tn + lane < P * q) buf[tn + lane] = SENT;
     if (tn + 32 + lane < P * q) buf[tn + 32 + lane] = SENT;
     const float4 *src = S.enc[(pc.z >> 16) & 0xff] + start;
-    if (lane == 0) S.desc[b] = make_uint4(tn | (q << 16), (pc.z & 0x1bffffffu) | flags, 0u, 0u);
+    if (lane == 0) S.desc[b] = make_uint4(tn | (q << 16), (pc.z & 0x19ffffffu) | flags, 0u, 0u);
     fence_proxy_async();          // the sentinel stores (generic proxy) before the bulk copy into the same buffer
     __syncwarp();                 // ... and every lane has read the cursor before lane 0 moves it
     if (lane == 0) {
@@ -691,13 +702,14 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
     ConsShared<R> *CS = reinterpret_cast<ConsShared<R> *>(smem_raw);
     // one "doorbell" mbarrier per producer: its consumers ring it whenever they release a buffer
     unsigned long long *bells = reinterpret_cast<unsigned long long *>(smem_raw + sizeof(ConsShared<R>) * N_CONS);
+    // tiles released so far by each consumer, four words per producer (its three consumers' counters are one 16-byte load)
+    uint32_t *released = reinterpret_cast<uint32_t *>(bells + N_PROD);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp < N_CONS && lane == 0) {
         ConsShared<R> &S = CS[warp];
         mbar_init(smem_u32(&S.full[0]), 1);
         mbar_init(smem_u32(&S.full[1]), 1);
-        mbar_init(smem_u32(&S.empty[0]), 1);
-        mbar_init(smem_u32(&S.empty[1]), 1);
+        released[(warp / CONS_PER_PROD) * 4 + warp % CONS_PER_PROD] = 0;
         S.p_npieces = 0; S.p_cur_piece = 0; S.p_j = 0; S.p_nparts = 1; S.p_seq = 0; S.p_state = 0;
         if (warp < N_PROD) mbar_init(smem_u32(&bells[warp]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -716,21 +728,25 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
         for (int i = 0; i < CONS_PER_PROD; i++)
             produce_next_task<R>(CS[pw * CONS_PER_PROD + i], planes, p, fc, tasks, ctl, n_tasks, lane);
         int remaining = CONS_PER_PROD;
-        const uint32_t bell = smem_u32(&bells[pw]);
+        const uint32_t bell = smem_u32(&bells[pw]), relw = smem_u32(&released[pw * 4]);
         uint32_t bq = 0;                            // doorbell phase this producer waits on next
         while (remaining > 0) {
             while (mbar_test(bell, bq & 1u)) bq++;  // catch up with the rings so far (an even lag behaves like none)
+            __syncwarp();
+            // a buffer is free when fewer than two of the tiles issued to its consumer are still unreleased
+            const uint4 rel = ld_volatile_shared_v4(relw);
+            const uint32_t rl[3] = {rel.x, rel.y, rel.z};
             bool progress = false;
 #pragma unroll
             for (int i = 0; i < CONS_PER_PROD; i++) {
                 const uint32_t t = tt[i];
-                if (t >> 31) continue;
-                ConsShared<R> &S = CS[pw * CONS_PER_PROD + i];
-                const int b = (int)(t & 1u);
-                // the buffer is free once the consumer has released its previous tile (non-blocking poll)
-                if (t >= 2 && !mbar_test(smem_u32(&S.empty[b]), ((t >> 1) - 1u) & 1u)) continue;
+                // a warp-uniform decision (vote): the lanes of this warp need not have loaded the counters at the same
+                // moment, and everything below is warp-synchronous
+                if (!__all_sync(0xffffffffu, !(t >> 31) && t - rl[i] < 2u)) continue;
+                if (!progress) fence_acq_rel_cta();  // the consumer's reads of the buffer (released with st.release) before our copy into it
                 progress = true;
-                if (produce_tile<R>(S, planes, p, fc, tasks, ctl, n_tasks, b, lane)) tt[i] = t + 1;
+                ConsShared<R> &S = CS[pw * CONS_PER_PROD + i];
+                if (produce_tile<R>(S, planes, p, fc, tasks, ctl, n_tasks, (int)(t & 1u), lane)) tt[i] = t + 1;
                 else { tt[i] = 1u << 31; remaining--; }
             }
             // nothing to do: every buffer is full.  Sleep in hardware on the doorbell (no issue slots) until one of
@@ -746,7 +762,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(CONS_REGS));
     ConsShared<R> &S = CS[warp];
     const uint32_t full0 = smem_u32(&S.full[0]), full1 = smem_u32(&S.full[1]);
-    const uint32_t emp0 = smem_u32(&S.empty[0]), emp1 = smem_u32(&S.empty[1]);
+    const uint32_t relw = smem_u32(&released[(warp / CONS_PER_PROD) * 4 + warp % CONS_PER_PROD]);
     const uint32_t bell = smem_u32(&bells[warp / CONS_PER_PROD]);
     u64 xi[2] = {0, 0}, yi[2] = {0, 0}, zi[2] = {0, 0};
     u64 gx[2] = {0, 0}, gy[2] = {0, 0}, gz[2] = {0, 0};
@@ -759,7 +775,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
         if (d0.y & D_END) break;
         if (d0.y & D_FIRST) {
             // ---- a new task: its header, and the lane's four sinks (slots past n repeat the last sink) ----
-            hslot = (int)((d0.y >> 26) & 1u);
+            hslot = (int)((d0.y >> 25) & 3u);
             const TaskHdr &h = S.hdr[hslot];
             L = (int)h.L; n = (int)h.n;
             P = 32 / L;
@@ -902,7 +918,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
         fence_proxy_async();
         __syncwarp();
         if (lane == 0) {
-            mbar_arrive(b ? emp1 : emp0);
+            st_release_shared(relw, t + 1u);        // tiles released so far
             mbar_arrive(bell);                      // wake the producer
         }
     }
@@ -1126,7 +1142,7 @@ static int launch_warp(nf_ctx *ctx, const nf_force_params &p, const ForceConsts 
                        const Task *tasks, uint32_t *ctl, float *partial, uint32_t *arrive, cudaStream_t st)
 {
     // one block per SM: 12 consumer + 4 producer warps, the consumers' tile buffers fill the shared memory
-    const size_t smem = sizeof(ConsShared<R>) * N_CONS + N_PROD * sizeof(unsigned long long);
+    const size_t smem = sizeof(ConsShared<R>) * N_CONS + N_PROD * (sizeof(unsigned long long) + 4 * sizeof(uint32_t));
     NF_CUDA(ctx, cudaFuncSetAttribute(k_forces_warp<R, MASS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const size_t want = (max_tasks(p) + N_CONS - 1) / N_CONS;
     size_t blocks = (size_t)ctx->sm_count;
