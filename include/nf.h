@@ -241,6 +241,40 @@ int nf_cell_vrms(nf_ctx *ctx, const float *vel_xyz, const uint32_t *perm, const 
                  int64_t N, int K, float *cell_vrms, float *vmax, void *stream);
 
 /*
+ * nf_timestep_terms -- the reduction of time-step criteria 2 and 3 from the per-cell
+ * quantities nf_forces_ex (a_max) and nf_cell_vrms (v_rms, maximum velocity) return:
+ *
+ *   criterion 2  "the step size must be less than TimeStepAccel times the maximum of v_rms/a_max computed within
+ *                each cell" (:194) ... "we also compute a global v_rms/a_max and use the maximum of the global and
+ *                cell-based values.  This protects us from taking catastrophically small time steps as a result of
+ *                abnormally cold cells" (:207).  A cold cell makes its own ratio SMALL, so the cell-based value that
+ *                the global one guards against is the smallest ratio over cells (reading c19); the largest
+ *                is returned too, for the literal reading.
+ *   criterion 3  "the step size times the maximum velocity must be less than 80% of a cell width" (:195).
+ *
+ *   cell_vrms, cell_amax   dev in   K^3 float32 each (nf_cell_vrms / nf_forces_ex)
+ *   cell_offset            dev in   K^3 + 1 uint64 (nf_bin): particle counts weight the global v_rms
+ *   vmax                   dev in, nullable  1 float32 (nf_cell_vrms)
+ *   out                    host out
+ *
+ * Cells that are empty or have a_max = 0 take no part in the cell ratios.  Each ratio is the float32 quotient
+ * v_rms / a_max (round to nearest), so minimum and maximum are exact and order-independent; the global v_rms is
+ * sqrt(sum_c n_c v_rms_c^2 / N) accumulated in double in a fixed order (deterministic).  Synchronises `stream`.
+ * The caller multiplies by its own TimeStepAccel (eta) and combines with criterion 1.
+ */
+typedef struct nf_timestep {
+    double ratio_cell_min;   /* min over cells of v_rms / a_max        (0 if no cell qualifies) */
+    double ratio_cell_max;   /* max over cells of v_rms / a_max */
+    double ratio_global;     /* global v_rms / global a_max            (0 if a_max = 0) */
+    double ratio_criterion2; /* max(ratio_global, ratio_cell_min): the step is eta times this (reading c19) */
+    double vrms_global, amax_global, vmax;
+    double drift_limit;      /* criterion 3: 0.8 * (box / K) / vmax    (infinity if vmax = 0 or not given) */
+    int64_t cells_used;      /* cells that entered the cell ratios */
+} nf_timestep;
+int nf_timestep_terms(nf_ctx *ctx, const float *cell_vrms, const float *cell_amax, const uint64_t *cell_offset,
+                      int K, float box, const float *vmax, nf_timestep *out, void *stream);
+
+/*
  * nf_forces_host -- the whole path from HOST buffers: H2D copy of the positions, nf_bin,
  * nf_forces, D2H copy of the accelerations (the paper's GPU rate "includes
  * PCIe bus transfer overheads").  All device buffers come from the context's scratch arena

@@ -12,6 +12,7 @@ from .nf_oracle import (  # noqa: F401
     cell_amax,
     kick_drift,
     cell_vrms,
+    timestep_terms,
     interactions,
     spline_over_r,
     plummer_over_r,

@@ -174,6 +174,30 @@ def cell_vrms(vel, key, ncell: int):
     return out, float(vmax.value)
 
 
+def timestep_terms(cell_vrms, cell_amax, cell_count, K: int, box: float, vmax=None) -> dict:
+    """Time-step criteria 2 and 3 written out, plain numpy.  Criterion 2: the step is
+    TimeStepAccel times a ratio v_rms / a_max; "we also compute a global v_rms/a_max and use the maximum of the global
+    and cell-based values.  This protects us from taking catastrophically small time steps as a result of abnormally
+    cold cells" -- a cold cell has a SMALL ratio, so the cell-based value is the minimum over cells (DESIGN.md reading
+    c19; the maximum over cells, the literal reading of :194, is returned beside it).  Each cell ratio is the float32
+    quotient; cells that are empty or have a_max = 0 are left out.  Criterion 3: step * vmax < 0.8 cell widths."""
+    v = np.asarray(cell_vrms, dtype=np.float32).ravel()
+    a = np.asarray(cell_amax, dtype=np.float32).ravel()
+    n = np.asarray(cell_count, dtype=np.int64).ravel()
+    use = (n > 0) & (a > 0)
+    q = (v[use] / a[use]).astype(np.float32)
+    N = int(n.sum())
+    vr = float(np.sqrt(np.sum(n[n > 0].astype(np.float64) * v[n > 0].astype(np.float64) ** 2) / N)) if N else 0.0
+    am = float(a[n > 0].max()) if N else 0.0
+    rg = vr / am if am > 0 else 0.0
+    rmin = float(q.min()) if q.size else 0.0
+    out = {"ratio_cell_min": rmin, "ratio_cell_max": float(q.max()) if q.size else 0.0, "ratio_global": rg,
+           "ratio_criterion2": max(rg, rmin), "vrms_global": vr, "amax_global": am, "cells_used": int(use.sum()),
+           "vmax": float(vmax) if vmax is not None else 0.0}
+    out["drift_limit"] = 0.8 * (float(box) / K) / out["vmax"] if out["vmax"] > 0 else float("inf")
+    return out
+
+
 def interactions(cell_count, K: int, R: int, sink_plane_lo: int = 0, sink_plane_hi=None) -> int:
     """I = sum_c n_c sum_{c' in N(c)} n_c' (ordered pairs, self pairs included)."""
     lib = _load()

@@ -4,7 +4,9 @@
 //
 // k_kick_drift   v <- v + a*kick ; x <- wrap(x + v*drift)       elementwise, HBM-bound (36 B / particle)
 // k_cell_vrms    per-cell rms speed in the cell order of nf_bin + global max |v_axis|
+// k_timestep_*   reduction of criteria 2 and 3 over the cells (min / max of v_rms / a_max, global v_rms and a_max)
 #include "nf_common.cuh"
+#include <math.h>
 
 namespace {
 
@@ -53,7 +55,100 @@ __global__ void __launch_bounds__(256) k_cell_vrms(const float *__restrict__ vel
     }
 }
 
+// Time-step terms.  Stage 1: each block reduces a contiguous range of cells to one record; stage 2: one block
+// reduces the records in index order.  Minimum / maximum of float32 values are order-independent; the double sum
+// is formed in a fixed tree order, so the result is the same from run to run.
+constexpr int TS_BLOCKS = 1024, TS_THREADS = 256;
+struct TsRec { float rmin, rmax, amax; unsigned int pad; double sum_nv2; unsigned long long n, used; };
+
+__device__ __forceinline__ void ts_merge(TsRec &a, const TsRec &b)
+{
+    a.rmin = fminf(a.rmin, b.rmin); a.rmax = fmaxf(a.rmax, b.rmax); a.amax = fmaxf(a.amax, b.amax);
+    a.sum_nv2 += b.sum_nv2; a.n += b.n; a.used += b.used;
+}
+__device__ __forceinline__ TsRec ts_block_reduce(TsRec r)
+{
+    __shared__ TsRec sh[TS_THREADS];
+    sh[threadIdx.x] = r;
+    __syncthreads();
+    for (int d = TS_THREADS / 2; d > 0; d >>= 1) {
+        if ((int)threadIdx.x < d) { TsRec a = sh[threadIdx.x]; ts_merge(a, sh[threadIdx.x + d]); sh[threadIdx.x] = a; }
+        __syncthreads();
+    }
+    return sh[0];
+}
+__device__ __forceinline__ TsRec ts_empty()
+{
+    TsRec r; r.rmin = 3.0e38f; r.rmax = 0.f; r.amax = 0.f; r.pad = 0; r.sum_nv2 = 0.0; r.n = 0; r.used = 0;
+    return r;
+}
+
+__global__ void __launch_bounds__(TS_THREADS) k_timestep_cells(const float *__restrict__ vrms, const float *__restrict__ amax,
+                                                               const uint64_t *__restrict__ off, size_t ncell, TsRec *__restrict__ rec)
+{
+    const size_t per = (ncell + gridDim.x - 1) / gridDim.x;
+    const size_t c0 = (size_t)blockIdx.x * per, c1 = c0 + per < ncell ? c0 + per : ncell;
+    TsRec r = ts_empty();
+    for (size_t c = c0 + threadIdx.x; c < c1; c += TS_THREADS) {
+        const unsigned long long n = off[c + 1] - off[c];
+        if (n == 0) continue;
+        const float v = vrms[c], a = amax[c];
+        r.sum_nv2 += (double)n * (double)v * (double)v;
+        r.n += n;
+        r.amax = fmaxf(r.amax, a);
+        if (a > 0.f) {
+            const float q = __fdiv_rn(v, a);
+            r.rmin = fminf(r.rmin, q); r.rmax = fmaxf(r.rmax, q); r.used++;
+        }
+    }
+    r = ts_block_reduce(r);
+    if (threadIdx.x == 0) rec[blockIdx.x] = r;
+}
+__global__ void __launch_bounds__(TS_THREADS) k_timestep_final(const TsRec *__restrict__ rec, int nrec, TsRec *__restrict__ out)
+{
+    TsRec r = ts_empty();
+    for (int i = threadIdx.x; i < nrec; i += TS_THREADS) ts_merge(r, rec[i]);
+    r = ts_block_reduce(r);
+    if (threadIdx.x == 0) *out = r;
+}
+
 }  // namespace
+
+int nf_timestep_terms(nf_ctx *ctx, const float *cell_vrms, const float *cell_amax, const uint64_t *cell_offset,
+                      int K, float box, const float *vmax, nf_timestep *out, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, K >= 1 && K <= NF_MAX_K, "nf_timestep_terms: bad K");
+    NF_ARG(ctx, cell_vrms && cell_amax && cell_offset && out, "nf_timestep_terms: null argument");
+    NF_ARG(ctx, box > 0.0f && box < 3.0e38f, "box must be positive and finite");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t ncell = (size_t)K * K * K;
+    const int nb = (int)(ncell < (size_t)TS_BLOCKS * TS_THREADS ? (ncell + TS_THREADS - 1) / TS_THREADS : TS_BLOCKS);
+    NF_TRY(nf_scratch_reserve(ctx, (size_t)(nb + 2) * sizeof(TsRec) + 1024));
+    nf_scratch_reset(ctx);
+    TsRec *rec = nf_scratch_take<TsRec>(ctx, (size_t)nb + 1);
+    if (!rec) { NF_SET_ERR(ctx, "nf_timestep_terms: internal scratch arena too small"); return NF_ERR_NOMEM; }
+    k_timestep_cells<<<nb, TS_THREADS, 0, st>>>(cell_vrms, cell_amax, cell_offset, ncell, rec);
+    NF_LAUNCHED(ctx);
+    k_timestep_final<<<1, TS_THREADS, 0, st>>>(rec, nb, rec + nb);
+    NF_LAUNCHED(ctx);
+    TsRec h;
+    float hv = 0.f;
+    NF_CUDA(ctx, cudaMemcpyAsync(&h, rec + nb, sizeof(TsRec), cudaMemcpyDeviceToHost, st));
+    if (vmax) NF_CUDA(ctx, cudaMemcpyAsync(&hv, vmax, sizeof(float), cudaMemcpyDeviceToHost, st));
+    NF_CUDA(ctx, cudaStreamSynchronize(st));
+    out->cells_used = (int64_t)h.used;
+    out->ratio_cell_min = h.used ? (double)h.rmin : 0.0;
+    out->ratio_cell_max = (double)h.rmax;
+    out->vrms_global = h.n ? sqrt(h.sum_nv2 / (double)h.n) : 0.0;
+    out->amax_global = (double)h.amax;
+    out->ratio_global = h.amax > 0.f ? out->vrms_global / (double)h.amax : 0.0;
+    out->ratio_criterion2 = out->ratio_global > out->ratio_cell_min ? out->ratio_global : out->ratio_cell_min;
+    out->vmax = (double)hv;
+    out->drift_limit = hv > 0.f ? 0.8 * ((double)box / (double)K) / (double)hv : INFINITY;
+    return NF_OK;
+}
 
 int nf_kick_drift_impl(nf_ctx *ctx, float *pos, float *vel, const float *acc, int64_t N, float kick, float drift, float box,
                        cudaStream_t st)

@@ -27,13 +27,22 @@ EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve
            "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host",
            "nf_bin_m", "nf_forces_ex", "nf_kick_drift", "nf_cell_vrms", "nf_stream_step_slabs",
            "nf_keys", "nf_forces_chunk", "nf_forces_host_m", "nf_regroup_plane", "nf_stream_step_regroup",
-           "nf_forces_host_begin", "nf_forces_host_end"]
+           "nf_forces_host_begin", "nf_forces_host_end", "nf_timestep_terms"]
 
 
 class NFError(RuntimeError):
     def __init__(self, status: int, msg: str):
         super().__init__(f"libnf status {status}: {msg}")
         self.status = status
+
+
+class TimeStep(ctypes.Structure):
+    _fields_ = [("ratio_cell_min", ctypes.c_double), ("ratio_cell_max", ctypes.c_double), ("ratio_global", ctypes.c_double),
+                ("ratio_criterion2", ctypes.c_double), ("vrms_global", ctypes.c_double), ("amax_global", ctypes.c_double),
+                ("vmax", ctypes.c_double), ("drift_limit", ctypes.c_double), ("cells_used", ctypes.c_int64)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
 
 
 class StreamStats(ctypes.Structure):
@@ -81,6 +90,8 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.nf_kick_drift.argtypes = [vp, vp, vp, vp, i64, f32, f32, f32, vp]
     lib.nf_cell_vrms.restype = i32
     lib.nf_cell_vrms.argtypes = [vp, vp, vp, vp, i64, i32, vp, vp, vp]
+    lib.nf_timestep_terms.restype = i32
+    lib.nf_timestep_terms.argtypes = [vp, vp, vp, vp, i32, f32, vp, ctypes.POINTER(TimeStep), vp]
     lib.nf_out_of_range.restype = i32
     lib.nf_out_of_range.argtypes = [vp, ctypes.POINTER(i64), vp]
     lib.nf_forces.restype = i32
@@ -267,6 +278,17 @@ class Context:
         self._check(self.lib.nf_cell_vrms(self._h, _ptr(vel), _ptr(b.perm) if original_order else None, _ptr(b.cell_offset),
                                           b.N, b.K, _ptr(vrms), _ptr(vmax), self._stream(stream)))
         return vrms, vmax
+
+    def timestep_terms(self, cell_vrms: torch.Tensor, cell_amax: torch.Tensor, b: Binned, vmax: Optional[torch.Tensor] = None,
+                       stream=None) -> dict:
+        """nf_timestep_terms: the reduction of time-step criteria 2 and 3 over the cells."""
+        ncell = b.K ** 3
+        for t in (cell_vrms, cell_amax):
+            assert t.is_cuda and t.dtype == torch.float32 and t.numel() == ncell and t.is_contiguous()
+        ts = TimeStep()
+        self._check(self.lib.nf_timestep_terms(self._h, _ptr(cell_vrms), _ptr(cell_amax), _ptr(b.cell_offset), b.K, float(b.box),
+                                               _ptr(vmax) if vmax is not None else None, ctypes.byref(ts), self._stream(stream)))
+        return ts.as_dict()
 
     def reserve_host(self, maxN: int, K: int):
         self._check(self.lib.nf_reserve_host(self._h, int(maxN), int(K)))

@@ -345,6 +345,34 @@ def test_cell_vrms_and_vmax(ctx):
     assert torch.equal(vrms2, vrms) and torch.equal(vmax2, vmax)
 
 
+def test_timestep_terms(ctx):
+    """nf_timestep_terms (criteria 2 and 3) against the oracle's numpy reduction, on the
+    a_max of a real force call and random velocities; minimum and maximum bit-exact, the double sums to rounding."""
+    cfg = inputs.scaled(inputs.config(3), 48 ** 3, 12)
+    cfg = inputs.dataclasses.replace(cfg, n_halos=10)
+    pos = inputs.make_positions(cfg).numpy()
+    rng = np.random.default_rng(17)
+    vel = (rng.standard_normal((cfg.N, 3)) * np.exp(rng.normal(0, 1.5, (cfg.N, 1)))).astype(np.float32)
+    b = ctx.bin(torch.from_numpy(pos).cuda(), cfg.K, cfg.box)
+    amax = torch.zeros(cfg.K ** 3, dtype=torch.float32, device="cuda")
+    ctx.forces(b, cfg.R, cfg.eps, cfg.Gm, cell_amax=amax)
+    vrms, vmax = ctx.cell_vrms(torch.from_numpy(vel).cuda(), b)
+    got = ctx.timestep_terms(vrms, amax, b, vmax)
+    ref = oracle.timestep_terms(vrms.cpu().numpy(), amax.cpu().numpy(), u32(b.cell_count), cfg.K, cfg.box, float(vmax.item()))
+    assert got["cells_used"] == ref["cells_used"] > 0
+    assert got["ratio_cell_min"] == ref["ratio_cell_min"] and got["ratio_cell_max"] == ref["ratio_cell_max"]
+    assert got["amax_global"] == ref["amax_global"] and got["vmax"] == ref["vmax"]
+    for k in ("vrms_global", "ratio_global", "ratio_criterion2", "drift_limit"):
+        assert abs(got[k] - ref[k]) <= 1e-12 * abs(ref[k]), (k, got[k], ref[k])
+    assert got == ctx.timestep_terms(vrms, amax, b, vmax)          # deterministic
+    # no velocities known: criterion 3 gives no bound; an all-empty box gives zeros
+    assert ctx.timestep_terms(vrms, amax, b)["drift_limit"] == float("inf")
+    e = ctx.bin(torch.empty(0, 3, device="cuda"), 3, 1.0)
+    z = torch.zeros(27, device="cuda")
+    t0 = ctx.timestep_terms(z, z, e)
+    assert t0["cells_used"] == 0 and t0["ratio_criterion2"] == 0.0 and t0["vrms_global"] == 0.0
+
+
 def test_step_cycle_force_kick_drift_rebin(ctx):
     """One slab-pipeline cycle on the device -- nf_bin, nf_forces_ex, nf_kick_drift, nf_bin again --
     against the same cycle on the oracle side.  The two sides' accelerations differ by rounding, so

@@ -524,3 +524,23 @@ def test_cell_vrms_definition():
     u = (3.0 * u / np.sqrt((u ** 2).sum(axis=1))[:, None]).astype(np.float32)
     got, _ = oracle.cell_vrms(u, key, K ** 3)
     assert np.allclose(got[np.bincount(key, minlength=K ** 3) > 0], 3.0, rtol=1e-6)
+
+
+def test_timestep_terms_hand_worked():
+    """Criteria 2 and 3 on a box worked by hand.  Four cells: A (n = 2, v_rms = 3,
+    a_max = 6), B (n = 6, v_rms = 1, a_max = 0.5), C empty, D (n = 2, v_rms = 2, a_max = 0: no ratio).
+    Cell ratios 0.5 and 2; global v_rms = sqrt((2*9 + 6*1 + 2*4) / 10) = sqrt(3.2); global a_max = 6."""
+    t = oracle.timestep_terms([3, 1, 7, 2], [6, 0.5, 9, 0], [2, 6, 0, 2], K=4, box=2.0, vmax=0.25)
+    assert t["cells_used"] == 2
+    assert t["ratio_cell_min"] == 0.5 and t["ratio_cell_max"] == 2.0
+    assert abs(t["vrms_global"] - np.sqrt(3.2)) < 1e-15
+    assert t["amax_global"] == 6.0                    # the empty cell's stale entries (7, 9) take no part
+    assert abs(t["ratio_global"] - np.sqrt(3.2) / 6.0) < 1e-15
+    # "use the maximum of the global and cell-based values ... protects us from ... abnormally cold cells": a cold
+    # cell (small v_rms, large a_max) must not shorten the step below the global value
+    assert t["ratio_criterion2"] == t["ratio_cell_min"] == 0.5        # here the cell value (0.5) exceeds the global 0.298
+    cold = oracle.timestep_terms([3, 1e-6, 7, 2], [6, 0.5, 9, 0], [2, 6, 0, 2], K=4, box=2.0, vmax=0.25)
+    assert cold["ratio_cell_min"] < 1e-5 and cold["ratio_criterion2"] == cold["ratio_global"]
+    # criterion 3: 0.8 * cell width / vmax = 0.8 * 0.5 / 0.25
+    assert abs(t["drift_limit"] - 1.6) < 1e-15
+    assert oracle.timestep_terms([1], [1], [1], K=1, box=1.0)["drift_limit"] == float("inf")
