@@ -610,14 +610,20 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
 
 // The next task for one consumer: pulled from the work list and prepared (header, piece table) as soon as the
 // last tile of the previous one has been issued, i.e. while the consumer still has up to two tiles to sweep.
+// The FIRST task of every consumer is assigned statically (`first` >= 0), interleaved over blocks and schedulers:
+// entry (c * N_PROD + scheduler) * blocks + block for consumer c of a scheduler, so that a work list shorter than a
+// few entries per warp is spread evenly over all SMs and schedulers instead of going to whichever blocks start
+// first (C1: 1200 tasks for 1776 consumer warps; 48 SMs used to get nothing).  Later tasks are pulled dynamically.
 template <int R>
 __device__ __noinline__ void produce_next_task(ConsShared<R> &S, const nf_plane_view *__restrict__ planes, const nf_force_params &p,
                                                const ForceConsts &fc, const Task *__restrict__ tasks, uint32_t *__restrict__ ctl,
-                                               uint32_t n_tasks, int lane)
+                                               uint32_t n_tasks, int lane, int first = -1)
 {
-    uint32_t ti = 0;
-    if (lane == 0) ti = atomicAdd(&ctl[0], 1u);
-    ti = __shfl_sync(0xffffffffu, ti, 0);
+    uint32_t ti = (uint32_t)first;
+    if (first < 0) {
+        if (lane == 0) ti = atomicAdd(&ctl[0], 1u) + gridDim.x * N_CONS;
+        ti = __shfl_sync(0xffffffffu, ti, 0);
+    }
     if (ti >= n_tasks) {
         if (lane == 0) S.p_state = 2u;            // work list exhausted: the consumer is told to stop at its next free buffer
         __syncwarp();
@@ -726,7 +732,8 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
 #pragma unroll
         for (int i = 0; i < CONS_PER_PROD; i++) tt[i] = 0;
         for (int i = 0; i < CONS_PER_PROD; i++)
-            produce_next_task<R>(CS[pw * CONS_PER_PROD + i], planes, p, fc, tasks, ctl, n_tasks, lane);
+            produce_next_task<R>(CS[pw * CONS_PER_PROD + i], planes, p, fc, tasks, ctl, n_tasks, lane,
+                                 (int)((i * N_PROD + pw) * gridDim.x + blockIdx.x));
         int remaining = CONS_PER_PROD;
         const uint32_t bell = smem_u32(&bells[pw]), relw = smem_u32(&released[pw * 4]);
         uint32_t bq = 0;                            // doorbell phase this producer waits on next
