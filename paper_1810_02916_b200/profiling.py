@@ -4,6 +4,9 @@
         per-kernel table of an `ncu --metrics gpu__time_duration.sum --csv` launch list
     python -m paper_1810_02916_b200.profiling full <raw.csv> <out.md> --title T --command C [--kernel REGEX] [--interactions I]
         the counters DESIGN.md quotes, from `ncu -i x.ncu-rep --page raw --csv`
+    python -m paper_1810_02916_b200.profiling sass <out.md>
+        SASS facts of the interaction kernel k_forces_warp<2, false> in the built libnf.so (cuobjdump -sass): mnemonic
+        counts that show the Blackwell instructions in use, and the body of the untracked (MODE 2) sweep loop
     python -m paper_1810_02916_b200.profiling traffic <workload> <ncu.csv> --command C
         records dram__bytes_read.sum / dram__bytes_write.sum of one interaction-kernel launch on <workload> in
         profiles/interaction_kernel_traffic.json together with the hash of the kernel sources it was captured
@@ -151,6 +154,75 @@ def cmd_full(a):
         fh.write("\n".join(out) + "\n")
 
 
+def cmd_sass(a):
+    import subprocess
+    lib = os.path.join(ROOT, "paper_1810_02916_b200", "libnf.so")
+    cmd = ["cuobjdump", "-sass", lib]
+    txt = subprocess.run(cmd, capture_output=True, text=True, check=True).stdout
+    m = re.search(r"Function : (\S*k_forces_warpILi2ELb0E\S*)(.*?)(?=\n\s*Function :|\Z)", txt, re.S)
+    if not m:
+        raise SystemExit("k_forces_warp<2, false> not found in " + lib)
+    lines = []
+    for l in m.group(2).splitlines():
+        mm = re.match(r"\s*/\*([0-9a-f]{4,5})\*/\s+(.*?);\s*/\*", l)
+        if mm:
+            lines.append((int(mm.group(1), 16), mm.group(2).strip()))
+    def opc(t):
+        f = t.split()
+        return (f[1] if f[0].startswith("@") else f[0]).split(".")[0]
+    cnt = {}
+    for _, t in lines:
+        cnt[opc(t)] = cnt.get(opc(t), 0) + 1
+    full = {}
+    for _, t in lines:
+        f = t.split()
+        k = f[1] if f[0].startswith("@") else f[0]
+        full[k] = full.get(k, 0) + 1
+    addr = {a_: i for i, (a_, _) in enumerate(lines)}
+    loops = []
+    for i, (a_, t) in enumerate(lines):
+        mm = re.search(r"\bBRA\s+0x([0-9a-f]+)", t)
+        if mm and "BRA.DIV" not in t:
+            tgt = int(mm.group(1), 16)
+            if tgt < a_ and tgt in addr:
+                body = lines[addr[tgt]:i + 1]
+                n2 = sum(1 for _, b in body if re.match(r"(@\S+\s+)?(FFMA2|FADD2|FMUL2)", b))
+                if n2 >= 100 and len(body) < 400:
+                    loops.append((tgt, a_, body, n2))
+    out = ["# SASS of the interaction kernel `k_forces_warp<2, false>` (built `libnf.so`, sm_100a)", "",
+           "Command: `python -m paper_1810_02916_b200.profiling sass <this file>`, i.e. `cuobjdump -sass paper_1810_02916_b200/libnf.so`",
+           f"on the library built from kernel sources sha256 {kernel_source_hash()[:16]}... (`python -m paper_1810_02916_b200.build`).", "",
+           f"Function `{m.group(1)}`: {len(lines)} instructions.", "",
+           "| mnemonic | count | what it shows |", "|---|---|---|"]
+    notes = {"UBLKCP": "cp.async.bulk (TMA 1-D bulk copy global -> shared)", "SYNCS": "mbarrier operations (arrive / expect_tx / try_wait)",
+             "FFMA2": "packed FP32 fused multiply-add (two sinks per instruction)", "FADD2": "packed FP32 add", "FMUL2": "packed FP32 multiply",
+             "FMNMX3": "three-input min: close-pair tracking of MODE 1", "FMNMX": "two-input min: the `min` form of Eq. 2 (MODE 0)",
+             "MUFU": "rsqrt (MUFU.RSQ) and the producer's reciprocal", "USETMAXREG": "setmaxnreg: registers moved from producers to consumers",
+             "LDS": "shared-memory loads (LDS.128 broadcast of a source)", "FENCE": "fence.proxy.async before a bulk copy reuses a buffer",
+             "NANOSLEEP": "the producer's timed sleep on its doorbell", "HMMA": "tensor-core MMA (none: not a contraction)", "UTCHMMA": "tcgen05 MMA (none)"}
+    for k in ["UBLKCP", "SYNCS", "USETMAXREG", "FFMA2", "FADD2", "FMUL2", "MUFU", "FMNMX3", "FMNMX", "LDS", "FENCE", "NANOSLEEP", "HMMA", "UTCHMMA"]:
+        out.append(f"| `{k}` | {cnt.get(k, 0)} | {notes[k]} |")
+    out += ["", "Sweep loops (backward branches enclosing >= 100 packed FP32 instructions):", "",
+            "| loop | instructions | FFMA2 | FADD2 | FMUL2 | MUFU.RSQ | FMNMX3 | FMNMX | LDS.128 | `.reuse` operands | which |", "|---|---|---|---|---|---|---|---|---|---|---|"]
+    mode2 = None
+    for tgt, a_, body, n2 in loops:
+        c = lambda pat: sum(1 for _, b in body if re.match(r"(@\S+\s+)?" + pat, b))
+        nm3, nm = c(r"FMNMX3"), c(r"FMNMX\b") + c(r"FMNMX\.")
+        which = "MODE 1 (tracked)" if nm3 else ("MODE 0 (min form)" if nm else "MODE 2 (untracked r^-3)")
+        if not nm3 and not nm and (mode2 is None or len(body) < len(mode2[2])):
+            mode2 = (tgt, a_, body)
+        out.append(f"| {tgt:#06x}-{a_:#06x} | {len(body)} | {c('FFMA2')} | {c('FADD2')} | {c('FMUL2')} | {c('MUFU.RSQ')} | {nm3} | {nm} | {c('LDS.128')} | "
+                   f"{sum(b.count('.reuse') for _, b in body)} | {which} |")
+    if mode2:
+        tgt, a_, body = mode2
+        out += ["", f"The MODE 2 loop ({tgt:#06x}-{a_:#06x}): 8 sources x 4 sinks per lane per iteration = 16 packed pairs x 11 FMA-pipe instructions + 32 MUFU.RSQ + 8 LDS.128.",
+                "First 48 instructions:", "", "```"]
+        out += [f"/*{x:04x}*/  {t}" for x, t in body[:48]]
+        out += ["```"]
+    with open(a.out, "w") as fh:
+        fh.write("\n".join(out) + "\n")
+
+
 def cmd_traffic(a):
     rd = wr = None
     t = None
@@ -189,9 +261,10 @@ def main():
     p.add_argument("--title", required=True); p.add_argument("--command", required=True); p.add_argument("--note", default="")
     p.add_argument("--kernel", default="k_forces_warp"); p.add_argument("--index", type=int, default=0)
     p.add_argument("--interactions", type=float, default=0.0)
+    p = sub.add_parser("sass"); p.add_argument("out")
     p = sub.add_parser("traffic"); p.add_argument("workload"); p.add_argument("csv"); p.add_argument("--command", required=True)
     a = ap.parse_args()
-    {"launches": cmd_launches, "full": cmd_full, "traffic": cmd_traffic}[a.what](a)
+    {"launches": cmd_launches, "full": cmd_full, "traffic": cmd_traffic, "sass": cmd_sass}[a.what](a)
 
 
 if __name__ == "__main__":
