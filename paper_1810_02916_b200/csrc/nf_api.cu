@@ -186,7 +186,7 @@ static int check_force_args(nf_ctx *ctx, int K, int R, float eps, float Gm, int 
     NF_ARG(ctx, eps > 0.0f && eps < 3.0e38f, "eps must be positive and finite");
     NF_ARG(ctx, Gm == Gm && fabsf(Gm) < 3.0e38f, "Gm must be finite");
     const int law = softening & NF_SOFT_LAW_MASK;
-    NF_ARG(ctx, (law == NF_SOFT_SPLINE || law == NF_SOFT_PLUMMER) && (softening & ~(NF_SOFT_LAW_MASK | NF_MASS_W)) == 0,
+    NF_ARG(ctx, (law == NF_SOFT_SPLINE || law == NF_SOFT_PLUMMER) && (softening & ~(NF_SOFT_LAW_MASK | NF_MASS_W | NF_DENSE_ORDER)) == 0,
            "unknown softening %d", softening);
     return NF_OK;
 }
@@ -210,8 +210,12 @@ static int forces_common(nf_ctx *ctx, const float *pos_sorted, const uint64_t *c
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = x_lo; p.sink_hi = x_hi;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
+    // in-cell ordering of dense cells (nf_dense.cu): asked for with NF_DENSE_ORDER, and automatic when the MEAN occupancy
+    // already says that cells are dense -- decided from the arguments alone, so that the same call always takes the same path
+    const bool dense = N >= NF_DENSE_N && ((softening & NF_DENSE_ORDER) || N / ((int64_t)K * K * K) >= 512);
+    p.softening = softening & ~NF_DENSE_ORDER;
     nf_scratch_reset(ctx);
-    NF_TRY(nf_scratch_reserve(ctx, forces_scratch_full(N, K)));
+    NF_TRY(nf_scratch_reserve(ctx, forces_scratch_full(N, K) + (dense ? nf_dense_scratch_bytes(N, K) : 0)));
     nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
     float4 *enc = nf_scratch_take<float4>(ctx, (size_t)N);
     float4 *enc_h = nf_scratch_take<float4>(ctx, (size_t)N);
@@ -219,8 +223,10 @@ static int forces_common(nf_ctx *ctx, const float *pos_sorted, const uint64_t *c
     cudaStream_t st = (cudaStream_t)stream;
     const float4 *ps = reinterpret_cast<const float4 *>(pos_sorted);
     NF_TRY(nf_encode_impl(ctx, p, ps, cell_offset, (size_t)K * K * K, enc, enc_h, st));
+    uint32_t *dinfo = nullptr;
+    if (dense) NF_TRY(nf_dense_order_impl(ctx, p, ps, cell_offset, N, enc, enc_h, &dinfo, st));
     if (cell_amax) NF_CUDA(ctx, cudaMemsetAsync(cell_amax, 0, sizeof(float) * (size_t)K * K * K, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, ps, enc, enc_h, cell_offset, perm, acc_xyz, cell_amax, st));
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, ps, enc, enc_h, cell_offset, perm, acc_xyz, cell_amax, dinfo, st));
     return nf_forces_impl(ctx, p, d_planes, st, true);
 }
 
@@ -318,7 +324,7 @@ int nf_forces_host_m(nf_ctx *ctx, const float *pos_host, const float *mass_host,
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
     NF_TRY(nf_encode_impl(ctx, p, reinterpret_cast<const float4 *>(sorted), off, ncell, enc, enc_h, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, acc, nullptr, st));
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, acc, nullptr, nullptr, st));
     NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
     NF_CUDA(ctx, cudaMemcpyAsync(acc_host, acc, n * 12, cudaMemcpyDeviceToHost, st));
     NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
@@ -416,7 +422,7 @@ int nf_forces_host_begin(nf_ctx *ctx, const float *pos_host, int64_t N, int K, i
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
     NF_TRY(nf_encode_impl(ctx, p, reinterpret_cast<const float4 *>(sorted), off, ncell, enc, enc_h, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, hp->acc[i], nullptr, st));
+    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, hp->acc[i], nullptr, nullptr, st));
     NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
     NF_CUDA(ctx, cudaMemcpyAsync(hp->h_bad + i, ctx->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     NF_CUDA(ctx, cudaEventRecord(hp->ev_done[i], st));

@@ -87,10 +87,12 @@ __device__ __forceinline__ unsigned same_digit_lanes(unsigned act, uint32_t d, u
 }
 
 // per-tile digit histogram -> hist[digit * ntiles + tile]
-__global__ void __launch_bounds__(RS_THREADS) k_radix_hist(const uint32_t *__restrict__ keys, int64_t N, Digit dg,
-                                                           uint32_t *__restrict__ hist, uint32_t ntiles)
+// n_dev (nullable): the element count lives on the device (at most N); tiles past it count nothing
+__global__ void __launch_bounds__(RS_THREADS) k_radix_hist(const uint32_t *__restrict__ keys, int64_t N, const uint32_t *__restrict__ n_dev,
+                                                           Digit dg, uint32_t *__restrict__ hist, uint32_t ntiles)
 {
     extern __shared__ uint32_t sh[];
+    if (n_dev) N = min(N, (int64_t)*n_dev);
     const uint32_t K = dg.K;
     for (uint32_t d = threadIdx.x; d < K; d += RS_THREADS) sh[d] = 0;
     __syncthreads();
@@ -111,11 +113,13 @@ __global__ void __launch_bounds__(RS_THREADS) k_radix_hist(const uint32_t *__res
 // 4-byte stores scattered over the whole array.  idx_in == nullptr means "identity" (first pass).
 // shared: cnt[RS_WARPS][K] | gdelta[K] | wsum[RS_WARPS] | skey[RS_TILE] | sidx[RS_TILE]
 __global__ void __launch_bounds__(RS_THREADS) k_radix_scatter(const uint32_t *__restrict__ keys_in, const uint32_t *__restrict__ idx_in,
-                                                              int64_t N, Digit dg,
+                                                              int64_t N, const uint32_t *__restrict__ n_dev, Digit dg,
                                                               const uint32_t *__restrict__ hist_scanned, uint32_t ntiles,
                                                               uint32_t *__restrict__ keys_out, uint32_t *__restrict__ idx_out)
 {
     extern __shared__ uint32_t sh[];
+    if (n_dev) N = min(N, (int64_t)*n_dev);
+    if ((int64_t)blockIdx.x * RS_TILE >= N) return;
     const uint32_t K = dg.K;
     uint32_t *gdelta = sh + (size_t)RS_WARPS * K;
     uint32_t *wsum = gdelta + K;
@@ -287,6 +291,29 @@ size_t nf_bin_scratch_bytes(int64_t N, int K, bool plane)
     return b + 4096;
 }
 
+// One stable LSD pass over (key, index) pairs by the digit (key >> shift) & (bins - 1), bins a power of two <= 1024.  The
+// element count may live on the device (n_dev, at most n_max).  hist: bins * ceil(n_max / RS_TILE) words; tmp32: its scan temp.
+size_t nf_radix_tiles(int64_t n_max) { return n_max > 0 ? ((size_t)n_max + RS_TILE - 1) / RS_TILE : 1; }
+int nf_radix_pass(nf_ctx *ctx, const uint32_t *kin, const uint32_t *iin, int64_t n_max, const uint32_t *n_dev, uint32_t bins,
+                  uint32_t shift, uint32_t *kout, uint32_t *iout, uint32_t *hist, uint32_t *tmp32, cudaStream_t st)
+{
+    if (n_max <= 0) return NF_OK;
+    const size_t ntiles = nf_radix_tiles(n_max);
+    Digit dg;
+    dg.div = 1u << shift; dg.K = bins; dg.sh = shift; dg.mask = bins - 1;
+    dg.nbits = 0;
+    while ((1u << dg.nbits) < bins) dg.nbits++;
+    const size_t sh_hist = (size_t)bins * sizeof(uint32_t);
+    const size_t sh_scat = ((size_t)bins * RS_WARPS + (size_t)bins + 32 + 2 * (size_t)RS_TILE) * sizeof(uint32_t);
+    k_radix_hist<<<(unsigned)ntiles, RS_THREADS, sh_hist, st>>>(kin, n_max, n_dev, dg, hist, (uint32_t)ntiles);
+    NF_LAUNCHED(ctx);
+    NF_TRY(nf_exclusive_scan_u32(ctx, hist, hist, (size_t)bins * ntiles, tmp32, st));
+    NF_CUDA(ctx, cudaFuncSetAttribute(k_radix_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh_scat));
+    k_radix_scatter<<<(unsigned)ntiles, RS_THREADS, sh_scat, st>>>(kin, iin, n_max, n_dev, dg, hist, (uint32_t)ntiles, kout, iout);
+    NF_LAUNCHED(ctx);
+    return NF_OK;
+}
+
 // a1 alone: keys (cx*K+cy)*K+cz of N positions, no histogram; out-of-range particles counted in counters[0]
 int nf_keys_impl(nf_ctx *ctx, const float *pos, int64_t N, int K, float box, uint32_t *keys, cudaStream_t st)
 {
@@ -344,11 +371,11 @@ int nf_bin_impl(nf_ctx *ctx, const float *pos, const float *mass, int64_t N, int
         if ((K & (K - 1)) == 0) { dg.sh = 0; while ((1u << dg.sh) < div) dg.sh++; }
         dg.nbits = 0;
         while ((1u << dg.nbits) < (uint32_t)K) dg.nbits++;
-        k_radix_hist<<<(unsigned)ntiles, RS_THREADS, sh_hist, st>>>(kin, N, dg, hist, (uint32_t)ntiles);
+        k_radix_hist<<<(unsigned)ntiles, RS_THREADS, sh_hist, st>>>(kin, N, nullptr, dg, hist, (uint32_t)ntiles);
         NF_LAUNCHED(ctx);
         NF_TRY(nf_exclusive_scan_u32(ctx, hist, hist, (size_t)K * ntiles, tmp32, st));
         NF_CUDA(ctx, cudaFuncSetAttribute(k_radix_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh_scat));
-        k_radix_scatter<<<(unsigned)ntiles, RS_THREADS, sh_scat, st>>>(kin, iin, N, dg, hist, (uint32_t)ntiles, kout, iout);
+        k_radix_scatter<<<(unsigned)ntiles, RS_THREADS, sh_scat, st>>>(kin, iin, N, nullptr, dg, hist, (uint32_t)ntiles, kout, iout);
         NF_LAUNCHED(ctx);
         kin = kout;
         iin = iout;

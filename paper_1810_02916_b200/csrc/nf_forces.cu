@@ -35,6 +35,7 @@ struct ForceConsts {
     float scale;        // 2^k
     float ws;           // cell width in internal units, (box / K) * scale
     float out_scale;    // Gm * scale^2: a = out_scale * sum f' d'
+    float box_far2;     // (eps' (1 + 4e-3))^2: two boxes further apart than this hold no pair inside eps (margin: float32 shifts, z-block encoding)
     float near_lo;      // -(ws/2 - eps' - margin): a sink offset below it (above its negative) is "near" that face of its cell
     int flags;          // FC_FAR_OK: a cell width exceeds eps, so cells two or more apart hold no pair inside eps;  FC_PLUMMER
 };
@@ -204,7 +205,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // of the encoding (<= 2^-23 ws) is the same size as that of the x/y column shifts, and
 // differences inside one cell stay exact.
 // ------------------------------------------------------------------------------------------
-constexpr int ZB = 8;
+constexpr int ZB = NF_ZB;
 
 __global__ void __launch_bounds__(256) k_encode(const float4 *__restrict__ pos, const uint64_t *__restrict__ off, size_t ncell, int K,
                                                 float scale, float ws, float4 *__restrict__ enc, float4 *__restrict__ enc_h)
@@ -452,6 +453,7 @@ struct TaskHdr {                            // what a consumer needs to know abo
     uint64_t s0;                            // first sink (slot in the plane's arrays)
     uint32_t n, L, cyz;
     uint32_t part, nparts, slot;                // source split: this entry is part `part` of `nparts`, partial sums in slots slot..slot+nparts-1
+    uint32_t eoff;                              // dense own cell: compact position of the task's first sink (nf_dense.cu), else 0xffffffff
 };
 
 template <int R>
@@ -465,10 +467,11 @@ struct ConsShared {
     unsigned long long full[2];
     // producer's cursor for this consumer
     uint32_t p_npieces, p_cur_piece, p_j, p_nparts, p_P, p_invP, p_seq, p_state;   // p_state 0: inside a task, 1: next tile starts a task, 2: stop
+    uint32_t p_tchunk0, p_tnchunk;          // dense own cell: first box and number of boxes (<= 3) of the task's sinks; 0 boxes = not dense
 };
 
 // ---- producer: everything about task ti that does not need the FMA pipe -------------------------------
-template <int R>
+template <int R, bool DENSE>
 __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view *__restrict__ planes, const nf_force_params &p,
                                              const ForceConsts &fc, const Task task, uint32_t seq, int lane)
 {
@@ -486,6 +489,8 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
     // which of the two encoded copies: the one whose z-blocks do not cut cz-R..cz+R (if any)
     const int zphi = ((cz - R + ZB * 4) / ZB != (cz + R + ZB * 4) / ZB) ? ZB / 2 : 0;
     const float4 *se = zphi ? sp.enc_h : sp.enc;
+    // dense own cell (nf_dense.cu): its encoded copies are ordered along a Morton curve with a box per 64 particles
+    const uint32_t own_di = (DENSE && p.dense_slot && sp.dinfo) ? sp.dinfo[task.cyz] : 0u;
     if (lane < W) {
         int px = sink_plane + lane - R;
         if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
@@ -497,7 +502,10 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
         h.se = se; h.acc = sp.acc; h.perm = sp.perm; h.amax = sp.amax; h.s0 = s0;
         h.n = (uint32_t)n; h.L = (uint32_t)L; h.cyz = task.cyz;
         h.part = task.part_slot & 0xffu; h.nparts = task.nparts; h.slot = task.part_slot >> 8;
+        h.eoff = own_di ? (own_di - 1u) * 64u + task.first : 0xffffffffu;
         S.hdr[seq & 3u] = h;
+        S.p_tchunk0 = own_di ? own_di - 1u + (task.first >> 6) : 0u;
+        S.p_tnchunk = own_di ? ((task.first + (uint32_t)n - 1u) >> 6) - (task.first >> 6) + 1u : 0u;
         S.p_P = (uint32_t)P;
         S.p_invP = (65536u + P - 1) / P;        // floor(x / P) == (x * inv_P) >> 16 for x < 1024
     }
@@ -519,7 +527,7 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
     int n_pieces = 0;
     for (int rb = 0; rb < NR; rb += 32) {
         const int r = rb + lane;
-        uint32_t st[W], cn[W];
+        uint32_t st[W], cn[W], di[W];
         int kz[W];
         bool newp[W];
         int np = 0;
@@ -533,6 +541,7 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
             else if (px < 0 || px >= p.n_planes) px = -1;
             const int qy = ((cy + dyi - R) % K + K) % K;
             const uint64_t *qo = px >= 0 ? planes[px].off + (size_t)qy * K : nullptr;
+            const uint32_t *qd = (DENSE && own_di && px >= 0 && planes[px].dinfo) ? planes[px].dinfo + (size_t)qy * K : nullptr;
             uint32_t prev_end = 0;
             int prev_k = 0;
             bool have = false;
@@ -541,8 +550,11 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
                 const int qz = ((cz + s - R) % K + K) % K;
                 st[s] = 0; cn[s] = 0;
                 if (qo) { st[s] = (uint32_t)qo[qz]; cn[s] = (uint32_t)(qo[qz + 1] - qo[qz]); }
+                di[s] = (DENSE && qd) ? qd[qz] : 0u;
                 kz[s] = (s - R) - ((qz + zphi) % ZB) + ((cz + zphi) % ZB);
-                const bool self = col == NR / 2 && s == R;    // the sinks' own cell: a piece of its own
+                // the sinks' own cell is a piece of its own, and so is every dense cell seen from a dense cell (its tiles get
+                // their law from the boxes, tile by tile)
+                const bool self = (col == NR / 2 && s == R) || di[s] != 0u;
                 newp[s] = cn[s] > 0 && (self || !(have && prev_end == st[s] && prev_k == kz[s]));
                 if (cn[s] > 0) { have = !self; prev_end = st[s] + cn[s]; prev_k = kz[s]; }
                 np += newp[s] ? 1 : 0;
@@ -578,7 +590,11 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
                     else if (own_col && s == R) mode = 0u;
                     else if (far_col) mode = 2u;
                     else if ((near & need) != need) mode = 2u;
-                    S.piece[slot] = make_uint4(st[s], cn[s], (uint32_t)col | ((uint32_t)(kz[s] + 128) << 8) | ((uint32_t)dxi << 16) | (mode << 27), 0u);
+                    // .w: balanced tile length (bits 0-8, set below) | first box of a dense cell << 9; .z bit 24: dense piece,
+                    // bits 29-31: the cell's place s in its column (both masked out of the descriptor)
+                    S.piece[slot] = make_uint4(st[s], cn[s], (uint32_t)col | ((uint32_t)(kz[s] + 128) << 8) | ((uint32_t)dxi << 16) | (mode << 27) |
+                                                                 (di[s] ? (1u << 24) | ((uint32_t)s << 29) : 0u),
+                                               di[s] ? (di[s] - 1u) << 9 : 0u);
                 } else {
                     S.piece[slot].y += cn[s];
                 }
@@ -591,14 +607,14 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
     for (int i = lane; i < n_pieces; i += 32) {
         const uint32_t cnt = S.piece[i].y;
         const uint32_t nt = (cnt + tile_max - 1) / tile_max;
-        S.piece[i].w = (cnt + nt - 1) / nt;
+        S.piece[i].w |= (cnt + nt - 1) / nt;
     }
     __syncwarp();
     // the entry's first tile: tile number `part` of the task's tile sequence (every nparts-th tile is its own)
     uint32_t cp = 0, j = task.part_slot & 0xffu;
     while (cp < (uint32_t)n_pieces) {
         const uint4 pc = S.piece[cp];
-        const uint32_t nt = (pc.y + pc.w - 1) / pc.w;
+        const uint32_t pw = pc.w & 0x1ffu, nt = (pc.y + pw - 1) / pw;
         if (j < nt) break;
         j -= nt;
         cp++;
@@ -614,7 +630,7 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
 // entry (c * N_PROD + scheduler) * blocks + block for consumer c of a scheduler, so that a work list shorter than a
 // few entries per warp is spread evenly over all SMs and schedulers instead of going to whichever blocks start
 // first (C1: 1200 tasks for 1776 consumer warps; 48 SMs used to get nothing).  Later tasks are pulled dynamically.
-template <int R>
+template <int R, bool DENSE>
 __device__ __noinline__ void produce_next_task(ConsShared<R> &S, const nf_plane_view *__restrict__ planes, const nf_force_params &p,
                                                const ForceConsts &fc, const Task *__restrict__ tasks, uint32_t *__restrict__ ctl,
                                                uint32_t n_tasks, int lane, int first = -1)
@@ -630,14 +646,14 @@ __device__ __noinline__ void produce_next_task(ConsShared<R> &S, const nf_plane_
         return;
     }
     const uint32_t seq = S.p_seq;
-    produce_task<R>(S, planes, p, fc, tasks[ti], seq, lane);
+    produce_task<R, DENSE>(S, planes, p, fc, tasks[ti], seq, lane);
     if (lane == 0) { S.p_seq = seq + 1; S.p_state = 1u; }     // 1: the next tile issued is the first of a task
     __syncwarp();
 }
 
 // The next tile for one consumer into its free buffer b.  Returns false when the work list is exhausted (the
 // consumer has then been told to stop).
-template <int R>
+template <int R, bool DENSE>
 __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view *__restrict__ planes, const nf_force_params &p,
                                           const ForceConsts &fc, const Task *__restrict__ tasks, uint32_t *__restrict__ ctl,
                                           uint32_t n_tasks, int b, int lane)
@@ -655,17 +671,18 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
     uint32_t flags = state == 1u ? (D_FIRST | (((S.p_seq - 1u) & 3u) << 25)) : 0u;      // bits 25-26: header slot
     const uint32_t cur_piece = S.p_cur_piece, cur_j = S.p_j, n_pieces = S.p_npieces;
     const uint4 pc = S.piece[cur_piece];
-    const uint32_t start = pc.x + cur_j * pc.w;
-    const uint32_t tn = min(pc.w, pc.y - cur_j * pc.w);
+    const uint32_t pcw = pc.w & 0x1ffu;            // balanced tile length of the piece
+    const uint32_t start = pc.x + cur_j * pcw;
+    const uint32_t tn = min(pcw, pc.y - cur_j * pcw);
     // the entry's next tile: nparts tiles further along the task's tile sequence
     const uint32_t nparts = S.p_nparts;
     uint32_t np = cur_piece, nj = cur_j + nparts;
     if (nparts == 1) {                          // not split (the usual case): no division
-        if (nj * pc.w >= pc.y) { np++; nj = 0; }
+        if (nj * pcw >= pc.y) { np++; nj = 0; }
     } else {
         while (np < n_pieces) {
             const uint4 qc = S.piece[np];
-            const uint32_t nt = (qc.y + qc.w - 1) / qc.w;
+            const uint32_t qw = qc.w & 0x1ffu, nt = (qc.y + qw - 1) / qw;
             if (nj < nt) break;
             nj -= nt;
             np++;
@@ -680,7 +697,34 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
     if (tn + lane < P * q) buf[tn + lane] = SENT;
     if (tn + 32 + lane < P * q) buf[tn + 32 + lane] = SENT;
     const float4 *src = S.enc[(pc.z >> 16) & 0xff] + start;
-    if (lane == 0) S.desc[b] = make_uint4(tn | (q << 16), (pc.z & 0x19ffffffu) | flags, 0u, 0u);
+    uint32_t meta = pc.z & 0x19ffffffu;
+    if (DENSE && ((pc.z >> 24) & 1u)) {
+        // A dense cell seen from a dense cell: the law of this tile follows from the boxes (one per 64 particles in Morton
+        // order) of the task's sinks (<= 3) and of the tile's sources (<= 9: a tile has at most 508 of them).  If every pair of boxes is further apart than
+        // eps, no pair of particles is inside eps and the untracked r^-3 sweep is exact (fn. 4); the tile of the
+        // own cell then holds none of the task's sinks either (no r = 0 pair).  Else: the min form for the own cell,
+        // tracking for the others.  Boxes are in scaled cell-centred offsets; the source cell's frame is shifted by whole cells.
+        const uint32_t o0 = cur_j * pcw, k0 = o0 >> 6, nk = ((o0 + tn - 1u) >> 6) - k0 + 1u;
+        const uint32_t ntc = S.p_tnchunk;
+        const int col = (int)(pc.z & 0xffu), dxi = (int)((pc.z >> 16) & 0xffu), dyi = col - dxi * (2 * R + 1), szi = (int)(pc.z >> 29);
+        bool nearp = false;
+        const uint32_t a = (uint32_t)lane / 10u, bq = (uint32_t)lane % 10u;     // 3 x 10 pairs of boxes, one per lane
+        if (a < ntc && bq < nk) {
+            const float *A = p.dense_box + 6 * (size_t)(S.p_tchunk0 + a), *B = p.dense_box + 6 * (size_t)((pc.w >> 9) + k0 + bq);
+            const float sh[3] = {(float)(dxi - R) * fc.ws, (float)(dyi - R) * fc.ws, (float)(szi - R) * fc.ws};
+            float g2 = 0.f;
+#pragma unroll
+            for (int ax = 0; ax < 3; ax++) {
+                const float g = fmaxf(fmaxf(A[ax] - (B[3 + ax] + sh[ax]), (B[ax] + sh[ax]) - A[3 + ax]), 0.f);
+                g2 = fmaf(g, g, g2);
+            }
+            nearp = !(g2 > fc.box_far2);
+        }
+        const bool own = col == (2 * R + 1) * (2 * R + 1) / 2 && szi == R;
+        const uint32_t mode = __any_sync(0xffffffffu, nearp) ? (own ? 0u : 1u) : 2u;
+        if (!(fc.flags & FC_PLUMMER)) meta = (meta & ~(3u << 27)) | (mode << 27);
+    }
+    if (lane == 0) S.desc[b] = make_uint4(tn | (q << 16), meta | flags, 0u, 0u);
     fence_proxy_async();          // the sentinel stores (generic proxy) before the bulk copy into the same buffer
     __syncwarp();                 // ... and every lane has read the cursor before lane 0 moves it
     if (lane == 0) {
@@ -693,11 +737,11 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
     }
     __syncwarp();
     // the task's last tile is on its way and its piece table is dead: prepare the next task now
-    if (last) produce_next_task<R>(S, planes, p, fc, tasks, ctl, n_tasks, lane);
+    if (last) produce_next_task<R, DENSE>(S, planes, p, fc, tasks, ctl, n_tasks, lane);
     return true;
 }
 
-template <int R, bool MASS>
+template <int R, bool MASS, bool DENSE>
 __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const nf_plane_view *__restrict__ planes, const nf_force_params p,
                                                                              const ForceConsts fc, const Task *__restrict__ tasks,
                                                                              uint32_t *__restrict__ ctl, float *__restrict__ partial,
@@ -732,7 +776,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
 #pragma unroll
         for (int i = 0; i < CONS_PER_PROD; i++) tt[i] = 0;
         for (int i = 0; i < CONS_PER_PROD; i++)
-            produce_next_task<R>(CS[pw * CONS_PER_PROD + i], planes, p, fc, tasks, ctl, n_tasks, lane,
+            produce_next_task<R, DENSE>(CS[pw * CONS_PER_PROD + i], planes, p, fc, tasks, ctl, n_tasks, lane,
                                  (int)((i * N_PROD + pw) * gridDim.x + blockIdx.x));
         int remaining = CONS_PER_PROD;
         const uint32_t bell = smem_u32(&bells[pw]), relw = smem_u32(&released[pw * 4]);
@@ -753,7 +797,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
                 if (!progress) fence_acq_rel_cta();  // the consumer's reads of the buffer (released with st.release) before our copy into it
                 progress = true;
                 ConsShared<R> &S = CS[pw * CONS_PER_PROD + i];
-                if (produce_tile<R>(S, planes, p, fc, tasks, ctl, n_tasks, (int)(t & 1u), lane)) tt[i] = t + 1;
+                if (produce_tile<R, DENSE>(S, planes, p, fc, tasks, ctl, n_tasks, (int)(t & 1u), lane)) tt[i] = t + 1;
                 else { tt[i] = 1u << 31; remaining--; }
             }
             // nothing to do: every buffer is full.  Sleep in hardware on the doorbell (no issue slots) until one of
@@ -905,7 +949,8 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
                             fz = (float)(ssz * (double)fc.out_scale);
                 a2max = fmaxf(a2max, fx * fx + fy * fy + fz * fz);
                 if (h.acc) {
-                    const uint64_t si = h.s0 + (uint64_t)i;
+                    // sorted slot of sink i: its encoded copy may sit elsewhere inside a dense cell (nf_dense.cu)
+                    const uint64_t si = (DENSE && h.eoff != 0xffffffffu) ? (uint64_t)p.dense_slot[h.eoff + (uint32_t)i] : h.s0 + (uint64_t)i;
                     const uint64_t o = h.perm ? (uint64_t)h.perm[si] : si;
                     h.acc[3 * o + 0] = fx;
                     h.acc[3 * o + 1] = fy;
@@ -958,7 +1003,7 @@ __global__ void __launch_bounds__(256) k_interactions(const uint32_t *__restrict
 }
 
 __global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
-                              const uint64_t *off, const uint32_t *perm, float *acc, float *amax)
+                              const uint64_t *off, const uint32_t *perm, float *acc, float *amax, const uint32_t *dinfo)
 {
     int cx = blockIdx.x * blockDim.x + threadIdx.x;
     if (cx >= K) return;
@@ -970,6 +1015,7 @@ __global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, c
     v.perm = perm;
     v.acc = acc;
     v.amax = amax ? amax + (size_t)cx * K * K : nullptr;
+    v.dinfo = dinfo ? dinfo + (size_t)cx * K * K : nullptr;
     planes[cx] = v;
 }
 
@@ -1022,6 +1068,7 @@ ForceConsts make_consts(const nf_force_params &p)
     fc.C = (float)(6.0 / (es * es * es * es * es));
     fc.r2_floor = plummer ? (float)(es * es) : 8.673617379884035e-19f;  // 2^-60
     fc.eps2_test = plummer ? 0.0f : (float)(es * es * 1.0001);
+    fc.box_far2 = (float)(es * es * 1.008);
     fc.out_scale = (float)((double)p.Gm * (double)scale * (double)scale);
     // sources two or more cells away are at least one cell width (minus rounding) from every sink of the cell
     // margin: 1e-3 of a cell for the float32 rounding of the cell assignment (a particle may sit a few ulp of
@@ -1117,11 +1164,18 @@ int nf_forces_init(nf_ctx *ctx)
 }
 
 int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
-                        const uint64_t *off, const uint32_t *perm, float *acc, float *cell_amax, cudaStream_t st)
+                        const uint64_t *off, const uint32_t *perm, float *acc, float *cell_amax, const uint32_t *dinfo, cudaStream_t st)
 {
-    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, enc, enc_h, off, perm, acc, cell_amax);
+    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, enc, enc_h, off, perm, acc, cell_amax, dinfo);
     NF_LAUNCHED(ctx);
     return NF_OK;
+}
+
+void nf_encode_consts(const nf_force_params &p, float *scale, float *ws)
+{
+    const ForceConsts fc = make_consts(p);
+    *scale = fc.scale;
+    *ws = fc.ws;
 }
 
 int nf_encode_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, float4 *enc,
@@ -1144,19 +1198,28 @@ int nf_interactions_planes(nf_ctx *ctx, const nf_force_params &p, const nf_plane
     return NF_OK;
 }
 
-template <int R, bool MASS>
-static int launch_warp(nf_ctx *ctx, const nf_force_params &p, const ForceConsts &fc, const nf_plane_view *d_planes,
+template <int R, bool MASS, bool DENSE>
+static int launch_warp_d(nf_ctx *ctx, const nf_force_params &p, const ForceConsts &fc, const nf_plane_view *d_planes,
                        const Task *tasks, uint32_t *ctl, float *partial, uint32_t *arrive, cudaStream_t st)
 {
     // one block per SM: 12 consumer + 4 producer warps, the consumers' tile buffers fill the shared memory
     const size_t smem = sizeof(ConsShared<R>) * N_CONS + N_PROD * (sizeof(unsigned long long) + 4 * sizeof(uint32_t));
-    NF_CUDA(ctx, cudaFuncSetAttribute(k_forces_warp<R, MASS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NF_CUDA(ctx, cudaFuncSetAttribute(k_forces_warp<R, MASS, DENSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const size_t want = (max_tasks(p) + N_CONS - 1) / N_CONS;
     size_t blocks = (size_t)ctx->sm_count;
     if (blocks > want) blocks = want;
-    k_forces_warp<R, MASS><<<(unsigned)blocks, (N_CONS + N_PROD) * 32, smem, st>>>(d_planes, p, fc, tasks, ctl, partial, arrive);
+    k_forces_warp<R, MASS, DENSE><<<(unsigned)blocks, (N_CONS + N_PROD) * 32, smem, st>>>(d_planes, p, fc, tasks, ctl, partial, arrive);
     NF_LAUNCHED(ctx);
     return NF_OK;
+}
+
+// the kernel with the dense-cell logic of nf_dense.cu is a separate instance: the common path pays nothing for it
+template <int R, bool MASS>
+static int launch_warp(nf_ctx *ctx, const nf_force_params &p, const ForceConsts &fc, const nf_plane_view *d_planes,
+                       const Task *tasks, uint32_t *ctl, float *partial, uint32_t *arrive, cudaStream_t st)
+{
+    if (p.dense_slot) return launch_warp_d<R, MASS, true>(ctx, p, fc, d_planes, tasks, ctl, partial, arrive, st);
+    return launch_warp_d<R, MASS, false>(ctx, p, fc, d_planes, tasks, ctl, partial, arrive, st);
 }
 
 int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d_planes,

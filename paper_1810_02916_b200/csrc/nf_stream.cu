@@ -217,6 +217,7 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
         S->h_views[q].perm = sl.perm;
         S->h_views[q].acc = sl.acc;
         S->h_views[q].amax = nullptr;
+        S->h_views[q].dinfo = nullptr;
     }
     NF_CUDA(ctx, cudaMemcpyAsync(S->d_views, S->h_views, sizeof(nf_plane_view) * NP, cudaMemcpyHostToDevice, st));
     NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st));

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libnf.so")
 NF_OK, NF_ERR_ARG, NF_ERR_NOMEM, NF_ERR_CUDA, NF_ERR_RANGE = 0, 1, 2, 3, 4
 SOFT_SPLINE, SOFT_PLUMMER = 0, 1
 NF_MASS_W = 0x100
+NF_DENSE_ORDER = 0x200
 _SOFT = {"spline": SOFT_SPLINE, "plummer": SOFT_PLUMMER}
 
 # every symbol include/nf.h declares
@@ -228,31 +229,34 @@ class Context:
 
     def forces_chunk(self, b: Binned, R: int, eps: float, Gm: float, x_lo: int, x_hi: int, softening: str = "spline",
                      original_order: bool = True, out: Optional[torch.Tensor] = None, stream=None,
-                     use_mass: bool = False, cell_amax: Optional[torch.Tensor] = None) -> torch.Tensor:
+                     use_mass: bool = False, cell_amax: Optional[torch.Tensor] = None, dense_order: bool = False) -> torch.Tensor:
         """nf_forces_chunk: accelerations of the particles in x-planes [x_lo, x_hi) only (rows of the other
         particles -- ghosts -- are left untouched); every particle of ``b`` acts as a source."""
         acc = out if out is not None else torch.zeros(b.N, 3, dtype=torch.float32, device=b.pos_sorted.device)
         assert acc.is_cuda and acc.dtype == torch.float32 and acc.shape == (b.N, 3) and acc.is_contiguous()
         self._check(self.lib.nf_forces_chunk(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset),
                                              _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
-                                             float(b.box), float(Gm), _SOFT[softening] | (NF_MASS_W if use_mass else 0),
+                                             float(b.box), float(Gm),
+                                             _SOFT[softening] | (NF_MASS_W if use_mass else 0) | (NF_DENSE_ORDER if dense_order else 0),
                                              int(x_lo), int(x_hi), _ptr(acc), _ptr(cell_amax), self._stream(stream)))
         return acc
 
     def forces(self, b: Binned, R: int, eps: float, Gm: float, softening: str = "spline",
                original_order: bool = True, out: Optional[torch.Tensor] = None, stream=None,
-               use_mass: bool = False, cell_amax: Optional[torch.Tensor] = None) -> torch.Tensor:
+               use_mass: bool = False, cell_amax: Optional[torch.Tensor] = None, dense_order: bool = False) -> torch.Tensor:
         """nf_forces: accelerations float32 [N, 3] (caller's order if original_order).
         use_mass: sources carry their masses in pos_sorted[:, 3] (NF_MASS_W; Gm is then G).
+        dense_order: NF_DENSE_ORDER, the in-cell ordering of dense cells (automatic when N / K^3 >= 512).
         cell_amax: float32 [K^3] device tensor to receive the per-cell max |a| (nf_forces_ex)."""
         acc = out if out is not None else torch.empty(b.N, 3, dtype=torch.float32, device=b.pos_sorted.device)
         assert acc.is_cuda and acc.dtype == torch.float32 and acc.shape == (b.N, 3) and acc.is_contiguous()
-        if use_mass or cell_amax is not None:
+        if use_mass or cell_amax is not None or dense_order:
             if cell_amax is not None:
                 assert cell_amax.is_cuda and cell_amax.dtype == torch.float32 and cell_amax.numel() == b.K ** 3 and cell_amax.is_contiguous()
             self._check(self.lib.nf_forces_ex(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset), _ptr(b.cell_count),
                                               _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
-                                              float(b.box), float(Gm), _SOFT[softening] | (NF_MASS_W if use_mass else 0),
+                                              float(b.box), float(Gm),
+                                              _SOFT[softening] | (NF_MASS_W if use_mass else 0) | (NF_DENSE_ORDER if dense_order else 0),
                                               _ptr(acc), _ptr(cell_amax), self._stream(stream)))
             return acc
         self._check(self.lib.nf_forces(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset), _ptr(b.cell_count),

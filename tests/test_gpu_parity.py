@@ -667,8 +667,9 @@ def test_stream_slabs_randomised(ctx, seed):
     assert stats["interactions"] == oracle.interactions(cnt, K, R, plane0 + R, plane0 + R + P)
 
 
+@pytest.mark.parametrize("dense_order", [False, True])
 @pytest.mark.parametrize("seed", list(range(6)))
-def test_forces_dense_cells_randomised(ctx, seed):
+def test_forces_dense_cells_randomised(ctx, seed, dense_order):
     """Few cells, many particles (cells of 10^3 - 6x10^4): full 128-sink tasks, the dense-cells-first
     part of the work list, columns cut into many tiles, K down to 2R+1; sampled sinks against the oracle."""
     rng = np.random.default_rng(4000 + seed)
@@ -688,13 +689,81 @@ def test_forces_dense_cells_randomised(ctx, seed):
     use_mass = rng.random() < 0.4
     mass = rng.uniform(0, 3, n).astype(np.float32) if use_mass else None
     b = ctx.bin(torch.from_numpy(pos).cuda(), K, box, mass=torch.from_numpy(mass).cuda() if use_mass else None)
-    acc = ctx.forces(b, R, eps, 1.0 / n, softening=softening, use_mass=use_mass).cpu().numpy()
+    acc = ctx.forces(b, R, eps, 1.0 / n, softening=softening, use_mass=use_mass, dense_order=dense_order).cpu().numpy()
     sink = np.sort(rng.choice(n, 3000, replace=False))
     ref = oracle.forces(pos, K, R, eps, box, 1.0 / n, sink_idx=sink, softening=softening, mass=mass)
     err = oracle.parity_error(acc[sink], ref)
     assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (seed, K, R, n, float(np.median(err)), float(err.max()))
     assert ctx.interactions(b, R) == oracle.interactions(u32(b.cell_count), K, R)
     assert int(u32(b.cell_count).max()) > 1000
+
+
+def test_forces_dense_order_clumps_across_faces(ctx):
+    """NF_DENSE_ORDER (in-cell Morton ordering of cells >= 4096 particles, boxes per 64 particles, tile-by-tile choice of
+    the law): clumps of 10^4 - 10^5 particles planted ON cell faces, edges and a corner, so that dense cells see dense
+    neighbours across every kind of boundary and close pairs straddle them; eps of the order of the clump's interparticle
+    spacing.  Sampled sinks against the oracle, the flag against no flag, determinism, the chunk call, masses."""
+    rng = np.random.default_rng(91)
+    K, R, box = 6, 2, 3.0
+    w = box / K
+    parts = [rng.random((20_000, 3)) * box]
+    for centre, m, sig in (((2.0, 2.5, 2.5), 60_000, 0.05), ((3.0, 3.0, 2.5), 40_000, 0.04), ((4.0, 4.0, 4.0), 80_000, 0.06),
+                           ((0.0, 0.5, 5.5), 30_000, 0.05), ((2.5, 2.5, 0.5), 12_000, 0.02)):
+        parts.append(np.array(centre) * w + sig * w * rng.standard_normal((m, 3)))
+    pos = np.mod(np.concatenate(parts), box).astype(np.float32)
+    pos = np.minimum(pos, np.nextafter(np.float32(box), np.float32(0)))
+    pos = pos[rng.permutation(pos.shape[0])]
+    n = pos.shape[0]
+    eps = 0.004 * w
+    mass = rng.uniform(0.5, 2.0, n).astype(np.float32)
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box)
+    assert int((u32(b.cell_count) >= 4096).sum()) >= 12
+    a_on = ctx.forces(b, R, eps, 1.0 / n, dense_order=True)
+    assert torch.equal(a_on, ctx.forces(b, R, eps, 1.0 / n, dense_order=True))          # deterministic
+    a_off = ctx.forces(b, R, eps, 1.0 / n)
+    sink = np.sort(rng.choice(n, 6000, replace=False))
+    ref = oracle.forces(pos, K, R, eps, box, 1.0 / n, sink_idx=sink)
+    for a in (a_on, a_off):
+        err = oracle.parity_error(a.cpu().numpy()[sink], ref)
+        assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (float(np.median(err)), float(err.max()))
+    d = oracle.parity_error(a_on.cpu().numpy(), a_off.cpu().numpy().astype(np.float64))
+    assert d.max() <= 1e-4, float(d.max())                         # every particle, flag against no flag
+    # the chunk call (two ranges) with the flag gives the same bits as the whole box with the flag
+    a_ch = torch.zeros_like(a_on)
+    ctx.forces_chunk(b, R, eps, 1.0 / n, 0, 3, out=a_ch, dense_order=True)
+    ctx.forces_chunk(b, R, eps, 1.0 / n, 3, K, out=a_ch, dense_order=True)
+    assert torch.equal(a_ch, a_on)
+    # masses and Plummer with the flag
+    bm = ctx.bin(torch.from_numpy(pos).cuda(), K, box, mass=torch.from_numpy(mass).cuda())
+    am = ctx.forces(bm, R, eps, 1.0, use_mass=True, dense_order=True).cpu().numpy()
+    refm = oracle.forces(pos, K, R, eps, box, 1.0, sink_idx=sink[:2000], mass=mass)
+    err = oracle.parity_error(am[sink[:2000]], refm)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
+    ap = ctx.forces(b, R, 5 * eps, 1.0 / n, softening="plummer", dense_order=True).cpu().numpy()
+    refp = oracle.forces(pos, K, R, 5 * eps, box, 1.0 / n, sink_idx=sink[:2000], softening="plummer")
+    err = oracle.parity_error(ap[sink[:2000]], refp)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
+
+
+def test_forces_dense_order_beyond_its_capacity(ctx):
+    """More particles in dense cells than the ordering takes per call (a quarter of N, at least 2^20): the cells past the
+    limit keep nf_bin's order and the old laws, next to cells that are ordered."""
+    rng = np.random.default_rng(92)
+    K, R, box = 5, 2, 1.0
+    w = box / K
+    parts = [(np.array(c) + 0.5) * w + 0.1 * w * rng.standard_normal((420_000, 3)).clip(-4.9, 4.9) for c in ((1, 2, 2), (2, 2, 2), (3, 2, 2))]
+    pos = np.concatenate(parts + [rng.random((5000, 3)) * box]).astype(np.float32)
+    pos = pos[rng.permutation(pos.shape[0])]
+    n = pos.shape[0]
+    eps = 0.01 * w
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box)
+    assert int((u32(b.cell_count) >= 4096).sum()) >= 3 and int(u32(b.cell_count)[u32(b.cell_count) >= 4096].sum()) > (1 << 20)
+    acc = ctx.forces(b, R, eps, 1.0 / n)                            # N / K^3 >= 512: the ordering is automatic
+    assert torch.equal(acc, ctx.forces(b, R, eps, 1.0 / n))
+    sink = np.sort(rng.choice(n, 1500, replace=False))
+    ref = oracle.forces(pos, K, R, eps, box, 1.0 / n, sink_idx=sink)
+    err = oracle.parity_error(acc.cpu().numpy()[sink], ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (float(np.median(err)), float(err.max()))
 
 
 # ------------------------------------------------- slab stream: plane faces and error paths
