@@ -521,8 +521,8 @@ def run_sharded(args, cfg):
 
 
 def sweep_small_configs(ctx, dev, steps=3, warmup=3):
-    """Interaction-kernel roofline fraction of C1, C2 and C3 in the same process (milliseconds each): the
-    other single-GPU configs of BASELINE.json beside the headline workload.  Same timing rules as the main
+    """Interaction-kernel roofline fraction of C1, C2 and C3 -- the other single-GPU configs of BASELINE.json beside the
+    headline workload -- and of D1, the one-dense-cell workload (config 6), in the same process (milliseconds each).  Same timing rules as the main
     line: W warm-up steps, the L2 flushed between timed steps (inputs smaller than the L2), CUDA events
     around the kernel inside nf_forces."""
     sm_max_mhz, _, _ = read_peaks()
@@ -530,7 +530,7 @@ def sweep_small_configs(ctx, dev, steps=3, warmup=3):
     peak = sms * sm_max_mhz * 1e6 * 2 * FP32_LANES_PER_SM
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     out = {}
-    for which in (1, 2, 3):
+    for which in (1, 2, 3, 6):
         cfg = inputs.config(which)
         pos = inputs.make_positions(cfg, device=dev)
         b = ctx.bin(pos, cfg.K, cfg.box)
@@ -567,7 +567,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--no-sweep", action="store_true", help="skip the C1-C3 kernel sweep of the default line")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the C1-C3 + D1 kernel sweep of the default line")
     ap.add_argument("--shard", action="store_true", help="use the x-slab sharded path (the default for --gpus N > 1) even on one GPU")
     ap.add_argument("--shard-backend", default="nccl", choices=["nccl", "gloo"],
                     help="gloo: debugging aid, every rank on cuda:0 with ghosts staged through host memory")

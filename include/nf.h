@@ -61,14 +61,15 @@ enum {
  * masses in the .w lane of pos_sorted (written by nf_bin_m) and `Gm` is then G alone:
  * a_i = G * sum_j m_j f(|d|) d.  The paper's runs use equal masses; SURVEY.md Sec. 8(f) rank 1. */
 #define NF_MASS_W 0x100
-/* Flag OR-ed into `softening` of nf_forces / nf_forces_ex / nf_forces_chunk: the box holds cells of thousands of particles
- * or more ("the largest cell has over 200,000 particles").  Such cells (>= 4096 particles; up to 2048 of them
- * and a quarter of the particles per call) get their internal encoded copies ordered along a Morton curve inside the cell,
- * with a bounding box per 64 particles, so that the kernel can prove most source tiles of a dense cell free of pairs inside
- * eps and sweep them with the bare 1/r^2 law instead of the min form of Eq. 2 -- exact, because the two agree for r >= eps
- * (fn. 4).  No output changes its order or meaning; accelerations change in the last bits only (another
- * summation order).  Taken automatically, flag or not, when the mean occupancy N / K^3 is at least 512.  Other calls
- * (nf_forces_host*, nf_stream_*) ignore the flag. */
+/* Flag OR-ed into the `softening` argument of every force call (nf_forces*, nf_forces_host*, nf_stream_*): the box holds
+ * cells of thousands of particles or more ("the largest cell has over 200,000 particles").  Such cells
+ * (>= 4096 particles; up to 2048 of them and a quarter of the particles -- at least 2^20 -- per box, or per plane in the
+ * slab stream) get their INTERNAL encoded copies ordered along a Morton curve inside the cell, with a bounding box per 64
+ * particles, so that the kernel can prove most source tiles of a dense cell free of pairs inside eps and sweep them with
+ * the bare 1/r^2 law instead of the min form of Eq. 2 -- exact, because the two agree for r >= eps (fn. 4).
+ * No output changes its order or meaning; accelerations change in the last bits only (another summation order), and
+ * remain bit-reproducible from call to call.  Taken automatically, flag or not, when the mean occupancy (N / K^3; in the
+ * slab stream the fullest plane's n / K^2) is at least 512: the decision depends on the arguments alone. */
 #define NF_DENSE_ORDER 0x200
 #define NF_SOFT_LAW_MASK 0xff
 

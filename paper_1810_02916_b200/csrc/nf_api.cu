@@ -191,6 +191,41 @@ static int check_force_args(nf_ctx *ctx, int K, int R, float eps, float Gm, int 
     return NF_OK;
 }
 
+// Arena bytes of the in-cell ordering of dense cells for a whole box (temporaries + its three outputs), 0 when not taken
+static size_t dense_full_bytes(int64_t N, int K, int softening)
+{
+    const size_t ncell = (size_t)K * K * K;
+    if (!nf_dense_wanted(N, ncell, softening)) return 0;
+    const size_t cap = nf_dense_cap(N);
+    return nf_dense_scratch_bytes(N, ncell) + nf_align_up(ncell * 4, 256) + nf_align_up(cap * 4, 256) + nf_align_up(cap / 64 * 24, 256) + 1024;
+}
+
+// Encoded copies of a whole box, the in-cell ordering of its dense cells where it is wanted (nf_dense.cu; outputs taken
+// from the arena), and the plane table.  Clears NF_DENSE_ORDER in p.softening and sets p.dense.
+static int encode_full(nf_ctx *ctx, nf_force_params &p, const float4 *ps, const uint64_t *off, const uint32_t *perm, int64_t N,
+                       float4 *enc, float4 *enc_h, nf_plane_view *d_planes, float *acc, float *cell_amax, cudaStream_t st)
+{
+    const int K = p.K;
+    const size_t ncell = (size_t)K * K * K;
+    const bool dense = nf_dense_wanted(N, ncell, p.softening);
+    p.softening &= ~NF_DENSE_ORDER;
+    NF_TRY(nf_encode_impl(ctx, p, ps, off, ncell, enc, enc_h, st));
+    uint32_t *dinfo = nullptr, *dslot = nullptr;
+    float *dbox = nullptr;
+    if (dense) {
+        const size_t cap = nf_dense_cap(N);
+        dinfo = nf_scratch_take<uint32_t>(ctx, ncell);
+        dslot = nf_scratch_take<uint32_t>(ctx, cap);
+        dbox = nf_scratch_take<float>(ctx, cap / 64 * 6);
+        if (!dinfo || !dslot || !dbox) { NF_SET_ERR(ctx, "nf_forces: internal scratch arena too small (dense-cell ordering)"); return NF_ERR_NOMEM; }
+        const size_t mark = ctx->scratch_used;
+        NF_TRY(nf_dense_order_impl(ctx, p, ps, off, ncell, N, enc, enc_h, dinfo, dslot, dbox, st));
+        ctx->scratch_used = mark;                  // its temporaries are dead once enqueued work is ordered: same stream
+        p.dense = 1;
+    }
+    return nf_fill_planes_full(ctx, d_planes, K, ps, enc, enc_h, off, perm, acc, cell_amax, dinfo, dslot, dbox, st);
+}
+
 // nf_forces / nf_forces_ex / nf_forces_chunk: sinks are the particles of the x-planes [x_lo, x_hi)
 static int forces_common(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset, const uint32_t *perm, int64_t N, int K,
                          int R, float eps, float box, float Gm, int softening, int x_lo, int x_hi, float *acc_xyz, float *cell_amax,
@@ -210,23 +245,16 @@ static int forces_common(nf_ctx *ctx, const float *pos_sorted, const uint64_t *c
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = x_lo; p.sink_hi = x_hi;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
-    // in-cell ordering of dense cells (nf_dense.cu): asked for with NF_DENSE_ORDER, and automatic when the MEAN occupancy
-    // already says that cells are dense -- decided from the arguments alone, so that the same call always takes the same path
-    const bool dense = N >= NF_DENSE_N && ((softening & NF_DENSE_ORDER) || N / ((int64_t)K * K * K) >= 512);
-    p.softening = softening & ~NF_DENSE_ORDER;
     nf_scratch_reset(ctx);
-    NF_TRY(nf_scratch_reserve(ctx, forces_scratch_full(N, K) + (dense ? nf_dense_scratch_bytes(N, K) : 0)));
+    NF_TRY(nf_scratch_reserve(ctx, forces_scratch_full(N, K) + dense_full_bytes(N, K, softening)));
     nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
     float4 *enc = nf_scratch_take<float4>(ctx, (size_t)N);
     float4 *enc_h = nf_scratch_take<float4>(ctx, (size_t)N);
     if (!d_planes || !enc || !enc_h) { NF_SET_ERR(ctx, "nf_forces: internal scratch arena too small"); return NF_ERR_NOMEM; }
     cudaStream_t st = (cudaStream_t)stream;
     const float4 *ps = reinterpret_cast<const float4 *>(pos_sorted);
-    NF_TRY(nf_encode_impl(ctx, p, ps, cell_offset, (size_t)K * K * K, enc, enc_h, st));
-    uint32_t *dinfo = nullptr;
-    if (dense) NF_TRY(nf_dense_order_impl(ctx, p, ps, cell_offset, N, enc, enc_h, &dinfo, st));
     if (cell_amax) NF_CUDA(ctx, cudaMemsetAsync(cell_amax, 0, sizeof(float) * (size_t)K * K * K, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, ps, enc, enc_h, cell_offset, perm, acc_xyz, cell_amax, dinfo, st));
+    NF_TRY(encode_full(ctx, p, ps, cell_offset, perm, N, enc, enc_h, d_planes, acc_xyz, cell_amax, st));
     return nf_forces_impl(ctx, p, d_planes, st, true);
 }
 
@@ -269,7 +297,7 @@ static size_t host_path_bytes(int64_t N, int K)
     const size_t n = (size_t)(N > 0 ? N : 1), ncell = (size_t)K * K * K;
     size_t b = nf_align_up(n * 12, 256) * 2 + nf_align_up(n * 16, 256) + 2 * nf_align_up(n * 4, 256) +
                nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256);
-    return b + nf_bin_scratch_bytes(N, K, false) + forces_scratch_full(N, K) + 4096;
+    return b + nf_bin_scratch_bytes(N, K, false) + forces_scratch_full(N, K) + dense_full_bytes(N, K, NF_DENSE_ORDER) + 4096;
 }
 
 int nf_reserve_host(nf_ctx *ctx, int64_t maxN, int K)
@@ -323,8 +351,7 @@ int nf_forces_host_m(nf_ctx *ctx, const float *pos_host, const float *mass_host,
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
-    NF_TRY(nf_encode_impl(ctx, p, reinterpret_cast<const float4 *>(sorted), off, ncell, enc, enc_h, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, acc, nullptr, nullptr, st));
+    NF_TRY(encode_full(ctx, p, reinterpret_cast<const float4 *>(sorted), off, perm, N, enc, enc_h, d_planes, acc, nullptr, st));
     NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
     NF_CUDA(ctx, cudaMemcpyAsync(acc_host, acc, n * 12, cudaMemcpyDeviceToHost, st));
     NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters, ctx->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
@@ -373,7 +400,8 @@ int nf_forces_host_begin(nf_ctx *ctx, const float *pos_host, int64_t N, int K, i
         fp.K = K; fp.n_planes = K; fp.sink_lo = 0; fp.sink_hi = K; fp.max_sinks = N;
         const size_t wl = nf_forces_scratch_bytes(fp), bs = nf_bin_scratch_bytes(N, K, false);
         const size_t need = 4 * nf_align_up(n * 12, 256) + 3 * nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
-                            nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256) + (wl > bs ? wl : bs) + 8192;
+                            nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256) + (wl > bs ? wl : bs) +
+                            dense_full_bytes(N, K, NF_DENSE_ORDER) + 8192;
         NF_TRY(nf_scratch_reserve(ctx, need));
         nf_scratch_reset(ctx);
         for (int i = 0; i < 2; i++) {
@@ -421,8 +449,7 @@ int nf_forces_host_begin(nf_ctx *ctx, const float *pos_host, int64_t N, int K, i
     nf_force_params p{};
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = 0; p.sink_hi = K;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
-    NF_TRY(nf_encode_impl(ctx, p, reinterpret_cast<const float4 *>(sorted), off, ncell, enc, enc_h, st));
-    NF_TRY(nf_fill_planes_full(ctx, d_planes, K, reinterpret_cast<const float4 *>(sorted), enc, enc_h, off, perm, hp->acc[i], nullptr, nullptr, st));
+    NF_TRY(encode_full(ctx, p, reinterpret_cast<const float4 *>(sorted), off, perm, N, enc, enc_h, d_planes, hp->acc[i], nullptr, st));
     NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
     NF_CUDA(ctx, cudaMemcpyAsync(hp->h_bad + i, ctx->counters, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     NF_CUDA(ctx, cudaEventRecord(hp->ev_done[i], st));

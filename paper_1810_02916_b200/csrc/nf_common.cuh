@@ -107,7 +107,10 @@ struct nf_plane_view {
     const uint32_t *perm;     // nullable
     float *acc;               // output for this plane (n x 3), nullable for ghost planes
     float *amax;              // nullable: K*K per-cell maxima of |a| (zeroed by the caller; integer atomicMax on the float bits)
-    const uint32_t *dinfo;    // nullable: K*K words, 0 = cell not dense, else (compact offset of the cell / 64) + 1 (nf_dense.cu)
+    // in-cell ordering of this plane's dense cells (nf_dense.cu); all null = none
+    const uint32_t *dinfo;    // K*K words, 0 = cell not dense, else (compact offset of the cell / 64) + 1
+    const uint32_t *dslot;    // compact position -> slot (within this plane's arrays) of the particle whose encoded copy sits there
+    const float *dbox;        // per 64 compact positions: lo.xyz, hi.xyz of the scaled cell-centred offsets
 };
 struct nf_force_params {
     int K;            // cells per side in y and z
@@ -118,9 +121,7 @@ struct nf_force_params {
     float eps, box, Gm;
     int softening;
     long long max_sinks;  // upper bound on the particles in the sink planes (sizes the work list)
-    // in-cell spatial ordering of dense cells (nf_dense.cu); null = none
-    const uint32_t *dense_slot;   // compact position -> slot (within its plane's arrays) of the particle whose encoded copy sits there
-    const float *dense_box;       // per 64 compact positions: lo.xyz, hi.xyz of the scaled cell-centred offsets
+    int dense;            // 1: some plane view carries the in-cell ordering of dense cells (selects the kernel instance with that logic)
 };
 size_t nf_forces_scratch_bytes(const nf_force_params &p);
 // d_planes: DEVICE array of p.n_planes views (fill with nf_fill_planes_full or copy from pinned memory)
@@ -128,7 +129,8 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
                    cudaStream_t st, bool record_timing);
 // the full box seen as K planes sharing one set of arrays: plane cx starts at cell cx*K*K
 int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
-                        const uint64_t *off, const uint32_t *perm, float *acc, float *cell_amax, const uint32_t *dinfo, cudaStream_t st);
+                        const uint64_t *off, const uint32_t *perm, float *acc, float *cell_amax, const uint32_t *dinfo, const uint32_t *dslot,
+                        const float *dbox, cudaStream_t st);
 // enc[s], enc_h[s] = the two encoded copies of pos[s] for the ncell cells described by off (cell index % K = cz);
 // they depend on p.eps, p.box, p.K
 int nf_encode_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, float4 *enc,
@@ -136,13 +138,18 @@ int nf_encode_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, con
 // In-cell ordering of dense cells (nf_dense.cu), full box only.  Cells of at least NF_DENSE_N particles get their ENCODED
 // copies (enc, enc_h: what the interaction kernel reads) re-ordered along a Morton curve inside the cell, with a box per 64
 // particles, so that the kernel can prove most (task, tile) pairs free of pairs inside eps.  dinfo: K^3 words out.
-// Scratch comes from the arena.  Sets p.dense_slot / p.dense_box.
+// `off` describes ncell cells whose index modulo K is cz (the full box: K^3 cells; one plane: K^2).  Outputs: dinfo
+// (ncell words), dslot (nf_dense_cap(N) words), dbox (nf_dense_cap(N) / 64 * 6 floats) -- caller-owned, they must live as
+// long as the encoded copies; temporaries come from the arena (nf_dense_scratch_bytes).
 constexpr int NF_ZB = 8;                // cells per z-block of the encoding (nf_forces.cu k_encode)
 constexpr int NF_DENSE_N = 4096;
 constexpr int NF_DENSE_MAX_CELLS = 2048;
-size_t nf_dense_scratch_bytes(int64_t N, int K);
-int nf_dense_order_impl(nf_ctx *ctx, nf_force_params &p, const float4 *pos, const uint64_t *off, int64_t N, float4 *enc, float4 *enc_h,
-                        uint32_t **dinfo_out, cudaStream_t st);
+uint32_t nf_dense_cap(int64_t N);
+size_t nf_dense_scratch_bytes(int64_t N, size_t ncell);
+// is the ordering taken for a set of N particles in ncell cells?  From the arguments alone (the same call always takes the same path)
+static inline bool nf_dense_wanted(int64_t N, size_t ncell, int softening) { return N >= NF_DENSE_N && ((softening & NF_DENSE_ORDER) || (size_t)N / ncell >= 512); }
+int nf_dense_order_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, int64_t N,
+                        float4 *enc, float4 *enc_h, uint32_t *dinfo, uint32_t *dslot, float *dbox, cudaStream_t st);
 size_t nf_radix_tiles(int64_t n_max);
 int nf_radix_pass(nf_ctx *ctx, const uint32_t *kin, const uint32_t *iin, int64_t n_max, const uint32_t *n_dev, uint32_t bins,
                   uint32_t shift, uint32_t *kout, uint32_t *iout, uint32_t *hist, uint32_t *tmp32, cudaStream_t st);

@@ -130,42 +130,40 @@ __global__ void __launch_bounds__(256) k_dense_finish(const float4 *__restrict__
     }
 }
 
-uint32_t dense_cap(int64_t N)
+}  // namespace
+
+// compact positions the ordering takes per call: a quarter of the particles, at least 2^20, at most 2^28
+uint32_t nf_dense_cap(int64_t N)
 {
     const int64_t c = N / 4 > (1 << 20) ? N / 4 : (1 << 20);
     return (uint32_t)(c < (1ll << 28) ? c : (1ll << 28)) & ~63u;
 }
 
-}  // namespace
-
-size_t nf_dense_scratch_bytes(int64_t N, int K)
+size_t nf_dense_scratch_bytes(int64_t N, size_t ncell)
 {
-    const size_t ncell = (size_t)K * K * K, cap = dense_cap(N);
-    size_t b = 5 * nf_align_up(ncell * sizeof(uint32_t), 256);                                  // n64, one, coff, rank, dinfo
+    const size_t cap = nf_dense_cap(N);
+    size_t b = 4 * nf_align_up(ncell * sizeof(uint32_t), 256);                                  // n64, one, coff, rank
     b += 2 * nf_align_up(nf_scan_temp_elems(ncell) * sizeof(uint32_t), 256);
-    b += 4 * nf_align_up(cap * sizeof(uint32_t), 256);                                          // key / index ping-pong
-    b += nf_align_up((cap / 64) * 6 * sizeof(float), 256);                                      // boxes
+    b += 3 * nf_align_up(cap * sizeof(uint32_t), 256);                                          // key ping-pong, one index buffer (the other is dslot)
     b += nf_align_up((size_t)NF_DENSE_MAX_CELLS * sizeof(DenseCell), 256) + 256;
     b += nf_align_up(256 * nf_radix_tiles(cap) * sizeof(uint32_t), 256);                        // digit histograms
     b += nf_align_up(nf_scan_temp_elems(256 * nf_radix_tiles(cap)) * sizeof(uint32_t), 256);
     return b + 4096;
 }
 
-int nf_dense_order_impl(nf_ctx *ctx, nf_force_params &p, const float4 *pos, const uint64_t *off, int64_t N, float4 *enc, float4 *enc_h,
-                        uint32_t **dinfo_out, cudaStream_t st)
+int nf_dense_order_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, int64_t N,
+                        float4 *enc, float4 *enc_h, uint32_t *dinfo, uint32_t *dslot, float *dbox, cudaStream_t st)
 {
     const int K = p.K;
-    const size_t ncell = (size_t)K * K * K;
-    const uint32_t cap = dense_cap(N);
+    const uint32_t cap = nf_dense_cap(N);
     uint32_t *n64 = nf_scratch_take<uint32_t>(ctx, ncell);
     uint32_t *one = nf_scratch_take<uint32_t>(ctx, ncell);
     uint32_t *coff = nf_scratch_take<uint32_t>(ctx, ncell);
     uint32_t *rank = nf_scratch_take<uint32_t>(ctx, ncell);
-    uint32_t *dinfo = nf_scratch_take<uint32_t>(ctx, ncell);
     uint32_t *stmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(ncell));
     uint32_t *keyA = nf_scratch_take<uint32_t>(ctx, cap), *keyB = nf_scratch_take<uint32_t>(ctx, cap);
-    uint32_t *idxA = nf_scratch_take<uint32_t>(ctx, cap), *idxB = nf_scratch_take<uint32_t>(ctx, cap);
-    float *box = nf_scratch_take<float>(ctx, (size_t)(cap / 64) * 6);
+    uint32_t *idxA = nf_scratch_take<uint32_t>(ctx, cap), *idxB = dslot;
+    float *box = dbox;
     DenseCell *dcell = nf_scratch_take<DenseCell>(ctx, NF_DENSE_MAX_CELLS);
     uint32_t *nd = nf_scratch_take<uint32_t>(ctx, 64);
     const size_t nt = nf_radix_tiles(cap);
@@ -193,8 +191,5 @@ int nf_dense_order_impl(nf_ctx *ctx, nf_force_params &p, const float4 *pos, cons
     const unsigned grid = (unsigned)(nchunk / 8 < 148 * 16 ? (nchunk + 7) / 8 : 148 * 16);
     k_dense_finish<<<grid, 256, 0, st>>>(pos, keyA, idxA, nd, dcell, K, scale, ws, enc, enc_h, idxB, box, nchunk);
     NF_LAUNCHED(ctx);
-    p.dense_slot = idxB;
-    p.dense_box = box;
-    *dinfo_out = dinfo;
     return NF_OK;
 }

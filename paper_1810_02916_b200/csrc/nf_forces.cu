@@ -453,7 +453,7 @@ struct TaskHdr {                            // what a consumer needs to know abo
     uint64_t s0;                            // first sink (slot in the plane's arrays)
     uint32_t n, L, cyz;
     uint32_t part, nparts, slot;                // source split: this entry is part `part` of `nparts`, partial sums in slots slot..slot+nparts-1
-    uint32_t eoff;                              // dense own cell: compact position of the task's first sink (nf_dense.cu), else 0xffffffff
+    const uint32_t *eslot;                      // dense own cell (nf_dense.cu): sorted slot of each of the task's sinks, else null
 };
 
 template <int R>
@@ -467,7 +467,9 @@ struct ConsShared {
     unsigned long long full[2];
     // producer's cursor for this consumer
     uint32_t p_npieces, p_cur_piece, p_j, p_nparts, p_P, p_invP, p_seq, p_state;   // p_state 0: inside a task, 1: next tile starts a task, 2: stop
-    uint32_t p_tchunk0, p_tnchunk;          // dense own cell: first box and number of boxes (<= 3) of the task's sinks; 0 boxes = not dense
+    uint32_t p_tnchunk;                     // dense own cell: number of boxes (<= 3) of the task's sinks; 0 = not dense
+    const float *p_tbox;                    // ... and the first of them
+    const float *dbox[W];                   // boxes of the W source planes (by dx + R)
 };
 
 // ---- producer: everything about task ti that does not need the FMA pipe -------------------------------
@@ -490,22 +492,25 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
     const int zphi = ((cz - R + ZB * 4) / ZB != (cz + R + ZB * 4) / ZB) ? ZB / 2 : 0;
     const float4 *se = zphi ? sp.enc_h : sp.enc;
     // dense own cell (nf_dense.cu): its encoded copies are ordered along a Morton curve with a box per 64 particles
-    const uint32_t own_di = (DENSE && p.dense_slot && sp.dinfo) ? sp.dinfo[task.cyz] : 0u;
+    const uint32_t own_di = (DENSE && sp.dinfo) ? sp.dinfo[task.cyz] : 0u;
     if (lane < W) {
         int px = sink_plane + lane - R;
         if (p.periodic_x) px = (px % p.n_planes + p.n_planes) % p.n_planes;
         else if (px < 0 || px >= p.n_planes) px = -1;
         S.enc[lane] = px >= 0 ? (zphi ? planes[px].enc_h : planes[px].enc) : nullptr;
+        if (DENSE) S.dbox[lane] = px >= 0 ? planes[px].dbox : nullptr;
     }
     if (lane == 0) {
         TaskHdr h;
         h.se = se; h.acc = sp.acc; h.perm = sp.perm; h.amax = sp.amax; h.s0 = s0;
         h.n = (uint32_t)n; h.L = (uint32_t)L; h.cyz = task.cyz;
         h.part = task.part_slot & 0xffu; h.nparts = task.nparts; h.slot = task.part_slot >> 8;
-        h.eoff = own_di ? (own_di - 1u) * 64u + task.first : 0xffffffffu;
+        h.eslot = own_di ? sp.dslot + (size_t)(own_di - 1u) * 64u + task.first : nullptr;
         S.hdr[seq & 3u] = h;
-        S.p_tchunk0 = own_di ? own_di - 1u + (task.first >> 6) : 0u;
-        S.p_tnchunk = own_di ? ((task.first + (uint32_t)n - 1u) >> 6) - (task.first >> 6) + 1u : 0u;
+        if (DENSE) {
+            S.p_tbox = own_di ? sp.dbox + 6 * (size_t)(own_di - 1u + (task.first >> 6)) : nullptr;
+            S.p_tnchunk = own_di ? ((task.first + (uint32_t)n - 1u) >> 6) - (task.first >> 6) + 1u : 0u;
+        }
         S.p_P = (uint32_t)P;
         S.p_invP = (65536u + P - 1) / P;        // floor(x / P) == (x * inv_P) >> 16 for x < 1024
     }
@@ -710,7 +715,7 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
         bool nearp = false;
         const uint32_t a = (uint32_t)lane / 10u, bq = (uint32_t)lane % 10u;     // 3 x 10 pairs of boxes, one per lane
         if (a < ntc && bq < nk) {
-            const float *A = p.dense_box + 6 * (size_t)(S.p_tchunk0 + a), *B = p.dense_box + 6 * (size_t)((pc.w >> 9) + k0 + bq);
+            const float *A = S.p_tbox + 6 * (size_t)a, *B = S.dbox[dxi] + 6 * (size_t)((pc.w >> 9) + k0 + bq);
             const float sh[3] = {(float)(dxi - R) * fc.ws, (float)(dyi - R) * fc.ws, (float)(szi - R) * fc.ws};
             float g2 = 0.f;
 #pragma unroll
@@ -950,7 +955,7 @@ __global__ void __launch_bounds__((N_CONS + N_PROD) * 32, 1) k_forces_warp(const
                 a2max = fmaxf(a2max, fx * fx + fy * fy + fz * fz);
                 if (h.acc) {
                     // sorted slot of sink i: its encoded copy may sit elsewhere inside a dense cell (nf_dense.cu)
-                    const uint64_t si = (DENSE && h.eoff != 0xffffffffu) ? (uint64_t)p.dense_slot[h.eoff + (uint32_t)i] : h.s0 + (uint64_t)i;
+                    const uint64_t si = (DENSE && h.eslot) ? (uint64_t)h.eslot[i] : h.s0 + (uint64_t)i;
                     const uint64_t o = h.perm ? (uint64_t)h.perm[si] : si;
                     h.acc[3 * o + 0] = fx;
                     h.acc[3 * o + 1] = fy;
@@ -1003,7 +1008,8 @@ __global__ void __launch_bounds__(256) k_interactions(const uint32_t *__restrict
 }
 
 __global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
-                              const uint64_t *off, const uint32_t *perm, float *acc, float *amax, const uint32_t *dinfo)
+                              const uint64_t *off, const uint32_t *perm, float *acc, float *amax, const uint32_t *dinfo,
+                              const uint32_t *dslot, const float *dbox)
 {
     int cx = blockIdx.x * blockDim.x + threadIdx.x;
     if (cx >= K) return;
@@ -1016,6 +1022,8 @@ __global__ void k_fill_planes(nf_plane_view *planes, int K, const float4 *pos, c
     v.acc = acc;
     v.amax = amax ? amax + (size_t)cx * K * K : nullptr;
     v.dinfo = dinfo ? dinfo + (size_t)cx * K * K : nullptr;
+    v.dslot = dslot;
+    v.dbox = dbox;
     planes[cx] = v;
 }
 
@@ -1164,9 +1172,10 @@ int nf_forces_init(nf_ctx *ctx)
 }
 
 int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float4 *pos, const float4 *enc, const float4 *enc_h,
-                        const uint64_t *off, const uint32_t *perm, float *acc, float *cell_amax, const uint32_t *dinfo, cudaStream_t st)
+                        const uint64_t *off, const uint32_t *perm, float *acc, float *cell_amax, const uint32_t *dinfo, const uint32_t *dslot,
+                        const float *dbox, cudaStream_t st)
 {
-    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, enc, enc_h, off, perm, acc, cell_amax, dinfo);
+    k_fill_planes<<<(K + 127) / 128, 128, 0, st>>>(d_planes, K, pos, enc, enc_h, off, perm, acc, cell_amax, dinfo, dslot, dbox);
     NF_LAUNCHED(ctx);
     return NF_OK;
 }
@@ -1218,7 +1227,7 @@ template <int R, bool MASS>
 static int launch_warp(nf_ctx *ctx, const nf_force_params &p, const ForceConsts &fc, const nf_plane_view *d_planes,
                        const Task *tasks, uint32_t *ctl, float *partial, uint32_t *arrive, cudaStream_t st)
 {
-    if (p.dense_slot) return launch_warp_d<R, MASS, true>(ctx, p, fc, d_planes, tasks, ctl, partial, arrive, st);
+    if (p.dense) return launch_warp_d<R, MASS, true>(ctx, p, fc, d_planes, tasks, ctl, partial, arrive, st);
     return launch_warp_d<R, MASS, false>(ctx, p, fc, d_planes, tasks, ctl, partial, arrive, st);
 }
 

@@ -28,6 +28,10 @@ struct Slot {
     float *vel;        // n x 3 (nf_stream_step_slabs only)
     float *part_pos;   // n x 3, n x 3 (nf_stream_step_regroup only): the drifted plane as [to plane-1 | stay | to plane+1]
     float *part_vel;
+    // in-cell ordering of the plane's dense cells (nf_dense.cu), null when the pass does not take it
+    uint32_t *dinfo;   // K*K
+    uint32_t *dslot;   // nf_dense_cap(n)
+    float *dbox;       // nf_dense_cap(n) / 64 * 6
 };
 
 // the kick + drift epilogue of nf_stream_step_slabs (null pointers: plain nf_stream_slabs)
@@ -109,7 +113,8 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
     NF_ARG(ctx, P <= K, "P = %d sink planes exceed K = %d", P, K);
     NF_ARG(ctx, eps > 0.0f && eps < 3.0e38f, "eps must be positive and finite");
     NF_ARG(ctx, box > 0.0f && box < 3.0e38f, "box must be positive and finite");
-    NF_ARG(ctx, softening == NF_SOFT_SPLINE || softening == NF_SOFT_PLUMMER, "unknown softening %d (the slab stream carries no masses)", softening);
+    NF_ARG(ctx, (softening & ~NF_DENSE_ORDER) == NF_SOFT_SPLINE || (softening & ~NF_DENSE_ORDER) == NF_SOFT_PLUMMER,
+           "unknown softening %d (the slab stream carries no masses)", softening);
     const int NP = P + 2 * R, NS = in.nseg;
     const bool regroup = step && step->out_seg_n;
     NF_ARG(ctx, NS >= 1 && NS <= 3, "a plane has 1 to 3 host segments");
@@ -153,7 +158,12 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
         ctx->slab_state = S;
     }
     const size_t n = (size_t)max_n;
-    const size_t slot_bytes = nf_align_up(n * 12, 256) + 3 * nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
+    // in-cell ordering of dense cells, plane by plane: asked for, or the fullest plane's mean occupancy says so
+    const bool dense = nf_dense_wanted(max_n, ncell, softening);
+    softening &= ~NF_DENSE_ORDER;
+    const size_t dcap = dense ? nf_dense_cap(max_n) : 0;
+    const size_t dense_bytes = dense ? nf_align_up(ncell * 4, 256) + nf_align_up(dcap * 4, 256) + nf_align_up(dcap / 64 * 24, 256) : 0;
+    const size_t slot_bytes = dense_bytes + nf_align_up(n * 12, 256) + 3 * nf_align_up(n * 16, 256) + nf_align_up(n * 4, 256) +
                               nf_align_up(ncell * 4, 256) + nf_align_up((ncell + 1) * 8, 256) + nf_align_up(n * 12, 256) +
                               (step ? nf_align_up(n * 12, 256) : 0) + (regroup ? 2 * nf_align_up(n * 12, 256) : 0);
     const size_t need = slot_bytes * W;
@@ -177,6 +187,7 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
     nf_force_params fp{};
     fp.K = K; fp.n_planes = NP; fp.periodic_x = 0; fp.R = R; fp.eps = eps; fp.box = box; fp.Gm = Gm; fp.softening = softening;
     fp.sink_lo = 0; fp.sink_hi = 1; fp.max_sinks = max_n;     // one sink plane per nf_forces_impl call
+    fp.dense = dense ? 1 : 0;
     if (regroup && P > S->segn_cap) {
         NF_CUDA(ctx, cudaDeviceSynchronize());
         if (S->d_segn) NF_CUDA(ctx, cudaFree(S->d_segn));
@@ -188,7 +199,7 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
     }
     // binning, the force work list and the regrouping of a plane take their scratch one after the other
     NF_TRY(nf_scratch_reserve(ctx, nf_bin_scratch_bytes(max_n, K, true) + nf_forces_scratch_bytes(fp) +
-                                       (regroup ? nf_regroup_scratch_bytes(max_n) : 0)));
+                                       (regroup ? nf_regroup_scratch_bytes(max_n) : 0) + (dense ? nf_dense_scratch_bytes(max_n, ncell) : 0)));
 
     std::vector<Slot> slots(W);
     for (int s = 0; s < W; s++) {
@@ -206,6 +217,12 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
         slots[s].part_pos = regroup ? (float *)b : nullptr;
         if (regroup) b += nf_align_up(n * 12, 256);
         slots[s].part_vel = regroup ? (float *)b : nullptr;
+        if (regroup) b += nf_align_up(n * 12, 256);
+        slots[s].dinfo = dense ? (uint32_t *)b : nullptr;
+        if (dense) b += nf_align_up(ncell * 4, 256);
+        slots[s].dslot = dense ? (uint32_t *)b : nullptr;
+        if (dense) b += nf_align_up(dcap * 4, 256);
+        slots[s].dbox = dense ? (float *)b : nullptr;
     }
     // plane views (device pointers are fixed by the slot assignment q % W)
     for (int q = 0; q < NP; q++) {
@@ -217,7 +234,9 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
         S->h_views[q].perm = sl.perm;
         S->h_views[q].acc = sl.acc;
         S->h_views[q].amax = nullptr;
-        S->h_views[q].dinfo = nullptr;
+        S->h_views[q].dinfo = sl.dinfo;
+        S->h_views[q].dslot = sl.dslot;
+        S->h_views[q].dbox = sl.dbox;
     }
     NF_CUDA(ctx, cudaMemcpyAsync(S->d_views, S->h_views, sizeof(nf_plane_view) * NP, cudaMemcpyHostToDevice, st));
     NF_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st));
@@ -266,6 +285,9 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
         // counters[0] accumulates out-of-range / wrong-plane particles over all planes
         NF_TRY(nf_bin_impl(ctx, sl.raw, nullptr, plane_n[q], K, box, cx, sl.sorted, sl.perm, sl.count, sl.off, st));
         NF_TRY(nf_encode_impl(ctx, fp, (const float4 *)sl.sorted, sl.off, ncell, (float4 *)sl.enc, (float4 *)sl.enc_h, st));
+        if (dense)
+            NF_TRY(nf_dense_order_impl(ctx, fp, (const float4 *)sl.sorted, sl.off, ncell, plane_n[q], (float4 *)sl.enc, (float4 *)sl.enc_h,
+                                       sl.dinfo, sl.dslot, sl.dbox, st));
         NF_CUDA(ctx, cudaEventRecord(bin1[q], st));
 
         const int sp = q - R;        // chunk plane whose neighbourhood is now complete

@@ -22,6 +22,13 @@ NF_MASS_W = 0x100
 NF_DENSE_ORDER = 0x200
 _SOFT = {"spline": SOFT_SPLINE, "plummer": SOFT_PLUMMER}
 
+def _soft_code(softening: str) -> int:
+    """'spline' or 'plummer', optionally followed by '+dense' (NF_DENSE_ORDER: in-cell ordering of dense cells)."""
+    base, _, opt = softening.partition("+")
+    assert opt in ("", "dense"), softening
+    return _SOFT[base] | (NF_DENSE_ORDER if opt else 0)
+
+
 # every symbol include/nf.h declares
 EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve", "nf_bin",
            "nf_out_of_range", "nf_forces", "nf_interactions", "nf_spline_equivalent_eps",
@@ -237,7 +244,7 @@ class Context:
         self._check(self.lib.nf_forces_chunk(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset),
                                              _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
                                              float(b.box), float(Gm),
-                                             _SOFT[softening] | (NF_MASS_W if use_mass else 0) | (NF_DENSE_ORDER if dense_order else 0),
+                                             _soft_code(softening) | (NF_MASS_W if use_mass else 0) | (NF_DENSE_ORDER if dense_order else 0),
                                              int(x_lo), int(x_hi), _ptr(acc), _ptr(cell_amax), self._stream(stream)))
         return acc
 
@@ -256,12 +263,12 @@ class Context:
             self._check(self.lib.nf_forces_ex(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset), _ptr(b.cell_count),
                                               _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
                                               float(b.box), float(Gm),
-                                              _SOFT[softening] | (NF_MASS_W if use_mass else 0) | (NF_DENSE_ORDER if dense_order else 0),
+                                              _soft_code(softening) | (NF_MASS_W if use_mass else 0) | (NF_DENSE_ORDER if dense_order else 0),
                                               _ptr(acc), _ptr(cell_amax), self._stream(stream)))
             return acc
         self._check(self.lib.nf_forces(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset), _ptr(b.cell_count),
                                        _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
-                                       float(b.box), float(Gm), _SOFT[softening], _ptr(acc), self._stream(stream)))
+                                       float(b.box), float(Gm), _soft_code(softening), _ptr(acc), self._stream(stream)))
         return acc
 
     def kick_drift(self, pos: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, kick: float, drift: float,
@@ -313,11 +320,11 @@ class Context:
         if mass_host is not None:
             assert (not mass_host.is_cuda) and mass_host.dtype == torch.float32 and mass_host.shape == (N,) and mass_host.is_contiguous()
             self._check(self.lib.nf_forces_host_m(self._h, _ptr(pos_host), _ptr(mass_host), N, int(K), int(R), float(eps),
-                                                  float(box), float(Gm), _SOFT[softening] | NF_MASS_W, _ptr(out),
+                                                  float(box), float(Gm), _soft_code(softening) | NF_MASS_W, _ptr(out),
                                                   self._stream(stream)), allow=allow)
             return out
         self._check(self.lib.nf_forces_host(self._h, _ptr(pos_host), N, int(K), int(R), float(eps), float(box),
-                                            float(Gm), _SOFT[softening], _ptr(out), self._stream(stream)), allow=allow)
+                                            float(Gm), _soft_code(softening), _ptr(out), self._stream(stream)), allow=allow)
         return out
 
     def forces_host_begin(self, pos_host: torch.Tensor, K: int, R: int, eps: float, box: float, Gm: float, out: torch.Tensor,
@@ -328,7 +335,7 @@ class Context:
             assert (not t.is_cuda) and t.dtype == torch.float32 and t.dim() == 2 and t.shape[1] == 3 and t.is_contiguous() and t.is_pinned()
         assert out.shape == pos_host.shape
         self._check(self.lib.nf_forces_host_begin(self._h, _ptr(pos_host), pos_host.shape[0], int(K), int(R), float(eps), float(box),
-                                                  float(Gm), _SOFT[softening], _ptr(out), self._stream(stream)))
+                                                  float(Gm), _soft_code(softening), _ptr(out), self._stream(stream)))
 
     def forces_host_end(self, strict: bool = False):
         """nf_forces_host_end: wait for the oldest step in flight; its ``out`` tensor is then complete."""
@@ -370,7 +377,7 @@ class Context:
         acc_ptrs = (ctypes.c_void_p * P)(*[t.data_ptr() if t.shape[0] else None for t in out])
         stats = StreamStats()
         self._check(self.lib.nf_stream_slabs(self._h, pos_ptrs, ns, int(P), int(K), int(R), float(eps), float(box),
-                                             int(plane0), float(Gm), _SOFT[softening], acc_ptrs, ctypes.byref(stats),
+                                             int(plane0), float(Gm), _soft_code(softening), acc_ptrs, ctypes.byref(stats),
                                              self._stream(stream)), allow=() if strict else (NF_ERR_RANGE,))
         return out, stats.as_dict()
 
@@ -389,7 +396,7 @@ class Context:
         ns = (ctypes.c_int64 * NP)(*[t.shape[0] for t in planes])
         stats = StreamStats()
         self._check(self.lib.nf_stream_step_slabs(self._h, tab(planes), tab(vels), ns, int(P), int(K), int(R), float(eps), float(box),
-                                                  int(plane0), float(Gm), _SOFT[softening], float(kick), float(drift),
+                                                  int(plane0), float(Gm), _soft_code(softening), float(kick), float(drift),
                                                   tab(pos_out), tab(vel_out), tab(acc) if acc is not None else None,
                                                   ctypes.byref(stats), self._stream(stream)))
         return pos_out, vel_out, acc, stats.as_dict()
@@ -444,7 +451,7 @@ class Context:
         out_n = (ctypes.c_int64 * (3 * P))()
         stats = StreamStats()
         self._check(self.lib.nf_stream_step_regroup(self._h, pos_ptrs, vel_ptrs, ns, int(P), int(K), int(R), float(eps), float(box),
-                                                    int(plane0), float(Gm), _SOFT[softening], float(kick), float(drift),
+                                                    int(plane0), float(Gm), _soft_code(softening), float(kick), float(drift),
                                                     tab(out_pos), tab(out_vel), out_n, tab(acc) if acc is not None else None,
                                                     ctypes.byref(stats), self._stream(stream)),
                     allow=() if strict else (NF_ERR_RANGE,))

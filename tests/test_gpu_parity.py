@@ -745,6 +745,51 @@ def test_forces_dense_order_clumps_across_faces(ctx):
     assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL
 
 
+def test_dense_order_host_paths_and_stream(ctx):
+    """The in-cell ordering of dense cells on the other call paths: nf_forces_host and the nf_forces_host_begin / _end
+    pipeline give the bits of nf_forces with the flag, and nf_stream_slabs orders the dense cells of every plane it loads
+    (clumps on a plane face, so dense cells see dense cells of the next plane; x open inside the chunk)."""
+    rng = np.random.default_rng(93)
+    K, R, box = 8, 1, 4.0
+    w = box / K
+    parts = [rng.random((6000, 3)) * box]
+    for centre, m, sig in (((3.0, 3.5, 3.5), 50_000, 0.05), ((4.0, 4.0, 4.0), 70_000, 0.06), ((5.0, 0.0, 7.5), 30_000, 0.04)):
+        parts.append(np.array(centre) * w + sig * w * rng.standard_normal((m, 3)))
+    pos = np.mod(np.concatenate(parts), box).astype(np.float32)
+    pos = np.minimum(pos, np.nextafter(np.float32(box), np.float32(0)))
+    pos = pos[rng.permutation(pos.shape[0])]
+    n, eps, Gm = pos.shape[0], 0.004 * w, 1.0 / pos.shape[0]
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box)
+    assert int((u32(b.cell_count) >= 4096).sum()) >= 8
+    a_dev = ctx.forces(b, R, eps, Gm, dense_order=True).cpu()
+    hpos = torch.from_numpy(pos).pin_memory()
+    assert torch.equal(ctx.forces_host(hpos, K, R, eps, box, Gm, softening="spline+dense"), a_dev)
+    outs = [torch.empty(n, 3).pin_memory() for _ in range(2)]
+    ctx.forces_host_begin(hpos, K, R, eps, box, Gm, outs[0], softening="spline+dense")
+    ctx.forces_host_begin(hpos, K, R, eps, box, Gm, outs[1], softening="spline+dense")
+    ctx.forces_host_end(); ctx.forces_host_end()
+    assert torch.equal(outs[0], a_dev) and torch.equal(outs[1], a_dev)
+    # the slab stream over planes 2..6 (sinks 3..5): filed by the oracle's keys
+    keys, _ = oracle.keys(pos, K, box)
+    cx = (keys // (K * K)).astype(np.int64)
+    plane0, P = 2, 3
+    planes = [torch.from_numpy(pos[cx == plane0 + q].copy()).pin_memory() for q in range(P + 2 * R)]
+    allpos = torch.cat(planes).numpy()
+    starts = np.cumsum([0] + [p.shape[0] for p in planes])
+    sink_idx = np.arange(starts[R], starts[R + P])
+    Gs = 1.0 / allpos.shape[0]
+    # x is open inside the chunk: the oracle sees only the chunk's particles, in a box whose other planes are empty
+    ref = oracle.forces(allpos, K, R, eps, box, Gs, sink_idx=sink_idx)
+    out_d, st_d = ctx.stream_slabs(planes, P, K, R, eps, box, plane0, Gs, softening="spline+dense")
+    out_n, st_n = ctx.stream_slabs(planes, P, K, R, eps, box, plane0, Gs)
+    for out in (out_d, out_n):
+        err = oracle.parity_error(torch.cat(out).numpy(), ref)
+        assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (float(np.median(err)), float(err.max()))
+    assert st_d["interactions"] == st_n["interactions"] and st_d["out_of_range"] == 0
+    out_d2, _ = ctx.stream_slabs(planes, P, K, R, eps, box, plane0, Gs, softening="spline+dense")
+    assert all(torch.equal(a, c) for a, c in zip(out_d, out_d2))
+
+
 def test_forces_dense_order_beyond_its_capacity(ctx):
     """More particles in dense cells than the ordering takes per call (a quarter of N, at least 2^20): the cells past the
     limit keep nf_bin's order and the old laws, next to cells that are ordered."""
