@@ -5,7 +5,10 @@ is a thin marshalling layer over the C functions of the same name (prefix ``nfo_
 arithmetic lives in nf_oracle.c, each routine citing the PAPER.md passage it follows.
 
 Parity status: every function is pinned by tests/test_oracle_pins.py (brute force, closed
-forms, invariants); nothing here is "parity unpinned".
+forms, invariants); nothing here is "parity unpinned" except kick_drift against the paper (it prints no
+formula; pinned to the textbook leapfrog, reading c20).  timestep_terms (criteria 2 and 3,
+PAPER.md:193-195, :207) is plain numpy in this file and pinned by a hand-worked four-cell box; which
+extremum over cells criterion 2 takes is DESIGN.md reading c19.
 """
 from __future__ import annotations
 

@@ -5,7 +5,7 @@
     python -m paper_1810_02916_b200.profiling full <raw.csv> <out.md> --title T --command C [--kernel REGEX] [--interactions I]
         the counters DESIGN.md quotes, from `ncu -i x.ncu-rep --page raw --csv`
     python -m paper_1810_02916_b200.profiling sass <out.md>
-        SASS facts of the interaction kernel k_forces_warp<2, false> in the built libnf.so (cuobjdump -sass): mnemonic
+        SASS facts of the interaction kernel k_forces_warp<2, false, false> (R = 2, no masses, no dense-cell logic) in the built libnf.so (cuobjdump -sass): mnemonic
         counts that show the Blackwell instructions in use, and the body of the untracked (MODE 2) sweep loop
     python -m paper_1810_02916_b200.profiling traffic <workload> <ncu.csv> --command C
         records dram__bytes_read.sum / dram__bytes_write.sum of one interaction-kernel launch on <workload> in
@@ -159,9 +159,9 @@ def cmd_sass(a):
     lib = os.path.join(ROOT, "paper_1810_02916_b200", "libnf.so")
     cmd = ["cuobjdump", "-sass", lib]
     txt = subprocess.run(cmd, capture_output=True, text=True, check=True).stdout
-    m = re.search(r"Function : (\S*k_forces_warpILi2ELb0E\S*)(.*?)(?=\n\s*Function :|\Z)", txt, re.S)
+    m = re.search(r"Function : (\S*k_forces_warpILi2ELb0ELb0E\S*)(.*?)(?=\n\s*Function :|\Z)", txt, re.S)
     if not m:
-        raise SystemExit("k_forces_warp<2, false> not found in " + lib)
+        raise SystemExit("k_forces_warp<2, false, false> not found in " + lib)
     lines = []
     for l in m.group(2).splitlines():
         mm = re.match(r"\s*/\*([0-9a-f]{4,5})\*/\s+(.*?);\s*/\*", l)
@@ -189,7 +189,7 @@ def cmd_sass(a):
                 n2 = sum(1 for _, b in body if re.match(r"(@\S+\s+)?(FFMA2|FADD2|FMUL2)", b))
                 if n2 >= 100 and len(body) < 400:
                     loops.append((tgt, a_, body, n2))
-    out = ["# SASS of the interaction kernel `k_forces_warp<2, false>` (built `libnf.so`, sm_100a)", "",
+    out = ["# SASS of the interaction kernel `k_forces_warp<2, false, false>` (built `libnf.so`, sm_100a)", "",
            "Command: `python -m paper_1810_02916_b200.profiling sass <this file>`, i.e. `cuobjdump -sass paper_1810_02916_b200/libnf.so`",
            f"on the library built from kernel sources sha256 {kernel_source_hash()[:16]}... (`python -m paper_1810_02916_b200.build`).", "",
            f"Function `{m.group(1)}`: {len(lines)} instructions.", "",
