@@ -34,7 +34,7 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "nf.h"), __file__]
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f != "probe_sweep.cu"] + [os.path.join(HERE, "..", "include", "nf.h"), __file__]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
@@ -66,5 +66,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_probe() -> str:
+    """csrc/probe_sweep.cu -> ./probe_sweep: the sweep loops of the interaction kernel in isolation (a measuring tool)."""
+    out = os.path.join(HERE, "probe_sweep")
+    cmd = [os.environ.get("NVCC", "nvcc")] + NVCC_FLAGS[:5] + ["--ftz=true", "-o", out, os.path.join(CSRC, "probe_sweep.cu")]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed compiling probe_sweep.cu")
+    return out
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--probe" in sys.argv:
+        print(build_probe())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
