@@ -549,7 +549,33 @@ def sweep_small_configs(ctx, dev, steps=3, warmup=3):
                 k_ms.append(k)
                 s_ms.append(e0.elapsed_time(e1))
         k = sum(k_ms) / len(k_ms)
-        out[cfg.name] = {"kernel_ms": k, "step_ms": sum(s_ms) / len(s_ms), "interactions": I,
+        graph_ms = None
+        if which == 1:
+            # the smallest config is launch-bound (~45 launches for 0.3 ms of kernels): the same step replayed from a CUDA graph
+            try:
+                st = torch.cuda.Stream()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.stream(st):
+                    ctx.bin(pos, cfg.K, cfg.box, out=b, stream=st)
+                    ctx.forces(b, cfg.R, cfg.eps, cfg.Gm, out=acc, stream=st)
+                    st.synchronize()
+                    g.capture_begin()
+                    ctx.bin(pos, cfg.K, cfg.box, out=b, stream=st)
+                    ctx.forces(b, cfg.R, cfg.eps, cfg.Gm, out=acc, stream=st)
+                    g.capture_end()
+                torch.cuda.synchronize()
+                g.replay()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for _ in range(20):
+                    g.replay()
+                e1.record()
+                torch.cuda.synchronize()
+                graph_ms = e0.elapsed_time(e1) / 20
+                del g
+            except Exception:
+                graph_ms = None
+        out[cfg.name] = {"kernel_ms": k, "step_ms": sum(s_ms) / len(s_ms), "step_ms_cuda_graph": graph_ms, "interactions": I,
                          "frac": FLOP_PER_INTERACTION * I / (k * 1e-3) / peak,
                          "interactions_per_s_step": I / (sum(s_ms) / len(s_ms) * 1e-3)}
         del pos, b, acc

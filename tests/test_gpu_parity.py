@@ -182,6 +182,42 @@ def test_two_particle_closed_form_gpu(ctx):
     assert (ctx.forces(b, R, eps, Gm).cpu().numpy() == 0).all()
 
 
+def test_step_is_capturable_in_a_cuda_graph(ctx):
+    """nf_bin + nf_forces enqueue only stream-ordered work once the scratch is reserved (include/nf.h), so a step can be
+    captured in a CUDA graph and replayed (what a launch-bound small problem wants): same bits as the direct calls."""
+    cfg = inputs.config(1)
+    pos = inputs.make_positions(cfg, device="cuda")
+    ctx.reserve(cfg.N, cfg.K)
+    b = ctx.bin(pos, cfg.K, cfg.box)
+    acc = torch.empty(cfg.N, 3, device="cuda")
+    ctx.forces(b, cfg.R, cfg.eps, cfg.Gm, out=acc)
+    ref, ref_perm = acc.clone(), b.perm.clone()
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        ctx.bin(pos, cfg.K, cfg.box, out=b, stream=s)
+        ctx.forces(b, cfg.R, cfg.eps, cfg.Gm, out=acc, stream=s)
+        s.synchronize()
+        g.capture_begin()
+        ctx.bin(pos, cfg.K, cfg.box, out=b, stream=s)
+        ctx.forces(b, cfg.R, cfg.eps, cfg.Gm, out=acc, stream=s)
+        g.capture_end()
+    torch.cuda.synchronize()
+    for _ in range(3):
+        acc.zero_()
+        b.perm.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(acc, ref) and torch.equal(b.perm, ref_perm)
+    # new positions in the same buffer: the replay bins and computes them
+    pos2 = inputs.make_positions(inputs.dataclasses.replace(cfg, seed=cfg.seed + 5), device="cuda")
+    pos.copy_(pos2)
+    g.replay()
+    torch.cuda.synchronize()
+    b2 = ctx.bin(pos2, cfg.K, cfg.box)
+    assert torch.equal(acc, ctx.forces(b2, cfg.R, cfg.eps, cfg.Gm))
+
+
 def test_forces_sorted_order_and_determinism(ctx):
     cfg = inputs.scaled(inputs.config(3), 50_000, 8)
     pos = inputs.make_positions(cfg).cuda()
