@@ -132,13 +132,17 @@ static size_t forces_scratch_full(int64_t N, int K)
     return nf_forces_scratch_bytes(p) + 2 * nf_align_up((size_t)(N > 0 ? N : 1) * 16, 256);   // + the two encoded copies
 }
 
+static size_t dense_full_bytes(int64_t N, int K, int softening);
+
 int nf_reserve(nf_ctx *ctx, int64_t maxN, int K)
 {
     if (!ctx) return NF_ERR_ARG;
     NF_TRY(check_common(ctx, maxN, K, 1.0f));
     NF_CUDA(ctx, cudaSetDevice(ctx->device));
     size_t need = nf_bin_scratch_bytes(maxN, K, false);
-    size_t f = forces_scratch_full(maxN, K);
+    // (the in-cell ordering of dense cells is reserved for where it is automatic; a call that asks for it with
+    // NF_DENSE_ORDER on a sparser box grows the arena once)
+    size_t f = forces_scratch_full(maxN, K) + dense_full_bytes(maxN, K, 0);
     return nf_scratch_reserve(ctx, need > f ? need : f);
 }
 
