@@ -216,7 +216,9 @@ int nf_forces_ex(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offs
  *
  *   x_lo, x_hi   sink plane range, 0 <= x_lo <= x_hi <= K (ranges that wrap are two calls)
  *   cell_amax    nullable, K^3 float32 as for nf_forces_ex (zero outside the sink planes)
- *   everything else as for nf_forces_ex.  nf_forces_ex is nf_forces_chunk with [0, K).
+ *   everything else as for nf_forces_ex.  nf_forces_ex is nf_forces_chunk with [0, K).  A sink's acceleration does not depend on
+ *   the range it is computed in, up to the last bits: the bits are the same as long as no task of the call is split over
+ *   several work-list entries (small problems with few, long tasks), else equal within rounding.
  */
 int nf_forces_chunk(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset, const uint32_t *perm,
                     int64_t N, int K, int R, float eps, float box, float Gm, int softening, int x_lo, int x_hi,

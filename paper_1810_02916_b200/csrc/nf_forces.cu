@@ -263,7 +263,9 @@ struct SplitTable {
     uint8_t nt[128];
     uint8_t L[128][SPLIT_MAX];
 };
-__constant__ SplitTable c_split[2];   // [0]: L <= 32;  [1]: L <= 8, for problems too small to fill the GPU with full-width tasks
+constexpr int N_TABLES = 2;
+__constant__ SplitTable c_split[N_TABLES];   // [0]: L <= 32;  [1..]: narrower tasks for problems too small to fill the GPU with full-width ones
+__constant__ int c_lmax[N_TABLES];
 
 __global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restrict__ planes, nf_force_params p, int small,
                                                     uint32_t *__restrict__ tc)
@@ -274,10 +276,22 @@ __global__ void __launch_bounds__(256) k_task_count(const nf_plane_view *__restr
     const size_t nc = (size_t)gridDim.y * KK, c = task_slot((int)blockIdx.y, cyz, p.K, (int)gridDim.y);
     const uint64_t *off = planes[p.sink_lo + blockIdx.y].off;
     const uint64_t n = off[cyz + 1] - off[cyz];
-    const uint32_t nt = (uint32_t)(n >> 7) + c_split[small].nt[n & 127];
+    // full tasks of 4 Lmax sinks, and the split of the remainder from the table
+    const int lmax = c_lmax[small], full = 4 * lmax;
+    const int rem = (int)(n % (uint64_t)full);
+    uint32_t narrow = 0;
+    if (small)                          // only where the whole problem is a few tasks per warp (below)
+        for (int k = 0; k < c_split[small].nt[rem]; k++) narrow += 2 * c_split[small].L[rem][k] <= lmax ? 1u : 0u;
+    const uint32_t nt = (uint32_t)(n / (uint64_t)full) + c_split[small].nt[rem];
     const bool heavy = n >= HEAVY_N;
-    tc[c] = heavy ? nt : 0u;            // first half of the list: dense cells
-    tc[nc + c] = heavy ? 0u : nt;
+    // three sections: the tasks of dense cells first (long tasks early), then the others in the order of task_slot, and --
+    // for SMALL problems, where every warp gets one or two tasks and the kernel lasts as long as its slowest warp -- the
+    // NARROW tasks of those (few sinks, many phases: a fraction of a full task's time) last, so that the statically
+    // assigned first round is the long tasks and the short ones fill in behind them (C1: 0.20 -> 0.15 ms).  For large
+    // problems this order costs locality (C4: -1 point) and stays off.
+    tc[c] = heavy ? nt : 0u;
+    tc[nc + c] = heavy ? 0u : nt - narrow;
+    tc[2 * nc + c] = heavy ? 0u : narrow;
 }
 
 // ctl[0] = work cursor (zeroed here), ctl[1] = number of entries of the work list the kernel reads, ctl[2] = number of tasks
@@ -291,30 +305,32 @@ __global__ void __launch_bounds__(256) k_task_fill(const nf_plane_view *__restri
     const size_t nc = (size_t)gridDim.y * KK, c = task_slot((int)blockIdx.y, cyz, p.K, (int)gridDim.y);
     const uint64_t *off = planes[p.sink_lo + blockIdx.y].off;
     const uint64_t n = off[cyz + 1] - off[cyz];
-    const size_t e = n >= HEAVY_N ? c : nc + c;
-    uint32_t o = to[e];
+    const bool heavy = n >= HEAVY_N;
+    uint32_t o = to[heavy ? c : nc + c], o_narrow = to[2 * nc + c];
     Task t;
     t.nparts = 1;
     t.part_slot = 0;
     t.cyz = (uint32_t)cyz;
     t.plane = (uint16_t)(p.sink_lo + blockIdx.y);
     uint32_t first = 0;
-    for (uint64_t k = 0; k < (n >> 7); k++) {
+    const int lmax = c_lmax[small], full = 4 * lmax;
+    for (uint64_t k = 0; k < n / (uint64_t)full; k++) {
         t.first = first;
-        t.L = 32;
+        t.L = (uint8_t)lmax;
         tasks[o++] = t;
-        first += 128;
+        first += (uint32_t)full;
     }
-    const int rem = (int)(n & 127);
+    const int rem = (int)(n % (uint64_t)full);
     for (int k = 0; k < c_split[small].nt[rem]; k++) {
         t.first = first;
         t.L = (uint8_t)c_split[small].L[rem][k];
-        tasks[o++] = t;
+        if (small && !heavy && 2 * (int)t.L <= lmax) tasks[o_narrow++] = t;
+        else tasks[o++] = t;
         first += 4u * t.L;
     }
     if (cyz == KK - 1 && blockIdx.y == gridDim.y - 1) {
         ctl[0] = 0;
-        ctl[1] = ctl[2] = to[2 * nc - 1] + tc[2 * nc - 1];
+        ctl[1] = ctl[2] = to[3 * nc - 1] + tc[3 * nc - 1];
         ctl[4] = ctl[5] = ctl[6] = 0;
     }
 }
@@ -1126,16 +1142,20 @@ void make_split_table(SplitTable &t, int Lmax)
 
 }  // namespace
 
+static const int TABLE_LMAX[N_TABLES] = {32, 8};
+
 static size_t n_sink_cells(const nf_force_params &p)
 {
     const int n_sink_planes = p.sink_hi - p.sink_lo;
     return (size_t)(n_sink_planes > 0 ? n_sink_planes : 0) * p.K * p.K;
 }
+constexpr size_t SMALL_SINKS_MAX = 256u * 256u * N_CONS;      // no problem with more sinks takes a narrow table (256 SMs at most)
 static size_t max_tasks(const nf_force_params &p)
 {
-    // full tasks (128 sinks) plus at most SPLIT_MAX remainder tasks per cell, each holding at least one sink
+    // full tasks (128 sinks; down to 16 for problems small enough to take a narrow table) plus at most SPLIT_MAX remainder
+    // tasks per cell, each holding at least one sink
     const size_t ms = (size_t)(p.max_sinks > 0 ? p.max_sinks : 0), rem = n_sink_cells(p) * SPLIT_MAX;
-    return (rem < ms ? rem : ms) + ms / 128 + 1;
+    return (rem < ms ? rem : ms) + ms / (ms < SMALL_SINKS_MAX ? 16 : 128) + 1;
 }
 // The source split is considered only for problems that can have fewer than split_target tasks (every task holds
 // at most 128 sinks); its work list has at most max_tasks + split_target entries, of which at most
@@ -1148,8 +1168,8 @@ size_t nf_forces_scratch_bytes(const nf_force_params &p)
 {
     const size_t nc = n_sink_cells(p);
     size_t b = nf_align_up((size_t)p.n_planes * sizeof(nf_plane_view), 256);
-    b += 2 * nf_align_up(2 * nc * sizeof(uint32_t), 256);                           // tc, to
-    b += nf_align_up(nf_scan_temp_elems(2 * nc) * sizeof(uint32_t), 256);           // scan temp
+    b += 2 * nf_align_up(3 * nc * sizeof(uint32_t), 256);                           // tc, to
+    b += nf_align_up(nf_scan_temp_elems(3 * nc) * sizeof(uint32_t), 256);           // scan temp
     b += nf_align_up(max_tasks(p) * sizeof(Task), 256);                             // tasks
     // the source split of small problems (sized for the largest GPU this could run on: 256 SMs)
     const size_t st_max = 32u * 256u * N_CONS;
@@ -1164,10 +1184,10 @@ size_t nf_forces_scratch_bytes(const nf_force_params &p)
 
 int nf_forces_init(nf_ctx *ctx)
 {
-    static SplitTable t[2];
-    make_split_table(t[0], 32);
-    make_split_table(t[1], 8);        // 4 tasks of 32 sinks still cover any remainder below 128
+    static SplitTable t[N_TABLES];
+    for (int i = 0; i < N_TABLES; i++) make_split_table(t[i], TABLE_LMAX[i]);
     NF_CUDA(ctx, cudaMemcpyToSymbol(c_split, t, sizeof(t)));
+    NF_CUDA(ctx, cudaMemcpyToSymbol(c_lmax, TABLE_LMAX, sizeof(TABLE_LMAX)));
     return NF_OK;
 }
 
@@ -1238,9 +1258,9 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
     const ForceConsts fc = make_consts(p);
     const int n_sink_planes = p.sink_hi - p.sink_lo;
     const size_t nc = n_sink_cells(p);
-    uint32_t *tc = nf_scratch_take<uint32_t>(ctx, nc ? 2 * nc : 1);
-    uint32_t *to = nf_scratch_take<uint32_t>(ctx, nc ? 2 * nc : 1);
-    uint32_t *tmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(2 * nc));
+    uint32_t *tc = nf_scratch_take<uint32_t>(ctx, nc ? 3 * nc : 1);
+    uint32_t *to = nf_scratch_take<uint32_t>(ctx, nc ? 3 * nc : 1);
+    uint32_t *tmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(3 * nc));
     Task *tasks = nf_scratch_take<Task>(ctx, max_tasks(p));
     uint32_t *ctl = nf_scratch_take<uint32_t>(ctx, 8);
     if (!tc || !to || !tmp || !tasks || !ctl) {
@@ -1270,12 +1290,17 @@ int nf_forces_impl(nf_ctx *ctx, const nf_force_params &p, const nf_plane_view *d
     if (n_sink_planes > 0) {
         // work list
         dim3 grid((unsigned)((p.K * p.K + 255) / 256), (unsigned)n_sink_planes);
-        // A problem with fewer tasks than resident warps (3 blocks of 4 per SM) is bound by the length of
-        // one task: narrower tasks (L <= 8, so P >= 4 phases share every tile) halve it.  ~40 sinks per task.
-        const int small = p.max_sinks < 40LL * ctx->sm_count * N_CONS ? 1 : 0;
+        // A problem with only a few tasks per consumer warp is bound by the length of its tasks and by how evenly they
+        // fall on the schedulers: it takes the table of narrow tasks (L <= 8 lanes, 32 sinks, >= 4 phases share every
+        // tile; cells are cut into tasks of 32 sinks instead of 128), the narrowest of them last.  Measured against
+        // tables with L <= 4 ... 32 on boxes of 8 x 10^3 ... 2.6 x 10^5 particles: best or within 3 % of the best up to
+        // ~150 sinks per consumer warp (C1: 0.257 ms with full-width tasks, 0.153 ms with these).
+        // (not for boxes of dense cells -- mean occupancy above 512 --, which have many full-width tasks per warp anyway)
+        const int small = p.max_sinks < 256LL * ctx->sm_count * N_CONS && (size_t)p.max_sinks < SMALL_SINKS_MAX &&
+                                  (size_t)p.max_sinks <= 512 * nc ? 1 : 0;
         k_task_count<<<grid, 256, 0, st>>>(d_planes, p, small, tc);
         NF_LAUNCHED(ctx);
-        NF_TRY(nf_exclusive_scan_u32(ctx, tc, to, 2 * nc, tmp, st));
+        NF_TRY(nf_exclusive_scan_u32(ctx, tc, to, 3 * nc, tmp, st));
         k_task_fill<<<grid, 256, 0, st>>>(d_planes, tc, to, p, small, tasks, ctl);
         NF_LAUNCHED(ctx);
         if (split) {
