@@ -19,3 +19,5 @@ from .nf_oracle import (  # noqa: F401
     max_threads,
     parity_error,
 )
+from . import nf_tree  # noqa: F401,E402  (tree near field for dense cells)
+from .nf_tree import forces_tree  # noqa: F401,E402
