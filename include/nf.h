@@ -225,6 +225,40 @@ int nf_forces_chunk(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_o
                     float *acc_xyz, float *cell_amax, void *stream);
 
 /*
+ * nf_forces_tree -- nf_forces_ex with a TREE for the sources of dense cells ("Future versions of Abacus
+ * will employ trees in the near-field domain, especially for dense cells"; "the largest cell has over
+ * 200,000 particles").  The paper names the idea and prints no algorithm; the one built
+ * here is stated in DESIGN.md (readings t1-t6) and followed step by step by oracle/nf_tree.py:
+ *
+ *   - a cell of >= 4096 particles is DENSE (the cells NF_DENSE_ORDER orders: at most 2048 of them and
+ *     min(max(N/4, 2^20), 2^28) particles in 64-aligned sizes, taken in cell order; further ones are not dense);
+ *   - its particles, in Morton order of their cell-centred offsets, form leaves of 64 and nodes of 8 children up to a
+ *     root; a node has the bounding box of its particles, their mass and centre of mass;
+ *   - sinks are taken 64 at a time (consecutive in their cell) with their bounding box; such a group meets each dense
+ *     cell among its (2R+1)^3 neighbours by walking that cell's tree: a node whose box is further from the group's box
+ *     than eps and than (its diagonal / theta) acts as ONE particle at its centre of mass (1/r^2); any other node is
+ *     opened, and a leaf that is not accepted is summed particle by particle with the softened law of `softening`;
+ *   - sources of cells that are not dense are summed directly, exactly as by nf_forces_ex.
+ *
+ *   theta       opening angle, 0 <= theta < 1.  theta = 0 accepts nothing: the result is the direct sum (nf_forces_ex up
+ *               to summation order).  For theta > 0 the result is an APPROXIMATION: per accepted node the error is at
+ *               most G M / D^2 * (1/(1-theta)^2 - 1 - 2 theta), D the distance to its centre of mass.
+ *   everything else as for nf_forces_ex (NF_MASS_W allowed; NF_DENSE_ORDER implied).  cell_amax is computed from the
+ *   final accelerations.  Asynchronous on `stream`; deterministic (bit-reproducible from call to call).
+ *   The box must be whole (no chunk / slab / host variant).
+ *
+ * nf_tree_stats -- what the last nf_forces_tree on this context evaluated (synchronises `stream`):
+ *   node_interactions  sum over (sink, accepted node) pairs
+ *   leaf_interactions  sum over (sink, particle of an opened leaf) pairs
+ * The walk's decisions are taken in float32 in a fixed order of rounded operations, so both counts are exact
+ * properties of the input (the oracle reproduces them bit for bit).
+ */
+int nf_forces_tree(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset, const uint32_t *perm, int64_t N,
+                   int K, int R, float eps, float box, float Gm, int softening, float theta, float *acc_xyz,
+                   float *cell_amax, void *stream);
+int nf_tree_stats(nf_ctx *ctx, int64_t *node_interactions, int64_t *leaf_interactions, void *stream);
+
+/*
  * nf_kick_drift -- the leapfrog updates that follow the force in the slab pipeline (Table 1
  * "Kick", "Drift").  The paper gives no formula, so the
  * factors are the caller's (they absorb the cosmological prefactors of the time step):

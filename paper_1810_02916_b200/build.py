@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnf.so")
-SOURCES = ["nf_api.cu", "nf_scan.cu", "nf_bin.cu", "nf_forces.cu", "nf_stream.cu", "nf_step.cu", "nf_regroup.cu", "nf_dense.cu"]
+SOURCES = ["nf_api.cu", "nf_scan.cu", "nf_bin.cu", "nf_forces.cu", "nf_stream.cu", "nf_step.cu", "nf_regroup.cu", "nf_dense.cu", "nf_tree.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",

@@ -206,12 +206,14 @@ static size_t dense_full_bytes(int64_t N, int K, int softening)
 
 // Encoded copies of a whole box, the in-cell ordering of its dense cells where it is wanted (nf_dense.cu; outputs taken
 // from the arena), and the plane table.  Clears NF_DENSE_ORDER in p.softening and sets p.dense.
+struct TreeHandles { uint32_t *dinfo, *dslot; nf_dense_keep keep; };
 static int encode_full(nf_ctx *ctx, nf_force_params &p, const float4 *ps, const uint64_t *off, const uint32_t *perm, int64_t N,
-                       float4 *enc, float4 *enc_h, nf_plane_view *d_planes, float *acc, float *cell_amax, cudaStream_t st)
+                       float4 *enc, float4 *enc_h, nf_plane_view *d_planes, float *acc, float *cell_amax, cudaStream_t st,
+                       TreeHandles *tree = nullptr)
 {
     const int K = p.K;
     const size_t ncell = (size_t)K * K * K;
-    const bool dense = nf_dense_wanted(N, ncell, p.softening);
+    const bool dense = nf_dense_wanted(N, ncell, p.softening | (tree ? NF_DENSE_ORDER : 0));
     p.softening &= ~NF_DENSE_ORDER;
     NF_TRY(nf_encode_impl(ctx, p, ps, off, ncell, enc, enc_h, st));
     uint32_t *dinfo = nullptr, *dslot = nullptr;
@@ -222,18 +224,32 @@ static int encode_full(nf_ctx *ctx, nf_force_params &p, const float4 *ps, const 
         dslot = nf_scratch_take<uint32_t>(ctx, cap);
         dbox = nf_scratch_take<float>(ctx, cap / 64 * 6);
         if (!dinfo || !dslot || !dbox) { NF_SET_ERR(ctx, "nf_forces: internal scratch arena too small (dense-cell ordering)"); return NF_ERR_NOMEM; }
+        nf_dense_keep keep{nullptr, nullptr};
+        float4 *sentinel = nullptr;
+        if (tree) {                                // nf_tree.cu builds on the table of dense cells; the kernel needs a sentinel tile
+            keep.dcell = nf_scratch_take<nf_dense_cell>(ctx, NF_DENSE_MAX_CELLS);
+            keep.nd = nf_scratch_take<uint32_t>(ctx, 64);
+            sentinel = nf_scratch_take<float4>(ctx, 16);
+            if (!keep.dcell || !keep.nd || !sentinel) { NF_SET_ERR(ctx, "nf_forces_tree: internal scratch arena too small"); return NF_ERR_NOMEM; }
+        }
         const size_t mark = ctx->scratch_used;
-        NF_TRY(nf_dense_order_impl(ctx, p, ps, off, ncell, N, enc, enc_h, dinfo, dslot, dbox, st));
+        NF_TRY(nf_dense_order_impl(ctx, p, ps, off, ncell, N, enc, enc_h, dinfo, dslot, dbox, st, tree ? &keep : nullptr));
         ctx->scratch_used = mark;                  // its temporaries are dead once enqueued work is ordered: same stream
         p.dense = 1;
+        if (tree) {
+            NF_TRY(nf_tree_sentinel(ctx, sentinel, st));
+            p.tree = 1; p.sentinel = sentinel;
+            tree->dinfo = dinfo; tree->dslot = dslot; tree->keep = keep;
+        }
     }
-    return nf_fill_planes_full(ctx, d_planes, K, ps, enc, enc_h, off, perm, acc, cell_amax, dinfo, dslot, dbox, st);
+    // with the tree the per-cell maxima come from the final accelerations (nf_tree.cu), not from the kernel's epilogue
+    return nf_fill_planes_full(ctx, d_planes, K, ps, enc, enc_h, off, perm, acc, p.tree ? nullptr : cell_amax, dinfo, dslot, dbox, st);
 }
 
 // nf_forces / nf_forces_ex / nf_forces_chunk: sinks are the particles of the x-planes [x_lo, x_hi)
 static int forces_common(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset, const uint32_t *perm, int64_t N, int K,
                          int R, float eps, float box, float Gm, int softening, int x_lo, int x_hi, float *acc_xyz, float *cell_amax,
-                         void *stream)
+                         void *stream, bool tree = false, float theta = 0.f)
 {
     NF_TRY(check_common(ctx, N, K, box));
     NF_TRY(check_force_args(ctx, K, R, eps, Gm, softening));
@@ -250,7 +266,10 @@ static int forces_common(nf_ctx *ctx, const float *pos_sorted, const uint64_t *c
     p.K = K; p.n_planes = K; p.periodic_x = 1; p.sink_lo = x_lo; p.sink_hi = x_hi;
     p.R = R; p.eps = eps; p.box = box; p.Gm = Gm; p.softening = softening; p.max_sinks = N;
     nf_scratch_reset(ctx);
-    NF_TRY(nf_scratch_reserve(ctx, forces_scratch_full(N, K) + dense_full_bytes(N, K, softening)));
+    const size_t ncell = (size_t)K * K * K;
+    tree = tree && N >= NF_DENSE_N;                    // no cell can be dense below that: the plain path
+    NF_TRY(nf_scratch_reserve(ctx, forces_scratch_full(N, K) + dense_full_bytes(N, K, softening | (tree ? NF_DENSE_ORDER : 0)) +
+                                       (tree ? nf_tree_scratch_bytes(N, ncell) : 0)));
     nf_plane_view *d_planes = nf_scratch_take<nf_plane_view>(ctx, (size_t)K);
     float4 *enc = nf_scratch_take<float4>(ctx, (size_t)N);
     float4 *enc_h = nf_scratch_take<float4>(ctx, (size_t)N);
@@ -258,8 +277,32 @@ static int forces_common(nf_ctx *ctx, const float *pos_sorted, const uint64_t *c
     cudaStream_t st = (cudaStream_t)stream;
     const float4 *ps = reinterpret_cast<const float4 *>(pos_sorted);
     if (cell_amax) NF_CUDA(ctx, cudaMemsetAsync(cell_amax, 0, sizeof(float) * (size_t)K * K * K, st));
-    NF_TRY(encode_full(ctx, p, ps, cell_offset, perm, N, enc, enc_h, d_planes, acc_xyz, cell_amax, st));
-    return nf_forces_impl(ctx, p, d_planes, st, true);
+    TreeHandles th{};
+    NF_TRY(encode_full(ctx, p, ps, cell_offset, perm, N, enc, enc_h, d_planes, acc_xyz, cell_amax, st, tree ? &th : nullptr));
+    NF_TRY(nf_forces_impl(ctx, p, d_planes, st, true));
+    if (tree) NF_TRY(nf_tree_forces_impl(ctx, p, theta, ps, cell_offset, perm, N, th.dinfo, th.dslot, th.keep, acc_xyz, cell_amax, st));
+    return NF_OK;
+}
+
+int nf_forces_tree(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset, const uint32_t *perm, int64_t N, int K, int R,
+                   float eps, float box, float Gm, int softening, float theta, float *acc_xyz, float *cell_amax, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, theta >= 0.0f && theta < 1.0f, "nf_forces_tree: theta = %g outside [0, 1)", (double)theta);
+    return forces_common(ctx, pos_sorted, cell_offset, perm, N, K, R, eps, box, Gm, softening, 0, K, acc_xyz, cell_amax, stream, true, theta);
+}
+
+int nf_tree_stats(nf_ctx *ctx, int64_t *node_interactions, int64_t *leaf_interactions, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, node_interactions && leaf_interactions, "nf_tree_stats: null output");
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    NF_CUDA(ctx, cudaMemcpyAsync(ctx->h_counters + 8, ctx->counters + 8, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    NF_CUDA(ctx, cudaStreamSynchronize(st));
+    *node_interactions = (int64_t)ctx->h_counters[8];
+    *leaf_interactions = (int64_t)ctx->h_counters[9];
+    return NF_OK;
 }
 
 int nf_forces(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_offset,

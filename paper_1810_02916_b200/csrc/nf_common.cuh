@@ -122,6 +122,8 @@ struct nf_force_params {
     int softening;
     long long max_sinks;  // upper bound on the particles in the sink planes (sizes the work list)
     int dense;            // 1: some plane view carries the in-cell ordering of dense cells (selects the kernel instance with that logic)
+    int tree;             // 1 (needs dense): the sources of dense cells are left to the tree near field (nf_tree.cu) -- the interaction kernel skips them
+    const float4 *sentinel;   // tree: two far-away massless sources, the only tile of a task that has no other source left
 };
 size_t nf_forces_scratch_bytes(const nf_force_params &p);
 // d_planes: DEVICE array of p.n_planes views (fill with nf_fill_planes_full or copy from pinned memory)
@@ -148,8 +150,21 @@ uint32_t nf_dense_cap(int64_t N);
 size_t nf_dense_scratch_bytes(int64_t N, size_t ncell);
 // is the ordering taken for a set of N particles in ncell cells?  From the arguments alone (the same call always takes the same path)
 static inline bool nf_dense_wanted(int64_t N, size_t ncell, int softening) { return N >= NF_DENSE_N && ((softening & NF_DENSE_ORDER) || (size_t)N / ncell >= 512); }
+struct nf_dense_cell { unsigned long long c0; uint32_t coff, cell, n, pad; };   // first slot, compact offset (64-aligned), cell index, particles
+// keep (nullable): where the caller wants the table of dense cells (NF_DENSE_MAX_CELLS entries, by rank) and two counters
+// (compact length, number of dense cells) to outlive the call -- nf_tree.cu builds on them
+struct nf_dense_keep { nf_dense_cell *dcell; uint32_t *nd; };
 int nf_dense_order_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, int64_t N,
-                        float4 *enc, float4 *enc_h, uint32_t *dinfo, uint32_t *dslot, float *dbox, cudaStream_t st);
+                        float4 *enc, float4 *enc_h, uint32_t *dinfo, uint32_t *dslot, float *dbox, cudaStream_t st,
+                        const nf_dense_keep *keep = nullptr);
+// Tree near field for dense cells (nf_tree.cu, readings t1-t6), whole box only.  Runs after the
+// interaction kernel (which skipped the sources of dense cells: p.tree) and ADDS the dense cells' attraction to acc.
+size_t nf_tree_scratch_bytes(int64_t N, size_t ncell);
+int nf_tree_forces_impl(nf_ctx *ctx, const nf_force_params &p, float theta, const float4 *pos, const uint64_t *off, const uint32_t *perm,
+                        int64_t N, const uint32_t *dinfo, const uint32_t *dslot, const nf_dense_keep &keep, float *acc,
+                        float *cell_amax, cudaStream_t st);
+// writes the two sentinel sources (p.sentinel); part of the tree path, launched before the interaction kernel
+int nf_tree_sentinel(nf_ctx *ctx, float4 *sentinel, cudaStream_t st);
 size_t nf_radix_tiles(int64_t n_max);
 int nf_radix_pass(nf_ctx *ctx, const uint32_t *kin, const uint32_t *iin, int64_t n_max, const uint32_t *n_dev, uint32_t bins,
                   uint32_t shift, uint32_t *kout, uint32_t *iout, uint32_t *hist, uint32_t *tmp32, cudaStream_t st);

@@ -23,7 +23,7 @@ namespace {
 constexpr uint32_t PAD = 0xffffffffu;
 constexpr uint32_t MORTON_BITS = 21, MORTON_MASK = (1u << MORTON_BITS) - 1;
 
-struct DenseCell { unsigned long long c0; uint32_t coff, cell, n, pad; };
+using DenseCell = nf_dense_cell;
 
 __device__ __forceinline__ uint32_t spread3(uint32_t v)      // 7 bits -> every third bit
 {
@@ -66,14 +66,17 @@ __global__ void __launch_bounds__(256) k_dense_keys(const float4 *__restrict__ p
         dc.c0 = c0; dc.coff = o; dc.cell = (uint32_t)c; dc.n = n; dc.pad = 0;
         dcell[r] = dc;
         atomicMax(nd, o + m);                        // integer: order-independent
+        atomicAdd(nd + 1, 1u);                       // number of dense cells taken
     }
     for (uint32_t j = lane; j < m; j += 32) {
         uint32_t k = MORTON_MASK, i = PAD;           // padding sorts behind the cell's particles
         if (j < n) {
             const float4 q = pos[c0 + j];
-            const int qx = min(127, max(0, (int)((q.x * invw + 0.5f) * 128.0f)));
-            const int qy = min(127, max(0, (int)((q.y * invw + 0.5f) * 128.0f)));
-            const int qz = min(127, max(0, (int)((q.z * invw + 0.5f) * 128.0f)));
+            // every operation rounded to float32, no fused multiply-add: the order is part of the tree's definition
+            // (reading t2) and the oracle takes the same decision in the same precision
+            const int qx = min(127, max(0, (int)__fmul_rn(__fadd_rn(__fmul_rn(q.x, invw), 0.5f), 128.0f)));
+            const int qy = min(127, max(0, (int)__fmul_rn(__fadd_rn(__fmul_rn(q.y, invw), 0.5f), 128.0f)));
+            const int qz = min(127, max(0, (int)__fmul_rn(__fadd_rn(__fmul_rn(q.z, invw), 0.5f), 128.0f)));
             k = spread3((uint32_t)qz) | (spread3((uint32_t)qy) << 1) | (spread3((uint32_t)qx) << 2);
             i = j;
         }
@@ -152,7 +155,8 @@ size_t nf_dense_scratch_bytes(int64_t N, size_t ncell)
 }
 
 int nf_dense_order_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, int64_t N,
-                        float4 *enc, float4 *enc_h, uint32_t *dinfo, uint32_t *dslot, float *dbox, cudaStream_t st)
+                        float4 *enc, float4 *enc_h, uint32_t *dinfo, uint32_t *dslot, float *dbox, cudaStream_t st,
+                        const nf_dense_keep *keep)
 {
     const int K = p.K;
     const uint32_t cap = nf_dense_cap(N);
@@ -164,8 +168,8 @@ int nf_dense_order_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos
     uint32_t *keyA = nf_scratch_take<uint32_t>(ctx, cap), *keyB = nf_scratch_take<uint32_t>(ctx, cap);
     uint32_t *idxA = nf_scratch_take<uint32_t>(ctx, cap), *idxB = dslot;
     float *box = dbox;
-    DenseCell *dcell = nf_scratch_take<DenseCell>(ctx, NF_DENSE_MAX_CELLS);
-    uint32_t *nd = nf_scratch_take<uint32_t>(ctx, 64);
+    DenseCell *dcell = keep ? keep->dcell : nf_scratch_take<DenseCell>(ctx, NF_DENSE_MAX_CELLS);
+    uint32_t *nd = keep ? keep->nd : nf_scratch_take<uint32_t>(ctx, 64);
     const size_t nt = nf_radix_tiles(cap);
     uint32_t *hist = nf_scratch_take<uint32_t>(ctx, 256 * nt);
     uint32_t *htmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(256 * nt));
@@ -175,7 +179,7 @@ int nf_dense_order_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos
     }
     float scale, ws;
     nf_encode_consts(p, &scale, &ws);
-    NF_CUDA(ctx, cudaMemsetAsync(nd, 0, sizeof(uint32_t), st));
+    NF_CUDA(ctx, cudaMemsetAsync(nd, 0, 2 * sizeof(uint32_t), st));
     k_dense_mark<<<(unsigned)((ncell + 255) / 256), 256, 0, st>>>(off, ncell, n64, one);
     NF_LAUNCHED(ctx);
     NF_TRY(nf_exclusive_scan_u32(ctx, n64, coff, ncell, stmp, st));

@@ -370,6 +370,7 @@ __global__ void __launch_bounds__(256) k_split_measure(const nf_plane_view *__re
                 const int qy = ((cy + dy) % K + K) % K;
                 for (int dz = -R; dz <= R; dz++) {
                     const int qz = ((cz + dz) % K + K) % K;
+                    if (p.tree && planes[px].dinfo && planes[px].dinfo[qy * K + qz]) continue;   // swept by the tree, not here
                     S += off[qy * K + qz + 1] - off[qy * K + qz];
                 }
             }
@@ -562,7 +563,7 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
             else if (px < 0 || px >= p.n_planes) px = -1;
             const int qy = ((cy + dyi - R) % K + K) % K;
             const uint64_t *qo = px >= 0 ? planes[px].off + (size_t)qy * K : nullptr;
-            const uint32_t *qd = (DENSE && own_di && px >= 0 && planes[px].dinfo) ? planes[px].dinfo + (size_t)qy * K : nullptr;
+            const uint32_t *qd = (DENSE && (own_di || p.tree) && px >= 0 && planes[px].dinfo) ? planes[px].dinfo + (size_t)qy * K : nullptr;
             uint32_t prev_end = 0;
             int prev_k = 0;
             bool have = false;
@@ -572,6 +573,8 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
                 st[s] = 0; cn[s] = 0;
                 if (qo) { st[s] = (uint32_t)qo[qz]; cn[s] = (uint32_t)(qo[qz + 1] - qo[qz]); }
                 di[s] = (DENSE && qd) ? qd[qz] : 0u;
+                // tree near field (nf_tree.cu): the sources of dense cells are its business, for every sink
+                if (DENSE && p.tree && di[s]) { cn[s] = 0; di[s] = 0u; }
                 kz[s] = (s - R) - ((qz + zphi) % ZB) + ((cz + zphi) % ZB);
                 // the sinks' own cell is a piece of its own, and so is every dense cell seen from a dense cell (its tiles get
                 // their law from the boxes, tile by tile)
@@ -624,6 +627,16 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
         n_pieces += __shfl_sync(0xffffffffu, incl, 31);
     }
     __syncwarp();
+    if (DENSE && p.tree && n_pieces == 0) {
+        // every source of this task went to the tree: its one tile is two massless sources far away (zero force), so
+        // that the task still has a first and a last tile
+        if (lane == 0) {
+            S.enc[0] = p.sentinel;
+            S.piece[0] = make_uint4(0u, 2u, (128u << 8) | (2u << 27), 0u);
+        }
+        n_pieces = 1;
+        __syncwarp();
+    }
     // balanced tile length of every piece (no division on the per-tile path)
     for (int i = lane; i < n_pieces; i += 32) {
         const uint32_t cnt = S.piece[i].y;

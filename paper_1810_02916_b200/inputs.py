@@ -278,3 +278,19 @@ def select_box(pos: torch.Tensor, lo, hi, box: float) -> torch.Tensor:
         else:
             mask &= (x >= l_w) | (x < h_w)
     return torch.nonzero(mask).flatten()
+
+
+def clumps(seed: int, K: int, box: float, clumps_, n_bg: int):
+    """Seeded numpy test input for dense cells: uniform balls inside chosen cells plus a uniform background.
+    clumps_: list of (cell (cx, cy, cz), n, radius in cell widths, centre offset in cell widths).  float32 [N, 3],
+    shuffled.  (The late-time state of PAPER.md:75 in miniature: a few cells with thousands of particles.)"""
+    import numpy as np
+    rng = np.random.default_rng(seed)
+    w = box / K
+    parts = [rng.random((n_bg, 3)) * box]
+    for (c, n, rad, ctr) in clumps_:
+        d = rng.normal(size=(n, 3))
+        d *= (rng.random(n) ** (1.0 / 3.0) / np.linalg.norm(d, axis=1))[:, None] * rad * w
+        parts.append((np.array(c) + 0.5 + np.array(ctr)) * w + d)
+    pos = np.concatenate(parts) % box
+    return np.ascontiguousarray(pos[rng.permutation(pos.shape[0])], dtype=np.float32)

@@ -35,7 +35,7 @@ EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve
            "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host",
            "nf_bin_m", "nf_forces_ex", "nf_kick_drift", "nf_cell_vrms", "nf_stream_step_slabs",
            "nf_keys", "nf_forces_chunk", "nf_forces_host_m", "nf_regroup_plane", "nf_stream_step_regroup",
-           "nf_forces_host_begin", "nf_forces_host_end", "nf_timestep_terms"]
+           "nf_forces_host_begin", "nf_forces_host_end", "nf_timestep_terms", "nf_forces_tree", "nf_tree_stats"]
 
 
 class NFError(RuntimeError):
@@ -94,6 +94,10 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.nf_bin_m.argtypes = [vp, vp, vp, i64, i32, f32, vp, vp, vp, vp, vp]
     lib.nf_forces_ex.restype = i32
     lib.nf_forces_ex.argtypes = [vp, vp, vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp, vp]
+    lib.nf_forces_tree.restype = i32
+    lib.nf_forces_tree.argtypes = [vp, vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, f32, vp, vp, vp]
+    lib.nf_tree_stats.restype = i32
+    lib.nf_tree_stats.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
     lib.nf_kick_drift.restype = i32
     lib.nf_kick_drift.argtypes = [vp, vp, vp, vp, i64, f32, f32, f32, vp]
     lib.nf_cell_vrms.restype = i32
@@ -270,6 +274,27 @@ class Context:
                                        _ptr(b.perm) if original_order else None, b.N, b.K, int(R), float(eps),
                                        float(b.box), float(Gm), _soft_code(softening), _ptr(acc), self._stream(stream)))
         return acc
+
+    def forces_tree(self, b: Binned, R: int, eps: float, Gm: float, theta: float, softening: str = "spline",
+                    original_order: bool = True, out: Optional[torch.Tensor] = None, stream=None, use_mass: bool = False,
+                    cell_amax: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """nf_forces_tree: nf_forces_ex with the sources of dense cells (>= 4096 particles) met through a tree with
+        opening angle theta (readings t1-t6).  theta = 0 is the direct sum."""
+        acc = out if out is not None else torch.empty(b.N, 3, dtype=torch.float32, device=b.pos_sorted.device)
+        assert acc.is_cuda and acc.dtype == torch.float32 and acc.shape == (b.N, 3) and acc.is_contiguous()
+        if cell_amax is not None:
+            assert cell_amax.is_cuda and cell_amax.dtype == torch.float32 and cell_amax.numel() == b.K ** 3 and cell_amax.is_contiguous()
+        self._check(self.lib.nf_forces_tree(self._h, _ptr(b.pos_sorted), _ptr(b.cell_offset), _ptr(b.perm) if original_order else None,
+                                            b.N, b.K, int(R), float(eps), float(b.box), float(Gm),
+                                            _soft_code(softening) | (NF_MASS_W if use_mass else 0), float(theta),
+                                            _ptr(acc), _ptr(cell_amax), self._stream(stream)))
+        return acc
+
+    def tree_stats(self, stream=None) -> dict:
+        """nf_tree_stats: (sink, accepted node) and (sink, particle of an opened leaf) pairs of the last forces_tree."""
+        a, b_ = ctypes.c_int64(0), ctypes.c_int64(0)
+        self._check(self.lib.nf_tree_stats(self._h, ctypes.byref(a), ctypes.byref(b_), self._stream(stream)))
+        return {"node": int(a.value), "leaf": int(b_.value)}
 
     def kick_drift(self, pos: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, kick: float, drift: float,
                    box: float, stream=None):

@@ -5,19 +5,11 @@ import numpy as np
 
 import oracle
 from oracle import nf_tree
+from paper_1810_02916_b200 import inputs
 
 
 def clumpy(seed, K, box, clumps, n_bg):
-    """clumps: list of (cell (cx,cy,cz), n, radius in cell widths, centre offset in cell widths)."""
-    rng = np.random.default_rng(seed)
-    w = box / K
-    parts = [rng.random((n_bg, 3)) * box]
-    for (c, n, rad, ctr) in clumps:
-        d = rng.normal(size=(n, 3))
-        d *= (rng.random(n) ** (1.0 / 3.0) / np.linalg.norm(d, axis=1))[:, None] * rad * w
-        parts.append((np.array(c) + 0.5 + np.array(ctr)) * w + d)
-    pos = np.concatenate(parts) % box
-    return np.ascontiguousarray(pos[rng.permutation(pos.shape[0])], dtype=np.float32)
+    return inputs.clumps(seed, K, box, clumps, n_bg)
 
 
 def test_theta_zero_is_the_direct_sum_and_counts_every_pair():
