@@ -10,13 +10,14 @@ the one DESIGN.md states (readings t1-t6, "Tree near field"), step by step:
   t1  A cell is DENSE when it holds >= 4096 particles.  (Capacity rule of the implementation, part of the definition: the
       dense cells taken are, in cell order, the first 2048 whose 64-aligned sizes add up to at most
       cap(N) = min(max(N/4, 2^20), 2^28) rounded down to 64; further ones are treated as not dense.)
-  t2  Inside a dense cell the particles are ordered by a 21-bit Morton code of their float32 cell-centred offset o
-      (7 bits per axis, q = clamp(int(((o * (K/box)) + 0.5) * 128), 0, 127), every operation rounded to float32, x the most
-      significant axis), ties in the stable order of the binning.
-  t3  LEAVES are runs of 64 consecutive particles of that order; a node of level l holds 8 consecutive nodes of level
+  t2  Inside a dense cell the particles are ordered by the 21-bit Hilbert index (Skilling's construction) of their float32
+      cell-centred offset o (7 bits per axis, q = clamp(int(((o * (K/box)) + 0.5) * 128), 0, 127), every operation
+      rounded to float32, x the most significant axis), ties in the stable order of the binning.  (A Hilbert run is a
+      compact blob; a Morton run jumps across the cell at octant boundaries and its bounding box with it.)
+  t3  LEAVES are runs of 16 consecutive particles of that order; a node of level l holds 8 consecutive nodes of level
       l-1, up to a single root.  A node carries the bounding box of its particles' float32 offsets, its mass M and its
       centre of mass.
-  t4  SINK GROUPS are runs of 64 consecutive particles of a cell, in Morton order if the cell is dense and in the binned
+  t4  SINK GROUPS are runs of 64 consecutive particles of a cell, in Hilbert order if the cell is dense and in the binned
       order if not; a group carries the bounding box of its float32 offsets.
   t5  A group meets a dense cell at cell displacement delta (|delta| <= R per axis, periodic) by walking its tree from
       the root.  With sh = float32(delta) * float32(box/K), a node box shifted by sh, g = the per-axis gap between the two
@@ -34,7 +35,7 @@ monopole bound: for a sink at distance D from the centre of mass of a node whose
 The float32 decisions (t2, t5) are taken in the same precision by the CUDA path, so the two walks are the same walk;
 everything else here is double precision from the caller's float32 positions, as in nf_oracle.c.
 
-Pins (tests/test_oracle_pins.py): theta = 0 equals nf_oracle.forces; a far, tight dense cell seen from a single sink
+Pins (tests/test_tree_oracle_pins.py): theta = 0 equals nf_oracle.forces; a far, tight dense cell seen from a single sink
 equals the hand formula G M (c - x)/|c - x|^3; the error against the direct sum respects the bound above sink by sink and
 falls with theta; conservation of the interaction count at theta = 0 (every sink meets every source of a dense neighbour).
 """
@@ -46,7 +47,8 @@ import numpy as np
 
 from . import nf_oracle as _o
 
-LEAF = 64
+LEAF = 16
+GROUP = 64
 FANOUT = 8
 DENSE_N = 4096
 DENSE_MAX_CELLS = 2048
@@ -68,23 +70,47 @@ def dense_cells(cell_count, N: int):
     return big & (rank < DENSE_MAX_CELLS) & (coff + n64 <= dense_cap(int(N)))
 
 
-def morton_order(off32, K: int, box: float):
+def hilbert_index(q, bits: int = 7):
+    """Hilbert index of integer grid points q [n, 3] (J. Skilling, "Programming the Hilbert curve", AIP Conf. Proc. 707,
+    2004: the transpose construction), axis 0 the most significant.  Consecutive indices are face-adjacent cells."""
+    X = [np.array(q[:, a], dtype=np.uint32) for a in range(3)]
+    Q = 1 << (bits - 1)
+    while Q > 1:
+        P = np.uint32(Q - 1)
+        for i in range(3):
+            hit = (X[i] & np.uint32(Q)) != 0
+            t = (X[0] ^ X[i]) & P
+            x0 = np.where(hit, X[0] ^ P, X[0] ^ t)       # invert the low bits of X[0] / exchange them with X[i]'s
+            xi = np.where(hit, X[i], X[i] ^ t)
+            X[i] = xi
+            X[0] = x0
+        Q >>= 1
+    X[1] = X[1] ^ X[0]                                   # Gray encode
+    X[2] = X[2] ^ X[1]
+    t = np.zeros_like(X[0])
+    Q = 1 << (bits - 1)
+    while Q > 1:
+        t = np.where((X[2] & np.uint32(Q)) != 0, t ^ np.uint32(Q - 1), t)
+        Q >>= 1
+    h = np.zeros_like(X[0])
+    for b in range(bits):
+        for a in range(3):
+            h |= (((X[a] ^ t) >> b) & 1) << (3 * b + (2 - a))
+    return h
+
+
+def hilbert_order(off32, K: int, box: float):
     """t2: the in-cell order (indices into the cell's particles in binned order)."""
     invw = f32(K) / f32(box)
     o = np.asarray(off32, dtype=f32)
     t = ((o * invw).astype(f32) + f32(0.5)).astype(f32)
     q = np.clip((t * f32(128.0)).astype(f32).astype(np.int32), 0, 127).astype(np.uint32)
-    code = np.zeros(o.shape[0], dtype=np.uint32)
-    for b in range(7):
-        code |= ((q[:, 2] >> b) & 1) << (3 * b)
-        code |= ((q[:, 1] >> b) & 1) << (3 * b + 1)
-        code |= ((q[:, 0] >> b) & 1) << (3 * b + 2)
-    return np.argsort(code, kind="stable")
+    return np.argsort(hilbert_index(q, 7), kind="stable")
 
 
 def build_tree(off32, xg, m):
     """t3: levels[0] = leaves ... levels[-1] = root; each a dict of lo, hi (float32 [n,3]), mass, com (float64).
-    off32, xg (double global positions), m (double masses) are in Morton order."""
+    off32, xg (double global positions), m (double masses) are in Hilbert order."""
     n = off32.shape[0]
     nl = (n + LEAF - 1) // LEAF
     lo = np.empty((nl, 3), dtype=f32)
@@ -194,7 +220,7 @@ def forces_tree(pos, K: int, R: int, eps: float, box: float, Gm: float, theta: f
     trees = {}
     for c in np.nonzero(dense)[0]:
         s = np.arange(off[c], off[c + 1])
-        order = morton_order(offs32[s], K, box)
+        order = hilbert_order(offs32[s], K, box)
         s = s[order]
         trees[int(c)] = (s, build_tree(offs32[s], xg[perm[s]], m_all[perm[s]]))
     cw32 = f32(box) / f32(K)
@@ -213,8 +239,8 @@ def forces_tree(pos, K: int, R: int, eps: float, box: float, Gm: float, theta: f
         if not nb:
             continue
         s_c = trees[int(c)][0] if dense[c] else np.arange(off[c], off[c + 1])
-        for g0 in range(0, s_c.shape[0], LEAF):
-            gs = s_c[g0:g0 + LEAF]                       # t4: sorted slots of the group's sinks
+        for g0 in range(0, s_c.shape[0], GROUP):
+            gs = s_c[g0:g0 + GROUP]                      # t4: sorted slots of the group's sinks
             if not stats and not wanted[perm[gs]].any():
                 continue
             glo = offs32[gs].min(axis=0)

@@ -138,7 +138,7 @@ int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float
 int nf_encode_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, float4 *enc,
                    float4 *enc_h, cudaStream_t st);
 // In-cell ordering of dense cells (nf_dense.cu), full box only.  Cells of at least NF_DENSE_N particles get their ENCODED
-// copies (enc, enc_h: what the interaction kernel reads) re-ordered along a Morton curve inside the cell, with a box per 64
+// copies (enc, enc_h: what the interaction kernel reads) re-ordered along a Hilbert curve inside the cell, with a box per 64
 // particles, so that the kernel can prove most (task, tile) pairs free of pairs inside eps.  dinfo: K^3 words out.
 // `off` describes ncell cells whose index modulo K is cz (the full box: K^3 cells; one plane: K^2).  Outputs: dinfo
 // (ncell words), dslot (nf_dense_cap(N) words), dbox (nf_dense_cap(N) / 64 * 6 floats) -- caller-owned, they must live as

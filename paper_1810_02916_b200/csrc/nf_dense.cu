@@ -3,7 +3,7 @@
 // PAPER.md:75 "the largest cell has over 200,000 particles" (the late-time, clustered state) and :107, where the paper
 // reports its own slowdown there.  Inside such a cell every tile of sources holds pairs closer than eps to some of a
 // task's sinks, so the whole own-cell sweep has to evaluate the min form of Eq. 2.  With the
-// particles of the cell ordered along a space-filling curve, 128 consecutive sinks and 446 consecutive sources are compact
+// particles of the cell ordered along a space-filling curve (Hilbert's), 128 consecutive sinks and 446 consecutive sources are compact
 // blobs, and a bounding box per 64 particles lets the kernel's producer PROVE that a (task, tile) pair holds no pair
 // inside eps -- then the cheaper r^-3 sweep is exact (the two laws agree for r >= eps).
 //
@@ -11,7 +11,8 @@
 // output keep nf_bin's stable order.  `slot` maps an encoded position back to the sorted slot of its particle.
 //
 //   k_dense_mark     per cell: is it dense (>= NF_DENSE_N particles)?  rank and 64-aligned compact offset by two scans
-//   k_dense_keys     dense cells: key = rank << 21 | 21-bit Morton code of the cell-centred offset, index = in-cell index
+//   k_dense_cells    which dense cells take part (capacity), their table by rank
+//   k_dense_keys     per compact position: key = rank << 21 | 21-bit Hilbert index of the cell-centred offset, index = in-cell index
 //   nf_radix_pass    4 stable LSD passes of 8 bits over the compact array (its length lives on the device)
 //   k_dense_finish   encoded copies in the new order, slot map, one box per 64 compact positions
 //
@@ -44,45 +45,77 @@ __global__ void __launch_bounds__(256) k_dense_mark(const uint64_t *__restrict__
     one[c] = d ? 1u : 0u;
 }
 
-// one warp per cell.  coff / rank: exclusive scans of n64 / one.  A dense cell takes part while its rank and the end of its
-// compact range stay below the limits (the cells that do form a prefix of the dense cells in cell order).
-__global__ void __launch_bounds__(256) k_dense_keys(const float4 *__restrict__ pos, const uint64_t *__restrict__ off, size_t ncell,
-                                                    const uint32_t *__restrict__ n64, const uint32_t *__restrict__ coff,
-                                                    const uint32_t *__restrict__ rank, uint32_t cap, float invw,
-                                                    uint32_t *__restrict__ dinfo, DenseCell *__restrict__ dcell,
-                                                    uint32_t *__restrict__ key, uint32_t *__restrict__ idx, uint32_t *__restrict__ nd)
+// 21-bit Hilbert index of a point of the 128^3 grid (J. Skilling, "Programming the Hilbert curve", AIP Conf. Proc. 707,
+// 2004: the transpose construction, restated): consecutive indices are face-adjacent grid cells, so a run of consecutive
+// particles is a compact blob -- a Morton run jumps across the cell wherever it crosses an octant boundary, and its
+// bounding box with it.  Integer arithmetic only: part of the tree's definition (reading t2).
+__device__ __forceinline__ uint32_t hilbert3(uint32_t x, uint32_t y, uint32_t z)
 {
-    const size_t c = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    uint32_t X[3] = {x, y, z};
+    for (uint32_t Q = 64u; Q > 1u; Q >>= 1) {
+        const uint32_t P = Q - 1u;
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            if (X[i] & Q) X[0] ^= P;                                    // invert the low bits of X[0]
+            else { const uint32_t t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }   // exchange the low bits of X[0] and X[i]
+        }
+    }
+    X[1] ^= X[0]; X[2] ^= X[1];                                       // Gray encode
+    uint32_t t = 0;
+    for (uint32_t Q = 64u; Q > 1u; Q >>= 1)
+        if (X[2] & Q) t ^= Q - 1u;
+    X[0] ^= t; X[1] ^= t; X[2] ^= t;
+    return spread3(X[2]) | (spread3(X[1]) << 1) | (spread3(X[0]) << 2);
+}
+
+// one thread per cell.  coff / rank: exclusive scans of n64 / one.  A dense cell takes part while its rank and the end of its
+// compact range stay below the limits (the cells that do form a prefix of the dense cells in cell order).
+__global__ void __launch_bounds__(256) k_dense_cells(const uint64_t *__restrict__ off, size_t ncell, const uint32_t *__restrict__ n64,
+                                                     const uint32_t *__restrict__ coff, const uint32_t *__restrict__ rank, uint32_t cap,
+                                                     uint32_t *__restrict__ dinfo, DenseCell *__restrict__ dcell, uint32_t *__restrict__ nd)
+{
+    const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= ncell) return;
-    const int lane = threadIdx.x & 31;
     const uint32_t m = n64[c];
     const bool dense = m != 0 && rank[c] < (uint32_t)NF_DENSE_MAX_CELLS && (unsigned long long)coff[c] + m <= cap;
-    if (lane == 0) dinfo[c] = dense ? (coff[c] >> 6) + 1u : 0u;
+    dinfo[c] = dense ? (coff[c] >> 6) + 1u : 0u;
     if (!dense) return;
-    const uint64_t c0 = off[c];
-    const uint32_t n = (uint32_t)(off[c + 1] - c0), o = coff[c], r = rank[c];
-    if (lane == 0) {
-        DenseCell dc;
-        dc.c0 = c0; dc.coff = o; dc.cell = (uint32_t)c; dc.n = n; dc.pad = 0;
-        dcell[r] = dc;
-        atomicMax(nd, o + m);                        // integer: order-independent
-        atomicAdd(nd + 1, 1u);                       // number of dense cells taken
-    }
-    for (uint32_t j = lane; j < m; j += 32) {
-        uint32_t k = MORTON_MASK, i = PAD;           // padding sorts behind the cell's particles
-        if (j < n) {
-            const float4 q = pos[c0 + j];
+    DenseCell dc;
+    dc.c0 = off[c]; dc.coff = coff[c]; dc.cell = (uint32_t)c; dc.n = (uint32_t)(off[c + 1] - off[c]); dc.pad = 0;
+    dcell[rank[c]] = dc;
+    atomicMax(nd, coff[c] + m);                  // integer: order-independent
+    atomicAdd(nd + 1, 1u);                       // number of dense cells taken
+}
+
+// one thread per compact position: key = rank << 21 | Hilbert index of the cell-centred offset, index = in-cell index
+__global__ void __launch_bounds__(256) k_dense_keys(const float4 *__restrict__ pos, const uint32_t *__restrict__ nd,
+                                                    const DenseCell *__restrict__ dcell, uint32_t cap, float invw,
+                                                    uint32_t *__restrict__ key, uint32_t *__restrict__ idx)
+{
+    const uint32_t n_d = nd[0], ndense = nd[1];
+    for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < n_d; t += gridDim.x * blockDim.x) {
+        uint32_t lo = 0, hi = ndense;            // the dense cell this position belongs to: last rank with coff <= t
+        while (hi - lo > 1) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (dcell[mid].coff <= t) lo = mid; else hi = mid;
+        }
+        const DenseCell dc = dcell[lo];
+        const uint32_t j = t - dc.coff;
+        uint32_t k = MORTON_MASK, i = PAD;       // padding sorts behind the cell's particles
+        if (j < dc.n) {
+            const float4 q = pos[dc.c0 + j];
             // every operation rounded to float32, no fused multiply-add: the order is part of the tree's definition
             // (reading t2) and the oracle takes the same decision in the same precision
             const int qx = min(127, max(0, (int)__fmul_rn(__fadd_rn(__fmul_rn(q.x, invw), 0.5f), 128.0f)));
             const int qy = min(127, max(0, (int)__fmul_rn(__fadd_rn(__fmul_rn(q.y, invw), 0.5f), 128.0f)));
             const int qz = min(127, max(0, (int)__fmul_rn(__fadd_rn(__fmul_rn(q.z, invw), 0.5f), 128.0f)));
-            k = spread3((uint32_t)qz) | (spread3((uint32_t)qy) << 1) | (spread3((uint32_t)qx) << 2);
+            k = hilbert3((uint32_t)qx, (uint32_t)qy, (uint32_t)qz);
             i = j;
         }
-        key[o + j] = (r << MORTON_BITS) | k;
-        idx[o + j] = i;
+        key[t] = (lo << MORTON_BITS) | k;
+        idx[t] = i;
     }
+    (void)cap;
 }
 
 // one warp per 64 compact positions (a "chunk"; cells start on chunk boundaries)
@@ -184,8 +217,9 @@ int nf_dense_order_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos
     NF_LAUNCHED(ctx);
     NF_TRY(nf_exclusive_scan_u32(ctx, n64, coff, ncell, stmp, st));
     NF_TRY(nf_exclusive_scan_u32(ctx, one, rank, ncell, stmp, st));
-    k_dense_keys<<<(unsigned)((ncell + 7) / 8), 256, 0, st>>>(pos, off, ncell, n64, coff, rank, cap, (float)K / p.box, dinfo, dcell, keyA,
-                                                               idxA, nd);
+    k_dense_cells<<<(unsigned)((ncell + 255) / 256), 256, 0, st>>>(off, ncell, n64, coff, rank, cap, dinfo, dcell, nd);
+    NF_LAUNCHED(ctx);
+    k_dense_keys<<<(unsigned)(cap / 256 < 148u * 8u ? (cap + 255) / 256 : 148u * 8u), 256, 0, st>>>(pos, nd, dcell, cap, (float)K / p.box, keyA, idxA);
     NF_LAUNCHED(ctx);
     NF_TRY(nf_radix_pass(ctx, keyA, idxA, cap, nd, 256, 0, keyB, idxB, hist, htmp, st));
     NF_TRY(nf_radix_pass(ctx, keyB, idxB, cap, nd, 256, 8, keyA, idxA, hist, htmp, st));

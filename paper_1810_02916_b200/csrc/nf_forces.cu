@@ -508,7 +508,7 @@ __device__ __noinline__ void produce_task(ConsShared<R> &S, const nf_plane_view 
     // which of the two encoded copies: the one whose z-blocks do not cut cz-R..cz+R (if any)
     const int zphi = ((cz - R + ZB * 4) / ZB != (cz + R + ZB * 4) / ZB) ? ZB / 2 : 0;
     const float4 *se = zphi ? sp.enc_h : sp.enc;
-    // dense own cell (nf_dense.cu): its encoded copies are ordered along a Morton curve with a box per 64 particles
+    // dense own cell (nf_dense.cu): its encoded copies are ordered along a Hilbert curve with a box per 64 particles
     const uint32_t own_di = (DENSE && sp.dinfo) ? sp.dinfo[task.cyz] : 0u;
     if (lane < W) {
         int px = sink_plane + lane - R;
@@ -733,7 +733,7 @@ __device__ __noinline__ bool produce_tile(ConsShared<R> &S, const nf_plane_view 
     const float4 *src = S.enc[(pc.z >> 16) & 0xff] + start;
     uint32_t meta = pc.z & 0x19ffffffu;
     if (DENSE && ((pc.z >> 24) & 1u)) {
-        // A dense cell seen from a dense cell: the law of this tile follows from the boxes (one per 64 particles in Morton
+        // A dense cell seen from a dense cell: the law of this tile follows from the boxes (one per 64 particles in Hilbert
         // order) of the task's sinks (<= 3) and of the tile's sources (<= 9: a tile has at most 508 of them).  If every pair of boxes is further apart than
         // eps, no pair of particles is inside eps and the untracked r^-3 sweep is exact (fn. 4); the tile of the
         // own cell then holds none of the task's sinks either (no r = 0 pair).  Else: the min form for the own cell,

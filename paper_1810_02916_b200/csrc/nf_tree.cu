@@ -5,10 +5,10 @@
 // one DESIGN.md states (readings t1-t6), the same one oracle/nf_tree.py follows on the CPU:
 //
 //   t1  dense cell = a cell of nf_dense.cu's in-cell ordering (>= NF_DENSE_N particles, within its capacity)
-//   t2  its particles in Morton order of their cell-centred offsets (k_dense_keys)
-//   t3  leaves = 64 consecutive particles (one "chunk" of the compact array), a node of level l = 8 nodes of level l-1,
-//       up to one root; a node carries the box of its particles' offsets, its mass and its centre of mass
-//   t4  sink group = 64 consecutive particles of a cell (Morton order in a dense cell, binned order elsewhere) and
+//   t2  its particles in Hilbert order of their cell-centred offsets (k_dense_keys)
+//   t3  leaves = 16 consecutive particles (a quarter of a 64-particle "chunk" of the compact array), a node of level l =
+//       8 nodes of level l-1, up to one root; a node carries the box of its particles' offsets, its mass and its centre of mass
+//   t4  sink group = 64 consecutive particles of a cell (Hilbert order in a dense cell, binned order elsewhere) and
 //       the box of their offsets
 //   t5  a group walks the tree of every dense cell among its (2R+1)^3 neighbours from the root: a node is ACCEPTED when
 //       the gap d between the two boxes and the node's diagonal s satisfy d^2 > eps^2 and s^2 < theta^2 d^2 (float32,
@@ -19,7 +19,7 @@
 //       dense source cells when p.tree is set
 //
 //   k_tree_layout    one thread: per dense cell the number of nodes of every level and where they start
-//   k_tree_leaves    one warp per chunk: Morton-ordered copy of (offset, mass), the leaf's box, mass, centre of mass
+//   k_tree_leaves    one warp per chunk: Hilbert-ordered copy of (offset, mass); box, mass, centre of mass of its four leaves
 //   k_tree_level     level l from level l-1
 //   k_tree_items     per cell: number of sink groups if any neighbour cell is dense (scanned into the work list)
 //   k_tree_walk      one warp per sink group: the walk of t5 with a bounded depth-first stack in shared memory; ADDS to acc
@@ -31,7 +31,8 @@
 
 namespace {
 
-constexpr int MAXLEV = 9;                       // 2^22 leaves at most (2^28 compact positions): 8 levels above them
+constexpr int LEAF = 16;                        // particles per leaf (t3); sink groups are 64 (t4)
+constexpr int MAXLEV = 9;                       // 2^24 leaves at most (2^28 compact positions): 8 levels above them
 constexpr uint32_t PAD = 0xffffffffu;
 constexpr int WALK_WARPS = 8;
 constexpr int STACK_CAP = 256 * MAXLEV + 64;    // depth-first over batches of 32 nodes: at most 8 * 32 pending per level
@@ -54,7 +55,7 @@ __global__ void k_tree_layout(const nf_dense_cell *__restrict__ dcell, const uin
         const nf_dense_cell dc = dcell[r];
         TreeCell t;
         t.c0 = dc.c0; t.coff = dc.coff; t.n = dc.n; t.pad = 0;
-        uint32_t m = (dc.n + 63u) >> 6;
+        uint32_t m = (dc.n + (uint32_t)LEAF - 1u) / (uint32_t)LEAF;
         int l = 0;
         for (;; l++) {
             t.base[l] = next; t.cnt[l] = m;
@@ -96,41 +97,41 @@ __global__ void __launch_bounds__(256) k_tree_leaves(const float4 *__restrict__ 
         const uint32_t t0 = ch * 64u;
         if (t0 >= n_d) return;
         const uint32_t r = cell_of_chunk(tcell, ndense, t0);
-        const uint32_t node = tcell[r].base[0] + ((t0 - tcell[r].coff) >> 6);
-        float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
-        double sm = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
+        const uint32_t leaf0 = (t0 - tcell[r].coff) / (uint32_t)LEAF, nleaf = tcell[r].cnt[0], base = tcell[r].base[0];
+        // positions t0 + 32 h + lane: lanes 0-15 / 16-31 of round h are leaf 2h / 2h + 1 of this chunk
 #pragma unroll
         for (int h = 0; h < 2; h++) {
+            float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+            double sm = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
             const uint32_t t = t0 + 32u * h + lane;
             const uint32_t s = dslot[t];
             float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
             if (s != PAD) {
                 o = pos[s];
                 if (!MASS) o.w = 1.0f;
-                lo[0] = fminf(lo[0], o.x); hi[0] = fmaxf(hi[0], o.x);
-                lo[1] = fminf(lo[1], o.y); hi[1] = fmaxf(hi[1], o.y);
-                lo[2] = fminf(lo[2], o.z); hi[2] = fmaxf(hi[2], o.z);
-                sm += (double)o.w; sx += (double)o.w * (double)o.x; sy += (double)o.w * (double)o.y; sz += (double)o.w * (double)o.z;
+                lo[0] = hi[0] = o.x; lo[1] = hi[1] = o.y; lo[2] = hi[2] = o.z;
+                sm = (double)o.w; sx = (double)o.w * (double)o.x; sy = (double)o.w * (double)o.y; sz = (double)o.w * (double)o.z;
             }
             tpos[t] = o;
-        }
 #pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
+            for (int d = 8; d > 0; d >>= 1) {            // within each half-warp: one leaf
 #pragma unroll
-            for (int a = 0; a < 3; a++) {
-                lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], d));
-                hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], d));
+                for (int a = 0; a < 3; a++) {
+                    lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], d));
+                    hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], d));
+                }
+                sm += __shfl_xor_sync(0xffffffffu, sm, d);
+                sx += __shfl_xor_sync(0xffffffffu, sx, d);
+                sy += __shfl_xor_sync(0xffffffffu, sy, d);
+                sz += __shfl_xor_sync(0xffffffffu, sz, d);
             }
-            sm += __shfl_xor_sync(0xffffffffu, sm, d);
-            sx += __shfl_xor_sync(0xffffffffu, sx, d);
-            sy += __shfl_xor_sync(0xffffffffu, sy, d);
-            sz += __shfl_xor_sync(0xffffffffu, sz, d);
-        }
-        if (lane == 0) {
-            const double inv = sm != 0.0 ? 1.0 / sm : 0.0;
-            nlo[node] = make_float4(lo[0], lo[1], lo[2], (float)sm);
-            nhi[node] = make_float4(hi[0], hi[1], hi[2], 0.f);
-            ncom[node] = make_float4((float)(sx * inv), (float)(sy * inv), (float)(sz * inv), (float)sm);
+            const uint32_t leaf = leaf0 + 2u * h + (lane >> 4);
+            if ((lane & 15) == 0 && leaf < nleaf) {
+                const double inv = sm != 0.0 ? 1.0 / sm : 0.0;
+                nlo[base + leaf] = make_float4(lo[0], lo[1], lo[2], (float)sm);
+                nhi[base + leaf] = make_float4(hi[0], hi[1], hi[2], 0.f);
+                ncom[base + leaf] = make_float4((float)(sx * inv), (float)(sy * inv), (float)(sz * inv), (float)sm);
+            }
         }
     }
 }
@@ -318,6 +319,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                             const uint32_t lm = __ballot_sync(0xffffffffu, openl);
                             if (openl) S.leaves[__popc(lm & ((1u << lane) - 1u))] = k;
                             nleaf = __popc(lm);
+                            st_leaf += (unsigned long long)__reduce_add_sync(0xffffffffu, openl ? min((uint32_t)LEAF, T.n - (uint32_t)LEAF * k) : 0u) * nsink;
                             // opened nodes -> their children on the stack
                             const bool openn = have && !acc_it && l > 0;
                             uint32_t nch = 0;
@@ -336,15 +338,19 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                             sp += tot;
                             __syncwarp();
                         }
-                        // the leaves opened by this batch, particle by particle with the full law
-                        for (uint32_t i = 0; i < nleaf; i++) {
-                            const uint32_t k = S.leaves[i];
-                            const size_t t0 = (size_t)T.coff + 64u * (size_t)k;
-                            S.stage[lane] = P.tpos[t0 + lane];
-                            S.stage[32 + lane] = P.tpos[t0 + 32 + lane];
+                        // the leaves opened by this batch, four at a time, particle by particle with the full law
+                        for (uint32_t i = 0; i < nleaf; i += 4) {
+#pragma unroll
+                            for (int rr = 0; rr < 2; rr++) {
+                                const uint32_t li = i + 2u * rr + ((uint32_t)lane >> 4);
+                                float4 q = make_float4(0.f, 0.f, 0.f, 0.f);            // massless filler
+                                if (li < nleaf) q = P.tpos[(size_t)T.coff + (size_t)LEAF * S.leaves[li] + (lane & 15)];
+                                S.stage[32 * rr + lane] = q;
+                            }
                             __syncwarp();
-                            const uint32_t np = min(64u, T.n - 64u * k);
-                            st_leaf += (unsigned long long)np * nsink;
+                            const uint32_t np = (uint32_t)LEAF * min(4u, nleaf - i);
+                            float lx[2] = {0.f, 0.f}, ly[2] = {0.f, 0.f}, lz[2] = {0.f, 0.f};     // formed from zero, then added: shorter sums
+#pragma unroll 4
                             for (uint32_t j = 0; j < np; j++) {
                                 const float4 q = S.stage[j];
 #pragma unroll
@@ -352,13 +358,17 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                                     const float ddx = q.x - px[h], ddy = q.y - py[h], ddz = q.z - pz[h];
                                     const float r2 = ddx * ddx + ddy * ddy + ddz * ddz;
                                     const float f = law_full(r2, P.eps2, inv_eps, inv_eps3, P.plummer) * q.w;
-                                    ax[h] += f * ddx; ay[h] += f * ddy; az[h] += f * ddz;
+                                    lx[h] += f * ddx; ly[h] += f * ddy; lz[h] += f * ddz;
                                 }
                             }
+#pragma unroll
+                            for (int h = 0; h < 2; h++) { ax[h] += lx[h]; ay[h] += ly[h]; az[h] += lz[h]; }
                             __syncwarp();
                         }
                         // accepted nodes: evaluate when the list could not take another batch, or at the end of the walk
                         if (nlist > (uint32_t)(LIST_CAP - 32) || (sp == 0 && nlist > 0)) {
+                            float lx[2] = {0.f, 0.f}, ly[2] = {0.f, 0.f}, lz[2] = {0.f, 0.f};
+#pragma unroll 4
                             for (uint32_t j = 0; j < nlist; j++) {
                                 const float4 q = S.list[j];
 #pragma unroll
@@ -369,9 +379,11 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                                     if (P.plummer) { const float ri = rsqrtf(r2 + P.eps2); f = ri * ri * ri; }
                                     else { const float ri = rsqrtf(r2); f = ri * ri * ri; }
                                     f *= q.w;
-                                    ax[h] += f * ddx; ay[h] += f * ddy; az[h] += f * ddz;
+                                    lx[h] += f * ddx; ly[h] += f * ddy; lz[h] += f * ddz;
                                 }
                             }
+#pragma unroll
+                            for (int h = 0; h < 2; h++) { ax[h] += lx[h]; ay[h] += ly[h]; az[h] += lz[h]; }
                             nlist = 0;
                             __syncwarp();
                         }
@@ -413,7 +425,7 @@ __global__ void __launch_bounds__(256) k_tree_amax(const uint64_t *__restrict__ 
     if (lane == 0) amax[c] = sqrtf(m);
 }
 
-size_t tree_nodes_max(int64_t N) { return (size_t)(nf_dense_cap(N) / 64) * 8 / 7 + (size_t)MAXLEV * NF_DENSE_MAX_CELLS + 64; }
+size_t tree_nodes_max(int64_t N) { return (size_t)(nf_dense_cap(N) / LEAF) * 8 / 7 + (size_t)MAXLEV * NF_DENSE_MAX_CELLS + 64; }
 
 }  // namespace
 
@@ -462,9 +474,9 @@ int nf_tree_forces_impl(nf_ctx *ctx, const nf_force_params &p, float theta, cons
     NF_LAUNCHED(ctx);
     // levels above the leaves: a cell of n particles has ceil(log8(n / 64)) of them; the box holds at most N particles
     int maxlev = 1;
-    for (uint64_t m = ((uint64_t)N + 63) / 64; m > 1; m = (m + 7) / 8) maxlev++;
+    for (uint64_t m = ((uint64_t)N + LEAF - 1) / LEAF; m > 1; m = (m + 7) / 8) maxlev++;
     for (int l = 1; l < maxlev && l < MAXLEV; l++) {
-        const uint64_t per = (((uint64_t)N + 63) / 64 >> (3 * l)) + 1;
+        const uint64_t per = (((uint64_t)N + LEAF - 1) / LEAF >> (3 * l)) + 1;
         dim3 g((unsigned)((per + 127) / 128 < 64 ? (per + 127) / 128 : 64), NF_DENSE_MAX_CELLS);
         k_tree_level<<<g, 128, 0, st>>>(keep.nd, tcell, l, nlo, nhi, ncom);
         NF_LAUNCHED(ctx);

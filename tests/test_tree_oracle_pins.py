@@ -32,7 +32,7 @@ def test_theta_zero_is_the_direct_sum_and_counts_every_pair():
 def test_far_tight_dense_cell_is_a_point_mass_hand_formula():
     """One dense cell holding a tight ball, single sinks two cells away (one of them through the periodic wrap):
     with theta = 0.5 the root is accepted and the acceleration is G M (c - x)/|c - x|^3 by hand."""
-    K, R, box, eps, Gm = 5, 2, 5.0, 0.01, 2.5e-4
+    K, R, box, eps, Gm = 5, 2, 5.0, 0.2, 2.5e-4          # eps wider than the ball: no node can be accepted inside it
     rng = np.random.default_rng(3)
     ball = (np.array([2.5, 2.5, 0.5]) + 0.01 * rng.normal(size=(4096, 3))).astype(np.float32)
     s1 = np.array([[4.3, 2.4, 0.6]], dtype=np.float32)      # delta = (-2, 0, 0), no wrap
@@ -84,27 +84,44 @@ def test_error_bound_sink_by_sink_and_convergence():
     assert rms[1] / np.sqrt((mag ** 2).mean()) < 5e-3
 
 
-def test_morton_order_and_boxes_invariants():
+def test_hilbert_index_brute_force():
+    """Every point of the 16^3 grid gets its own index and consecutive indices are face-adjacent cells -- the defining
+    property of the curve, checked exhaustively; x is the most significant axis (the curve ends at (15, 0, 0))."""
+    n = 16
+    g = np.stack(np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij"), -1).reshape(-1, 3).astype(np.uint32)
+    h = nf_tree.hilbert_index(g, 4)
+    assert sorted(h.tolist()) == list(range(n ** 3))
+    path = g[np.argsort(h)].astype(int)
+    assert (np.abs(np.diff(path, axis=0)).sum(axis=1) == 1).all()
+    assert path[0].tolist() == [0, 0, 0] and path[-1].tolist() == [n - 1, 0, 0]
+    # the 7-bit curve used by the tree: a sample of consecutive indices, found by inverting on the full grid of one octant pair
+    g7 = np.stack(np.meshgrid(np.arange(128), np.arange(64, 72), np.arange(128), indexing="ij"), -1).reshape(-1, 3).astype(np.uint32)
+    h7 = nf_tree.hilbert_index(g7, 7)
+    o = np.argsort(h7)
+    hs, ps = h7[o].astype(np.int64), g7[o].astype(int)
+    adj = np.diff(hs) == 1
+    assert adj.sum() > 10000 and (np.abs(np.diff(ps, axis=0)).sum(axis=1)[adj] == 1).all()
+
+
+def test_hilbert_order_and_boxes_invariants():
     K, box = 3, 3.0
     rng = np.random.default_rng(7)
     off = ((rng.random((5000, 3)) - 0.5) * (box / K) * 0.999).astype(np.float32)
-    order = nf_tree.morton_order(off, K, box)
+    order = nf_tree.hilbert_order(off, K, box)
     assert sorted(order.tolist()) == list(range(5000))
     o = off[order]
-    # the eight octants of the cell are contiguous along the curve, x the most significant axis
-    octant = 4 * (o[:, 0] >= 0) + 2 * (o[:, 1] >= 0) + (o[:, 2] >= 0)
-    assert (np.diff(octant) >= 0).all()
-    # ... and so are the 64 sub-octants inside them
+    # each of the eight octants of the cell is one contiguous run along the curve, and so is each of the 64 sub-octants
     w = box / K
-    sub = np.floor((o / w + 0.5) * 4).astype(int)
-    sub2 = 0
-    for bit in (1, 0):
-        sub2 = sub2 * 8 + 4 * ((sub[:, 0] >> bit) & 1) + 2 * ((sub[:, 1] >> bit) & 1) + ((sub[:, 2] >> bit) & 1)
-    assert (np.diff(sub2) >= 0).all()
+    for parts in (2, 4):
+        sub = np.floor((o / w + 0.5) * parts).astype(int)
+        ident = (sub[:, 0] * parts + sub[:, 1]) * parts + sub[:, 2]
+        assert (np.diff(ident) != 0).sum() + 1 == parts ** 3
+    # the curve starts in the octant of the low corner and ends across the cell in x
+    assert (o[0] < 0).all() and o[-1, 0] > 0 and (o[-1, 1:] < 0).all()
     m = rng.random(5000) + 0.5
     xg = o.astype(np.float64) + 1.5
     levels = nf_tree.build_tree(o, xg, m)
-    assert [L["mass"].shape[0] for L in levels] == [79, 10, 2, 1]
+    assert [L["mass"].shape[0] for L in levels] == [313, 40, 5, 1]
     assert abs(levels[-1]["mass"][0] - m.sum()) < 1e-9
     assert np.allclose(levels[-1]["com"][0], (m[:, None] * xg).sum(axis=0) / m.sum(), rtol=0, atol=1e-12)
     assert (levels[-1]["lo"][0] == o.min(axis=0)).all() and (levels[-1]["hi"][0] == o.max(axis=0)).all()
@@ -112,8 +129,8 @@ def test_morton_order_and_boxes_invariants():
         for k in range(levels[l]["mass"].shape[0]):
             ch = slice(8 * k, 8 * k + 8)
             assert (levels[l]["lo"][k] <= levels[l - 1]["lo"][ch]).all() and (levels[l]["hi"][k] >= levels[l - 1]["hi"][ch]).all()
-    # a leaf's box is the box of ITS 64 particles
-    assert (levels[0]["lo"][3] == o[192:256].min(axis=0)).all() and (levels[0]["hi"][78] == o[78 * 64:].max(axis=0)).all()
+    # a leaf's box is the box of ITS 16 particles
+    assert (levels[0]["lo"][3] == o[48:64].min(axis=0)).all() and (levels[0]["hi"][312] == o[312 * 16:].max(axis=0)).all()
 
 
 def test_opening_criterion_by_hand():
