@@ -18,7 +18,9 @@ the one DESIGN.md states (readings t1-t6, "Tree near field"), step by step:
       l-1, up to a single root.  A node carries the bounding box of its particles' float32 offsets, its mass M and its
       centre of mass.
   t4  SINK GROUPS are runs of 64 consecutive particles of a cell, in Hilbert order if the cell is dense and in the binned
-      order if not; a group carries the bounding box of its float32 offsets.
+      order if not; a group carries the bounding box of its float32 offsets.  A group whose box is more than 3 times
+      larger (diagonal) than the smallest box of its four quarters walks quarter by quarter, and a quarter that is
+      itself that large walks sink by sink (group_parts): one outlier must not make a whole group open the whole tree.
   t5  A group meets a dense cell at cell displacement delta (|delta| <= R per axis, periodic) by walking its tree from
       the root.  With sh = float32(delta) * float32(box/K), a node box shifted by sh, g = the per-axis gap between the two
       boxes (0 when they overlap), d2 = (gx*gx + gy*gy) + gz*gz, s2 = (ex*ex + ey*ey) + ez*ez for the node's extents e
@@ -178,6 +180,41 @@ def walk(levels, glo, ghi, sh, eps, theta):
     raise AssertionError
 
 
+def _diag2(lo, hi):
+    e = (hi - lo).astype(f32)
+    ee = (e * e).astype(f32)
+    return f32(f32(ee[0] + ee[1]) + ee[2])
+
+
+def group_parts(o32, theta: float = 1.0):
+    """t4: how the (up to 64) sinks of a group walk -- a list of (box lo, box hi, member positions).  Normally all
+    together under the box of the group.  A group whose box is out of proportion (an outlier among its sinks makes every
+    node look close, and the walk opens the whole tree) walks in parts: with m = the smallest squared diagonal among the
+    boxes of its four quarters (16 consecutive sinks each; quarters of fewer than 8 sinks do not count, and with none
+    that counts the group is not split), the group is split when its own squared diagonal exceeds 9 m; then each quarter walks under its own box, except that a quarter whose squared diagonal
+    exceeds 9 m walks sink by sink (a point has no extent).  float32, every operation rounded.  With theta = 0 nothing
+    is ever accepted, no box is looked at, and the group walks as a whole."""
+    n = o32.shape[0]
+    lo, hi = o32.min(axis=0), o32.max(axis=0)
+    if f32(f32(theta) * f32(theta)) == 0:
+        return [(lo, hi, np.arange(n))]
+    quarters = [np.arange(16 * q, min(n, 16 * q + 16)) for q in range(4) if 16 * q < n]
+    d2q = [_diag2(o32[m].min(axis=0), o32[m].max(axis=0)) for m in quarters]
+    counted = [d2 for m, d2 in zip(quarters, d2q) if m.shape[0] >= 8]
+    if not counted:
+        return [(lo, hi, np.arange(n))]
+    lim = f32(f32(9.0) * min(counted))
+    if not _diag2(lo, hi) > lim:
+        return [(lo, hi, np.arange(n))]
+    parts = []
+    for m, d2 in zip(quarters, d2q):
+        if d2 > lim:
+            parts += [(o32[i], o32[i], np.array([i])) for i in m]
+        else:
+            parts.append((o32[m].min(axis=0), o32[m].max(axis=0), m))
+    return parts
+
+
 def _law(d, eps, softening):
     """|F|/r for displacement vectors d [.., 3]; r = 0 contributes nothing (reading c6)."""
     r2 = (d * d).sum(axis=-1)
@@ -243,31 +280,31 @@ def forces_tree(pos, K: int, R: int, eps: float, box: float, Gm: float, theta: f
             gs = s_c[g0:g0 + GROUP]                      # t4: sorted slots of the group's sinks
             if not stats and not wanted[perm[gs]].any():
                 continue
-            glo = offs32[gs].min(axis=0)
-            ghi = offs32[gs].max(axis=0)
-            xs = xg[perm[gs]]
-            for (D, dl, img) in nb:
-                src, levels = trees[int(D)]
-                sh = (np.array(dl, dtype=f32) * cw32).astype(f32)
-                nodes, leaves = walk(levels, glo, ghi, sh, eps, theta)
-                image = np.array(img, dtype=np.float64) * float(box)
-                if nodes:
-                    com = np.array([levels[l]["com"][k] for (l, k) in nodes]) + image
-                    M = np.array([levels[l]["mass"][k] for (l, k) in nodes])
-                    d = com[None, :, :] - xs[:, None, :]
-                    r2 = (d * d).sum(axis=-1)
-                    if softening == "plummer":
+            for (glo, ghi, members) in group_parts(offs32[gs], theta):
+                ps = gs[members]                         # t4: the sinks that walk together, and their box
+                xs = xg[perm[ps]]
+                for (D, dl, img) in nb:
+                    src, levels = trees[int(D)]
+                    sh = (np.array(dl, dtype=f32) * cw32).astype(f32)
+                    nodes, leaves = walk(levels, glo, ghi, sh, eps, theta)
+                    image = np.array(img, dtype=np.float64) * float(box)
+                    if nodes:
+                        com = np.array([levels[l]["com"][k] for (l, k) in nodes]) + image
+                        M = np.array([levels[l]["mass"][k] for (l, k) in nodes])
+                        d = com[None, :, :] - xs[:, None, :]
+                        r2 = (d * d).sum(axis=-1)
+                        if softening == "plummer":
+                            fr = _law(d, eps, softening)
+                        else:
+                            fr = 1.0 / (r2 * np.sqrt(r2))
+                        a_tree[perm[ps]] += Gm * ((M[None, :] * fr)[:, :, None] * d).sum(axis=1)
+                        st["node"] += len(nodes) * ps.shape[0]
+                    if leaves.size:
+                        idx = np.concatenate([src[k * LEAF:(k + 1) * LEAF] for k in leaves])
+                        d = (xg[perm[idx]] + image)[None, :, :] - xs[:, None, :]
                         fr = _law(d, eps, softening)
-                    else:
-                        fr = 1.0 / (r2 * np.sqrt(r2))
-                    a_tree[perm[gs]] += Gm * ((M[None, :] * fr)[:, :, None] * d).sum(axis=1)
-                    st["node"] += len(nodes) * gs.shape[0]
-                if leaves.size:
-                    idx = np.concatenate([src[k * LEAF:(k + 1) * LEAF] for k in leaves])
-                    d = (xg[perm[idx]] + image)[None, :, :] - xs[:, None, :]
-                    fr = _law(d, eps, softening)
-                    a_tree[perm[gs]] += Gm * ((m_all[perm[idx]][None, :] * fr)[:, :, None] * d).sum(axis=1)
-                    st["leaf"] += idx.shape[0] * gs.shape[0]
+                        a_tree[perm[ps]] += Gm * ((m_all[perm[idx]][None, :] * fr)[:, :, None] * d).sum(axis=1)
+                        st["leaf"] += idx.shape[0] * ps.shape[0]
     out = a + a_tree[want]
     return (out, st) if stats else out
 

@@ -22,7 +22,7 @@
 //   k_tree_leaves    one warp per chunk: Hilbert-ordered copy of (offset, mass); box, mass, centre of mass of its four leaves
 //   k_tree_level     level l from level l-1
 //   k_tree_items     per cell: number of sink groups if any neighbour cell is dense (scanned into the work list)
-//   k_tree_walk      one warp per sink group: the walk of t5 with a bounded depth-first stack in shared memory; ADDS to acc
+//   k_tree_walk      one warp per sink group (walking as a whole, or in parts when its box is out of proportion: t4): the walk of t5 with a bounded depth-first stack in shared memory; ADDS to acc
 //   k_tree_amax      per-cell maximum of |a| from the final accelerations
 //
 // Deterministic: every sink belongs to one warp, which visits cells, nodes and particles in a fixed order; the only
@@ -185,7 +185,10 @@ __global__ void __launch_bounds__(256) k_tree_items(const uint64_t *__restrict__
     ng[c] = g;
 }
 
+struct Part { float lo[3], hi[3]; unsigned long long mask; };   // sinks that walk together (bit 32 h + lane), and their box
+
 struct WalkShared {
+    Part parts[68];                // at most 3 quarters + 16 single sinks ... 64 single sinks
     uint32_t stack[STACK_CAP];
     float4 list[LIST_CAP];         // accepted nodes waiting to be evaluated: centre of mass, mass
     float4 stage[64];              // the particles of one leaf
@@ -254,20 +257,91 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
             if (valid[h]) {
                 const float4 o = P.pos[slot[h]];
                 sx[h] = o.x; sy[h] = o.y; sz[h] = o.z;
-                glo[0] = fminf(glo[0], o.x); ghi[0] = fmaxf(ghi[0], o.x);
-                glo[1] = fminf(glo[1], o.y); ghi[1] = fmaxf(ghi[1], o.y);
-                glo[2] = fminf(glo[2], o.z); ghi[2] = fmaxf(ghi[2], o.z);
             }
         }
+        // boxes of the four quarters (16 consecutive sinks: a half-warp of one round) and of the whole group
+        float qlo[2][3], qhi[2][3];                  // this lane's quarter in round h
+        const float mylo[2][3] = {{valid[0] ? sx[0] : 3.0e38f, valid[0] ? sy[0] : 3.0e38f, valid[0] ? sz[0] : 3.0e38f},
+                                  {valid[1] ? sx[1] : 3.0e38f, valid[1] ? sy[1] : 3.0e38f, valid[1] ? sz[1] : 3.0e38f}};
+        const float myhi[2][3] = {{valid[0] ? sx[0] : -3.0e38f, valid[0] ? sy[0] : -3.0e38f, valid[0] ? sz[0] : -3.0e38f},
+                                  {valid[1] ? sx[1] : -3.0e38f, valid[1] ? sy[1] : -3.0e38f, valid[1] ? sz[1] : -3.0e38f}};
 #pragma unroll
-        for (int d = 16; d > 0; d >>= 1)
+        for (int h = 0; h < 2; h++)
 #pragma unroll
             for (int a = 0; a < 3; a++) {
-                glo[a] = fminf(glo[a], __shfl_xor_sync(0xffffffffu, glo[a], d));
-                ghi[a] = fmaxf(ghi[a], __shfl_xor_sync(0xffffffffu, ghi[a], d));
+                float l = mylo[h][a], u = myhi[h][a];
+#pragma unroll
+                for (int d = 8; d > 0; d >>= 1) {
+                    l = fminf(l, __shfl_xor_sync(0xffffffffu, l, d));
+                    u = fmaxf(u, __shfl_xor_sync(0xffffffffu, u, d));
+                }
+                qlo[h][a] = l; qhi[h][a] = u;
             }
-        const uint32_t nsink = __popc(__ballot_sync(0xffffffffu, valid[0])) + __popc(__ballot_sync(0xffffffffu, valid[1]));
+        const uint32_t vm0 = __ballot_sync(0xffffffffu, valid[0]), vm1 = __ballot_sync(0xffffffffu, valid[1]);
+        const unsigned long long vmask = (unsigned long long)vm0 | ((unsigned long long)vm1 << 32);
+        // t4 (group_parts): the group walks as a whole unless its box is out of proportion to its quarters'
+        uint32_t nparts = 0;
+        {
+            float blo[4][3], bhi[4][3], d2q[4];
+            uint32_t cq[4];
+            float lim = 3.0e38f;
+            bool counted = false;
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                float s2 = 0.f;
+#pragma unroll
+                for (int a = 0; a < 3; a++) {
+                    blo[q][a] = __shfl_sync(0xffffffffu, qlo[q >> 1][a], 16 * (q & 1));
+                    bhi[q][a] = __shfl_sync(0xffffffffu, qhi[q >> 1][a], 16 * (q & 1));
+                    const float e = __fsub_rn(bhi[q][a], blo[q][a]);
+                    s2 = a == 0 ? __fmul_rn(e, e) : __fadd_rn(s2, __fmul_rn(e, e));
+                }
+                cq[q] = __popcll(vmask & (0xffffull << (16 * q)));
+                d2q[q] = s2;
+                if (cq[q] >= 8u) { lim = fminf(lim, s2); counted = true; }
+            }
+#pragma unroll
+            for (int a = 0; a < 3; a++) {
+                glo[a] = fminf(fminf(blo[0][a], blo[1][a]), fminf(blo[2][a], blo[3][a]));
+                ghi[a] = fmaxf(fmaxf(bhi[0][a], bhi[1][a]), fmaxf(bhi[2][a], bhi[3][a]));
+            }
+            float d2g = 0.f;
+#pragma unroll
+            for (int a = 0; a < 3; a++) {
+                const float e = __fsub_rn(ghi[a], glo[a]);
+                d2g = a == 0 ? __fmul_rn(e, e) : __fadd_rn(d2g, __fmul_rn(e, e));
+            }
+            lim = __fmul_rn(9.0f, lim);
+            if (!(counted && d2g > lim && P.th2 > 0.f)) {       // theta = 0 accepts nothing: no box matters, one walk
+                if (lane == 0) { Part &pt = S.parts[0]; pt.mask = vmask; for (int a = 0; a < 3; a++) { pt.lo[a] = glo[a]; pt.hi[a] = ghi[a]; } }
+                nparts = 1;
+            } else {
+#pragma unroll
+                for (int q = 0; q < 4; q++) {
+                    if (cq[q] == 0) continue;
+                    if (d2q[q] > lim) {                    // sink by sink
+                        for (uint32_t i = 0; i < cq[q]; i++) {
+                            const int src = 16 * (q & 1) + (int)i;
+                            const float x = __shfl_sync(0xffffffffu, sx[q >> 1], src), y = __shfl_sync(0xffffffffu, sy[q >> 1], src),
+                                        z = __shfl_sync(0xffffffffu, sz[q >> 1], src);
+                            if (lane == 0) { Part &pt = S.parts[nparts]; pt.mask = 1ull << (16 * q + i); pt.lo[0] = pt.hi[0] = x; pt.lo[1] = pt.hi[1] = y; pt.lo[2] = pt.hi[2] = z; }
+                            nparts++;
+                        }
+                    } else {
+                        if (lane == 0) { Part &pt = S.parts[nparts]; pt.mask = vmask & (0xffffull << (16 * q)); for (int a = 0; a < 3; a++) { pt.lo[a] = blo[q][a]; pt.hi[a] = bhi[q][a]; } }
+                        nparts++;
+                    }
+                }
+            }
+            __syncwarp();
+        }
         float ax[2] = {0.f, 0.f}, ay[2] = {0.f, 0.f}, az[2] = {0.f, 0.f};
+        for (uint32_t pi = 0; pi < nparts; pi++) {
+        const Part part = S.parts[pi];
+#pragma unroll
+        for (int a = 0; a < 3; a++) { glo[a] = part.lo[a]; ghi[a] = part.hi[a]; }
+        const bool act[2] = {(bool)((part.mask >> lane) & 1ull), (bool)((part.mask >> (32 + lane)) & 1ull)};
+        const uint32_t nsink = (uint32_t)__popcll(part.mask);
         for (int dx = -R; dx <= R; dx++)
             for (int dy = -R; dy <= R; dy++)
                 for (int dz = -R; dz <= R; dz++) {
@@ -362,7 +436,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                                 }
                             }
 #pragma unroll
-                            for (int h = 0; h < 2; h++) { ax[h] += lx[h]; ay[h] += ly[h]; az[h] += lz[h]; }
+                            for (int h = 0; h < 2; h++) if (act[h]) { ax[h] += lx[h]; ay[h] += ly[h]; az[h] += lz[h]; }
                             __syncwarp();
                         }
                         // accepted nodes: evaluate when the list could not take another batch, or at the end of the walk
@@ -383,12 +457,13 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                                 }
                             }
 #pragma unroll
-                            for (int h = 0; h < 2; h++) { ax[h] += lx[h]; ay[h] += ly[h]; az[h] += lz[h]; }
+                            for (int h = 0; h < 2; h++) if (act[h]) { ax[h] += lx[h]; ay[h] += ly[h]; az[h] += lz[h]; }
                             nlist = 0;
                             __syncwarp();
                         }
                     }
                 }
+        }   // parts
 #pragma unroll
         for (int h = 0; h < 2; h++)
             if (valid[h]) {

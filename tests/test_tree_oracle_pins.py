@@ -148,3 +148,30 @@ def test_opening_criterion_by_hand():
     assert nf_tree.accept(glo, ghi, nlo[2:3], nhi[2:3], np.array([2, 0, 0], dtype=f), 2.4, 1.0).tolist() == [True]
     assert nf_tree.accept(glo, ghi, nlo[2:3], nhi[2:3], np.array([2, 0, 0], dtype=f), 2.6, 1.0).tolist() == [False]
     assert nf_tree.accept(glo, ghi, nlo[2:3], nhi[2:3], np.array([-3, 0, 0], dtype=f), 1.3, 1.0).tolist() == [True]   # gap 1.4 on the other side
+
+
+def test_group_parts_by_hand():
+    f = np.float32
+    line = np.zeros((64, 3), dtype=f)
+    line[:, 0] = np.arange(64)
+    # a 4 x 4 x 4 lattice whose quarters are 4 x 4 x 1 slabs: group diagonal^2 = 27, quarters 18 -> walks as a whole
+    cube = np.array([[i % 4, (i // 4) % 4, i // 16] for i in range(64)], dtype=f)
+    p = nf_tree.group_parts(cube)
+    assert len(p) == 1 and p[0][2].tolist() == list(range(64)) and p[0][0].tolist() == [0, 0, 0] and p[0][1].tolist() == [3, 3, 3]
+    # a line of 64: extent 63 against 15 per quarter (63^2 > 9 * 15^2) -> four quarters, each under its own box
+    p = nf_tree.group_parts(line)
+    assert [(a[0], b[0], m.tolist()) for a, b, m in p] == [(16 * q, 16 * q + 15, list(range(16 * q, 16 * q + 16))) for q in range(4)]
+    # one outlier in the second quarter: that quarter walks sink by sink (point boxes), the others as quarters
+    out = line.copy()
+    out[20] = [1000, 0, 0]
+    p = nf_tree.group_parts(out)
+    assert [m.tolist() for _, _, m in p] == [list(range(16))] + [[i] for i in range(16, 32)] + [list(range(32, 48)), list(range(48, 64))]
+    assert all((a == b).all() and (a == out[m[0]]).all() for a, b, m in p[1:17])
+    assert sorted(i for _, _, m in p for i in m.tolist()) == list(range(64))
+    # a short group: the quarter of 4 sinks does not count (limit 9 * 15^2 = 2025 >= 19^2): as a whole; 7 sinks: nothing counts
+    assert len(nf_tree.group_parts(line[:20])) == 1 and len(nf_tree.group_parts(line[:7])) == 1
+    # ... but 24 sinks with the last 8 far away: the second quarter counts (8 sinks, extent 7) and the group splits
+    far = line[:24].copy()
+    far[16:, 0] += 500
+    p = nf_tree.group_parts(far)
+    assert [m.tolist() for _, _, m in p] == [list(range(16)), list(range(16, 24))]       # 15^2 <= 9 * 7^2: both stay quarters
