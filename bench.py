@@ -520,6 +520,141 @@ def run_sharded(args, cfg):
         dist.destroy_process_group()
 
 
+def run_tree(args, cfg):
+    """`--tree THETA`: the step with nf_forces_tree in place of nf_forces.
+    One GPU.  `value` counts the interactions the step EVALUATED (pairs of the interaction kernel for the sources that are
+    not in dense cells + (sink, particle of an opened leaf) + (sink, accepted node)); the direct sum's pair count of the
+    same box and the time of the direct step are reported beside it."""
+    import numpy as np
+    from paper_1810_02916_b200 import nf
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    theta = float(args.tree)
+    ctx = nf.Context(0)
+    pos = inputs.make_positions(cfg, device=dev)
+    N, K, R = cfg.N, cfg.K, cfg.R
+    b = ctx.bin(pos, K, cfg.box)
+    acc = torch.empty(N, 3, dtype=torch.float32, device=dev)
+    I_direct = ctx.interactions(b, R)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if N * 28 < (256 << 20) else None
+
+    def step_tree():
+        ctx.bin(pos, K, cfg.box, out=b)
+        ctx.forces_tree(b, R, cfg.eps, cfg.Gm, theta, out=acc)
+
+    def step_direct():
+        ctx.bin(pos, K, cfg.box, out=b)
+        ctx.forces(b, R, cfg.eps, cfg.Gm, out=acc)
+
+    def timed(step, steps, want_walk):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        walk, kern = [], []
+        torch.cuda.synchronize()
+        for s_ in range(steps):
+            if flush is not None:
+                flush.fill_(s_)
+            ev[s_][0].record()
+            step()
+            ev[s_][1].record()
+            kern.append(ctx.last_forces_timing()[0])
+            if want_walk:
+                walk.append(ctx.last_tree_timing())
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(c) for a, c in ev) / steps, sum(kern) / steps, (sum(walk) / steps if walk else None)
+
+    for _ in range(args.warmup):
+        step_direct()
+    direct_ms, direct_k_ms, _ = timed(step_direct, args.steps, False)
+    a_direct = acc.clone()
+    for _ in range(args.warmup):
+        step_tree()
+    sampler = ClockSampler(0)
+    launches0 = ctx.launch_count()
+    ms_per_step, k_ms, walk_ms = timed(step_tree, args.steps, True)
+    launches = ctx.launch_count() - launches0
+    clocks = sampler.stop()
+    st = ctx.tree_stats()
+    # pairs the interaction kernel still evaluated: sources of cells below the dense threshold (DESIGN.md reading t1)
+    cnt = b.cell_count.cpu().numpy().astype(np.int64).reshape(K, K, K)
+    coff, rank, dense = 0, 0, np.zeros(K ** 3, dtype=bool)
+    cap = min(max(N // 4, 1 << 20), 1 << 28) & ~63
+    for c, n in enumerate(cnt.ravel()):
+        if n >= 4096:
+            n64 = (int(n) + 63) & ~63
+            dense[c] = rank < 2048 and coff + n64 <= cap
+            coff += n64
+            rank += 1
+    light = np.where(dense.reshape(K, K, K), 0, cnt)
+    I_kernel = 0
+    for d in np.ndindex(2 * R + 1, 2 * R + 1, 2 * R + 1):
+        I_kernel += int((cnt * np.roll(light, shift=(R - d[0], R - d[1], R - d[2]), axis=(0, 1, 2))).sum())
+    I_eval = I_kernel + st["node"] + st["leaf"]
+    value = I_eval / (ms_per_step * 1e-3)
+    # how far the approximation is from the direct sum (both on the GPU, all sinks)
+    mag = a_direct.double().norm(dim=1)
+    err = (acc.double() - a_direct.double()).norm(dim=1) / torch.maximum(mag, mag.pow(2).mean().sqrt())
+    approx = {"against": "nf_forces of the same box (direct sum), all sinks", "median": float(err.median()),
+              "p99": float(err.kthvalue(int(0.99 * N)).values), "max": float(err.max())}
+    # ---- end to end: positions from pinned host memory, accelerations back into pinned host memory ----
+    e2e = None
+    if not args.no_e2e:
+        hpos = torch.empty(N, 3, dtype=torch.float32, pin_memory=True).copy_(pos)
+        hacc = torch.empty(N, 3, dtype=torch.float32, pin_memory=True)
+        dpos = torch.empty_like(pos)
+
+        def host_step():
+            dpos.copy_(hpos, non_blocking=True)
+            ctx.bin(dpos, K, cfg.box, out=b)
+            ctx.forces_tree(b, R, cfg.eps, cfg.Gm, theta, out=acc)
+            hacc.copy_(acc, non_blocking=True)
+            torch.cuda.synchronize()
+
+        host_step()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            host_step()
+        e_s = (time.perf_counter() - t0) / args.steps
+        e2e = {"value": I_eval / e_s, "unit": "interactions/s", "h2d_bytes_per_step": 12 * N, "d2h_bytes_per_step": 12 * N,
+               "ms_per_step": 1e3 * e_s, "api": "Context.bin + Context.forces_tree on positions copied from pinned host memory, accelerations copied back",
+               "result_checksum": float(hacc[:: max(1, N // 4096)].double().abs().sum())}
+    sm_max_mhz, hbm_gbs, peak_src = read_peaks()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak_tflops = sms * sm_max_mhz * 1e6 * 2 * FP32_LANES_PER_SM / 1e12
+    achieved = FLOP_PER_INTERACTION * (st["node"] + st["leaf"]) / (walk_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "tree walk (k_tree_walk)", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved / peak_tflops, "traffic": None,
+                "peak_source": f"{sms} SMs x {sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz) x 2 x {FP32_LANES_PER_SM} FP32 lanes",
+                "flop_per_interaction": FLOP_PER_INTERACTION, "kernel_ms": walk_ms, "kernel_share_of_step": walk_ms / ms_per_step,
+                "interaction_kernel_ms": k_ms,
+                "note": "node and leaf interactions both counted at the direct kernel's flop per interaction; the walk also tests boxes and moves a stack"}
+    cpu, parity = None, None
+    if not args.no_cpu:
+        from oracle import nf_tree
+        pos_np = pos.cpu().numpy()
+        sinks = np.sort(np.random.default_rng(ORACLE_SEED).choice(N, min(N, 384), replace=False))
+        t0 = time.perf_counter()
+        ref = nf_tree.forces_tree(pos_np, K, R, cfg.eps, cfg.box, cfg.Gm, theta, sink_idx=sinks)
+        sec = time.perf_counter() - t0
+        parity = parity_block(acc[torch.from_numpy(sinks).to(dev)].cpu().numpy(), ref)
+        cpu = {"value": len(sinks) * (I_eval / N) / sec, "unit": "interactions/s", "cores": 1, "kind": "oracle", "seconds": sec,
+               "sample": f"oracle/nf_tree.py forces_tree (numpy, one process) for {len(sinks)} seeded sinks of {cfg.name} -- every 64-sink group "
+                         f"that holds one of them is walked and summed; rate = sinks x mean evaluated interactions per sink / seconds"}
+    line = {"metric": "near_field_pairwise_interactions_per_s", "value": value, "unit": "interactions/s", "n_gpus": 1,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg.name + f" + tree theta={theta:g}", "N": N, "K": K, "R": R, "eps": cfg.eps, "box": cfg.box,
+                       "theta": theta, "interactions_per_step_per_gpu": I_eval,
+                       "l2": "flushed between timed steps (256 MiB write)" if flush is not None else "inputs larger than L2",
+                       "parallelism": "1 GPU"},
+            "tree": {"theta": theta, "node_interactions": st["node"], "leaf_interactions": st["leaf"], "interaction_kernel_pairs": I_kernel,
+                     "direct_sum_pairs": I_direct, "direct_step_ms": direct_ms, "speedup_over_direct_step": direct_ms / ms_per_step,
+                     "direct_equivalent_interactions_per_s": I_direct / (ms_per_step * 1e-3), "walk_ms": walk_ms,
+                     "approximation_error": approx},
+            "particles_per_s": N / (ms_per_step * 1e-3), "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "roofline": roofline, "cpu_baseline": cpu, "parity": parity, "sweep": None}
+    print(json.dumps(line), flush=True)
+
+
 def sweep_small_configs(ctx, dev, steps=3, warmup=3):
     """Interaction-kernel roofline fraction of C1, C2 and C3 -- the other single-GPU configs of BASELINE.json beside the
     headline workload -- and of D1, the one-dense-cell workload (config 6), in the same process (milliseconds each).  Same timing rules as the main
@@ -599,6 +734,8 @@ def main():
                     help="gloo: debugging aid, every rank on cuda:0 with ghosts staged through host memory")
     ap.add_argument("--n-side", type=int, default=0,
                     help="profiling aid: the same recipe at n_side^3 particles and K = n_side/4 (not the bench workload)")
+    ap.add_argument("--tree", type=float, default=None, metavar="THETA",
+                    help="time the step with nf_forces_tree (tree near field for dense cells, opening angle THETA) instead of nf_forces")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = max(args.warmup, 0)
@@ -614,6 +751,11 @@ def main():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     if cfg.kind == "slab":
         run_stream(args, cfg)
+        return
+    if args.tree is not None:
+        if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+            raise SystemExit("bench.py --tree: one GPU (the tree near field takes a whole box)")
+        run_tree(args, cfg)
         return
     if args.shard or int(os.environ.get("WORLD_SIZE", "1")) > 1:
         run_sharded(args, cfg)

@@ -257,6 +257,8 @@ int nf_forces_tree(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_of
                    int K, int R, float eps, float box, float Gm, int softening, float theta, float *acc_xyz,
                    float *cell_amax, void *stream);
 int nf_tree_stats(nf_ctx *ctx, int64_t *node_interactions, int64_t *leaf_interactions, void *stream);
+/* duration of the walk kernel of the last nf_forces_tree on this context (CUDA events on its stream; synchronises on the end event) */
+int nf_last_tree_timing(nf_ctx *ctx, float *walk_ms);
 
 /*
  * nf_kick_drift -- the leapfrog updates that follow the force in the slab pipeline (Table 1

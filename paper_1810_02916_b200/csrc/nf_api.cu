@@ -76,7 +76,8 @@ int nf_create(nf_ctx **out, int device)
         if (cudaMallocHost((void **)&ctx->h_counters, 16 * sizeof(unsigned long long)) != cudaSuccess) { rc = NF_ERR_NOMEM; break; }
         memset(ctx->h_counters, 0, 16 * sizeof(unsigned long long));
         if (cudaEventCreate(&ctx->ev_total0) != cudaSuccess || cudaEventCreate(&ctx->ev_kern0) != cudaSuccess ||
-            cudaEventCreate(&ctx->ev_kern1) != cudaSuccess || cudaEventCreate(&ctx->ev_total1) != cudaSuccess) { rc = NF_ERR_CUDA; break; }
+            cudaEventCreate(&ctx->ev_kern1) != cudaSuccess || cudaEventCreate(&ctx->ev_total1) != cudaSuccess ||
+            cudaEventCreate(&ctx->ev_walk0) != cudaSuccess || cudaEventCreate(&ctx->ev_walk1) != cudaSuccess) { rc = NF_ERR_CUDA; break; }
         if (cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking) != cudaSuccess ||
             cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking) != cudaSuccess) { rc = NF_ERR_CUDA; break; }
         rc = nf_forces_init(ctx);
@@ -102,6 +103,8 @@ int nf_destroy(nf_ctx *ctx)
     if (ctx->ev_kern0) cudaEventDestroy(ctx->ev_kern0);
     if (ctx->ev_kern1) cudaEventDestroy(ctx->ev_kern1);
     if (ctx->ev_total1) cudaEventDestroy(ctx->ev_total1);
+    if (ctx->ev_walk0) cudaEventDestroy(ctx->ev_walk0);
+    if (ctx->ev_walk1) cudaEventDestroy(ctx->ev_walk1);
     if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
     if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
     nf_slab_state_free(ctx);
@@ -290,6 +293,16 @@ int nf_forces_tree(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_of
     if (!ctx) return NF_ERR_ARG;
     NF_ARG(ctx, theta >= 0.0f && theta < 1.0f, "nf_forces_tree: theta = %g outside [0, 1)", (double)theta);
     return forces_common(ctx, pos_sorted, cell_offset, perm, N, K, R, eps, box, Gm, softening, 0, K, acc_xyz, cell_amax, stream, true, theta);
+}
+
+int nf_last_tree_timing(nf_ctx *ctx, float *walk_ms)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, walk_ms != nullptr, "nf_last_tree_timing: null output");
+    NF_ARG(ctx, ctx->tree_timed, "nf_last_tree_timing: no nf_forces_tree has walked a tree on this context yet");
+    NF_CUDA(ctx, cudaEventSynchronize(ctx->ev_walk1));
+    NF_CUDA(ctx, cudaEventElapsedTime(walk_ms, ctx->ev_walk0, ctx->ev_walk1));
+    return NF_OK;
 }
 
 int nf_tree_stats(nf_ctx *ctx, int64_t *node_interactions, int64_t *leaf_interactions, void *stream)

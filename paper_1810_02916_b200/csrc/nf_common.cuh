@@ -24,6 +24,8 @@ struct nf_ctx {
     // timing of the last nf_forces
     cudaEvent_t ev_total0, ev_kern0, ev_kern1, ev_total1;
     bool forces_timed;
+    cudaEvent_t ev_walk0, ev_walk1;   // around the walk kernel of the last nf_forces_tree
+    bool tree_timed;
     long long launches;  // kernels launched by this context since nf_create
     // slab streaming resources (created lazily)
     cudaStream_t s_h2d, s_d2h;

@@ -567,8 +567,11 @@ int nf_tree_forces_impl(nf_ctx *ctx, const nf_force_params &p, float theta, cons
     W.cw = p.box / (float)K; W.eps = p.eps; W.eps2 = p.eps * p.eps; W.th2 = theta * theta; W.Gm = p.Gm;
     const size_t smem = sizeof(WalkShared) * WALK_WARPS;
     NF_CUDA(ctx, cudaFuncSetAttribute(k_tree_walk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NF_CUDA(ctx, cudaEventRecord(ctx->ev_walk0, st));
     k_tree_walk<<<(unsigned)ctx->sm_count * 2, WALK_WARPS * 32, smem, st>>>(W);
     NF_LAUNCHED(ctx);
+    NF_CUDA(ctx, cudaEventRecord(ctx->ev_walk1, st));
+    ctx->tree_timed = true;
     if (cell_amax) {
         k_tree_amax<<<(unsigned)((ncell + 7) / 8), 256, 0, st>>>(off, perm, acc, ncell, cell_amax);
         NF_LAUNCHED(ctx);

@@ -35,7 +35,7 @@ EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve
            "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host",
            "nf_bin_m", "nf_forces_ex", "nf_kick_drift", "nf_cell_vrms", "nf_stream_step_slabs",
            "nf_keys", "nf_forces_chunk", "nf_forces_host_m", "nf_regroup_plane", "nf_stream_step_regroup",
-           "nf_forces_host_begin", "nf_forces_host_end", "nf_timestep_terms", "nf_forces_tree", "nf_tree_stats"]
+           "nf_forces_host_begin", "nf_forces_host_end", "nf_timestep_terms", "nf_forces_tree", "nf_tree_stats", "nf_last_tree_timing"]
 
 
 class NFError(RuntimeError):
@@ -96,6 +96,8 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.nf_forces_ex.argtypes = [vp, vp, vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, vp, vp, vp]
     lib.nf_forces_tree.restype = i32
     lib.nf_forces_tree.argtypes = [vp, vp, vp, vp, i64, i32, i32, f32, f32, f32, i32, f32, vp, vp, vp]
+    lib.nf_last_tree_timing.restype = i32
+    lib.nf_last_tree_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     lib.nf_tree_stats.restype = i32
     lib.nf_tree_stats.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
     lib.nf_kick_drift.restype = i32
@@ -289,6 +291,12 @@ class Context:
                                             _soft_code(softening) | (NF_MASS_W if use_mass else 0), float(theta),
                                             _ptr(acc), _ptr(cell_amax), self._stream(stream)))
         return acc
+
+    def last_tree_timing(self) -> float:
+        """Milliseconds of the walk kernel of the last forces_tree (CUDA events on its stream)."""
+        t = ctypes.c_float(0)
+        self._check(self.lib.nf_last_tree_timing(self._h, ctypes.byref(t)))
+        return float(t.value)
 
     def tree_stats(self, stream=None) -> dict:
         """nf_tree_stats: (sink, accepted node) and (sink, particle of an opened leaf) pairs of the last forces_tree."""

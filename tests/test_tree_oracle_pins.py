@@ -1,6 +1,6 @@
 """Pins for the tree near field oracle (oracle/nf_tree.py, readings t1-t6).  Every check compares it
 with something other than itself: the direct-sum oracle (itself pinned by test_oracle_pins.py), a hand formula, the
-classical monopole error bound, geometric invariants of the Morton order and of the boxes."""
+classical monopole error bound, geometric invariants of the Hilbert order and of the boxes."""
 import numpy as np
 
 import oracle
