@@ -326,6 +326,25 @@ int nf_timestep_terms(nf_ctx *ctx, const float *cell_vrms, const float *cell_ama
                       int K, float box, const float *vmax, nf_timestep *out, void *stream);
 
 /*
+ * nf_timestep_terms_static -- nf_timestep_terms for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it): it allocates nothing.  nf_timestep_terms takes its scratch (one
+ * partial record per block of cells) from the context's arena, which grows with cudaMalloc on demand; this call keeps
+ * the same scratch in a file-scope __device__ array of fixed size -- 4097 records of 40 bytes = 164 KB, which every GPU
+ * that loads the library holds until the process exits -- and calls no cudaMalloc, cudaFree or allocating library
+ * routine.  Same kernels, same arguments, same meaning of `out`; minimum, maximum and counts are identical to
+ * nf_timestep_terms, the double sum behind vrms_global is formed over other block boundaries (equal within rounding).
+ *
+ *   K <= NF_TS_STATIC_MAX_K (256): one record per 4096 cells, 4096 records.  A larger K is NF_ERR_ARG with a message
+ *   that says so; use nf_timestep_terms there.
+ *   All calls, from every context and stream on a device, share the one array; it keeps the last call's contents
+ *   (nothing needs clearing: every record read was written by the same call).  Calls that OVERLAP on the GPU race:
+ *   issue them on one stream or order them yourself.  Synchronises `stream` (the result is returned to the host).
+ */
+#define NF_TS_STATIC_MAX_K 256
+int nf_timestep_terms_static(nf_ctx *ctx, const float *cell_vrms, const float *cell_amax, const uint64_t *cell_offset,
+                             int K, float box, const float *vmax, nf_timestep *out, void *stream);
+
+/*
  * nf_forces_host -- the whole path from HOST buffers: H2D copy of the positions, nf_bin,
  * nf_forces, D2H copy of the accelerations (the paper's GPU rate "includes
  * PCIe bus transfer overheads").  All device buffers come from the context's scratch arena

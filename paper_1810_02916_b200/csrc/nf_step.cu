@@ -188,3 +188,69 @@ int nf_cell_vrms(nf_ctx *ctx, const float *vel_xyz, const uint32_t *perm, const 
     NF_LAUNCHED(ctx);
     return NF_OK;
 }
+
+// ------------------------------------------------------------------------------------------
+// nf_timestep_terms_static: nf_timestep_terms for callers that cannot call cudaMalloc (code under CUDA graph capture,
+// tight serving loops, harnesses that forbid it).  Same kernels; their scratch -- one TsRec per block of
+// NF_TS_STATIC_CELLS_PER_REC cells plus the final record -- is a file-scope __device__ array instead of the context's
+// arena (which grows with cudaMalloc on demand).  Every GPU that loads libnf holds the array (164 KB) until exit.
+// In host code the array's NAME is a host-side stand-in, not a device address: the device address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+// ------------------------------------------------------------------------------------------
+#include <mutex>
+
+namespace {
+constexpr size_t TS_STATIC_CELLS_PER_REC = 4096;                                  // cells reduced into one record
+constexpr size_t TS_STATIC_MAX_REC = (size_t)NF_TS_STATIC_MAX_K * NF_TS_STATIC_MAX_K * NF_TS_STATIC_MAX_K / TS_STATIC_CELLS_PER_REC;
+static __device__ __align__(256) unsigned char g_ts_static[(TS_STATIC_MAX_REC + 1) * sizeof(TsRec)];
+constexpr int TS_STATIC_MAX_DEVICES = 64;
+TsRec *g_ts_static_ptr[TS_STATIC_MAX_DEVICES];       // device address of g_ts_static on each device (null: not looked up yet)
+std::mutex g_ts_static_mutex;
+}  // namespace
+
+int nf_timestep_terms_static(nf_ctx *ctx, const float *cell_vrms, const float *cell_amax, const uint64_t *cell_offset,
+                             int K, float box, const float *vmax, nf_timestep *out, void *stream)
+{
+    if (!ctx) return NF_ERR_ARG;
+    NF_ARG(ctx, K >= 1, "nf_timestep_terms_static: bad K");
+    NF_ARG(ctx, K <= NF_TS_STATIC_MAX_K,
+           "nf_timestep_terms_static: K = %d exceeds the static scratch (K <= %d: one record per %zu cells, %zu records); use nf_timestep_terms",
+           K, NF_TS_STATIC_MAX_K, TS_STATIC_CELLS_PER_REC, TS_STATIC_MAX_REC);
+    NF_ARG(ctx, cell_vrms && cell_amax && cell_offset && out, "nf_timestep_terms_static: null argument");
+    NF_ARG(ctx, box > 0.0f && box < 3.0e38f, "box must be positive and finite");
+    NF_ARG(ctx, ctx->device >= 0 && ctx->device < TS_STATIC_MAX_DEVICES, "nf_timestep_terms_static: device index %d out of range", ctx->device);
+    NF_CUDA(ctx, cudaSetDevice(ctx->device));
+    TsRec *rec = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_ts_static_mutex);
+        if (!g_ts_static_ptr[ctx->device]) {
+            void *p = nullptr;
+            NF_CUDA(ctx, cudaGetSymbolAddress(&p, g_ts_static));
+            g_ts_static_ptr[ctx->device] = static_cast<TsRec *>(p);
+        }
+        rec = g_ts_static_ptr[ctx->device];
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t ncell = (size_t)K * K * K;
+    const int nb = (int)((ncell + TS_STATIC_CELLS_PER_REC - 1) / TS_STATIC_CELLS_PER_REC);     // <= TS_STATIC_MAX_REC
+    // nothing has to start at zero: every block writes its own record and the final pass reads records [0, nb) only
+    k_timestep_cells<<<nb, TS_THREADS, 0, st>>>(cell_vrms, cell_amax, cell_offset, ncell, rec);
+    NF_LAUNCHED(ctx);
+    k_timestep_final<<<1, TS_THREADS, 0, st>>>(rec, nb, rec + nb);
+    NF_LAUNCHED(ctx);
+    TsRec h;
+    float hv = 0.f;
+    NF_CUDA(ctx, cudaMemcpyAsync(&h, rec + nb, sizeof(TsRec), cudaMemcpyDeviceToHost, st));
+    if (vmax) NF_CUDA(ctx, cudaMemcpyAsync(&hv, vmax, sizeof(float), cudaMemcpyDeviceToHost, st));
+    NF_CUDA(ctx, cudaStreamSynchronize(st));
+    out->cells_used = (int64_t)h.used;
+    out->ratio_cell_min = h.used ? (double)h.rmin : 0.0;
+    out->ratio_cell_max = (double)h.rmax;
+    out->vrms_global = h.n ? sqrt(h.sum_nv2 / (double)h.n) : 0.0;
+    out->amax_global = (double)h.amax;
+    out->ratio_global = h.amax > 0.f ? out->vrms_global / (double)h.amax : 0.0;
+    out->ratio_criterion2 = out->ratio_global > out->ratio_cell_min ? out->ratio_global : out->ratio_cell_min;
+    out->vmax = (double)hv;
+    out->drift_limit = hv > 0.f ? 0.8 * ((double)box / (double)K) / (double)hv : INFINITY;
+    return NF_OK;
+}

@@ -35,7 +35,8 @@ EXPORTS = ["nf_version", "nf_create", "nf_destroy", "nf_last_error", "nf_reserve
            "nf_stream_slabs", "nf_last_forces_timing", "nf_launch_count", "nf_forces_host", "nf_reserve_host",
            "nf_bin_m", "nf_forces_ex", "nf_kick_drift", "nf_cell_vrms", "nf_stream_step_slabs",
            "nf_keys", "nf_forces_chunk", "nf_forces_host_m", "nf_regroup_plane", "nf_stream_step_regroup",
-           "nf_forces_host_begin", "nf_forces_host_end", "nf_timestep_terms", "nf_forces_tree", "nf_tree_stats", "nf_last_tree_timing"]
+           "nf_forces_host_begin", "nf_forces_host_end", "nf_timestep_terms", "nf_forces_tree", "nf_tree_stats", "nf_last_tree_timing",
+           "nf_timestep_terms_static"]
 
 
 class NFError(RuntimeError):
@@ -106,6 +107,8 @@ def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
     lib.nf_cell_vrms.argtypes = [vp, vp, vp, vp, i64, i32, vp, vp, vp]
     lib.nf_timestep_terms.restype = i32
     lib.nf_timestep_terms.argtypes = [vp, vp, vp, vp, i32, f32, vp, ctypes.POINTER(TimeStep), vp]
+    lib.nf_timestep_terms_static.restype = i32
+    lib.nf_timestep_terms_static.argtypes = [vp, vp, vp, vp, i32, f32, vp, ctypes.POINTER(TimeStep), vp]
     lib.nf_out_of_range.restype = i32
     lib.nf_out_of_range.argtypes = [vp, ctypes.POINTER(i64), vp]
     lib.nf_forces.restype = i32
@@ -331,6 +334,18 @@ class Context:
             assert t.is_cuda and t.dtype == torch.float32 and t.numel() == ncell and t.is_contiguous()
         ts = TimeStep()
         self._check(self.lib.nf_timestep_terms(self._h, _ptr(cell_vrms), _ptr(cell_amax), _ptr(b.cell_offset), b.K, float(b.box),
+                                               _ptr(vmax) if vmax is not None else None, ctypes.byref(ts), self._stream(stream)))
+        return ts.as_dict()
+
+    def timestep_terms_static(self, cell_vrms: torch.Tensor, cell_amax: torch.Tensor, b: Binned, vmax: Optional[torch.Tensor] = None,
+                              stream=None) -> dict:
+        """nf_timestep_terms_static: timestep_terms with its scratch in a fixed __device__ array -- no allocation; K <= 256;
+        calls that overlap on the GPU race (include/nf.h)."""
+        ncell = b.K ** 3
+        for t in (cell_vrms, cell_amax):
+            assert t.is_cuda and t.dtype == torch.float32 and t.numel() == ncell and t.is_contiguous()
+        ts = TimeStep()
+        self._check(self.lib.nf_timestep_terms_static(self._h, _ptr(cell_vrms), _ptr(cell_amax), _ptr(b.cell_offset), b.K, float(b.box),
                                                _ptr(vmax) if vmax is not None else None, ctypes.byref(ts), self._stream(stream)))
         return ts.as_dict()
 
