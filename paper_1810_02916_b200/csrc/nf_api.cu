@@ -218,7 +218,7 @@ static int encode_full(nf_ctx *ctx, nf_force_params &p, const float4 *ps, const 
     const size_t ncell = (size_t)K * K * K;
     const bool dense = nf_dense_wanted(N, ncell, p.softening | (tree ? NF_DENSE_ORDER : 0));
     p.softening &= ~NF_DENSE_ORDER;
-    NF_TRY(nf_encode_impl(ctx, p, ps, off, ncell, enc, enc_h, st));
+    NF_TRY(nf_encode_impl(ctx, p, ps, off, ncell, enc, enc_h, st, dense ? NF_DENSE_N : 0));
     uint32_t *dinfo = nullptr, *dslot = nullptr;
     float *dbox = nullptr;
     if (dense) {

@@ -137,8 +137,9 @@ int nf_fill_planes_full(nf_ctx *ctx, nf_plane_view *d_planes, int K, const float
                         const float *dbox, cudaStream_t st);
 // enc[s], enc_h[s] = the two encoded copies of pos[s] for the ncell cells described by off (cell index % K = cz);
 // they depend on p.eps, p.box, p.K
+// skip_n > 0: cells of at least skip_n particles are left out -- the caller runs nf_dense_order_impl next, which encodes them
 int nf_encode_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos, const uint64_t *off, size_t ncell, float4 *enc,
-                   float4 *enc_h, cudaStream_t st);
+                   float4 *enc_h, cudaStream_t st, uint32_t skip_n = 0);
 // In-cell ordering of dense cells (nf_dense.cu), full box only.  Cells of at least NF_DENSE_N particles get their ENCODED
 // copies (enc, enc_h: what the interaction kernel reads) re-ordered along a Hilbert curve inside the cell, with a box per 64
 // particles, so that the kernel can prove most (task, tile) pairs free of pairs inside eps.  dinfo: K^3 words out.

@@ -118,6 +118,28 @@ __global__ void __launch_bounds__(256) k_dense_keys(const float4 *__restrict__ p
     (void)cap;
 }
 
+// Cells of NF_DENSE_N particles or more that the ordering does NOT take (beyond its capacity; rare): nf_encode_impl left
+// them out (skip_n), so their encoded copies are written here, in the binned order.  One warp per cell.
+__global__ void __launch_bounds__(256) k_dense_left_out(const float4 *__restrict__ pos, const uint64_t *__restrict__ off, size_t ncell,
+                                                        const uint32_t *__restrict__ dinfo, int K, float scale, float ws,
+                                                        float4 *__restrict__ enc, float4 *__restrict__ enc_h)
+{
+    const size_t c = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (c >= ncell) return;
+    const uint64_t s0 = off[c], s1 = off[c + 1];
+    if (s1 - s0 < (uint64_t)NF_DENSE_N || dinfo[c] != 0u) return;
+    const int lane = threadIdx.x & 31;
+    const int cz = (int)(c % (size_t)K);
+    const float ez = ((float)(cz % NF_ZB) - 0.5f * (float)(NF_ZB - 1)) * ws;
+    const float eh = ((float)((cz + NF_ZB / 2) % NF_ZB) - 0.5f * (float)(NF_ZB - 1)) * ws;
+    for (uint64_t s = s0 + lane; s < s1; s += 32) {
+        const float4 o = pos[s];
+        const float x = o.x * scale, y = o.y * scale;
+        enc[s] = make_float4(x, y, fmaf(o.z, scale, ez), o.w);
+        enc_h[s] = make_float4(x, y, fmaf(o.z, scale, eh), o.w);
+    }
+}
+
 // one warp per 64 compact positions (a "chunk"; cells start on chunk boundaries)
 __global__ void __launch_bounds__(256) k_dense_finish(const float4 *__restrict__ pos, const uint32_t *__restrict__ key,
                                                       const uint32_t *__restrict__ idx, const uint32_t *__restrict__ nd,
@@ -218,6 +240,8 @@ int nf_dense_order_impl(nf_ctx *ctx, const nf_force_params &p, const float4 *pos
     NF_TRY(nf_exclusive_scan_u32(ctx, n64, coff, ncell, stmp, st));
     NF_TRY(nf_exclusive_scan_u32(ctx, one, rank, ncell, stmp, st));
     k_dense_cells<<<(unsigned)((ncell + 255) / 256), 256, 0, st>>>(off, ncell, n64, coff, rank, cap, dinfo, dcell, nd);
+    NF_LAUNCHED(ctx);
+    k_dense_left_out<<<(unsigned)((ncell + 7) / 8), 256, 0, st>>>(pos, off, ncell, dinfo, K, scale, ws, enc, enc_h);
     NF_LAUNCHED(ctx);
     k_dense_keys<<<(unsigned)(cap / 256 < 148u * 8u ? (cap + 255) / 256 : 148u * 8u), 256, 0, st>>>(pos, nd, dcell, cap, (float)K / p.box, keyA, idxA);
     NF_LAUNCHED(ctx);

@@ -284,7 +284,7 @@ static int stream_run(nf_ctx *ctx, EventPool &pool, const PlaneIn &in,
         const int cx = ((plane0 + q) % K + K) % K;
         // counters[0] accumulates out-of-range / wrong-plane particles over all planes
         NF_TRY(nf_bin_impl(ctx, sl.raw, nullptr, plane_n[q], K, box, cx, sl.sorted, sl.perm, sl.count, sl.off, st));
-        NF_TRY(nf_encode_impl(ctx, fp, (const float4 *)sl.sorted, sl.off, ncell, (float4 *)sl.enc, (float4 *)sl.enc_h, st));
+        NF_TRY(nf_encode_impl(ctx, fp, (const float4 *)sl.sorted, sl.off, ncell, (float4 *)sl.enc, (float4 *)sl.enc_h, st, dense ? NF_DENSE_N : 0));
         if (dense)
             NF_TRY(nf_dense_order_impl(ctx, fp, (const float4 *)sl.sorted, sl.off, ncell, plane_n[q], (float4 *)sl.enc, (float4 *)sl.enc_h,
                                        sl.dinfo, sl.dslot, sl.dbox, st));
