@@ -22,7 +22,9 @@
 //   k_tree_leaves    one warp per chunk: Hilbert-ordered copy of (offset, mass); box, mass, centre of mass of its four leaves
 //   k_tree_level     level l from level l-1
 //   k_tree_items     per cell: number of sink groups if any neighbour cell is dense (scanned into the work list)
-//   k_tree_walk      one warp per sink group (walking as a whole, or in parts when its box is out of proportion: t4): the walk of t5 with a bounded depth-first stack in shared memory; ADDS to acc
+//   k_tree_walk<1>   one warp per sink group: in how many parts it walks (t4: as a whole, or in parts when its box is out of
+//                    proportion); scanned into the work list of (group, part) pairs
+//   k_tree_walk<0>   one warp per (group, part): the walk of t5 with a bounded depth-first stack in shared memory; ADDS to acc
 //   k_tree_amax      per-cell maximum of |a| from the final accelerations
 //
 // Deterministic: every sink belongs to one warp, which visits cells, nodes and particles in a fixed order; the only
@@ -199,6 +201,8 @@ struct WalkParams {
     const float4 *pos; const uint64_t *off; const uint32_t *perm; const uint32_t *dinfo; const uint32_t *dslot;
     const TreeCell *tcell; const uint32_t *crank; const float4 *tpos; const float4 *nlo; const float4 *nhi; const float4 *ncom;
     const uint32_t *goff;          // exclusive scan of the groups per cell, ncell + 1 entries
+    uint32_t *np;                  // parts per group (t4), written by the counting instance
+    const uint32_t *poff;          // exclusive scan of np: the work list is over (group, part) pairs
     float *acc; unsigned long long *stats; uint32_t *cursor;
     size_t ncell; int K, R, plummer; float cw, eps, eps2, th2, Gm;
 };
@@ -216,28 +220,45 @@ __device__ __forceinline__ float law_full(float r2, float eps2, float inv_eps, f
     return fminf(poly, ri * ri * ri);               // fn. 4: the spline is the smaller of the two
 }
 
+// COUNT: one warp per group, writes the number of parts the group walks in (t4) and nothing else.  Else: one warp per
+// (group, part) pair pulled from a cursor -- a group that walks in up to 64 parts is up to 64 work items, not one item
+// 19 walks long (that one item used to be the kernel's tail: SMs 63 % busy).
+template <bool COUNT>
 __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WalkShared &S = reinterpret_cast<WalkShared *>(smem_raw)[threadIdx.x >> 5];
     const int lane = threadIdx.x & 31;
     const int K = P.K, R = P.R;
-    const uint32_t n_items = P.goff[P.ncell];
+    const uint32_t n_groups = P.goff[P.ncell];
+    const uint32_t n_items = COUNT ? n_groups : P.poff[n_groups];
     const float inv_eps = 1.0f / P.eps, inv_eps3 = inv_eps * inv_eps * inv_eps;
     unsigned long long st_node = 0, st_leaf = 0;
-    for (;;) {
+    for (uint32_t round = 0;; round++) {
         uint32_t item = 0;
-        if (lane == 0) item = atomicAdd(P.cursor, 1u);
-        item = __shfl_sync(0xffffffffu, item, 0);
+        if (COUNT) item = (round * gridDim.x + blockIdx.x) * WALK_WARPS + (threadIdx.x >> 5);
+        else {
+            if (lane == 0) item = atomicAdd(P.cursor, 1u);
+            item = __shfl_sync(0xffffffffu, item, 0);
+        }
         if (item >= n_items) break;
-        // the cell of this group: last c with goff[c] <= item
+        uint32_t grp = item, pk = 0;
+        if (!COUNT) {                            // the group of this item: last grp with poff[grp] <= item
+            uint32_t lo_g = 0, hi_g = n_groups;
+            while (hi_g - lo_g > 1) {
+                const uint32_t mid = (lo_g + hi_g) >> 1;
+                if (P.poff[mid] <= item) lo_g = mid; else hi_g = mid;
+            }
+            grp = lo_g; pk = item - P.poff[lo_g];
+        }
+        // the cell of this group: last c with goff[c] <= grp
         size_t lo_c = 0, hi_c = P.ncell;
         while (hi_c - lo_c > 1) {
             const size_t mid = (lo_c + hi_c) >> 1;
-            if (P.goff[mid] <= item) lo_c = mid; else hi_c = mid;
+            if (P.goff[mid] <= grp) lo_c = mid; else hi_c = mid;
         }
         const size_t c = lo_c;
-        const uint32_t g = item - P.goff[c];
+        const uint32_t g = grp - P.goff[c];
         const int cz = (int)(c % K), cy = (int)((c / K) % K), cx = (int)(c / ((size_t)K * K));
         const uint64_t c0 = P.off[c], c1 = P.off[c + 1];
         const uint32_t own = P.dinfo[c];
@@ -335,9 +356,14 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
             }
             __syncwarp();
         }
+        if (COUNT) {
+            if (lane == 0) P.np[grp] = nparts;
+            __syncwarp();
+            continue;
+        }
         float ax[2] = {0.f, 0.f}, ay[2] = {0.f, 0.f}, az[2] = {0.f, 0.f};
-        for (uint32_t pi = 0; pi < nparts; pi++) {
-        const Part part = S.parts[pi];
+        {
+        const Part part = S.parts[pk];
 #pragma unroll
         for (int a = 0; a < 3; a++) { glo[a] = part.lo[a]; ghi[a] = part.hi[a]; }
         const bool act[2] = {(bool)((part.mask >> lane) & 1ull), (bool)((part.mask >> (32 + lane)) & 1ull)};
@@ -463,15 +489,16 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                         }
                     }
                 }
-        }   // parts
 #pragma unroll
         for (int h = 0; h < 2; h++)
-            if (valid[h]) {
+            if (valid[h] && act[h]) {
                 const uint64_t o = P.perm ? (uint64_t)P.perm[slot[h]] : slot[h];
                 P.acc[3 * o + 0] += P.Gm * ax[h];
                 P.acc[3 * o + 1] += P.Gm * ay[h];
                 P.acc[3 * o + 2] += P.Gm * az[h];
             }
+        }   // the part
+        __syncwarp();          // S.parts is rewritten by the next item
     }
     for (int d = 16; d > 0; d >>= 1) {
         st_node += __shfl_xor_sync(0xffffffffu, st_node, d);
@@ -500,6 +527,7 @@ __global__ void __launch_bounds__(256) k_tree_amax(const uint64_t *__restrict__ 
     if (lane == 0) amax[c] = sqrtf(m);
 }
 
+size_t tree_groups_max(int64_t N, size_t ncell) { return (size_t)N / 64 + ncell + 1; }    // sum over cells of ceil(n / 64)
 size_t tree_nodes_max(int64_t N) { return (size_t)(nf_dense_cap(N) / LEAF) * 8 / 7 + (size_t)MAXLEV * NF_DENSE_MAX_CELLS + 64; }
 
 }  // namespace
@@ -511,6 +539,8 @@ size_t nf_tree_scratch_bytes(int64_t N, size_t ncell)
     b += nf_align_up((size_t)NF_DENSE_MAX_CELLS * sizeof(TreeCell), 256) + nf_align_up(cap / 64 * sizeof(uint32_t), 256);
     b += nf_align_up(cap * sizeof(float4), 256) + 3 * nf_align_up(nn * sizeof(float4), 256);
     b += 2 * nf_align_up((ncell + 1) * sizeof(uint32_t), 256) + nf_align_up(nf_scan_temp_elems(ncell + 1) * sizeof(uint32_t), 256);
+    const size_t ng = tree_groups_max(N, ncell) + 1;
+    b += 2 * nf_align_up(ng * sizeof(uint32_t), 256) + nf_align_up(nf_scan_temp_elems(ng) * sizeof(uint32_t), 256);       // np, poff
     return b + 4096;
 }
 
@@ -534,7 +564,10 @@ int nf_tree_forces_impl(nf_ctx *ctx, const nf_force_params &p, float theta, cons
     float4 *nlo = nf_scratch_take<float4>(ctx, nn), *nhi = nf_scratch_take<float4>(ctx, nn), *ncom = nf_scratch_take<float4>(ctx, nn);
     uint32_t *ng = nf_scratch_take<uint32_t>(ctx, ncell + 1), *goff = nf_scratch_take<uint32_t>(ctx, ncell + 1);
     uint32_t *stmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(ncell + 1));
-    if (!tcell || !crank || !tpos || !nlo || !nhi || !ncom || !ng || !goff || !stmp) {
+    const size_t ngm = tree_groups_max(N, ncell) + 1;
+    uint32_t *np = nf_scratch_take<uint32_t>(ctx, ngm), *poff = nf_scratch_take<uint32_t>(ctx, ngm);
+    uint32_t *ptmp = nf_scratch_take<uint32_t>(ctx, nf_scan_temp_elems(ngm));
+    if (!tcell || !crank || !tpos || !nlo || !nhi || !ncom || !ng || !goff || !stmp || !np || !poff || !ptmp) {
         NF_SET_ERR(ctx, "nf_forces_tree: internal scratch arena too small");
         return NF_ERR_NOMEM;
     }
@@ -561,14 +594,21 @@ int nf_tree_forces_impl(nf_ctx *ctx, const nf_force_params &p, float theta, cons
     NF_TRY(nf_exclusive_scan_u32(ctx, ng, goff, ncell + 1, stmp, st));
     WalkParams W;
     W.pos = pos; W.off = off; W.perm = perm; W.dinfo = dinfo; W.dslot = dslot; W.tcell = tcell; W.crank = crank; W.tpos = tpos;
-    W.nlo = nlo; W.nhi = nhi; W.ncom = ncom; W.goff = goff; W.acc = acc; W.stats = stats;
+    W.nlo = nlo; W.nhi = nhi; W.ncom = ncom; W.goff = goff; W.np = np; W.poff = poff; W.acc = acc; W.stats = stats;
     W.cursor = reinterpret_cast<uint32_t *>(stats + 2);
     W.ncell = ncell; W.K = K; W.R = p.R; W.plummer = (p.softening & NF_SOFT_LAW_MASK) == NF_SOFT_PLUMMER ? 1 : 0;
     W.cw = p.box / (float)K; W.eps = p.eps; W.eps2 = p.eps * p.eps; W.th2 = theta * theta; W.Gm = p.Gm;
     const size_t smem = sizeof(WalkShared) * WALK_WARPS;
-    NF_CUDA(ctx, cudaFuncSetAttribute(k_tree_walk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NF_CUDA(ctx, cudaFuncSetAttribute(k_tree_walk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NF_CUDA(ctx, cudaFuncSetAttribute(k_tree_walk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // parts per group, scanned: the walk's work list is over (group, part) pairs
+    NF_CUDA(ctx, cudaMemsetAsync(np, 0, ngm * sizeof(uint32_t), st));
+    const size_t cblocks = (ngm + WALK_WARPS - 1) / WALK_WARPS;
+    k_tree_walk<true><<<(unsigned)(cblocks < (size_t)ctx->sm_count * 2 ? cblocks : (size_t)ctx->sm_count * 2), WALK_WARPS * 32, smem, st>>>(W);
+    NF_LAUNCHED(ctx);
+    NF_TRY(nf_exclusive_scan_u32(ctx, np, poff, ngm, ptmp, st));
     NF_CUDA(ctx, cudaEventRecord(ctx->ev_walk0, st));
-    k_tree_walk<<<(unsigned)ctx->sm_count * 2, WALK_WARPS * 32, smem, st>>>(W);
+    k_tree_walk<false><<<(unsigned)ctx->sm_count * 2, WALK_WARPS * 32, smem, st>>>(W);
     NF_LAUNCHED(ctx);
     NF_CUDA(ctx, cudaEventRecord(ctx->ev_walk1, st));
     ctx->tree_timed = true;
