@@ -39,6 +39,16 @@ constexpr uint32_t PAD = 0xffffffffu;
 constexpr int WALK_WARPS = 8;
 constexpr int STACK_CAP = 256 * MAXLEV + 64;    // depth-first over batches of 32 nodes: at most 8 * 32 pending per level
 constexpr int LIST_CAP = 64;
+constexpr float FILL = 1.0e15f;
+
+// packed float32 pairs (the two sinks a lane holds): one instruction for both, as in the interaction kernel
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk(float a, float b) { u64 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void upk(u64 r, float &a, float &b) { asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(r)); }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 
 struct TreeCell {
     unsigned long long c0;        // first sorted slot of the cell
@@ -107,7 +117,7 @@ __global__ void __launch_bounds__(256) k_tree_leaves(const float4 *__restrict__ 
             double sm = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
             const uint32_t t = t0 + 32u * h + lane;
             const uint32_t s = dslot[t];
-            float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+            float4 o = make_float4(FILL, FILL, FILL, 0.f);        // padding: massless and far away (r^-3 flushes to zero)
             if (s != PAD) {
                 o = pos[s];
                 if (!MASS) o.w = 1.0f;
@@ -190,12 +200,50 @@ __global__ void __launch_bounds__(256) k_tree_items(const uint64_t *__restrict__
 struct Part { float lo[3], hi[3]; unsigned long long mask; };   // sinks that walk together (bit 32 h + lane), and their box
 
 struct WalkShared {
-    Part parts[68];                // at most 3 quarters + 16 single sinks ... 64 single sinks
+    Part part;                     // the part this item walks
     uint32_t stack[STACK_CAP];
-    float4 list[LIST_CAP];         // accepted nodes waiting to be evaluated: centre of mass, mass
-    float4 stage[64];              // the particles of one leaf
-    uint32_t leaves[32];
+    ulonglong2 list[2 * LIST_CAP]; // accepted nodes waiting to be evaluated: (x,x | y,y), (z,z | m,m) -- duplicated for the packed sweep
+    ulonglong2 stage[2 * 64];      // the particles of up to four leaves, same layout
+    uint32_t leaves[32];           // leaves opened by a batch; bit 31: every pair of the leaf is further apart than eps
 };
+
+__device__ __forceinline__ void put_dup(ulonglong2 *dst, const float4 q)
+{
+    dst[0] = make_ulonglong2(pk(q.x, q.x), pk(q.y, q.y));
+    dst[1] = make_ulonglong2(pk(q.z, q.z), pk(q.w, q.w));
+}
+
+struct SweepConsts { u64 ie, ie3, six, m15, ten, eps2; };
+
+// n sources against the lane's two sinks (PX, PY, PZ), sums formed from zero into LX, LY, LZ.
+// LAW 0: m / r^2 (accepted nodes; leaves proven outside eps -- the spline equals it there, fn. 4)
+// LAW 1: the spline of Eq. 2 as min(poly, r^-3);  LAW 2: Plummer, Eq. 1
+template <int LAW>
+__device__ __forceinline__ void sweep2(const ulonglong2 *__restrict__ src, uint32_t n, u64 PX, u64 PY, u64 PZ, const SweepConsts &C,
+                                       u64 &LX, u64 &LY, u64 &LZ)
+{
+#pragma unroll 4
+    for (uint32_t j = 0; j < n; j++) {
+        const ulonglong2 xy = src[2 * j], zw = src[2 * j + 1];
+        const u64 DX = sub2(xy.x, PX), DY = sub2(xy.y, PY), DZ = sub2(zw.x, PZ);
+        u64 R2 = fma2(DZ, DZ, fma2(DY, DY, mul2(DX, DX)));
+        if (LAW == 2) R2 = add2(R2, C.eps2);
+        float a, b;
+        upk(R2, a, b);
+        if (LAW == 1) { a = fmaxf(a, 1.0e-30f); b = fmaxf(b, 1.0e-30f); }      // r = 0: the pair of a sink with itself
+        const u64 RI = pk(rsqrtf(a), rsqrtf(b));
+        u64 F = mul2(mul2(RI, RI), RI);
+        if (LAW == 1) {
+            const u64 U = mul2(mul2(R2, RI), C.ie);
+            const u64 POLY = mul2(fma2(U, fma2(U, C.six, C.m15), C.ten), C.ie3);
+            float f0, f1, p0, p1;
+            upk(F, f0, f1); upk(POLY, p0, p1);
+            F = pk(fminf(f0, p0), fminf(f1, p1));                               // fn. 4
+        }
+        F = mul2(F, zw.y);
+        LX = fma2(F, DX, LX); LY = fma2(F, DY, LY); LZ = fma2(F, DZ, LZ);
+    }
+}
 
 struct WalkParams {
     const float4 *pos; const uint64_t *off; const uint32_t *perm; const uint32_t *dinfo; const uint32_t *dslot;
@@ -207,24 +255,11 @@ struct WalkParams {
     size_t ncell; int K, R, plummer; float cw, eps, eps2, th2, Gm;
 };
 
-// |F|/r of the full softened law for one pair (r = 0 gives a finite factor; the displacement is then 0)
-__device__ __forceinline__ float law_full(float r2, float eps2, float inv_eps, float inv_eps3, int plummer)
-{
-    if (plummer) {
-        const float s = r2 + eps2, ri = rsqrtf(s);
-        return ri * ri * ri;
-    }
-    const float ri = rsqrtf(fmaxf(r2, 1.0e-30f));
-    const float u = r2 * ri * inv_eps;
-    const float poly = (10.0f + u * (6.0f * u - 15.0f)) * inv_eps3;
-    return fminf(poly, ri * ri * ri);               // fn. 4: the spline is the smaller of the two
-}
-
 // COUNT: one warp per group, writes the number of parts the group walks in (t4) and nothing else.  Else: one warp per
 // (group, part) pair pulled from a cursor -- a group that walks in up to 64 parts is up to 64 work items, not one item
 // 19 walks long (that one item used to be the kernel's tail: SMs 63 % busy).
 template <bool COUNT>
-__global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams P)
+__global__ void __launch_bounds__(WALK_WARPS * 32, 2) k_tree_walk(const WalkParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WalkShared &S = reinterpret_cast<WalkShared *>(smem_raw)[threadIdx.x >> 5];
@@ -233,6 +268,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
     const uint32_t n_groups = P.goff[P.ncell];
     const uint32_t n_items = COUNT ? n_groups : P.poff[n_groups];
     const float inv_eps = 1.0f / P.eps, inv_eps3 = inv_eps * inv_eps * inv_eps;
+    const SweepConsts SC = {pk(inv_eps, inv_eps), pk(inv_eps3, inv_eps3), pk(6.0f, 6.0f), pk(-15.0f, -15.0f), pk(10.0f, 10.0f), pk(P.eps2, P.eps2)};
     unsigned long long st_node = 0, st_leaf = 0;
     for (uint32_t round = 0;; round++) {
         uint32_t item = 0;
@@ -242,14 +278,14 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
             item = __shfl_sync(0xffffffffu, item, 0);
         }
         if (item >= n_items) break;
-        uint32_t grp = item, pk = 0;
+        uint32_t grp = item, part_k = 0;
         if (!COUNT) {                            // the group of this item: last grp with poff[grp] <= item
             uint32_t lo_g = 0, hi_g = n_groups;
             while (hi_g - lo_g > 1) {
                 const uint32_t mid = (lo_g + hi_g) >> 1;
                 if (P.poff[mid] <= item) lo_g = mid; else hi_g = mid;
             }
-            grp = lo_g; pk = item - P.poff[lo_g];
+            grp = lo_g; part_k = item - P.poff[lo_g];
         }
         // the cell of this group: last c with goff[c] <= grp
         size_t lo_c = 0, hi_c = P.ncell;
@@ -334,7 +370,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
             }
             lim = __fmul_rn(9.0f, lim);
             if (!(counted && d2g > lim && P.th2 > 0.f)) {       // theta = 0 accepts nothing: no box matters, one walk
-                if (lane == 0) { Part &pt = S.parts[0]; pt.mask = vmask; for (int a = 0; a < 3; a++) { pt.lo[a] = glo[a]; pt.hi[a] = ghi[a]; } }
+                if (lane == 0 && !COUNT) { Part &pt = S.part; pt.mask = vmask; for (int a = 0; a < 3; a++) { pt.lo[a] = glo[a]; pt.hi[a] = ghi[a]; } }
                 nparts = 1;
             } else {
 #pragma unroll
@@ -345,11 +381,11 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                             const int src = 16 * (q & 1) + (int)i;
                             const float x = __shfl_sync(0xffffffffu, sx[q >> 1], src), y = __shfl_sync(0xffffffffu, sy[q >> 1], src),
                                         z = __shfl_sync(0xffffffffu, sz[q >> 1], src);
-                            if (lane == 0) { Part &pt = S.parts[nparts]; pt.mask = 1ull << (16 * q + i); pt.lo[0] = pt.hi[0] = x; pt.lo[1] = pt.hi[1] = y; pt.lo[2] = pt.hi[2] = z; }
+                            if (lane == 0 && !COUNT && nparts == part_k) { Part &pt = S.part; pt.mask = 1ull << (16 * q + i); pt.lo[0] = pt.hi[0] = x; pt.lo[1] = pt.hi[1] = y; pt.lo[2] = pt.hi[2] = z; }
                             nparts++;
                         }
                     } else {
-                        if (lane == 0) { Part &pt = S.parts[nparts]; pt.mask = vmask & (0xffffull << (16 * q)); for (int a = 0; a < 3; a++) { pt.lo[a] = blo[q][a]; pt.hi[a] = bhi[q][a]; } }
+                        if (lane == 0 && !COUNT && nparts == part_k) { Part &pt = S.part; pt.mask = vmask & (0xffffull << (16 * q)); for (int a = 0; a < 3; a++) { pt.lo[a] = blo[q][a]; pt.hi[a] = bhi[q][a]; } }
                         nparts++;
                     }
                 }
@@ -363,7 +399,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
         }
         float ax[2] = {0.f, 0.f}, ay[2] = {0.f, 0.f}, az[2] = {0.f, 0.f};
         {
-        const Part part = S.parts[pk];
+        const Part part = S.part;
 #pragma unroll
         for (int a = 0; a < 3; a++) { glo[a] = part.lo[a]; ghi[a] = part.hi[a]; }
         const bool act[2] = {(bool)((part.mask >> lane) & 1ull), (bool)((part.mask >> (32 + lane)) & 1ull)};
@@ -380,6 +416,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                     float px[2], py[2], pz[2];
 #pragma unroll
                     for (int h = 0; h < 2; h++) { px[h] = sx[h] - sh[0]; py[h] = sy[h] - sh[1]; pz[h] = sz[h] - sh[2]; }
+                    const u64 PX = pk(px[0], px[1]), PY = pk(py[0], py[1]), PZ = pk(pz[0], pz[1]);
                     uint32_t sp = 0, nlist = 0;
                     if (lane == 0) S.stack[0] = (T.nlev - 1u) << 26;
                     sp = 1;
@@ -388,7 +425,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                         uint32_t nleaf = 0;
                         if (sp > 0) {
                             const uint32_t nb = min(32u, sp);
-                            bool have = (uint32_t)lane < nb, acc_it = false;
+                            bool have = (uint32_t)lane < nb, acc_it = false, far_eps = false;
                             uint32_t l = 0, k = 0, node = 0;
                             if (have) {
                                 const uint32_t e = S.stack[sp - 1u - lane];
@@ -405,19 +442,20 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                                     d2 = q == 0 ? __fmul_rn(gp, gp) : __fadd_rn(d2, __fmul_rn(gp, gp));
                                     s2 = q == 0 ? __fmul_rn(e1, e1) : __fadd_rn(s2, __fmul_rn(e1, e1));
                                 }
-                                acc_it = d2 > P.eps2 && s2 < __fmul_rn(P.th2, d2);
+                                far_eps = d2 > P.eps2;
+                                acc_it = far_eps && s2 < __fmul_rn(P.th2, d2);
                             }
                             sp -= nb;
                             __syncwarp();
                             // accepted nodes -> list
                             const uint32_t am = __ballot_sync(0xffffffffu, have && acc_it);
-                            if (have && acc_it) S.list[nlist + __popc(am & ((1u << lane) - 1u))] = P.ncom[node];
+                            if (have && acc_it) put_dup(S.list + 2 * (nlist + __popc(am & ((1u << lane) - 1u))), P.ncom[node]);
                             nlist += __popc(am);
                             st_node += (unsigned long long)__popc(am) * nsink;
                             // opened leaves -> this batch's leaf list
                             const bool openl = have && !acc_it && l == 0;
                             const uint32_t lm = __ballot_sync(0xffffffffu, openl);
-                            if (openl) S.leaves[__popc(lm & ((1u << lane) - 1u))] = k;
+                            if (openl) S.leaves[__popc(lm & ((1u << lane) - 1u))] = k | (far_eps ? 1u << 31 : 0u);
                             nleaf = __popc(lm);
                             st_leaf += (unsigned long long)__reduce_add_sync(0xffffffffu, openl ? min((uint32_t)LEAF, T.n - (uint32_t)LEAF * k) : 0u) * nsink;
                             // opened nodes -> their children on the stack
@@ -438,50 +476,38 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                             sp += tot;
                             __syncwarp();
                         }
-                        // the leaves opened by this batch, four at a time, particle by particle with the full law
+                        // the leaves opened by this batch, four at a time, particle by particle: the full softened law, or the
+                        // bare m / r^2 where the boxes prove every pair of the leaf further apart than eps (the same values)
                         for (uint32_t i = 0; i < nleaf; i += 4) {
 #pragma unroll
                             for (int rr = 0; rr < 2; rr++) {
                                 const uint32_t li = i + 2u * rr + ((uint32_t)lane >> 4);
-                                float4 q = make_float4(0.f, 0.f, 0.f, 0.f);            // massless filler
-                                if (li < nleaf) q = P.tpos[(size_t)T.coff + (size_t)LEAF * S.leaves[li] + (lane & 15)];
-                                S.stage[32 * rr + lane] = q;
+                                float4 q = make_float4(FILL, FILL, FILL, 0.f);           // massless filler
+                                if (li < nleaf) q = P.tpos[(size_t)T.coff + (size_t)LEAF * (S.leaves[li] & 0x7fffffffu) + (lane & 15)];
+                                put_dup(S.stage + 2 * (32 * rr + lane), q);
                             }
                             __syncwarp();
-                            const uint32_t np = (uint32_t)LEAF * min(4u, nleaf - i);
-                            float lx[2] = {0.f, 0.f}, ly[2] = {0.f, 0.f}, lz[2] = {0.f, 0.f};     // formed from zero, then added: shorter sums
-#pragma unroll 4
-                            for (uint32_t j = 0; j < np; j++) {
-                                const float4 q = S.stage[j];
-#pragma unroll
-                                for (int h = 0; h < 2; h++) {
-                                    const float ddx = q.x - px[h], ddy = q.y - py[h], ddz = q.z - pz[h];
-                                    const float r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-                                    const float f = law_full(r2, P.eps2, inv_eps, inv_eps3, P.plummer) * q.w;
-                                    lx[h] += f * ddx; ly[h] += f * ddy; lz[h] += f * ddz;
-                                }
+                            const uint32_t nl = min(4u, nleaf - i);
+                            u64 LX = 0, LY = 0, LZ = 0;                                   // formed from zero, then added: shorter sums
+                            for (uint32_t q4 = 0; q4 < nl; q4++) {
+                                const ulonglong2 *src = S.stage + 2 * LEAF * q4;
+                                if (P.plummer) sweep2<2>(src, LEAF, PX, PY, PZ, SC, LX, LY, LZ);
+                                else if (S.leaves[i + q4] >> 31) sweep2<0>(src, LEAF, PX, PY, PZ, SC, LX, LY, LZ);
+                                else sweep2<1>(src, LEAF, PX, PY, PZ, SC, LX, LY, LZ);
                             }
+                            float lx[2], ly[2], lz[2];
+                            upk(LX, lx[0], lx[1]); upk(LY, ly[0], ly[1]); upk(LZ, lz[0], lz[1]);
 #pragma unroll
                             for (int h = 0; h < 2; h++) if (act[h]) { ax[h] += lx[h]; ay[h] += ly[h]; az[h] += lz[h]; }
                             __syncwarp();
                         }
                         // accepted nodes: evaluate when the list could not take another batch, or at the end of the walk
                         if (nlist > (uint32_t)(LIST_CAP - 32) || (sp == 0 && nlist > 0)) {
-                            float lx[2] = {0.f, 0.f}, ly[2] = {0.f, 0.f}, lz[2] = {0.f, 0.f};
-#pragma unroll 4
-                            for (uint32_t j = 0; j < nlist; j++) {
-                                const float4 q = S.list[j];
-#pragma unroll
-                                for (int h = 0; h < 2; h++) {
-                                    const float ddx = q.x - px[h], ddy = q.y - py[h], ddz = q.z - pz[h];
-                                    const float r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-                                    float f;
-                                    if (P.plummer) { const float ri = rsqrtf(r2 + P.eps2); f = ri * ri * ri; }
-                                    else { const float ri = rsqrtf(r2); f = ri * ri * ri; }
-                                    f *= q.w;
-                                    lx[h] += f * ddx; ly[h] += f * ddy; lz[h] += f * ddz;
-                                }
-                            }
+                            u64 LX = 0, LY = 0, LZ = 0;
+                            if (P.plummer) sweep2<2>(S.list, nlist, PX, PY, PZ, SC, LX, LY, LZ);
+                            else sweep2<0>(S.list, nlist, PX, PY, PZ, SC, LX, LY, LZ);
+                            float lx[2], ly[2], lz[2];
+                            upk(LX, lx[0], lx[1]); upk(LY, ly[0], ly[1]); upk(LZ, lz[0], lz[1]);
 #pragma unroll
                             for (int h = 0; h < 2; h++) if (act[h]) { ax[h] += lx[h]; ay[h] += ly[h]; az[h] += lz[h]; }
                             nlist = 0;
@@ -498,7 +524,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_tree_walk(const WalkParams 
                 P.acc[3 * o + 2] += P.Gm * az[h];
             }
         }   // the part
-        __syncwarp();          // S.parts is rewritten by the next item
+        __syncwarp();          // S.part is rewritten by the next item
     }
     for (int d = 16; d > 0; d >>= 1) {
         st_node += __shfl_xor_sync(0xffffffffu, st_node, d);
