@@ -48,6 +48,8 @@ __device__ __forceinline__ void upk(u64 r, float &a, float &b) { asm("mov.b64 {%
 __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
 __device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+// MUFU.RSQ alone: rsqrtf() without -ftz wraps it in a range fix-up for denormals (2 FSETP + 4 FMUL per pair); no argument here is one
+__device__ __forceinline__ float rsq(float a) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
 __device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 
 struct TreeCell {
@@ -231,7 +233,7 @@ __device__ __forceinline__ void sweep2(const ulonglong2 *__restrict__ src, uint3
         float a, b;
         upk(R2, a, b);
         if (LAW == 1) { a = fmaxf(a, 1.0e-30f); b = fmaxf(b, 1.0e-30f); }      // r = 0: the pair of a sink with itself
-        const u64 RI = pk(rsqrtf(a), rsqrtf(b));
+        const u64 RI = pk(rsq(a), rsq(b));
         u64 F = mul2(mul2(RI, RI), RI);
         if (LAW == 1) {
             const u64 U = mul2(mul2(R2, RI), C.ie);
