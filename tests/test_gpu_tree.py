@@ -124,3 +124,32 @@ def test_tree_rejects_bad_theta(ctx):
     for th in (-0.1, 1.0, float("nan")):
         with pytest.raises(nf.NFError):
             ctx.forces_tree(b2, 1, 0.01, 1e-3, th)
+
+
+@pytest.mark.parametrize("seed", [101, 102, 103, 104, 105])
+def test_tree_randomised(ctx, seed):
+    """Seeded random boxes: 1-3 clumps of 4096-9000 particles of random place, radius and offset, random K, R, eps, theta,
+    softening law and masses.  Counts bit for bit, every sink within the bars."""
+    rng = np.random.default_rng(seed)
+    K = int(rng.integers(3, 7))
+    R = 2 if (K >= 5 and rng.integers(0, 2)) else 1
+    box = float(rng.choice([1.0, 3.0, 500.0]))
+    w = box / K
+    eps = float(w * rng.choice([0.002, 0.01, 0.05, 0.2]))
+    theta = float(rng.choice([0.2, 0.4, 0.6, 0.8, 0.95]))
+    cl = []
+    for _ in range(int(rng.integers(1, 4))):
+        rad = float(rng.choice([0.02, 0.1, 0.3, 0.49]))
+        cl.append((tuple(int(x) for x in rng.integers(0, K, 3)), int(rng.choice([4096, 4100, 5000, 9000])), rad,
+                   tuple(float(x) for x in rng.uniform(-0.4, 0.4, 3) * (0.5 - rad))))
+    softening = str(rng.choice(["spline", "spline", "plummer"]))
+    pos = inputs.clumps(seed, K, box, cl, int(rng.choice([0, 300, 3000])))
+    N = pos.shape[0]
+    m = (rng.random(N) + 0.5).astype(np.float32) if rng.integers(0, 2) else None
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box, mass=torch.from_numpy(m).cuda() if m is not None else None)
+    acc = ctx.forces_tree(b, R, eps, 1e-3, theta, softening=softening, use_mass=m is not None).cpu().numpy()
+    st = ctx.tree_stats()
+    ref, st_ref = nf_tree.forces_tree(pos, K, R, eps, box, 1e-3, theta, softening=softening, mass=m, stats=True)
+    assert st["node"] == st_ref["node"] and st["leaf"] == st_ref["leaf"]
+    err = oracle.parity_error(acc, ref)
+    assert np.isfinite(acc).all() and np.median(err) < MEDIAN_TOL and err.max() < MAX_TOL, (np.median(err), err.max())
