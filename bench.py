@@ -577,7 +577,7 @@ def run_tree(args, cfg):
     # pairs the interaction kernel still evaluated: sources of cells below the dense threshold (reading t1)
     cnt = b.cell_count.cpu().numpy().astype(np.int64).reshape(K, K, K)
     coff, rank, dense = 0, 0, np.zeros(K ** 3, dtype=bool)
-    cap = min(max(N // 4, 1 << 20), 1 << 28) & ~63
+    cap = min(max(N, 1 << 20) + 64 * 2048, 1 << 28) & ~63
     for c, n in enumerate(cnt.ravel()):
         if n >= 4096:
             n64 = (int(n) + 63) & ~63

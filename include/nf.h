@@ -66,7 +66,7 @@ enum {
 #define NF_MASS_W 0x100
 /* Flag OR-ed into the `softening` argument of every force call (nf_forces*, nf_forces_host*, nf_stream_*): the box holds
  * cells of thousands of particles or more ("the largest cell has over 200,000 particles").  Such cells
- * (>= 4096 particles; up to 2048 of them and a quarter of the particles -- at least 2^20 -- per box, or per plane in the
+ * (>= 4096 particles; up to 2048 of them and 2^28 particles per box, or per plane in the
  * slab stream) get their INTERNAL encoded copies ordered along a Hilbert curve inside the cell, with a bounding box per 64
  * particles, so that the kernel can prove most source tiles of a dense cell free of pairs inside eps and sweep them with
  * the bare 1/r^2 law instead of the min form of Eq. 2 -- exact, because the two agree for r >= eps (fn. 4).
@@ -231,7 +231,7 @@ int nf_forces_chunk(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_o
  * here is stated in DESIGN.md (readings t1-t6) and followed step by step by oracle/nf_tree.py:
  *
  *   - a cell of >= 4096 particles is DENSE (the cells NF_DENSE_ORDER orders: at most 2048 of them and
- *     min(max(N/4, 2^20), 2^28) particles in 64-aligned sizes, taken in cell order; further ones are not dense);
+ *     2^28 particles in 64-aligned sizes, taken in cell order; further ones are not dense);
  *   - its particles, in Hilbert order of their cell-centred offsets, form leaves of 16 and nodes of 8 children up to a
  *     root; a node has the bounding box of its particles, their mass and centre of mass;
  *   - sinks are taken 64 at a time (consecutive in their cell) with their bounding box; such a group meets each dense

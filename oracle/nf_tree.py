@@ -9,7 +9,8 @@ the one DESIGN.md states (readings t1-t6, "Tree near field"), step by step:
 
   t1  A cell is DENSE when it holds >= 4096 particles.  (Capacity rule of the implementation, part of the definition: the
       dense cells taken are, in cell order, the first 2048 whose 64-aligned sizes add up to at most
-      cap(N) = min(max(N/4, 2^20), 2^28) rounded down to 64; further ones are treated as not dense.)
+      cap(N) = min(max(N, 2^20) + 64 * 2048, 2^28) rounded down to 64 -- room for every particle unless N > 2^28 --; further
+      ones are treated as not dense.)
   t2  Inside a dense cell the particles are ordered by the 21-bit Hilbert index (Skilling's construction) of their float32
       cell-centred offset o (7 bits per axis, q = clamp(int(((o * (K/box)) + 0.5) * 128), 0, 127), every operation
       rounded to float32, x the most significant axis), ties in the stable order of the binning.  (A Hilbert run is a
@@ -58,7 +59,7 @@ f32 = np.float32
 
 
 def dense_cap(N: int) -> int:
-    c = max(N // 4, 1 << 20)
+    c = max(N, 1 << 20) + 64 * DENSE_MAX_CELLS
     return min(c, 1 << 28) & ~63
 
 
@@ -253,17 +254,22 @@ def forces_tree(pos, K: int, R: int, eps: float, box: float, Gm: float, theta: f
     a_tree = np.zeros((N, 3))
     xg = pos.astype(np.float64)
     st = dict(node=0, leaf=0, direct=0)
-    # trees of the dense cells
+    # trees of the dense cells, built when first needed
     trees = {}
-    for c in np.nonzero(dense)[0]:
-        s = np.arange(off[c], off[c + 1])
-        order = hilbert_order(offs32[s], K, box)
-        s = s[order]
-        trees[int(c)] = (s, build_tree(offs32[s], xg[perm[s]], m_all[perm[s]]))
+
+    def tree_of(c):
+        if c not in trees:
+            s = np.arange(off[c], off[c + 1])
+            s = s[hilbert_order(offs32[s], K, box)]
+            trees[c] = (s, build_tree(offs32[s], xg[perm[s]], m_all[perm[s]]))
+        return trees[c]
+
     cw32 = f32(box) / f32(K)
     deltas = list(itertools.product(range(-R, R + 1), repeat=3))
     cells = np.nonzero(cnt > 0)[0]
     for c in cells:
+        if not stats and not wanted[perm[off[c]:off[c + 1]]].any():
+            continue
         cz, cy, cx = int(c % K), int((c // K) % K), int(c // (K * K))
         nb = []
         for (dx, dy, dz) in deltas:
@@ -275,7 +281,7 @@ def forces_tree(pos, K: int, R: int, eps: float, box: float, Gm: float, theta: f
                 st["direct"] += int(cnt[c]) * int(cnt[D])
         if not nb:
             continue
-        s_c = trees[int(c)][0] if dense[c] else np.arange(off[c], off[c + 1])
+        s_c = tree_of(int(c))[0] if dense[c] else np.arange(off[c], off[c + 1])
         for g0 in range(0, s_c.shape[0], GROUP):
             gs = s_c[g0:g0 + GROUP]                      # t4: sorted slots of the group's sinks
             if not stats and not wanted[perm[gs]].any():
@@ -284,7 +290,7 @@ def forces_tree(pos, K: int, R: int, eps: float, box: float, Gm: float, theta: f
                 ps = gs[members]                         # t4: the sinks that walk together, and their box
                 xs = xg[perm[ps]]
                 for (D, dl, img) in nb:
-                    src, levels = trees[int(D)]
+                    src, levels = tree_of(int(D))
                     sh = (np.array(dl, dtype=f32) * cw32).astype(f32)
                     nodes, leaves = walk(levels, glo, ghi, sh, eps, theta)
                     image = np.array(img, dtype=np.float64) * float(box)

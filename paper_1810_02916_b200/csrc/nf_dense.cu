@@ -190,10 +190,11 @@ __global__ void __launch_bounds__(256) k_dense_finish(const float4 *__restrict__
 
 }  // namespace
 
-// compact positions the ordering takes per call: a quarter of the particles, at least 2^20, at most 2^28
+// compact positions the ordering takes per call: room for every particle in 64-aligned cells (N + 64 per dense cell), at
+// least 2^20 + 2^17, at most 2^28
 uint32_t nf_dense_cap(int64_t N)
 {
-    const int64_t c = N / 4 > (1 << 20) ? N / 4 : (1 << 20);
+    const int64_t c = (N > (1 << 20) ? N : (1 << 20)) + 64ll * NF_DENSE_MAX_CELLS;
     return (uint32_t)(c < (1ll << 28) ? c : (1ll << 28)) & ~63u;
 }
 

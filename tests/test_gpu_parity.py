@@ -826,9 +826,9 @@ def test_dense_order_host_paths_and_stream(ctx):
     assert all(torch.equal(a, c) for a, c in zip(out_d, out_d2))
 
 
-def test_forces_dense_order_beyond_its_capacity(ctx):
-    """More particles in dense cells than the ordering takes per call (a quarter of N, at least 2^20): the cells past the
-    limit keep nf_bin's order and the old laws, next to cells that are ordered."""
+def test_forces_dense_order_most_particles_in_dense_cells(ctx):
+    """Three neighbouring cells of 4.2x10^5 particles each, 99.6 % of the box: all of it is ordered (the ordering has room for
+    every particle), dense cells are each other's neighbours across faces."""
     rng = np.random.default_rng(92)
     K, R, box = 5, 2, 1.0
     w = box / K
@@ -844,6 +844,36 @@ def test_forces_dense_order_beyond_its_capacity(ctx):
     sink = np.sort(rng.choice(n, 1500, replace=False))
     ref = oracle.forces(pos, K, R, eps, box, 1.0 / n, sink_idx=sink)
     err = oracle.parity_error(acc.cpu().numpy()[sink], ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (float(np.median(err)), float(err.max()))
+
+
+def test_forces_dense_order_beyond_its_capacity(ctx):
+    """More dense cells than the ordering takes per call (2048): K = 13, every one of the 2197 cells holds ~4300 particles.
+    The cells past the limit (the last ~150 in cell order) keep nf_bin's order and the old laws -- their encoded copies come
+    from k_dense_left_out --, next to cells that are ordered."""
+    rng = np.random.default_rng(93)
+    K, R, box = 13, 1, 1.0
+    n = K ** 3 * 4300
+    pos = rng.random((n, 3), dtype=np.float32)
+    pos[pos >= 1.0] = 0.5
+    eps = 0.01 * box / K
+    b = ctx.bin(torch.from_numpy(pos).cuda(), K, box)
+    cnt = u32(b.cell_count)
+    assert int((cnt >= 4096).sum()) > 2048 + 50
+    acc = ctx.forces(b, R, eps, 1.0 / n)                            # N / K^3 >= 512: the ordering is automatic
+    assert torch.equal(acc, ctx.forces(b, R, eps, 1.0 / n))
+    # sinks from the first cells (ordered), the last cells (left out) and anywhere
+    key, _ = oracle.keys(pos, K, box)
+    sink = np.sort(np.concatenate([np.nonzero(key < 30)[0][:400], np.nonzero(key >= K ** 3 - 30)[0][:400], rng.choice(n, 400, replace=False)]))
+    ref = oracle.forces(pos, K, R, eps, box, 1.0 / n, sink_idx=sink)
+    err = oracle.parity_error(acc.cpu().numpy()[sink], ref)
+    assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (float(np.median(err)), float(err.max()))
+    # the tree takes the same 2048 cells and leaves the others to the direct sum: the oracle follows the same rule
+    a_t = ctx.forces_tree(b, R, eps, 1.0 / n, 0.6).cpu().numpy()
+    from oracle import nf_tree
+    sink_t = sink[::6]
+    ref_t = nf_tree.forces_tree(pos, K, R, eps, box, 1.0 / n, 0.6, sink_idx=sink_t)
+    err = oracle.parity_error(a_t[sink_t], ref_t)
     assert np.median(err) <= MEDIAN_TOL and err.max() <= MAX_TOL, (float(np.median(err)), float(err.max()))
 
 
