@@ -655,6 +655,36 @@ def run_tree(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def run_occupancy(args):
+    """`--occupancy`: the interaction kernel on boxes whose cells ALL hold exactly n particles (uniform inside the cell), K = 48,
+    R = 2: kernel time and fraction of the FP32 roofline as a function of the occupancy, i.e. of the task shape (L = ceil(n/4)
+    lanes, P = floor(32/L) phases) and of the tile length (5n sources per column).  A measuring aid for DESIGN.md Sec. 11."""
+    from paper_1810_02916_b200 import nf
+    dev = torch.device("cuda", 0)
+    ctx = nf.Context(0)
+    K, R, box = 48, 2, 1.0
+    w = box / K
+    g = torch.Generator(device=dev)
+    g.manual_seed(5)
+    cells = torch.stack(torch.meshgrid(torch.arange(K), torch.arange(K), torch.arange(K), indexing="ij"), -1).reshape(-1, 3).to(dev).float()
+    sm_max_mhz, _, peak_src = read_peaks()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak = sms * sm_max_mhz * 1e6 * 2 * FP32_LANES_PER_SM
+    rows = []
+    for n in (4, 8, 12, 16, 20, 24, 28, 32, 36, 40, 44, 48, 52, 56, 60, 64, 72, 80, 96, 112, 128):
+        pos = ((cells[:, None, :] + 0.02 + 0.96 * torch.rand(K ** 3, n, 3, generator=g, device=dev)) * w).reshape(-1, 3).contiguous()
+        b = ctx.bin(pos, K, box)
+        I = ctx.interactions(b, R)
+        ts = []
+        for s_ in range(args.warmup + args.steps):
+            ctx.forces(b, R, 0.01 * w, 1.0)
+            if s_ >= args.warmup:
+                ts.append(ctx.last_forces_timing()[0])
+        k_ms = statistics.median(ts)
+        rows.append({"n": n, "kernel_ms": k_ms, "frac": FLOP_PER_INTERACTION * I / (k_ms * 1e-3) / peak})
+    print(json.dumps({"occupancy_sweep": rows, "K": K, "R": R, "peak_source": f"{sms} SMs x {sm_max_mhz:.0f} MHz ({peak_src})"}), flush=True)
+
+
 def sweep_small_configs(ctx, dev, steps=3, warmup=3):
     """Interaction-kernel roofline fraction of C1, C2 and C3 -- the other single-GPU configs of BASELINE.json beside the
     headline workload -- and of D1, the one-dense-cell workload (config 6), in the same process (milliseconds each).  Same timing rules as the main
@@ -734,6 +764,8 @@ def main():
                     help="gloo: debugging aid, every rank on cuda:0 with ghosts staged through host memory")
     ap.add_argument("--n-side", type=int, default=0,
                     help="profiling aid: the same recipe at n_side^3 particles and K = n_side/4 (not the bench workload)")
+    ap.add_argument("--occupancy", action="store_true",
+                    help="measuring aid: kernel efficiency on boxes whose cells all hold exactly n particles, n = 4 ... 128")
     ap.add_argument("--tree", type=float, default=None, metavar="THETA",
                     help="time the step with nf_forces_tree (tree near field for dense cells, opening angle THETA) instead of nf_forces")
     args = ap.parse_args()
@@ -751,6 +783,9 @@ def main():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     if cfg.kind == "slab":
         run_stream(args, cfg)
+        return
+    if args.occupancy:
+        run_occupancy(args)
         return
     if args.tree is not None:
         if int(os.environ.get("WORLD_SIZE", "1")) > 1:
