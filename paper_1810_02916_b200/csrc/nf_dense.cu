@@ -22,7 +22,7 @@
 namespace {
 
 constexpr uint32_t PAD = 0xffffffffu;
-constexpr uint32_t MORTON_BITS = 21, MORTON_MASK = (1u << MORTON_BITS) - 1;
+constexpr uint32_t CURVE_BITS = 21, CURVE_MASK = (1u << CURVE_BITS) - 1;
 
 using DenseCell = nf_dense_cell;
 
@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(256) k_dense_keys(const float4 *__restrict__ p
         }
         const DenseCell dc = dcell[lo];
         const uint32_t j = t - dc.coff;
-        uint32_t k = MORTON_MASK, i = PAD;       // padding sorts behind the cell's particles
+        uint32_t k = CURVE_MASK, i = PAD;       // padding sorts behind the cell's particles
         if (j < dc.n) {
             const float4 q = pos[dc.c0 + j];
             // every operation rounded to float32, no fused multiply-add: the order is part of the tree's definition
@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(256) k_dense_keys(const float4 *__restrict__ p
             k = hilbert3((uint32_t)qx, (uint32_t)qy, (uint32_t)qz);
             i = j;
         }
-        key[t] = (lo << MORTON_BITS) | k;
+        key[t] = (lo << CURVE_BITS) | k;
         idx[t] = i;
     }
     (void)cap;
@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(256) k_dense_finish(const float4 *__restrict__
     for (uint32_t ch = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); ch < nchunk_max; ch += gridDim.x * (blockDim.x >> 5)) {
         const uint32_t t0 = ch * 64u;
         if (t0 >= n_d) return;
-        const DenseCell dc = dcell[key[t0] >> MORTON_BITS];
+        const DenseCell dc = dcell[key[t0] >> CURVE_BITS];
         const int cz = (int)(dc.cell % (uint32_t)K);
         const float ez = ((float)(cz % NF_ZB) - 0.5f * (float)(NF_ZB - 1)) * ws;
         const float eh = ((float)((cz + NF_ZB / 2) % NF_ZB) - 0.5f * (float)(NF_ZB - 1)) * ws;

@@ -735,7 +735,7 @@ def test_forces_dense_cells_randomised(ctx, seed, dense_order):
 
 
 def test_forces_dense_order_clumps_across_faces(ctx):
-    """NF_DENSE_ORDER (in-cell Morton ordering of cells >= 4096 particles, boxes per 64 particles, tile-by-tile choice of
+    """NF_DENSE_ORDER (in-cell Hilbert ordering of cells >= 4096 particles, boxes per 64 particles, tile-by-tile choice of
     the law): clumps of 10^4 - 10^5 particles planted ON cell faces, edges and a corner, so that dense cells see dense
     neighbours across every kind of boundary and close pairs straddle them; eps of the order of the clump's interparticle
     spacing.  Sampled sinks against the oracle, the flag against no flag, determinism, the chunk call, masses."""
