@@ -754,7 +754,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number 1..5 (default 4 = C4; 5 = slab streaming); 6 = one dense cell of 4x10^5 particles (profiling workload)")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number 1..5 (default 4 = C4; 5 = slab streaming); 6 = one dense cell of 4x10^5 particles (profiling workload); 7 = the C3 recipe at K = 16: 254 dense cells (for --tree)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

@@ -79,7 +79,12 @@ def config(which: int) -> Config:
         # over 200,000 particles"): one cell of ~4x10^5 particles in an otherwise almost empty K = 5 box
         N = 400_000
         return Config("D1-one-dense-cell-4e5", N, 5, 2, 1.0, 0.01 * 0.2, 1.0 / N, s, "onecell")
-    raise ValueError("config number must be 1..5 (6: the one-dense-cell profiling workload)")
+    if which == 7:
+        # not a BASELINE.json config: the C3 recipe on a grid four times coarser -- 4096 particles per cell on average, 254
+        # cells of >= 4096 (the largest 1.2x10^5) holding half the particles and neighbouring one another: the tree near
+        # field (nf_forces_tree) with many trees
+        return scaled(dataclasses.replace(config(3), seed=s), 256 ** 3, 16, name="D2-clustered-256^3-K16")
+    raise ValueError("config number must be 1..5 (6: the one-dense-cell profiling workload, 7: many dense cells)")
 
 
 def scaled(cfg: Config, N: int, K: int, name: Optional[str] = None) -> Config:
