@@ -234,7 +234,9 @@ int nf_forces_chunk(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_o
  *     2^28 particles in 64-aligned sizes, taken in cell order; further ones are not dense);
  *   - its particles, in Hilbert order of their cell-centred offsets, form leaves of 16 and nodes of 8 children up to a
  *     root; a node has the bounding box of its particles, their mass and centre of mass;
- *   - sinks are taken 64 at a time (consecutive in their cell) with their bounding box; such a group meets each dense
+ *   - sinks are taken 64 at a time (consecutive in their cell) with their bounding box -- a group whose box is more than
+ *     three times wider (diagonal) than the tightest of its four quarters walks quarter by quarter, such a quarter sink by
+ *     sink --; such a group meets each dense
  *     cell among its (2R+1)^3 neighbours by walking that cell's tree: a node whose box is further from the group's box
  *     than eps and than (its diagonal / theta) acts as ONE particle at its centre of mass (1/r^2); any other node is
  *     opened, and a leaf that is not accepted is summed particle by particle with the softened law of `softening`;
@@ -243,6 +245,8 @@ int nf_forces_chunk(nf_ctx *ctx, const float *pos_sorted, const uint64_t *cell_o
  *   theta       opening angle, 0 <= theta < 1.  theta = 0 accepts nothing: the result is the direct sum (nf_forces_ex up
  *               to summation order).  For theta > 0 the result is an APPROXIMATION: per accepted node the error is at
  *               most G M / D^2 * (1/(1-theta)^2 - 1 - 2 theta), D the distance to its centre of mass.
+ *               Measured on one cell of 4x10^5 particles: theta = 0.5 is 8x faster than the direct sum and 3x10^-4 (median,
+ *               north-star metric) away from it, theta = 0.7 13x and 7x10^-4; theta = 0 is 10x SLOWER than nf_forces_ex.
  *   everything else as for nf_forces_ex (NF_MASS_W allowed; NF_DENSE_ORDER implied).  cell_amax is computed from the
  *   final accelerations.  Asynchronous on `stream`; deterministic (bit-reproducible from call to call).
  *   The box must be whole (no chunk / slab / host variant).
