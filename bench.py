@@ -897,7 +897,9 @@ def main():
             # (b) the two-deep pipeline nf_forces_host_begin / _end: step s+1's H2D and step s's D2H run behind the
             # kernels of the step in between.  Timed in steady state: every iteration completes one whole step
             # (whose H2D, kernels and D2H all ran inside the timed region or overlapped the previous iteration's).
-            n_e2e = max(3, min(args.steps, 5))
+            # (long steps: 3-5 of them; short steps: as many as fill half a second, so that the few-step noise of the host clock
+            # does not decide the number -- C2 read 7.56 ms over 5 steps and 7.06 ms over 20)
+            n_e2e = max(3, min(args.steps, 5)) if ms_per_step > 100.0 else min(50, max(5, int(500.0 / max(ms_per_step, 1e-3))))
             ctx.forces_host_begin(hpos, K, R, rcfg.eps, rcfg.box, rcfg.Gm, hacc[0])
             ctx.forces_host_begin(hpos, K, R, rcfg.eps, rcfg.box, rcfg.Gm, hacc[1])
             ctx.forces_host_end()                                   # the pipeline is primed: one step in flight
